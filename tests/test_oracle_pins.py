@@ -1,0 +1,555 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix.
+
+The paper (arxiv 2309.15861) prints no worked numerical example, so the oracle
+is pinned to closed forms, invariants, special cases that reduce to textbook
+results, statistical laws with a known expectation, and brute force on tiny
+inputs (SURVEY.md §8(c) "Pins").  None of these tests touches the CUDA path.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+from conftest import ROOT
+
+C = 0.299792458
+ALPHA = 7.2973525693e-3
+
+
+def one_segment(x0=0.0, y0=0.0, z0=10000.0, t0=0.0, d=(0.0, 0.0, -1.0), length=1.0, gamma=1e7,
+                charge=-1.0, dE=1.0):
+    s = np.zeros(1, dtype=W.SEGMENT_DTYPE)
+    d = np.asarray(d, dtype=np.float64)
+    d = d / np.linalg.norm(d)
+    s["x0"], s["y0"], s["z0"], s["t0"] = x0, y0, z0, t0
+    s["dx"], s["dy"], s["dz"] = d
+    s["length"], s["gamma"], s["charge"], s["dE"] = length, gamma, charge, dE
+    return s
+
+
+ATM1 = W.atmosphere_single_layer()
+ATM5 = W.atmosphere_five_layer()
+PAR = W.default_params()
+
+
+# ------------------------------------------------------------------ Philox / uniforms
+def test_philox_known_answer_vectors():
+    n = 0
+    with open(os.path.join(ROOT, "tests", "golden", "philox4x32_10_kat.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            w = [int(x, 16) for x in line.split()]
+            assert O.philox4x32_10(w[0:4], w[4:6]) == w[6:10]
+            n += 1
+    assert n == 3
+
+
+def test_philox_is_a_bijection_of_the_counter_on_a_sample():
+    # distinct counters -> distinct outputs (Philox is a keyed permutation of the 128-bit counter)
+    outs = {tuple(O.philox4x32_10([j, 7, 0, t], [5, 9])) for j in range(2000) for t in (0, 1)}
+    assert len(outs) == 4000
+
+
+def test_uniform_construction_R19():
+    assert O.uniform(0) == 2.0 ** -24
+    assert O.uniform(0xFFFFFFFF) == 1.0 - 2.0 ** -24
+    assert O.uniform(0x1FF) == 2.0 ** -24            # low 9 bits are dropped
+    assert O.uniform(0x200) == 1.5 * 2.0 ** -23
+    rng = np.random.default_rng(0)
+    for r in rng.integers(0, 2 ** 32, 200):
+        u = O.uniform(int(r))
+        assert 0.0 < u < 1.0 and float(np.float32(u)) == u   # exactly representable in fp32
+
+
+def test_uniform_stream_mean_and_variance():
+    u = np.array([O.uniform(x) for j in range(4000) for x in O.philox4x32_10([j, 1, 0, 0], [42, 0])])
+    assert abs(u.mean() - 0.5) < 4 * math.sqrt(1 / 12 / len(u))
+    assert abs(u.var() - 1 / 12) < 0.003
+
+
+# ------------------------------------------------------------------ atmosphere
+def test_column_depth_single_layer(golden_closed_forms):
+    g = golden_closed_forms
+    assert O.depth(ATM1, 0.0) == pytest.approx(g["depth_h0_gcm2"], rel=1e-6)
+    assert O.depth(ATM1, 2000.0) == pytest.approx(g["depth_h2000_gcm2"], rel=1e-5)
+    for h in (0.0, 1234.0, 8400.0, 30000.0):
+        assert O.depth(ATM1, h) == pytest.approx(1.225e-3 * 840000.0 * math.exp(-h / 8400.0), rel=1e-14)
+        assert O.refractivity(ATM1, h) == pytest.approx(2.83e-4 * math.exp(-h / 8400.0), rel=1e-14)
+
+
+def test_five_layer_check_values_and_continuity(golden_closed_forms):
+    g = golden_closed_forms
+    for h, key in ((0, "five_layer_T_h0"), (2000, "five_layer_T_h2000"), (10000, "five_layer_T_h10000"),
+                   (40000, "five_layer_T_h40000")):
+        assert O.depth(ATM5, float(h)) == pytest.approx(g[key], rel=2e-4)
+    assert O.density(ATM5, 0.0) == pytest.approx(1.225e-3, rel=1e-12)
+    assert O.depth(ATM5, 112800.0) == pytest.approx(0.0, abs=1e-9)
+    for hb in (4000.0, 10000.0, 40000.0, 100000.0):          # T and rho continuous across boundaries
+        assert O.depth(ATM5, hb - 1e-6) == pytest.approx(O.depth(ATM5, hb), rel=1e-9)
+        assert O.density(ATM5, hb - 1e-6) == pytest.approx(O.density(ATM5, hb), rel=1e-9)
+
+
+def test_density_is_minus_dT_dh():
+    for atm in (ATM1, ATM5):
+        for h in (500.0, 3000.0, 7000.0, 25000.0, 60000.0):
+            dT = (O.depth(atm, h + 0.5) - O.depth(atm, h - 0.5)) / 1.0   # g/cm^2 per m
+            assert O.density(atm, h) == pytest.approx(-dT / 100.0, rel=1e-6)
+
+
+# ------------------------------------------------------------------ Cherenkov closed forms
+@pytest.mark.parametrize("h", [0, 2000, 8400, 10000])
+def test_cherenkov_angle_yield_and_threshold(golden_closed_forms, h):
+    g = golden_closed_forms
+    n = 1.0 + 2.83e-4 * math.exp(-h / 8400.0)
+    L = 2.0
+    seg = one_segment(z0=h + L / 2, length=L, gamma=1e7)       # midpoint altitude = h (R3)
+    st, f = O.preamble(ATM1, PAR, seg[0], 0)
+    assert st == 0
+    theta = math.atan2(f.sin_c, f.cos_c)
+    assert math.degrees(theta) == pytest.approx(g[f"theta_c_deg_h{h}"], abs=2e-5)
+    assert theta == pytest.approx(math.acos(1.0 / n), rel=1e-9)
+    assert f.sin_c ** 2 + f.cos_c ** 2 == pytest.approx(1.0, abs=1e-15)
+    # photons per metre at beta = 1, 300-600 nm
+    assert f.mu / L == pytest.approx(g[f"photons_per_m_h{h}"], rel=2e-4)
+    c_ft = 2 * math.pi * ALPHA * (1 / 300e-9 - 1 / 600e-9)
+    assert f.mu / L == pytest.approx(c_ft * (1.0 - 1.0 / n ** 2), rel=1e-9)
+    assert f.n_b == math.ceil(f.mu) and f.w0 == pytest.approx(f.mu / f.n_b, rel=1e-15)
+    # threshold: no photons just below gamma_th, photons just above
+    gth = (1.0 - 1.0 / n ** 2) ** -0.5
+    assert gth == pytest.approx(g[f"gamma_th_h{h}"], rel=2e-5)
+    st, f_lo = O.preamble(ATM1, PAR, one_segment(z0=h + L / 2, length=L, gamma=gth * (1 - 1e-4))[0], 0)
+    st, f_hi = O.preamble(ATM1, PAR, one_segment(z0=h + L / 2, length=100.0, gamma=gth * (1 + 1e-2),
+                                                 d=(1, 0, 0))[0], 0)
+    assert f_lo.n_b == 0 and f_hi.n_b > 0
+
+
+def test_theta_c_rad_sea_level(golden_closed_forms):
+    st, f = O.preamble(ATM1, PAR, one_segment(z0=0.5, length=1.0)[0], 0)
+    assert math.atan2(f.sin_c, f.cos_c) == pytest.approx(golden_closed_forms["theta_c_rad_h0"], abs=2e-7)
+
+
+def test_frank_tamm_constant(golden_closed_forms):
+    g = golden_closed_forms
+    assert 2 * math.pi * ALPHA == pytest.approx(g["two_pi_alpha"], rel=1e-9)
+    # the prefactor printed in PAPER.md:45, pi e^2 / (h eps0 c), from CODATA constants
+    e, hp, eps0, c0 = 1.602176634e-19, 6.62607015e-34, 8.8541878128e-12, 299792458.0
+    assert math.pi * e * e / (hp * eps0 * c0) == pytest.approx(g["two_pi_alpha"], rel=1e-8)
+    for lam1, lam2, key, scale in ((300.0, 600.0, "frank_tamm_per_m_300_600", 1.0),
+                                   (400.0, 700.0, "frank_tamm_per_cm_400_700", 0.01)):
+        par = W.default_params(lam1=lam1, lam2=lam2)
+        st, f = O.preamble(ATM1, par, one_segment(z0=0.5, length=1.0)[0], 0)
+        assert f.mu / f.sin_c ** 2 * scale == pytest.approx(g[key], abs=5.1e-3)   # fixture printed to 2 decimals
+    # charge enters as z^2, length linearly
+    st, f1 = O.preamble(ATM1, PAR, one_segment(z0=5000.0, length=1.0, d=(1, 0, 0))[0], 0)
+    st, f2 = O.preamble(ATM1, PAR, one_segment(z0=5000.0, length=3.0, d=(1, 0, 0), charge=2.0)[0], 0)
+    assert f2.mu == pytest.approx(12.0 * f1.mu, rel=1e-14)
+
+
+def test_bunching_R1():
+    seg = one_segment(z0=5000.0, length=10.0, d=(1, 0, 0))
+    st, f1 = O.preamble(ATM1, PAR, seg[0], 0)
+    st, f5 = O.preamble(ATM1, W.default_params(bunch_size=5.0), seg[0], 0)
+    assert f1.mu == f5.mu
+    assert f5.n_b == math.ceil(f5.mu / 5.0) and f5.w0 == pytest.approx(f5.mu / f5.n_b) and f5.w0 <= 5.0
+    assert f1.w0 <= 1.0
+
+
+def test_invalid_segments_are_rejected():
+    for kw in (dict(gamma=0.5), dict(length=-1.0), dict(gamma=float("nan")), dict(z0=float("inf"))):
+        st, f = O.preamble(ATM1, PAR, one_segment(**kw)[0], 0)
+        assert st == -1 and f.n_b == 0
+    s = one_segment()
+    s["dx"] = 0.1                                       # |d| off unity by more than 1e-3
+    st, f = O.preamble(ATM1, PAR, s[0], 0)
+    assert st == -1
+
+
+# ------------------------------------------------------------------ rotation
+def _random_dirs(n, seed):
+    rng = np.random.default_rng(seed)
+    v = rng.normal(size=(n, 3))
+    return v / np.linalg.norm(v, axis=1, keepdims=True)
+
+
+def test_rodrigues_matrix_invariants():
+    dirs = list(_random_dirs(50, 1)) + [np.array([0, 0, -1.0]), np.array([0, 0, 1.0]), np.array([1.0, 0, 0])]
+    for d in dirs:
+        st, f = O.preamble(ATM1, PAR, one_segment(z0=8000.0, d=d, length=1.0)[0], 0)
+        M = np.array([[f.M[i][j] for j in range(3)] for i in range(3)])
+        A = np.array(list(f.A))
+        dd = np.array(list(f.d))
+        assert np.allclose(M, M.T, atol=0)                         # symmetric
+        assert np.allclose(M @ M, np.eye(3), atol=1e-14)           # involution
+        assert np.linalg.det(M) == pytest.approx(1.0, abs=1e-14)   # proper rotation
+        assert np.allclose(M @ np.array([0, 0, -1.0]), dd, atol=1e-14)   # downward normal -> track direction
+        assert np.linalg.norm(A) == pytest.approx(1.0, abs=1e-15)
+        # geometric definition: rotation by pi about A (general axis-angle formula)
+        K = np.array([[0, -A[2], A[1]], [A[2], 0, -A[0]], [-A[1], A[0], 0]])
+        Rpi = np.eye(3) + math.sin(math.pi) * K + (1 - math.cos(math.pi)) * (K @ K)
+        assert np.allclose(M, Rpi, atol=1e-14)
+        if 1 - dd[2] >= 1e-12:                                     # A bisects d and -z
+            assert A @ dd == pytest.approx(A @ np.array([0, 0, -1.0]), abs=1e-14)
+
+
+def test_every_cherenkov_photon_lies_on_the_cone():
+    for d in _random_dirs(20, 2):
+        if d[2] > 0:
+            d = -d
+        seg = one_segment(z0=8000.0, d=d, length=25.0)
+        st, f = O.preamble(ATM1, PAR, seg[0], 0)
+        dd = np.array(list(f.d))
+        for j in range(0, f.n_b, max(1, f.n_b // 40)):
+            ph = O.make_photon(f, PAR, 11, j, 0)
+            v = np.array(list(ph.v))
+            e = np.array(list(ph.e))
+            assert v @ dd == pytest.approx(f.cos_c, abs=1e-14)     # v . d = cos(theta_c)
+            assert np.linalg.norm(v) == pytest.approx(1.0, abs=1e-14)
+            s = (e - np.array([seg["x0"][0], seg["y0"][0], seg["z0"][0]], dtype=np.float64)) @ dd
+            assert 0.0 < s < float(seg["length"][0])               # on the track
+            assert np.allclose(np.cross(e - np.array(list(f.p0)), dd), 0, atol=1e-8)
+            assert ph.t_e == pytest.approx(s * f.inv_beta_c, abs=1e-9)  # t0 = 0, moves at beta c
+            assert 300.0 < ph.lam < 600.0
+
+
+def test_azimuth_is_uniform_around_the_track():
+    seg = one_segment(z0=8000.0, d=(0.3, -0.2, -0.93), length=200.0)
+    st, f = O.preamble(ATM1, PAR, seg[0], 0)
+    dd = np.array(list(f.d))
+    e1 = np.cross(dd, [0, 0, 1.0]); e1 /= np.linalg.norm(e1)
+    e2 = np.cross(dd, e1)
+    phis = []
+    for j in range(f.n_b):
+        v = np.array(list(O.make_photon(f, PAR, 3, j, 0).v))
+        phis.append(math.atan2(v @ e2, v @ e1))
+    hist, _ = np.histogram(phis, bins=8, range=(-math.pi, math.pi))
+    exp = len(phis) / 8
+    assert ((hist - exp) ** 2 / exp).sum() < 24.3                 # chi2, 7 dof, p ~ 1e-3
+
+
+def test_wavelength_law_R4():
+    seg = one_segment(z0=3000.0, d=(1, 0, 0), length=300.0)
+    st, f = O.preamble(ATM1, PAR, seg[0], 0)
+    lam = np.array([O.make_photon(f, PAR, 5, j, 0).lam for j in range(f.n_b)])
+    n = len(lam)
+    assert n > 5000
+    inv = 1.0 / lam                                                # uniform on [1/600, 1/300]
+    lo, hi = 1 / 600.0, 1 / 300.0
+    assert abs(inv.mean() - (lo + hi) / 2) < 4 * (hi - lo) / math.sqrt(12 * n)
+    assert abs(np.median(lam) - 400.0) < 400.0 * 4 * 0.5 / math.sqrt(n) * 1.5   # median = 2/(1/l1 + 1/l2)
+    # fluorescence: uniform on [340, 450]
+    par = W.default_params(processes=W.PROC_FLUORESCENCE)
+    st, ff = O.preamble(ATM1, par, one_segment(dE=2000.0)[0], 1)
+    lf = np.array([O.make_photon(ff, par, 5, j, 1).lam for j in range(ff.n_b)])
+    assert ff.n_b == 8000 and lf.min() > 340 and lf.max() < 450
+    assert abs(lf.mean() - 395.0) < 4 * 110 / math.sqrt(12 * 8000)
+
+
+# ------------------------------------------------------------------ ray - sphere (R10)
+def _quadratic_hit(e, v, c, R):
+    """Independent formulation: |e + s v - c|^2 = R^2 has real roots and their mean is > 0."""
+    oc = e - c
+    b = 2.0 * (oc @ v)
+    cc = oc @ oc - R * R
+    disc = b * b - 4.0 * cc
+    return disc >= 0.0 and (-b / 2.0) > 0.0
+
+
+def test_ray_sphere_against_quadratic_solver_and_sampling():
+    rng = np.random.default_rng(3)
+    n_hit = 0
+    for i in range(1000):
+        c = np.array([rng.uniform(-50, 50), rng.uniform(-50, 50), 2000.0])
+        R = rng.uniform(1.0, 30.0)
+        e = c + np.array([rng.uniform(-200, 200), rng.uniform(-200, 200), rng.uniform(1.0, 3000.0)])
+        aim = c + rng.normal(size=3) * R * 0.8                     # aim near the sphere so ~half hit
+        v = aim - e
+        v /= np.linalg.norm(v)
+        if i % 10 == 0:
+            v = -v                                                 # upward rays never hit
+        hit, b2, s_c, s_pl, x, y = O.intersect(e, v, list(c) + [R])
+        expect = v[2] < 0 and _quadratic_hit(e, v, c, R)
+        assert hit == expect
+        # dense sampling of the ray: the smallest distance to the centre
+        s = np.linspace(0.0, 2 * np.linalg.norm(c - e), 20001)
+        dist = np.linalg.norm(e[None, :] + s[:, None] * v[None, :] - c[None, :], axis=1)
+        if abs(math.sqrt(max(b2, 0)) - R) > 0.05 and s_c > 1.0:
+            assert (dist.min() <= R) == (b2 <= R * R)
+        if v[2] < 0:
+            g = e + s_pl * v
+            assert g[2] == pytest.approx(c[2], abs=1e-9)
+            assert (x, y) == (pytest.approx(g[0] - c[0], abs=1e-9), pytest.approx(g[1] - c[1], abs=1e-9))
+        n_hit += hit
+    assert 200 < n_hit < 800
+
+
+def test_vertical_ray_hits_iff_offset_le_R():
+    for b, expect in ((5.999, True), (6.001, False), (0.0, True), (6.0, True)):
+        hit, b2, s_c, s_pl, x, y = O.intersect([b, 0, 5000.0], [0, 0, -1.0], [0, 0, 2000.0, 6.0])
+        assert hit == expect and b2 == pytest.approx(b * b, abs=1e-9) and s_pl == 3000.0 and x == b
+    # emission inside the sphere moving away from the centre, and below the centre plane: miss (R10)
+    assert not O.intersect([0, 0, 1999.0], [0, 0, -1.0], [0, 0, 2000.0, 6.0])[0]
+    assert not O.intersect([0, 0, 2001.0], [0, 0, 1.0], [0, 0, 2000.0, 6.0])[0]
+
+
+def test_impact_parameter_is_rotation_invariant():
+    rng = np.random.default_rng(4)
+    for _ in range(100):
+        e, c = rng.normal(size=3) * 1000, rng.normal(size=3) * 10
+        v = rng.normal(size=3); v /= np.linalg.norm(v)
+        Q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+        _, b2a, sca, *_ = O.intersect(e, v, list(c) + [6.0])
+        _, b2b, scb, *_ = O.intersect(Q @ e, Q @ v, list(Q @ c) + [6.0])
+        assert b2a == pytest.approx(b2b, rel=1e-9, abs=1e-6) and sca == pytest.approx(scb, rel=1e-12, abs=1e-9)
+
+
+# ------------------------------------------------------------------ timing (R8)
+def test_vertical_ray_optical_delay(golden_closed_forms):
+    g = golden_closed_forms
+    t = O.arrival_time(ATM1, 10000.0, 2000.0, -1.0, 8000.0, 0.0)
+    vac = 8000.0 / C
+    assert vac == pytest.approx(g["vertical_10km_2km_vacuum_ns"], abs=1e-3)
+    assert t - vac == pytest.approx(g["vertical_10km_2km_excess_ns"], abs=1e-5)
+    assert (t - vac) * C == pytest.approx(g["vertical_10km_2km_excess_m"], abs=1e-6)
+    # slant: both the geometric and the excess path scale with 1/|v_z|
+    vz = -0.8
+    ts = O.arrival_time(ATM1, 10000.0, 2000.0, vz, 8000.0 / 0.8, 0.0)
+    assert ts == pytest.approx(t / 0.8, rel=1e-14)
+
+
+def test_optical_delay_equals_numerical_integral_five_layer():
+    # integral of eta(h) dh from 2 km to 30 km by the trapezoid rule on a fine grid
+    h = np.linspace(2000.0, 30000.0, 280001)
+    eta = np.array([O.refractivity(ATM5, x) for x in h[::100]])
+    integral = np.trapezoid(eta, h[::100])
+    t = O.arrival_time(ATM5, 30000.0, 2000.0, -1.0, 28000.0, 0.0)
+    assert (t - 28000.0 / C) * C == pytest.approx(integral, rel=1e-6)
+
+
+# ------------------------------------------------------------------ transmission (R17)
+def _atm_with_tau(tau):
+    return W.atmosphere_five_layer(tau=np.asarray(tau, dtype=np.float32))
+
+
+def test_transmission_special_cases():
+    assert O.transmission(ATM5, 5000.0, 400.0, -0.7) == 1.0            # no table -> weights unchanged
+    assert O.transmission(_atm_with_tau(np.zeros((64, 32))), 5000.0, 400.0, -0.7) == 1.0
+    atm = _atm_with_tau(np.full((64, 32), 0.25))
+    for vz in (-1.0, -0.5, -0.123):
+        assert O.transmission(atm, 7000.0, 433.0, vz) == pytest.approx(math.exp(-0.25 / abs(vz)), rel=1e-7)
+
+
+def test_optical_depth_is_bilinear_and_clamped():
+    i, j = np.meshgrid(np.arange(64), np.arange(32), indexing="ij")
+    atm = _atm_with_tau(0.5 * i + 0.25 * j)                             # linear table -> exact reproduction
+    dl = 300.0 / 31
+    for h, lam in ((2000.0, 300.0), (2750.0, 300.0 + 3.5 * dl), (33499.0, 599.0), (12345.0, 456.7)):
+        fh, fl = (h - 2000.0) / 500.0, (lam - 300.0) / dl
+        assert O.optical_depth(atm, h, lam) == pytest.approx(0.5 * fh + 0.25 * fl, rel=1e-6, abs=1e-6)
+    assert O.optical_depth(atm, 0.0, 100.0) == pytest.approx(0.0, abs=1e-12)        # clamped low
+    assert O.optical_depth(atm, 1e6, 1e4) == pytest.approx(0.5 * 63 + 0.25 * 31, rel=1e-7)  # clamped high
+    rng = np.random.default_rng(5)
+    tau = rng.random((64, 32)).astype(np.float32)
+    atm = _atm_with_tau(tau)
+    for _ in range(50):                                                # grid nodes are reproduced
+        a, b = rng.integers(0, 64), rng.integers(0, 32)
+        assert O.optical_depth(atm, 2000.0 + 500.0 * a, 300.0 + dl * b) == pytest.approx(float(tau[a, b]), abs=2e-6)
+
+
+# ------------------------------------------------------------------ whole-path pins
+def test_isotropic_acceptance_fraction():
+    """Fraction of isotropic rays from distance D hitting a sphere R is (1 - sqrt(1 - R^2/D^2))/2 = 0.1
+    for R = 600, D = 1000 (SURVEY.md §8(c) pin "Isotropic acceptance")."""
+    par = W.default_params(processes=W.PROC_FLUORESCENCE, seed=77)
+    seg = one_segment(z0=3000.0, length=1e-3, gamma=100.0, dE=250000.0)   # 1e6 photons, 1000 m above the centre
+    tel = np.array([[0, 0, 2000.0, 600.0]], dtype=np.float32)
+    r = O.run(ATM5, tel, seg, par)
+    n = int(r["counters"][1])
+    assert n == 1_000_000 and int(r["counts"][0, 1]) == n
+    frac = int(r["tallies"]["hits"][0]) / n
+    assert abs(frac - 0.1) < 4 * math.sqrt(0.1 * 0.9 / n)
+    assert abs(int(r["counters"][2]) / n - 0.5) < 4 * 0.5 / math.sqrt(n)   # half go upward
+    assert r["tallies"]["sum_w"][0] == pytest.approx(r["tallies"]["hits"][0] * 1.0, rel=1e-12)
+
+
+def test_beaming_weight_and_equal_expectation(golden_closed_forms):
+    g = golden_closed_forms
+    par_b = W.default_params(processes=W.PROC_FLUORESCENCE, fl_beam_telescope=0)
+    tel = np.array([[0, 0, 2000.0, 600.0]], dtype=np.float32)
+    seg = one_segment(z0=3000.0, length=1e-3, gamma=100.0, dE=50000.0)     # 2e5 photons
+    st, f = O.preamble(ATM5, par_b, seg[0], 1, beam_tel=tel[0].astype(np.float64))
+    omega = 2 * math.pi * f.one_minus_cos_ab
+    assert omega == pytest.approx(g["omega_2deg_sr"], rel=1e-6)
+    assert f.w0 == pytest.approx(g["omega_2deg_over_4pi"], rel=1e-6)        # mu / n_b = 1 here
+    # all beamed photons stay inside the cone around the line of sight (straight down here)
+    for j in range(0, 2000, 7):
+        v = np.array(list(O.make_photon(f, par_b, 0, j, 1).v))
+        assert v @ np.array([0, 0, -1.0]) >= math.cos(math.radians(2.0)) - 1e-15
+    # equal expectation of the weighted tally when the cone (40 deg) covers the sphere (36.87 deg)
+    par_iso = W.default_params(processes=W.PROC_FLUORESCENCE, seed=5)
+    par_40 = W.default_params(processes=W.PROC_FLUORESCENCE, seed=6, fl_beam_telescope=0,
+                              fl_beam_halfangle=math.radians(40.0))
+    ri = O.run(ATM5, tel, seg, par_iso)
+    rb = O.run(ATM5, tel, seg, par_40)
+    n = 200_000
+    assert int(rb["counters"][2]) == 0                                       # none upward when beamed down
+    exp = 0.1 * n
+    sig_i = math.sqrt(n * 0.1 * 0.9)
+    p_b = 0.2 / (1 - math.cos(math.radians(40.0)))                           # hit probability inside the cone
+    w_b = (1 - math.cos(math.radians(40.0))) / 2
+    sig_b = w_b * math.sqrt(n * p_b * (1 - p_b))
+    assert abs(ri["tallies"]["sum_w"][0] - exp) < 4 * sig_i
+    assert abs(rb["tallies"]["sum_w"][0] - exp) < 4 * sig_b
+    assert rb["tallies"]["hits"][0] > 3 * ri["tallies"]["hits"][0]           # beaming buys statistics
+
+
+def test_beamed_line_of_sight_points_at_the_telescope():
+    par_b = W.default_params(processes=W.PROC_FLUORESCENCE, fl_beam_telescope=0, fl_beam_halfangle=1e-4)
+    tel = np.array([10000.0, 0.0, 2000.0, 6.0])
+    seg = one_segment(x0=100.0, y0=-50.0, z0=9000.0, d=(0.1, 0.2, -0.97), length=10.0, dE=100.0)
+    st, f = O.preamble(ATM5, par_b, seg[0], 1, beam_tel=tel)
+    mid = np.array(list(f.p0)) + 0.5 * f.L * np.array(list(f.d))
+    los = tel[:3] - mid
+    los /= np.linalg.norm(los)
+    for j in range(20):
+        v = np.array(list(O.make_photon(f, par_b, 9, j, 1).v))
+        assert math.acos(min(1.0, v @ los)) <= 1.0001e-4
+
+
+def test_cherenkov_ring_geometry():
+    """Vertical track, emission ~ point-like at dh above the plane: every ground point lies on the
+    circle of radius dh tan(theta_c) (SURVEY.md §8(c) pin "Ring geometry")."""
+    seg = one_segment(z0=10000.0, length=1e-2, gamma=1e6)
+    seg["t0"] = 0.0
+    par = W.default_params(bunch_size=1e-4, seed=3)                  # many bunches from a short track
+    tel = W.telescope_accept_all()
+    r = O.run(ATM1, tel, seg, par, record_capacity=100000)
+    rec = r["records"]
+    st, f = O.preamble(ATM1, par, seg[0], 0)
+    assert len(rec) == f.n_b > 1000
+    rad = np.hypot(rec["x"], rec["y"])
+    tan_c = f.sin_c / f.cos_c
+    assert np.all(np.abs(rad - 8000.0 * tan_c) <= 1e-2 * tan_c + 1e-9)
+    # direction cosines are those of the cone, and times follow the optical path
+    assert np.allclose(np.hypot(rec["cx"], rec["cy"]), f.sin_c, atol=1e-12)
+    t_exp = (8000.0 / f.cos_c) / C + 0.01 * (2.83e-4 / 1.225e-3) * (O.depth(ATM1, 2000.0) - O.depth(ATM1, 10000.0)) \
+        / f.cos_c / C
+    assert np.all(np.abs(rec["t"] - t_exp) < 1e-3)
+    assert np.allclose(rec["w"], f.w0, rtol=1e-15)
+
+
+def test_conservation_laws_config1_sample():
+    c = W.make_config("c1", 2000)
+    r = O.run(c["atmosphere"], c["telescopes"], c["segments"], c["params"], record_capacity=10000)
+    cnt = r["counters"]
+    assert cnt[0] == 2000 and cnt[1] == r["counts"].sum()
+    assert cnt[3] == r["tallies"]["hits"].sum() == cnt[4] == len(r["records"]) and cnt[5] == 0
+    assert r["tallies"]["sum_w"][0] == pytest.approx(r["records"]["w"].sum(), rel=1e-12)
+    assert r["tallies"]["sum_wt"][0] == pytest.approx((r["records"]["w"] * r["records"]["t"]).sum(), rel=1e-12)
+    # closed-form count: ceil of the Frank-Tamm yield from its textbook definition, vectorised in numpy
+    s = c["segments"]
+    z0, L, dz, gam = (s[k].astype(np.float64) for k in ("z0", "length", "dz", "gamma"))
+    n = 1.0 + 2.83e-4 * np.exp(-(z0 + 0.5 * L * dz) / 8400.0)
+    beta2 = 1.0 - 1.0 / gam ** 2
+    sin2 = np.maximum(1.0 - 1.0 / (beta2 * n * n), 0.0)
+    mu = 2 * math.pi * ALPHA * (1 / 300e-9 - 1 / 600e-9) * L * sin2
+    nb = np.ceil(mu).astype(np.int64)
+    mismatch = np.nonzero(nb != r["counts"][:, 0])[0]
+    # the naive 1 - 1/(beta n)^2 loses ~1e-12 relative: allow ceil() flips only where mu is within 1e-9 of an integer
+    assert all(abs(mu[i] - round(mu[i])) < 1e-9 for i in mismatch) and len(mismatch) <= 1
+    # segment ids are what the records say, and the split over threads changes nothing
+    r2 = O.run(c["atmosphere"], c["telescopes"], c["segments"], c["params"], record_capacity=10000, threads=3)
+    assert np.array_equal(r2["counts"], r["counts"]) and np.array_equal(r2["tallies"]["hits"], r["tallies"]["hits"])
+    assert np.array_equal(r2["records"]["id"], r["records"]["id"])
+    assert ((r["records"]["id"] >> 25) < 2000).all()
+
+
+def test_first_segment_id_makes_batches_independent_of_batching():
+    c = W.make_config("c1", 600)
+    full = O.run(c["atmosphere"], c["telescopes"], c["segments"], c["params"], record_capacity=5000)
+    a = O.run(c["atmosphere"], c["telescopes"], c["segments"][:250], c["params"], record_capacity=5000)
+    b = O.run(c["atmosphere"], c["telescopes"], c["segments"][250:], c["params"], first_id=250, record_capacity=5000)
+    assert np.array_equal(np.concatenate([a["records"]["id"], b["records"]["id"]]), full["records"]["id"])
+    assert np.array_equal(a["tallies"]["hits"] + b["tallies"]["hits"], full["tallies"]["hits"])
+
+
+def test_both_processes_and_record_capacity():
+    c = W.make_config("c4", 300)
+    c["telescopes"] = W.telescope_accept_all()
+    r = O.run(c["atmosphere"], c["telescopes"], c["segments"], c["params"], record_capacity=1000)
+    cnt = r["counters"]
+    assert (r["counts"][:, 1] == np.ceil(4.0 * c["segments"]["dE"].astype(np.float64))).all()
+    assert cnt[1] == r["counts"].sum() and cnt[4] == 1000 and cnt[5] == cnt[3] - 1000
+    # accept-all sphere: every downward photon is a hit except those emitted (inside the sphere) with the
+    # closest approach behind them, s_c <= 0 (R10) -- near-horizontal fluorescence photons flying outward
+    down = int(cnt[1] - cnt[2])
+    assert int(cnt[3]) <= down and down - int(cnt[3]) < 0.005 * down
+    tags = (r["records"]["id"] >> 24) & 1
+    assert set(np.unique(tags)) <= {0, 1}
+    # transmission can only reduce the weight
+    assert (r["records"]["w"] <= 1.0 + 1e-12).all() and (r["records"]["w"] > 0).all()
+
+
+# ------------------------------------------------------------------ tiny brute-force case
+def test_tiny_case_against_pure_python_restatement():
+    """1 segment, <= 32 photons, 1 telescope, recomputed in pure Python with a different formulation:
+    Python-int Philox, rotation by pi about the bisector through the generic axis-angle formula, and a
+    quadratic-equation ray-sphere test."""
+    M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
+
+    def philox(ctr, key):
+        c, k = list(ctr), list(key)
+        for _ in range(10):
+            p0, p1 = M0 * c[0], M1 * c[2]
+            c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xFFFFFFFF]
+            k = [(k[0] + W0) & 0xFFFFFFFF, (k[1] + W1) & 0xFFFFFFFF]
+        return c
+
+    seg = one_segment(x0=3.0, y0=-2.0, z0=2600.0, d=(0.004, -0.003, -1.0), length=0.8, gamma=300.0)
+    seg["t0"] = -2.0
+    tel = np.array([[0.0, 0.0, 2000.0, 9.0]], dtype=np.float32)
+    par = W.default_params(seed=(7 << 32) | 12345)
+    r = O.run(ATM1, tel, seg, par, first_id=(1 << 33) + 5, record_capacity=100)
+    nb = int(r["counts"][0, 0])
+    assert 8 <= nb <= 32
+
+    s = seg[0]
+    p0 = np.array([s["x0"], s["y0"], s["z0"]], dtype=np.float64)
+    d = np.array([s["dx"], s["dy"], s["dz"]], dtype=np.float64)
+    d /= np.linalg.norm(d)
+    L, gam = float(s["length"]), float(s["gamma"])
+    n = 1.0 + 2.83e-4 * math.exp(-(p0[2] + 0.5 * L * d[2]) / 8400.0)
+    beta = math.sqrt(1.0 - 1.0 / gam ** 2)
+    theta = math.acos(1.0 / (beta * n))
+    mu = 2 * math.pi * ALPHA * (1 / 300e-9 - 1 / 600e-9) * L * math.sin(theta) ** 2
+    assert nb == math.ceil(mu)
+    A = d + np.array([0, 0, -1.0]); A /= np.linalg.norm(A)
+    K = np.array([[0, -A[2], A[1]], [A[2], 0, -A[0]], [-A[1], A[0], 0]])
+    Rpi = np.eye(3) + 2.0 * (K @ K)
+    S = (1 << 33) + 5
+    hits = []
+    for j in range(nb):
+        rr = philox([j, S & 0xFFFFFFFF, S >> 32, 0], [12345, 7])
+        u = [((x >> 9) + 0.5) / 2 ** 23 for x in rr]
+        e = p0 + u[0] * L * d
+        phi = 2 * math.pi * u[1]
+        p = np.array([math.cos(phi) * math.sin(theta), math.sin(phi) * math.sin(theta), -math.cos(theta)])
+        v = Rpi @ p
+        if _quadratic_hit(e, v, tel[0, :3].astype(np.float64), 9.0):
+            sp = (2000.0 - e[2]) / v[2]
+            g = e + sp * v
+            t = -2.0 + u[0] * L / (beta * C) + (sp + 2.83e-4 * 8400.0 * (math.exp(-2000 / 8400.0)
+                                                                          - math.exp(-e[2] / 8400.0)) / abs(v[2])) / C
+            lam = 1.0 / (1 / 300.0 - u[2] * (1 / 300.0 - 1 / 600.0))
+            hits.append((j, g[0], g[1], v[0], v[1], t, lam, mu / nb))
+    rec = r["records"]
+    assert len(hits) == len(rec) >= 3
+    for h, q in zip(hits, rec):
+        assert (int(q["id"]) & 0xFFFFFF) == h[0] and (int(q["id"]) >> 25) == S
+        assert q["x"] == pytest.approx(h[1], abs=1e-7) and q["y"] == pytest.approx(h[2], abs=1e-7)
+        assert q["cx"] == pytest.approx(h[3], abs=1e-10) and q["cy"] == pytest.approx(h[4], abs=1e-10)
+        assert q["t"] == pytest.approx(h[5], abs=1e-8) and q["lam"] == pytest.approx(h[6], rel=1e-12)
+        assert q["w"] == pytest.approx(h[7], rel=1e-9)
