@@ -1,0 +1,188 @@
+/*
+ * c8opt.h -- C-ABI boundary of the B200-native optical photon path.
+ *
+ * The path (arxiv 2309.15861, Baack & Alameddine, ICRC2023; cited as
+ * PAPER.md:<line>; "R<n>" = a reading listed in DESIGN.md §2):
+ *
+ *   charged-particle track segment
+ *     -> Cherenkov photons   (Frank-Tamm yield PAPER.md:43-45, homogeneous step
+ *                             PAPER.md:47, cone generated downward and rotated by
+ *                             the 180-degree Rodrigues matrix PAPER.md:49-73)
+ *     -> fluorescence photons (constant yield x energy loss, positions uniform
+ *                             along the track, isotropic PAPER.md:29-35, or
+ *                             beamed toward a telescope PAPER.md:39)
+ *     -> straight-line propagation with the optical-path arrival time and an
+ *        optional transmission weight (R8, R17)
+ *     -> telescope-sphere intersection (BASELINE.json north_star, R10)
+ *     -> per-telescope tally, or compacted 28-byte photon-bunch records.
+ *
+ * All of it runs in hand-written CUDA kernels for sm_100a.  There is no CPU
+ * fallback: without a CUDA device every entry point that needs one returns
+ * C8OPT_ERR_CUDA.
+ *
+ * Conventions
+ *   - plain C types only; "host" / "device" is stated for every pointer.
+ *   - return value: 0 = OK, negative = error code below; the message of the
+ *     last error of a context is available from c8opt_last_error().
+ *   - units: metres, nanoseconds, nanometres (wavelength), g/cm^2 (depth), MeV.
+ *   - geometry: flat atmosphere, z up = altitude above sea level (R9).
+ *   - one context per host thread; calls on one context must not overlap.
+ */
+#ifndef C8OPT_H
+#define C8OPT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define C8OPT_OK              0
+#define C8OPT_ERR_ARGUMENT   (-1)  /* null pointer, bad size, non-monotone layers, ...   */
+#define C8OPT_ERR_CUDA       (-2)  /* CUDA runtime error or no sm_100 device             */
+#define C8OPT_ERR_CAPACITY   (-3)  /* photon-output region overflowed (records dropped)  */
+
+#define C8OPT_MAX_LAYERS      8
+#define C8OPT_MAX_TELESCOPES  4096
+
+#define C8OPT_PROC_CHERENKOV     1u   /* bit 0 of c8opt_run_params.processes */
+#define C8OPT_PROC_FLUORESCENCE  2u   /* bit 1 */
+#define C8OPT_MODE_TALLY   0u
+#define C8OPT_MODE_OUTPUT  1u
+
+typedef struct c8opt_ctx c8opt_ctx;   /* opaque, owned by the library */
+
+/* One atmosphere layer: column depth T(h) = a + b exp(-h / c) [g/cm^2] for
+ * h >= h_lo (layer 0 also covers h < h_lo of layer 0).  Density is -dT/dh.
+ * (BASELINE.json configs[1] "T(h)=a_i+b_i*exp(-h/c_i)"; R18.) */
+typedef struct { double h_lo_m, a_gcm2, b_gcm2, c_m; } c8opt_layer;
+
+/* Atmosphere descriptor (host memory, copied by c8opt_create_atmosphere).
+ * Refractivity n(h) - 1 = eta0 * rho(h) / rho0.  tau is the optional vertical
+ * optical-depth table tau(h, lambda) from altitude h down to the observation
+ * level, row-major [tau_nh][tau_nl], bilinear, clamped at the edges (R17);
+ * tau == NULL or tau_nh == 0 means no absorption. */
+typedef struct {
+    int32_t     n_layers;                       /* 1 .. C8OPT_MAX_LAYERS, h_lo ascending */
+    c8opt_layer layers[C8OPT_MAX_LAYERS];
+    double      eta0, rho0_gcm3, h_obs_m;
+    int32_t     tau_nh, tau_nl;
+    double      tau_h0_m, tau_dh_m, tau_l0_nm, tau_dl_nm;
+    const float *tau;                           /* host */
+} c8opt_atmosphere_desc;
+
+/* One track segment, 48 bytes ("steps ... a couple of meters").
+ * (dx,dy,dz) is the unit direction (re-normalised in fp64; off unity by more
+ * than 1e-3 => the segment is counted invalid and emits nothing), gamma the
+ * Lorentz factor (> 1), charge in units of e, dE the energy loss over the
+ * segment (used by fluorescence only), flags bit 0 = muon label (ignored). */
+typedef struct {
+    float x0, y0, z0, t0_ns;
+    float dx, dy, dz, length_m;
+    float gamma, charge, dE_MeV;
+    uint32_t flags;
+} c8opt_segment;
+
+/* Run parameters (host memory, read during the call). */
+typedef struct {
+    uint64_t seed;                 /* Philox key = (seed[31:0], seed[63:32])  (R20)        */
+    uint32_t processes;            /* C8OPT_PROC_* bits                                     */
+    uint32_t mode;                 /* C8OPT_MODE_TALLY or C8OPT_MODE_OUTPUT                 */
+    double   lam1_nm, lam2_nm;     /* Cherenkov band (PAPER.md:45 integral over lambda)     */
+    double   bunch_size;           /* B: n_b = ceil(mu / B) bunches of weight mu / n_b (R1) */
+    double   fl_yield_per_MeV;     /* constant fluorescence yield (R13)        */
+    double   fl_lam1_nm, fl_lam2_nm;
+    int32_t  fl_beam_telescope;    /* -1 isotropic, else beam toward this telescope (R14)   */
+    int32_t  reserved;
+    double   fl_beam_halfangle_rad;
+} c8opt_run_params;
+
+/* Optional outputs of one propagate call; every pointer is DEVICE memory owned
+ * by the caller and may be NULL (all NULL / out == NULL in plain tally mode).
+ *   records      : photon-output mode; 7 floats per record {x, y, cos_x, cos_y,
+ *                  t, lambda, weight}: x, y on the horizontal plane through the
+ *                  telescope centre, relative to the centre (R11).  Telescope k
+ *                  owns records [tel_offset[k], tel_offset[k] + tel_capacity[k]);
+ *                  the library keeps one cursor per telescope in the context
+ *                  (cleared by c8opt_reset_tallies) so consecutive calls append.
+ *   ids          : parallel to records; (segment id << 25) | (process tag << 24)
+ *                  | photon index, for validation.
+ *   counts       : uint32[n][2], bunches n_b emitted by segment i for the
+ *                  Cherenkov (tag 0) and fluorescence (tag 1) process.
+ * Record order inside a telescope region is unspecified (R22). */
+typedef struct {
+    float          *records;
+    const uint64_t *tel_offset;      /* device, [n_tel], in records */
+    const uint64_t *tel_capacity;    /* device, [n_tel], in records */
+    uint64_t       *ids;
+    uint32_t       *counts;
+} c8opt_output;
+
+typedef struct { uint64_t hits; double sum_w; double sum_wt; } c8opt_tally;
+
+/* indices into the counters[8] array of c8opt_read_tallies */
+enum {
+    C8OPT_CNT_SEGMENTS = 0, C8OPT_CNT_GENERATED = 1, C8OPT_CNT_UPWARD = 2, C8OPT_CNT_HITS = 3,
+    C8OPT_CNT_RECORDS = 4, C8OPT_CNT_DROPPED = 5, C8OPT_CNT_INVALID = 6, C8OPT_CNT_UNUSED = 7
+};
+
+/* Validate the descriptor, build the layer / transmission tables and upload
+ * them to the current CUDA device.  *out receives a new context.
+ * Errors: ARGUMENT (null, n_layers out of range, h_lo not ascending, c <= 0,
+ * rho0 <= 0, bad tau shape), CUDA. */
+int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out);
+
+/* Replace the telescope set: xyzr is HOST float[n][4] = centre and radius of
+ * each sphere (BASELINE.json north_star "telescopes' spheres").  Builds the
+ * ground-plane candidate grid used when n is large and clears the tallies.
+ * Errors: ARGUMENT (n < 1 or > C8OPT_MAX_TELESCOPES, radius <= 0, non-finite). */
+int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n);
+
+/* Generate, propagate, intersect and tally / write the photons of n segments
+ * (DEVICE array d_seg) with global ids first_segment_id + i.  Asynchronous on
+ * `cuda_stream` (a cudaStream_t; NULL = default stream); accumulates into the
+ * context's tallies and counters, so many batches may precede one read.
+ * The random stream of photon j of segment S is Philox4x32-10 with
+ * counter (j, S[31:0], S[63:32], process tag) and key = seed (R20): results do
+ * not depend on how segments are batched.
+ * Errors: ARGUMENT (null, no telescopes, bad params, output mode without
+ * records / offsets), CUDA. */
+int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_t n,
+                             uint64_t first_segment_id, const c8opt_run_params *params,
+                             const c8opt_output *out, void *cuda_stream);
+
+/* Same path with the segments in HOST memory (pinned memory makes the copies
+ * asynchronous): the segment table is cut into chunks whose host->device copy
+ * overlaps the kernel of the previous chunk on two internal streams; returns
+ * after all work is enqueued, ordered after prior work on `cuda_stream`, and
+ * `cuda_stream` waits for it.  out->counts, if given, is still DEVICE memory. */
+int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, uint64_t n,
+                                  uint64_t first_segment_id, const c8opt_run_params *params,
+                                  const c8opt_output *out, void *cuda_stream);
+
+/* Synchronise with all work enqueued on the context and copy the results to
+ * HOST memory: host_out[n_tel] tallies, counters[8] (may be NULL),
+ * host_tel_count[n_tel] = records written per telescope (may be NULL).
+ * Returns C8OPT_ERR_CAPACITY if any record was dropped (results are still
+ * copied); ARGUMENT if n_tel differs from the telescope count. */
+int c8opt_read_tallies(c8opt_ctx *ctx, c8opt_tally *host_out, int32_t n_tel,
+                       uint64_t *counters, uint64_t *host_tel_count);
+
+/* Zero tallies, counters and the per-telescope record cursors (asynchronous
+ * on `cuda_stream`). */
+int c8opt_reset_tallies(c8opt_ctx *ctx, void *cuda_stream);
+
+void c8opt_destroy(c8opt_ctx *ctx);
+
+/* Message of the last error on this context (or of the last failed
+ * c8opt_create_atmosphere when ctx == NULL).  Never NULL. */
+const char *c8opt_last_error(const c8opt_ctx *ctx);
+
+/* Number of kernels launched by this context so far (for bench.py's
+ * gpu_launches). */
+uint64_t c8opt_launch_count(const c8opt_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* C8OPT_H */

@@ -1,0 +1,416 @@
+// c8opt.cu -- the C-ABI of include/c8opt.h: context, table upload, kernel launches.
+// No torch types; device memory for segments / records is the caller's.
+#include "../../include/c8opt.h"
+#include "c8opt_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+thread_local char g_create_error[256] = "";
+
+struct HostLayer { double h_lo, a, b, c; };
+
+}  // namespace
+
+struct c8opt_ctx {
+    int device = 0;
+    // atmosphere (host copies)
+    int n_layers = 0;
+    HostLayer layer[C8OPT_MAX_LAYERS];
+    double eta0 = 0, rho0 = 0, h_obs = 0;
+    int tau_nh = 0, tau_nl = 0;
+    double tau_h0 = 0, tau_dh = 1, tau_l0 = 0, tau_dl = 1;
+    float *d_tau = nullptr;
+    // telescopes
+    int n_tel = 0;
+    bool coplanar = true;
+    std::vector<double> tel_xyzr;          // absolute, as given (float -> double)
+    double x_ref = 0, y_ref = 0, z_ref = 0;
+    float4 *d_telA = nullptr;
+    float *d_telT = nullptr;
+    // results
+    c8::Tally *d_tallies = nullptr;
+    unsigned long long *d_counters = nullptr;   // [8]
+    unsigned long long *d_cursors = nullptr;    // [n_tel]
+    std::vector<unsigned long long> h_capacity; // capacities of the last output-mode call
+    bool have_capacity = false;
+    unsigned long long segments_total = 0;      // host-side running count (counter 0)
+    unsigned long long launches = 0;
+    // host-segment pipeline
+    cudaStream_t pipe_stream[2] = {nullptr, nullptr};
+    cudaEvent_t pipe_event[3] = {nullptr, nullptr, nullptr};
+    c8opt_segment *d_stage[2] = {nullptr, nullptr};
+    unsigned long long stage_segments = 0;
+    char error[256] = "";
+};
+
+namespace {
+
+int fail(c8opt_ctx *ctx, int code, const char *fmt, ...)
+{
+    char *dst = ctx ? ctx->error : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 256, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define C8_CUDA(ctx, call)                                                                        \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess)                                                                    \
+            return fail(ctx, C8OPT_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_));            \
+    } while (0)
+
+// column depth T(h) = a_i + b_i exp(-h / c_i), layer i = last one with h >= h_lo (host, fp64)
+double host_depth(const c8opt_ctx *c, double h)
+{
+    int i = 0;
+    for (int k = 1; k < c->n_layers; ++k) if (h >= c->layer[k].h_lo) i = k;
+    return c->layer[i].a + c->layer[i].b * std::exp(-h / c->layer[i].c);
+}
+
+size_t smem_bytes() { return sizeof(c8::TileSmem); }
+
+typedef void (*kernel_t)(const c8::KParams);
+
+kernel_t pick_kernel(bool coplanar, unsigned mode)
+{
+    if (mode == C8OPT_MODE_OUTPUT) return coplanar ? c8::propagate_kernel<true, 1> : c8::propagate_kernel<false, 1>;
+    return coplanar ? c8::propagate_kernel<true, 0> : c8::propagate_kernel<false, 0>;
+}
+
+// Validate params / outputs and fill the kernel parameter block (everything except seg / n / first_id).
+int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *out, c8::KParams *kp)
+{
+    if (!rp) return fail(ctx, C8OPT_ERR_ARGUMENT, "params is NULL");
+    if (ctx->n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no telescopes: call c8opt_add_telescopes first");
+    const unsigned procs = rp->processes;
+    if (procs == 0 || (procs & ~3u)) return fail(ctx, C8OPT_ERR_ARGUMENT, "processes must be a combination of bits 0 and 1");
+    if (rp->mode > 1u) return fail(ctx, C8OPT_ERR_ARGUMENT, "mode must be 0 (tally) or 1 (photon output)");
+    if (!(rp->bunch_size > 0.0) || !std::isfinite(rp->bunch_size)) return fail(ctx, C8OPT_ERR_ARGUMENT, "bunch_size must be > 0");
+    if (procs & C8OPT_PROC_CHERENKOV)
+        if (!(rp->lam1_nm > 0.0) || !(rp->lam2_nm > rp->lam1_nm)) return fail(ctx, C8OPT_ERR_ARGUMENT, "need 0 < lam1 < lam2");
+    if (procs & C8OPT_PROC_FLUORESCENCE) {
+        if (!(rp->fl_yield_per_MeV >= 0.0) || !(rp->fl_lam1_nm > 0.0) || !(rp->fl_lam2_nm >= rp->fl_lam1_nm))
+            return fail(ctx, C8OPT_ERR_ARGUMENT, "bad fluorescence yield / band");
+        if (rp->fl_beam_telescope >= ctx->n_tel) return fail(ctx, C8OPT_ERR_ARGUMENT, "fl_beam_telescope out of range");
+        if (rp->fl_beam_telescope >= 0 && !(rp->fl_beam_halfangle_rad > 0.0 && rp->fl_beam_halfangle_rad <= 3.14159265358979323846))
+            return fail(ctx, C8OPT_ERR_ARGUMENT, "fl_beam_halfangle_rad must be in (0, pi]");
+    }
+    if (rp->mode == C8OPT_MODE_OUTPUT && (!out || !out->records || !out->tel_offset || !out->tel_capacity))
+        return fail(ctx, C8OPT_ERR_ARGUMENT, "photon-output mode needs out->records, tel_offset and tel_capacity");
+
+    c8::KParams &P = *kp;
+    std::memset(&P, 0, sizeof(P));
+    P.n_layers = ctx->n_layers;
+    for (int i = 0; i < ctx->n_layers; ++i) {
+        P.layer[i] = c8::LayerD{ctx->layer[i].h_lo, ctx->layer[i].a, ctx->layer[i].b, ctx->layer[i].c};
+        P.layerf[i] = c8::LayerF{(float)ctx->layer[i].h_lo, (float)ctx->layer[i].a, (float)ctx->layer[i].b,
+                                 (float)(1.0 / ctx->layer[i].c)};
+    }
+    P.eta0 = ctx->eta0; P.rho0 = ctx->rho0;
+    P.kappa_m = (float)(0.01 * ctx->eta0 / ctx->rho0);
+    P.tau = ctx->d_tau; P.tau_nh = ctx->tau_nh; P.tau_nl = ctx->tau_nl;
+    P.tau_h0 = (float)ctx->tau_h0; P.tau_inv_dh = (float)(1.0 / ctx->tau_dh);
+    P.tau_l0 = (float)ctx->tau_l0; P.tau_inv_dl = (float)(1.0 / ctx->tau_dl);
+    P.n_tel = ctx->n_tel; P.telA = ctx->d_telA; P.telT = ctx->d_telT;
+    P.x_ref = ctx->x_ref; P.y_ref = ctx->y_ref; P.z_ref = ctx->z_ref;
+    P.key0 = (uint32_t)rp->seed; P.key1 = (uint32_t)(rp->seed >> 32);
+    P.processes = procs; P.n_procs = (procs == 3u) ? 2u : 1u;
+    if (procs & C8OPT_PROC_CHERENKOV) {
+        // PAPER.md:45 prefactor: pi e^2 / (h eps0 c0) = 2 pi alpha; the lambda integral of lambda^-2 in closed form (R2)
+        const double two_pi_alpha = 2.0 * 3.14159265358979323846 * 7.2973525693e-3;
+        P.c_ft = two_pi_alpha * (1.0 / rp->lam1_nm - 1.0 / rp->lam2_nm) * 1.0e9;
+        P.inv_lam1 = (float)(1.0 / rp->lam1_nm);
+        P.dinv_lam = (float)(1.0 / rp->lam1_nm - 1.0 / rp->lam2_nm);
+    }
+    P.bunch_size = rp->bunch_size; P.fl_yield = rp->fl_yield_per_MeV;
+    P.fl_lam1 = (float)rp->fl_lam1_nm; P.fl_dlam = (float)(rp->fl_lam2_nm - rp->fl_lam1_nm);
+    P.beam_tel = (procs & C8OPT_PROC_FLUORESCENCE) ? rp->fl_beam_telescope : -1;
+    if (P.beam_tel >= 0) {
+        P.beam_x = ctx->tel_xyzr[4 * P.beam_tel + 0]; P.beam_y = ctx->tel_xyzr[4 * P.beam_tel + 1];
+        P.beam_z = ctx->tel_xyzr[4 * P.beam_tel + 2];
+        const double sh = std::sin(0.5 * rp->fl_beam_halfangle_rad);
+        P.omc = 2.0 * sh * sh;
+    }
+    P.tallies = ctx->d_tallies; P.counters = ctx->d_counters; P.cursors = ctx->d_cursors;
+    if (out) {
+        if (rp->mode == C8OPT_MODE_OUTPUT) {
+            P.records = out->records; P.tel_offset = (const unsigned long long *)out->tel_offset;
+            P.tel_capacity = (const unsigned long long *)out->tel_capacity; P.ids = (unsigned long long *)out->ids;
+        }
+        P.counts = out->counts;
+    }
+    return C8OPT_OK;
+}
+
+int launch(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, const c8opt_segment *d_seg, unsigned long long n,
+           unsigned long long first_id, uint32_t *counts, cudaStream_t st)
+{
+    if (n == 0) return C8OPT_OK;
+    P.seg = reinterpret_cast<const float4 *>(d_seg);
+    P.n_seg = n; P.first_id = first_id; P.counts = counts;
+    const unsigned long long per_tile = c8::kTile / P.n_procs;
+    const unsigned long long tiles = (n + per_tile - 1) / per_tile;
+    if (tiles > 0x7fffffffull) return fail(ctx, C8OPT_ERR_ARGUMENT, "too many segments in one call");
+    kernel_t k = pick_kernel(ctx->coplanar, mode);
+    k<<<(unsigned)tiles, c8::kTile, smem_bytes(), st>>>(P);
+    C8_CUDA(ctx, cudaGetLastError());
+    ctx->launches += 1;
+    ctx->segments_total += n;
+    return C8OPT_OK;
+}
+
+int remember_capacity(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *out, cudaStream_t st)
+{
+    if (rp->mode != C8OPT_MODE_OUTPUT) return C8OPT_OK;
+    ctx->h_capacity.resize(ctx->n_tel);
+    C8_CUDA(ctx, cudaMemcpyAsync(ctx->h_capacity.data(), out->tel_capacity, sizeof(unsigned long long) * ctx->n_tel,
+                                 cudaMemcpyDeviceToHost, st));
+    ctx->have_capacity = true;
+    return C8OPT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
+{
+    if (!desc || !out) return fail(nullptr, C8OPT_ERR_ARGUMENT, "desc or out is NULL");
+    *out = nullptr;
+    if (desc->n_layers < 1 || desc->n_layers > C8OPT_MAX_LAYERS) return fail(nullptr, C8OPT_ERR_ARGUMENT, "n_layers out of range");
+    for (int i = 0; i < desc->n_layers; ++i) {
+        const c8opt_layer &l = desc->layers[i];
+        if (!std::isfinite(l.h_lo_m) || !std::isfinite(l.a_gcm2) || !std::isfinite(l.b_gcm2) || !(l.c_m > 0.0) || !std::isfinite(l.c_m))
+            return fail(nullptr, C8OPT_ERR_ARGUMENT, "layer %d: non-finite coefficient or c <= 0", i);
+        if (i > 0 && !(l.h_lo_m > desc->layers[i - 1].h_lo_m)) return fail(nullptr, C8OPT_ERR_ARGUMENT, "layer bounds must ascend");
+    }
+    if (!(desc->rho0_gcm3 > 0.0) || !std::isfinite(desc->eta0) || !(desc->eta0 >= 0.0) || !std::isfinite(desc->h_obs_m))
+        return fail(nullptr, C8OPT_ERR_ARGUMENT, "need rho0 > 0, eta0 >= 0, finite h_obs");
+    const bool has_tau = desc->tau != nullptr && desc->tau_nh > 0;
+    if (has_tau) {
+        if (desc->tau_nl < 1 || desc->tau_nh > 4096 || desc->tau_nl > 4096 || !(desc->tau_dh_m > 0.0) || !(desc->tau_dl_nm > 0.0))
+            return fail(nullptr, C8OPT_ERR_ARGUMENT, "bad transmission table shape / spacing");
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, C8OPT_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+        return fail(nullptr, C8OPT_ERR_CUDA, "cannot query the current CUDA device");
+    if (prop.major != 10) return fail(nullptr, C8OPT_ERR_CUDA, "device is sm_%d%d, this library is built for sm_100a only", prop.major, prop.minor);
+
+    c8opt_ctx *ctx = new (std::nothrow) c8opt_ctx();
+    if (!ctx) return fail(nullptr, C8OPT_ERR_ARGUMENT, "out of host memory");
+    ctx->device = dev;
+    ctx->n_layers = desc->n_layers;
+    for (int i = 0; i < desc->n_layers; ++i)
+        ctx->layer[i] = HostLayer{desc->layers[i].h_lo_m, desc->layers[i].a_gcm2, desc->layers[i].b_gcm2, desc->layers[i].c_m};
+    ctx->eta0 = desc->eta0; ctx->rho0 = desc->rho0_gcm3; ctx->h_obs = desc->h_obs_m;
+    cudaError_t e = cudaSuccess;
+    if (has_tau) {
+        ctx->tau_nh = desc->tau_nh; ctx->tau_nl = desc->tau_nl;
+        ctx->tau_h0 = desc->tau_h0_m; ctx->tau_dh = desc->tau_dh_m; ctx->tau_l0 = desc->tau_l0_nm; ctx->tau_dl = desc->tau_dl_nm;
+        const size_t bytes = sizeof(float) * (size_t)desc->tau_nh * (size_t)desc->tau_nl;
+        e = cudaMalloc(&ctx->d_tau, bytes);
+        if (e == cudaSuccess) e = cudaMemcpy(ctx->d_tau, desc->tau, bytes, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 8 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, 8 * sizeof(unsigned long long));
+    for (int m = 0; m < 2 && e == cudaSuccess; ++m)
+        for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
+            e = cudaFuncSetAttribute(pick_kernel(cp != 0, (unsigned)m), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes());
+    if (e != cudaSuccess) {
+        fail(nullptr, C8OPT_ERR_CUDA, "context setup: %s", cudaGetErrorString(e));
+        c8opt_destroy(ctx);
+        return C8OPT_ERR_CUDA;
+    }
+    *out = ctx;
+    return C8OPT_OK;
+}
+
+int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    if (!xyzr) return fail(ctx, C8OPT_ERR_ARGUMENT, "xyzr is NULL");
+    if (n < 1 || n > C8OPT_MAX_TELESCOPES) return fail(ctx, C8OPT_ERR_ARGUMENT, "telescope count %d out of range 1..%d", n, C8OPT_MAX_TELESCOPES);
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int k = 0; k < n; ++k) {
+        for (int i = 0; i < 4; ++i)
+            if (!std::isfinite(xyzr[4 * k + i])) return fail(ctx, C8OPT_ERR_ARGUMENT, "telescope %d: non-finite value", k);
+        if (!(xyzr[4 * k + 3] > 0.0f)) return fail(ctx, C8OPT_ERR_ARGUMENT, "telescope %d: radius must be > 0", k);
+        for (int i = 0; i < 3; ++i) { lo[i] = std::fmin(lo[i], xyzr[4 * k + i]); hi[i] = std::fmax(hi[i], xyzr[4 * k + i]); }
+    }
+    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    C8_CUDA(ctx, cudaDeviceSynchronize());
+    ctx->n_tel = 0;
+    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_tallies); cudaFree(ctx->d_cursors);
+    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_tallies = nullptr; ctx->d_cursors = nullptr;
+    ctx->tel_xyzr.assign(xyzr, xyzr + 4 * (size_t)n);
+    // reference point: centre of the bounding box; all device coordinates are relative to it
+    ctx->x_ref = 0.5 * (lo[0] + hi[0]); ctx->y_ref = 0.5 * (lo[1] + hi[1]); ctx->z_ref = 0.5 * (lo[2] + hi[2]);
+    ctx->coplanar = (lo[2] == hi[2]);
+    std::vector<float4> A(n);
+    std::vector<float> T(n);
+    for (int k = 0; k < n; ++k) {
+        const double x = xyzr[4 * k], y = xyzr[4 * k + 1], z = xyzr[4 * k + 2], r = xyzr[4 * k + 3];
+        A[k] = make_float4((float)(x - ctx->x_ref), (float)(y - ctx->y_ref), (float)(z - ctx->z_ref), (float)(r * r));
+        T[k] = (float)host_depth(ctx, z);
+    }
+    C8_CUDA(ctx, cudaMalloc(&ctx->d_telA, sizeof(float4) * n));
+    C8_CUDA(ctx, cudaMalloc(&ctx->d_telT, sizeof(float) * n));
+    C8_CUDA(ctx, cudaMalloc(&ctx->d_tallies, sizeof(c8::Tally) * n));
+    C8_CUDA(ctx, cudaMalloc(&ctx->d_cursors, sizeof(unsigned long long) * n));
+    C8_CUDA(ctx, cudaMemcpy(ctx->d_telA, A.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
+    C8_CUDA(ctx, cudaMemcpy(ctx->d_telT, T.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
+    ctx->n_tel = n;
+    ctx->have_capacity = false;
+    const int rc = c8opt_reset_tallies(ctx, nullptr);
+    if (rc != C8OPT_OK) return rc;
+    C8_CUDA(ctx, cudaDeviceSynchronize());
+    return C8OPT_OK;
+}
+
+int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_t n, uint64_t first_segment_id,
+                             const c8opt_run_params *params, const c8opt_output *out, void *cuda_stream)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    if (!d_seg && n) return fail(ctx, C8OPT_ERR_ARGUMENT, "d_seg is NULL");
+    c8::KParams P;
+    int rc = fill_params(ctx, params, out, &P);
+    if (rc != C8OPT_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = remember_capacity(ctx, params, out, st);
+    if (rc != C8OPT_OK) return rc;
+    return launch(ctx, P, params->mode, d_seg, n, first_segment_id, out ? out->counts : nullptr, st);
+}
+
+int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, uint64_t n, uint64_t first_segment_id,
+                                  const c8opt_run_params *params, const c8opt_output *out, void *cuda_stream)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    if (!h_seg && n) return fail(ctx, C8OPT_ERR_ARGUMENT, "h_seg is NULL");
+    c8::KParams P;
+    int rc = fill_params(ctx, params, out, &P);
+    if (rc != C8OPT_OK) return rc;
+    cudaStream_t user = (cudaStream_t)cuda_stream;
+    rc = remember_capacity(ctx, params, out, user);
+    if (rc != C8OPT_OK) return rc;
+    if (n == 0) return C8OPT_OK;
+    // chunking: ~1/8 of the table per chunk, between 32 Ki and 1 Mi segments, a multiple of the tile
+    unsigned long long chunk = (n + 7) / 8;
+    if (chunk < (1ull << 15)) chunk = 1ull << 15;
+    if (chunk > (1ull << 20)) chunk = 1ull << 20;
+    chunk = (chunk + c8::kTile - 1) / c8::kTile * c8::kTile;
+    if (!ctx->pipe_stream[0]) {
+        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->pipe_stream[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 3; ++i) C8_CUDA(ctx, cudaEventCreateWithFlags(&ctx->pipe_event[i], cudaEventDisableTiming));
+    }
+    if (ctx->stage_segments < chunk) {
+        for (int i = 0; i < 2; ++i) {
+            C8_CUDA(ctx, cudaStreamSynchronize(ctx->pipe_stream[i]));
+            cudaFree(ctx->d_stage[i]); ctx->d_stage[i] = nullptr;
+        }
+        ctx->stage_segments = 0;
+        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaMalloc(&ctx->d_stage[i], sizeof(c8opt_segment) * chunk));
+        ctx->stage_segments = chunk;
+    }
+    C8_CUDA(ctx, cudaEventRecord(ctx->pipe_event[2], user));
+    for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamWaitEvent(ctx->pipe_stream[i], ctx->pipe_event[2], 0));
+    int c = 0;
+    for (unsigned long long off = 0; off < n; off += chunk, ++c) {
+        const unsigned long long m = (n - off < chunk) ? (n - off) : chunk;
+        cudaStream_t st = ctx->pipe_stream[c & 1];
+        C8_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage[c & 1], h_seg + off, sizeof(c8opt_segment) * m, cudaMemcpyHostToDevice, st));
+        rc = launch(ctx, P, params->mode, ctx->d_stage[c & 1], m, first_segment_id + off,
+                    (out && out->counts) ? out->counts + 2 * off : nullptr, st);
+        if (rc != C8OPT_OK) return rc;
+    }
+    for (int i = 0; i < 2; ++i) {
+        C8_CUDA(ctx, cudaEventRecord(ctx->pipe_event[i], ctx->pipe_stream[i]));
+        C8_CUDA(ctx, cudaStreamWaitEvent(user, ctx->pipe_event[i], 0));
+    }
+    return C8OPT_OK;
+}
+
+int c8opt_read_tallies(c8opt_ctx *ctx, c8opt_tally *host_out, int32_t n_tel, uint64_t *counters, uint64_t *host_tel_count)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    if (!host_out) return fail(ctx, C8OPT_ERR_ARGUMENT, "host_out is NULL");
+    if (n_tel != ctx->n_tel || n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "n_tel = %d but the context has %d telescopes", n_tel, ctx->n_tel);
+    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    C8_CUDA(ctx, cudaDeviceSynchronize());
+    static_assert(sizeof(c8opt_tally) == sizeof(c8::Tally), "tally layout");
+    C8_CUDA(ctx, cudaMemcpy(host_out, ctx->d_tallies, sizeof(c8::Tally) * n_tel, cudaMemcpyDeviceToHost));
+    unsigned long long cnt[8];
+    C8_CUDA(ctx, cudaMemcpy(cnt, ctx->d_counters, sizeof(cnt), cudaMemcpyDeviceToHost));
+    std::vector<unsigned long long> cur(n_tel);
+    C8_CUDA(ctx, cudaMemcpy(cur.data(), ctx->d_cursors, sizeof(unsigned long long) * n_tel, cudaMemcpyDeviceToHost));
+    unsigned long long hits = 0, stored = 0, dropped = 0;
+    for (int k = 0; k < n_tel; ++k) {
+        hits += host_out[k].hits;
+        unsigned long long kept = cur[k];
+        if (ctx->have_capacity && kept > ctx->h_capacity[k]) { dropped += kept - ctx->h_capacity[k]; kept = ctx->h_capacity[k]; }
+        stored += kept;
+        if (host_tel_count) host_tel_count[k] = kept;
+    }
+    if (counters) {
+        counters[C8OPT_CNT_SEGMENTS] = ctx->segments_total;
+        counters[C8OPT_CNT_GENERATED] = cnt[1];
+        counters[C8OPT_CNT_UPWARD] = cnt[2];
+        counters[C8OPT_CNT_HITS] = hits;
+        counters[C8OPT_CNT_RECORDS] = stored;
+        counters[C8OPT_CNT_DROPPED] = dropped;
+        counters[C8OPT_CNT_INVALID] = cnt[6];
+        counters[C8OPT_CNT_UNUSED] = 0;
+    }
+    if (dropped) return fail(ctx, C8OPT_ERR_CAPACITY, "%llu photon records dropped: output capacity exceeded", dropped);
+    return C8OPT_OK;
+}
+
+int c8opt_reset_tallies(c8opt_ctx *ctx, void *cuda_stream)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    C8_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), st));
+    if (ctx->n_tel > 0) {
+        C8_CUDA(ctx, cudaMemsetAsync(ctx->d_tallies, 0, sizeof(c8::Tally) * ctx->n_tel, st));
+        C8_CUDA(ctx, cudaMemsetAsync(ctx->d_cursors, 0, sizeof(unsigned long long) * ctx->n_tel, st));
+    }
+    ctx->segments_total = 0;
+    return C8OPT_OK;
+}
+
+void c8opt_destroy(c8opt_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->pipe_stream[i]) cudaStreamDestroy(ctx->pipe_stream[i]);
+        cudaFree(ctx->d_stage[i]);
+    }
+    for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
+    cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT);
+    cudaFree(ctx->d_tallies); cudaFree(ctx->d_counters); cudaFree(ctx->d_cursors);
+    cudaGetLastError();
+    delete ctx;
+}
+
+const char *c8opt_last_error(const c8opt_ctx *ctx) { return ctx ? ctx->error : g_create_error; }
+
+uint64_t c8opt_launch_count(const c8opt_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the fp64 oracle, element by element,
+on the seeded synthetic configs of BASELINE.json (workloads.make_config).  Criteria (a)-(d) of
+north_star are asserted in tests/parity_util.compare with the tolerances written there.
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q
+"""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def c8():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import paper_2309_15861_b200 as c8
+    c8.lib()          # fail loudly if the CUDA extension is missing
+    return c8
+
+
+def _report(name, rep):
+    print(f"[parity {name}] " + " ".join(f"{k}={v}" for k, v in rep.items() if k != "flip_list"))
+    for rid, k, d in rep.get("flip_list", []):
+        print(f"[parity {name}] flip photon={rid:#x} tel={k} b-R={d:+.3e} m")
+
+
+def test_config1_records_and_tallies(c8):
+    """configs[0]: 10^4 electron segments, single-layer atmosphere, 1 telescope; every record compared."""
+    import parity_util as pu
+    cfg = wl.make_config("c1")
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("c1", rep)
+    assert rep["matched"] > 100
+
+
+def test_config1_tally_mode_equals_output_mode(c8):
+    import parity_util as pu
+    cfg = wl.make_config("c1")
+    a = pu.gpu_run(cfg, c8.MODE_TALLY)
+    b = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    assert np.array_equal(a["tallies"]["hits"], b["tallies"]["hits"])
+    assert np.allclose(a["tallies"]["sum_w"], b["tallies"]["sum_w"], rtol=1e-12)
+    assert a["counters"]["generated"] == b["counters"]["generated"]
+    assert a["counters"]["records"] == 0 and b["counters"]["records"] == b["counters"]["hits"]
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 257, 1000])
+def test_ragged_sizes(c8, n):
+    """Empty input, less than a warp, a tile plus one, several tiles with a ragged tail."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=max(n, 1))
+    cfg["segments"] = cfg["segments"][:n]
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report(f"ragged{n}", rep)
+
+
+def test_config2_subset_records(c8):
+    """configs[1] shape (5-layer atmosphere, 4 telescopes) on 50k segments: every record compared."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=50_000)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("c2-50k", rep)
+    assert rep["matched"] > 5000
+
+
+def test_config2_full_size_tally(c8):
+    """configs[1] at full size (10^6 segments) in the launch configuration bench.py times (tally mode)."""
+    import parity_util as pu
+    cfg = wl.make_config("c2")
+    g = pu.gpu_run(cfg, c8.MODE_TALLY)
+    o = pu.oracle_run(cfg, record_capacity=0)
+    rep = pu.compare(cfg, g, o, check_records=False)
+    _report("c2-full", rep)
+
+
+def test_batching_and_host_path_invariance(c8):
+    """Results do not depend on how segments are batched (R20), nor on the host-buffer entry point."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=100_000)
+    a = pu.gpu_run(cfg, c8.MODE_OUTPUT, first_id=7)
+    b = pu.gpu_run(cfg, c8.MODE_OUTPUT, first_id=7, chunks=3)
+    c = pu.gpu_run(cfg, c8.MODE_OUTPUT, first_id=7, host_segments=True)
+    for other in (b, c):
+        assert np.array_equal(a["counts"], other["counts"])
+        assert np.array_equal(a["tallies"]["hits"], other["tallies"]["hits"])
+        assert np.array_equal(a["records"]["id"], other["records"]["id"])
+        for f in ("x", "y", "cx", "cy", "t", "lam", "w"):
+            assert np.array_equal(a["records"][f], other["records"][f])
+        assert np.allclose(a["tallies"]["sum_w"], other["tallies"]["sum_w"], rtol=1e-12)
+    assert b["launches"] == 3 and c["launches"] >= 1
+
+
+def test_config3_fluorescence_isotropic_and_beamed(c8):
+    """configs[2]: fluorescence only, telescope at 10 km; isotropic (hit list identical) and beamed 2 deg."""
+    import parity_util as pu
+    for name in ("c3a", "c3b"):
+        cfg = wl.make_config(name, n_segments=200_000)
+        g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+        o = pu.oracle_run(cfg)
+        rep = pu.compare(cfg, g, o)
+        _report(name, rep)
+        if name == "c3b":
+            assert rep["matched"] > 100
+
+
+def test_isotropic_near_telescope(c8):
+    """Isotropic fluorescence with a big sphere nearby, so that the isotropic branch has many hits."""
+    import parity_util as pu
+    cfg = wl.make_config("c3a", n_segments=20_000)
+    cfg["telescopes"] = np.array([[300.0, 0.0, 2000.0, 150.0]], dtype=np.float32)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("iso-near", rep)
+    assert rep["matched"] > 200
+
+
+def test_config4_subsample(c8):
+    """configs[3] shape: both processes, 100 telescopes, 5 layers + transmission table; 1 % subsample."""
+    import parity_util as pu
+    cfg = wl.make_config("c4", n_segments=100_000)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("c4-1pct", rep)
+    assert rep["matched"] > 5000
+
+
+def test_non_coplanar_and_generic_tracks(c8):
+    """Telescopes at different altitudes (general q_z != 0 test) and tracks that are horizontal / upward
+    (generic Cherenkov projection), plus invalid segments."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=30_000)
+    tel = cfg["telescopes"].copy()
+    tel[:, 2] += np.array([0.0, 35.0, -20.0, 60.0], dtype=np.float32)
+    tel[:, 3] = np.array([6.0, 12.0, 25.0, 40.0], dtype=np.float32)
+    cfg["telescopes"] = tel
+    seg = cfg["segments"]
+    rng = np.random.Generator(np.random.PCG64(99))
+    # every 7th track gets a random direction (isotropic), so some are horizontal or upward
+    idx = np.arange(0, len(seg), 7)
+    v = rng.normal(size=(len(idx), 3))
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    v = v.astype(np.float32).astype(np.float64)
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    seg["dx"][idx], seg["dy"][idx], seg["dz"][idx] = v[:, 0], v[:, 1], v[:, 2]
+    seg["length"][idx] = np.minimum(seg["length"][idx], 5.0)
+    # invalid ones
+    seg["gamma"][11] = 0.5
+    seg["dx"][12] = np.nan
+    seg["length"][13] = -1.0
+    seg["dz"][14] *= 1.01
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("noncoplanar", rep)
+    assert g["counters"]["invalid"] == 4
+    assert rep["matched"] > 1000
+
+
+def test_output_capacity_overflow(c8):
+    """The kernel never writes past tel_capacity; the overflow is counted and reported as error -3."""
+    import parity_util as pu
+    cfg = wl.make_config("c1")
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=100)
+    assert g["counters"]["records"] == 100
+    assert g["counters"]["dropped"] == g["counters"]["hits"] - 100 > 0
+    assert len(g["records"]) == 100
+
+
+def test_accept_all_output(c8):
+    """config 5g shape (every downward photon is written) on 3000 segments: the dense record path."""
+    import parity_util as pu
+    cfg = wl.make_config("c5g", n_segments=3000)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=1 << 20)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("c5g-3k", rep)
+    assert rep["matched"] == g["counters"]["generated"] - g["counters"]["upward"]
