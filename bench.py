@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- photons generated + propagated per second (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (preamble, Philox draw, generation, propagation, sphere
+test, tally / record output: every row of SURVEY.md §8(a)) over one batch of synthetic segments.
+The default workload is BASELINE.json configs[1] ("c2": 10^6 shower-shaped segments, 5-layer
+atmosphere, 4 telescopes, tally mode), the configuration north_star quotes the target on.
+Prints ONE JSON line (rank 0).  See DESIGN.md §7 for how each field is measured.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "photons generated+propagated per second"
+UNIT = "photons/s"
+# algorithmic thread-instructions per photon: Philox 40 +
+# uniforms/generation/projection 40 + 8 per telescope tested + loop 10
+ALG_INSTR = {"c1": 98.0, "c2": 122.0, "c5": 122.0, "c3a": 110.0, "c3b": 120.0, "c4": 130.0}
+RECORD_BYTES = 28.0
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons, self.max_mhz = index, period_s, [], set(), None
+        self._stop_evt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_baseline(cfg: dict, target_s: float = 15.0) -> dict:
+    """Time the fp64 oracle, as it stands, on the host cores on a bounded sample of the workload."""
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    seg = cfg["segments"]
+    probe = min(len(seg), 2000)
+    t0 = time.perf_counter()
+    r = oracle.run(cfg["atmosphere"], cfg["telescopes"], seg[:probe], cfg["params"], want_counts=False, threads=1)
+    t1 = time.perf_counter() - t0
+    per_seg_core = max(t1 / probe, 1e-9)
+    n = int(min(len(seg), max(probe, target_s * cores / per_seg_core)))
+    t0 = time.perf_counter()
+    r = oracle.run(cfg["atmosphere"], cfg["telescopes"], seg[:n], cfg["params"], want_counts=False, threads=cores)
+    dt = time.perf_counter() - t0
+    photons = int(r["counters"][1])
+    return {"value": photons / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n} of {len(seg)} segments of {cfg['name']} ({photons} photons) in {dt:.2f} s, "
+                      f"{cores} threads over contiguous segment ranges"}
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle on host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    cfg = wl.make_config(args.workload, n_segments=args.segments)
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    seg = cfg["segments"]
+    # each step = a bounded sample of the workload sized for ~2 s on this box
+    t0 = time.perf_counter()
+    oracle.run(cfg["atmosphere"], cfg["telescopes"], seg[:2000], cfg["params"], want_counts=False, threads=1)
+    per_seg_core = (time.perf_counter() - t0) / min(2000, len(seg))
+    n = int(min(len(seg), max(2000, 2.0 * cores / per_seg_core)))
+    steps = max(1, min(args.steps, 20))
+    warm = max(0, min(args.warmup, 2))
+    photons = 0
+    for _ in range(warm):
+        oracle.run(cfg["atmosphere"], cfg["telescopes"], seg[:n], cfg["params"], want_counts=False, threads=cores)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        r = oracle.run(cfg["atmosphere"], cfg["telescopes"], seg[:n], cfg["params"], want_counts=False, threads=cores)
+        photons += int(r["counters"][1])
+    dt = time.perf_counter() - t0
+    v = photons / dt
+    sample = f"each step = first {n} of {len(seg)} segments of {cfg['name']}, {cores} threads"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+        "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "segments": len(seg), "sampled_segments_per_step": n},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3a", "c3b", "c4", "c5", "c5g"])
+    ap.add_argument("--segments", type=int, default=None, help="override the segment count of the workload")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2309_15861_b200 as c8
+    from paper_2309_15861_b200.sharding import shard_first_id
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the photon path has no CPU fallback")
+    c8.lib()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- inputs: every rank owns a full-size segment set of its own (weak scaling, independent showers)
+    cfg = wl.make_config(args.workload, n_segments=args.segments)
+    if world > 1:
+        cfg = wl.make_config(args.workload, n_segments=args.segments, seed_offset=rank)
+    seg = cfg["segments"]
+    n = len(seg)
+    first_id = shard_first_id(rank, n)
+    tel = np.asarray(cfg["telescopes"], dtype=np.float32)
+    n_tel = len(tel)
+    par = dict(cfg["params"])
+    output_mode = par["mode"] == c8.MODE_OUTPUT
+    ctx = c8.Context(cfg["atmosphere"])
+    ctx.add_telescopes(tel)
+    h_seg = torch.from_numpy(seg.view(np.uint8).reshape(n, 48).copy()).pin_memory()
+    d_seg = h_seg.to(dev)
+    kw = {}
+    cap = 0
+    if output_mode:
+        # capacity: one warm-up pass in tally mode gives the exact record count per telescope
+        p0 = dict(par); p0["mode"] = c8.MODE_TALLY
+        ctx.propagate_segments(d_seg, p0, n=n, first_segment_id=first_id)
+        t0_, _, _ = ctx.read_tallies()
+        caps = (t0_["hits"].astype(np.int64) + 1024)
+        offs = np.concatenate([[0], np.cumsum(caps)[:-1]])
+        cap = int(caps.sum())
+        kw = dict(records=torch.empty((cap, 7), dtype=torch.float32, device=dev),
+                  tel_offset=torch.from_numpy(offs).to(dev), tel_capacity=torch.from_numpy(caps).to(dev))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step(timed_events=None):
+        flush.fill_(1)                                   # L2 flush between steps (untimed)
+        ctx.reset_tallies()
+        if timed_events is not None:
+            timed_events[0].record(stream)
+        ctx.propagate_segments(d_seg, par, n=n, first_segment_id=first_id, **kw)
+        if timed_events is not None:
+            timed_events[1].record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    tallies, counters, tel_count = ctx.read_tallies()
+    photons_per_step = counters["generated"]
+    hits_per_step = counters["hits"]
+
+    # ---- timed region: exactly K steps, device time by CUDA events on the launching stream
+    events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches0 = ctx.launch_count
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        step(events[k])
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    if world > 1:
+        dist.barrier()
+    launches = ctx.launch_count - launches0
+    step_ms = np.array([a.elapsed_time(b) for a, b in events])
+    total_ms = float(step_ms.sum())
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        pc = torch.tensor([photons_per_step], dtype=torch.float64, device=dev)
+        dist.all_reduce(pc, op=dist.ReduceOp.SUM)
+        photons_all = float(pc.item())
+    else:
+        photons_all = float(photons_per_step)
+    value = photons_all * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the C-ABI with HOST buffers: H2D of the segments + kernel + D2H of the tallies
+    e2e = None
+    if not args.no_e2e:
+        for _ in range(2):
+            ctx.reset_tallies()
+            ctx.propagate_segments_host(h_seg, par, n=n, first_segment_id=first_id, **kw)
+            ctx.read_tallies()
+        ke = max(3, min(args.steps, 20))
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            ctx.reset_tallies()
+            ctx.propagate_segments_host(h_seg, par, n=n, first_segment_id=first_id, **kw)
+            ctx.read_tallies()                          # synchronises + D2H
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": photons_all * ke / dt, "unit": UNIT, "h2d_bytes_per_step": int(n * 48),
+               "d2h_bytes_per_step": int(n_tel * 24 + 8 * 8 + n_tel * 8), "steps": ke,
+               "note": "c8opt_propagate_segments_host from pinned host memory (chunked H2D overlapped with the kernels) "
+                       "+ c8opt_read_tallies; wall clock"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant (only) kernel
+    peaks = load_peaks()
+    per_launch_s = total_ms * 1e-3 / args.steps
+    if args.workload == "c5g":
+        bytes_per_launch = RECORD_BYTES * hits_per_step + 48.0 * n
+        roofline = {"bound": "hbm", "achieved": bytes_per_launch / per_launch_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "traffic": None, "peak_source": peaks["source"], "bytes_per_photon": RECORD_BYTES}
+    else:
+        instr = ALG_INSTR.get(args.workload, 122.0)
+        peak = 148 * 4 * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12            # thread-instructions / s, issue-slot peak
+        roofline = {"bound": "alu", "achieved": instr * photons_per_step / per_launch_s / 1e12, "peak": peak,
+                    "unit": "Tinstr/s", "traffic": None, "peak_source": "148 SM x 4 schedulers x 32 lanes x sm_max_mhz "
+                    f"({peaks['source']})", "alg_instr_per_photon": instr,
+                    "hbm_achieved_gbs": (48.0 * n + RECORD_BYTES * (hits_per_step if output_mode else 0)) / per_launch_s / 1e9}
+    roofline["frac"] = roofline["achieved"] / roofline["peak"]
+    roofline["kernel"] = "c8::propagate_kernel"
+    roofline["kernel_ms"] = per_launch_s * 1e3
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": cfg["name"], "segments_per_gpu": n, "photons_per_step_per_gpu": photons_per_step,
+                   "hits_per_step_per_gpu": hits_per_step, "telescopes": n_tel, "mode": "output" if output_mode else "tally",
+                   "l2": "flushed between steps (256 MiB fill, untimed)", "timing": "sum of per-step CUDA-event times",
+                   "parallelism": f"segments sharded over {world} GPU(s), no data-path collective"},
+        "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "wall_s_timed_region": wall, "step_ms_min_med_max": [float(step_ms.min()), float(np.median(step_ms)), float(step_ms.max())],
+    }
+    if not args.no_cpu_baseline and world == 1:
+        out["cpu_baseline"] = oracle_baseline(cfg)
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

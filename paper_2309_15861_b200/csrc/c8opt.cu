@@ -3,6 +3,7 @@
 #include "../../include/c8opt.h"
 #include "c8opt_kernels.cuh"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -28,12 +29,19 @@ struct c8opt_ctx {
     double tau_h0 = 0, tau_dh = 1, tau_l0 = 0, tau_dl = 1;
     float *d_tau = nullptr;
     // telescopes
-    int n_tel = 0;
+    int n_tel = 0, n_tel_pending = 0;
     bool coplanar = true;
     std::vector<double> tel_xyzr;          // absolute, as given (float -> double)
     double x_ref = 0, y_ref = 0, z_ref = 0;
     float4 *d_telA = nullptr;
     float *d_telT = nullptr;
+    std::vector<float4> h_telA;
+    std::vector<float> h_telT;
+    // ground-plane candidate grid (n_tel > kTelConstMax)
+    int tel_src = c8::TEL_CONST;
+    uint2 *d_grid = nullptr;
+    int grid_nx = 0, grid_ny = 0;
+    float grid_x0 = 0, grid_y0 = 0, grid_inv_cell = 0, grid_vzmin = 0;
     // results
     c8::Tally *d_tallies = nullptr;
     unsigned long long *d_counters = nullptr;   // [8]
@@ -81,10 +89,77 @@ size_t smem_bytes() { return sizeof(c8::TileSmem); }
 
 typedef void (*kernel_t)(const c8::KParams);
 
-kernel_t pick_kernel(bool coplanar, unsigned mode)
+template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar)
 {
-    if (mode == C8OPT_MODE_OUTPUT) return coplanar ? c8::propagate_kernel<true, 1> : c8::propagate_kernel<false, 1>;
-    return coplanar ? c8::propagate_kernel<true, 0> : c8::propagate_kernel<false, 0>;
+    return coplanar ? c8::propagate_kernel<TELSRC, true, NT> : c8::propagate_kernel<TELSRC, false, NT>;
+}
+
+// nt = number of constant-bank telescope slots the hot loop tests (n_tel rounded up to 1, 4 or 8)
+int padded_count(int n_tel) { return n_tel <= 1 ? 1 : (n_tel <= 4 ? 4 : 8); }
+
+kernel_t pick_kernel(int tel_src, bool coplanar, int nt)
+{
+    if (tel_src == c8::TEL_CONST) {
+        if (nt == 1) return pick_kernel2<c8::TEL_CONST, 1>(coplanar);
+        if (nt == 4) return pick_kernel2<c8::TEL_CONST, 4>(coplanar);
+        return pick_kernel2<c8::TEL_CONST, 8>(coplanar);
+    }
+    if (tel_src == c8::TEL_GRID) return pick_kernel2<c8::TEL_GRID, 0>(coplanar);
+    return pick_kernel2<c8::TEL_GLOBAL, 0>(coplanar);
+}
+
+// Ground-plane candidate grid: a photon with |v_z| >= vzmin that hits telescope k crosses the
+// plane z_ref within rho_k = R / vzmin + |c_z - z_ref| sqrt(1 / vzmin^2 - 1) of (c_x, c_y).  Every cell lists the
+// telescopes whose disc (bounding square, plus slack for fp32 rounding) touches it; at most 4 per cell, else the
+// resolution is doubled, and if that does not help the grid is not used (brute force from global memory).
+bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
+{
+    const double vzmin = 0.5, slack = 0.05;
+    const int n = ctx->n_tel_pending;
+    std::vector<double> rho(n);
+    double x_lo = INFINITY, x_hi = -INFINITY, y_lo = INFINITY, y_hi = -INFINITY, rho_max = 0;
+    for (int k = 0; k < n; ++k) {
+        const double r = std::sqrt((double)ctx->h_telA[k].w), dz = std::fabs((double)ctx->h_telA[k].z);
+        rho[k] = r / vzmin + dz * std::sqrt(1.0 / (vzmin * vzmin) - 1.0) + slack;
+        rho_max = std::fmax(rho_max, rho[k]);
+        x_lo = std::fmin(x_lo, ctx->h_telA[k].x - rho[k]); x_hi = std::fmax(x_hi, ctx->h_telA[k].x + rho[k]);
+        y_lo = std::fmin(y_lo, ctx->h_telA[k].y - rho[k]); y_hi = std::fmax(y_hi, ctx->h_telA[k].y + rho[k]);
+    }
+    const double ext = std::fmax(x_hi - x_lo, y_hi - y_lo);
+    int res = (int)std::ceil(ext / (2.0 * rho_max));
+    if (res < 1) res = 1;
+    if (res > 256) res = 256;
+    for (; res <= 1024; res *= 2) {
+        const double cell = ext / res * (1.0 + 1e-6);
+        const int nx = (int)std::ceil((x_hi - x_lo) / cell), ny = (int)std::ceil((y_hi - y_lo) / cell);
+        if (nx < 1 || ny < 1) return false;
+        std::vector<uint16_t> list((size_t)nx * ny * 4, 0xffffu);
+        bool ok = true;
+        for (int k = 0; k < n && ok; ++k) {
+            const int ix0 = std::max(0, (int)std::floor((ctx->h_telA[k].x - rho[k] - x_lo) / cell));
+            const int ix1 = std::min(nx - 1, (int)std::floor((ctx->h_telA[k].x + rho[k] - x_lo) / cell));
+            const int iy0 = std::max(0, (int)std::floor((ctx->h_telA[k].y - rho[k] - y_lo) / cell));
+            const int iy1 = std::min(ny - 1, (int)std::floor((ctx->h_telA[k].y + rho[k] - y_lo) / cell));
+            for (int iy = iy0; iy <= iy1 && ok; ++iy)
+                for (int ix = ix0; ix <= ix1; ++ix) {
+                    uint16_t *c = &list[((size_t)iy * nx + ix) * 4];
+                    int slot = 0;
+                    while (slot < 4 && c[slot] != 0xffffu) ++slot;
+                    if (slot == 4) { ok = false; break; }
+                    c[slot] = (uint16_t)k;
+                }
+        }
+        if (!ok) continue;
+        cells->resize((size_t)nx * ny);
+        for (size_t i = 0; i < cells->size(); ++i)
+            (*cells)[i] = make_uint2((uint32_t)list[4 * i] | ((uint32_t)list[4 * i + 1] << 16),
+                                     (uint32_t)list[4 * i + 2] | ((uint32_t)list[4 * i + 3] << 16));
+        ctx->grid_nx = nx; ctx->grid_ny = ny;
+        ctx->grid_x0 = (float)x_lo; ctx->grid_y0 = (float)y_lo;
+        ctx->grid_inv_cell = (float)(1.0 / cell); ctx->grid_vzmin = (float)vzmin;
+        return true;
+    }
+    return false;
 }
 
 // Validate params / outputs and fill the kernel parameter block (everything except seg / n / first_id).
@@ -122,8 +197,17 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     P.tau_h0 = (float)ctx->tau_h0; P.tau_inv_dh = (float)(1.0 / ctx->tau_dh);
     P.tau_l0 = (float)ctx->tau_l0; P.tau_inv_dl = (float)(1.0 / ctx->tau_dl);
     P.n_tel = ctx->n_tel; P.telA = ctx->d_telA; P.telT = ctx->d_telT;
+    if (ctx->tel_src == c8::TEL_CONST) {
+        for (int k = 0; k < c8::kTelConstMax; ++k) { P.tel_c[k] = make_float4(0.f, 0.f, 0.f, -1.f); P.telT_c[k] = 0.f; }   // R^2 = -1: never hit
+        for (int k = 0; k < ctx->n_tel; ++k) { P.tel_c[k] = ctx->h_telA[k]; P.telT_c[k] = ctx->h_telT[k]; }
+    }
+    P.grid = ctx->d_grid; P.grid_nx = ctx->grid_nx; P.grid_ny = ctx->grid_ny;
+    P.grid_x0 = ctx->grid_x0; P.grid_y0 = ctx->grid_y0; P.grid_inv_cell = ctx->grid_inv_cell; P.grid_vzmin = ctx->grid_vzmin;
     P.x_ref = ctx->x_ref; P.y_ref = ctx->y_ref; P.z_ref = ctx->z_ref;
-    P.key0 = (uint32_t)rp->seed; P.key1 = (uint32_t)(rp->seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        P.rk0[r] = (uint32_t)rp->seed + (uint32_t)r * 0x9E3779B9u;
+        P.rk1[r] = (uint32_t)(rp->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+    }
     P.processes = procs; P.n_procs = (procs == 3u) ? 2u : 1u;
     if (procs & C8OPT_PROC_CHERENKOV) {
         // PAPER.md:45 prefactor: pi e^2 / (h eps0 c0) = 2 pi alpha; the lambda integral of lambda^-2 in closed form (R2)
@@ -161,7 +245,7 @@ int launch(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, const c8opt_segment *d
     const unsigned long long per_tile = c8::kTile / P.n_procs;
     const unsigned long long tiles = (n + per_tile - 1) / per_tile;
     if (tiles > 0x7fffffffull) return fail(ctx, C8OPT_ERR_ARGUMENT, "too many segments in one call");
-    kernel_t k = pick_kernel(ctx->coplanar, mode);
+    kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel));
     k<<<(unsigned)tiles, c8::kTile, smem_bytes(), st>>>(P);
     C8_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
@@ -229,9 +313,10 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
     }
     if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 8 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, 8 * sizeof(unsigned long long));
-    for (int m = 0; m < 2 && e == cudaSuccess; ++m)
-        for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
-            e = cudaFuncSetAttribute(pick_kernel(cp != 0, (unsigned)m), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes());
+    for (int ts = 0; ts < 3 && e == cudaSuccess; ++ts)
+        for (int nt = 1; nt <= 8 && e == cudaSuccess; nt *= (nt == 1 ? 4 : 2))
+            for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
+                e = cudaFuncSetAttribute(pick_kernel(ts, cp != 0, nt), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes());
     if (e != cudaSuccess) {
         fail(nullptr, C8OPT_ERR_CUDA, "context setup: %s", cudaGetErrorString(e));
         c8opt_destroy(ctx);
@@ -256,14 +341,15 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     C8_CUDA(ctx, cudaSetDevice(ctx->device));
     C8_CUDA(ctx, cudaDeviceSynchronize());
     ctx->n_tel = 0;
-    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_tallies); cudaFree(ctx->d_cursors);
-    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_tallies = nullptr; ctx->d_cursors = nullptr;
+    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_tallies); cudaFree(ctx->d_cursors); cudaFree(ctx->d_grid);
+    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_tallies = nullptr; ctx->d_cursors = nullptr; ctx->d_grid = nullptr;
     ctx->tel_xyzr.assign(xyzr, xyzr + 4 * (size_t)n);
     // reference point: centre of the bounding box; all device coordinates are relative to it
     ctx->x_ref = 0.5 * (lo[0] + hi[0]); ctx->y_ref = 0.5 * (lo[1] + hi[1]); ctx->z_ref = 0.5 * (lo[2] + hi[2]);
     ctx->coplanar = (lo[2] == hi[2]);
-    std::vector<float4> A(n);
-    std::vector<float> T(n);
+    std::vector<float4> &A = ctx->h_telA;
+    std::vector<float> &T = ctx->h_telT;
+    A.resize(n); T.resize(n);
     for (int k = 0; k < n; ++k) {
         const double x = xyzr[4 * k], y = xyzr[4 * k + 1], z = xyzr[4 * k + 2], r = xyzr[4 * k + 3];
         A[k] = make_float4((float)(x - ctx->x_ref), (float)(y - ctx->y_ref), (float)(z - ctx->z_ref), (float)(r * r));
@@ -275,6 +361,18 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     C8_CUDA(ctx, cudaMalloc(&ctx->d_cursors, sizeof(unsigned long long) * n));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telA, A.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telT, T.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
+    ctx->tel_src = c8::TEL_CONST;
+    if (n > c8::kTelConstMax) {
+        std::vector<uint2> cells;
+        ctx->n_tel_pending = n;
+        if (build_grid(ctx, &cells)) {
+            C8_CUDA(ctx, cudaMalloc(&ctx->d_grid, sizeof(uint2) * cells.size()));
+            C8_CUDA(ctx, cudaMemcpy(ctx->d_grid, cells.data(), sizeof(uint2) * cells.size(), cudaMemcpyHostToDevice));
+            ctx->tel_src = c8::TEL_GRID;
+        } else {
+            ctx->tel_src = c8::TEL_GLOBAL;
+        }
+    }
     ctx->n_tel = n;
     ctx->have_capacity = false;
     const int rc = c8opt_reset_tallies(ctx, nullptr);
@@ -403,7 +501,7 @@ void c8opt_destroy(c8opt_ctx *ctx)
         cudaFree(ctx->d_stage[i]);
     }
     for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
-    cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT);
+    cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_grid);
     cudaFree(ctx->d_tallies); cudaFree(ctx->d_counters); cudaFree(ctx->d_cursors);
     cudaGetLastError();
     delete ctx;

@@ -12,7 +12,11 @@
 // walks a contiguous 1/8 of it 32 photons at a time, so every lane always has a photon
 // regardless of how many photons each segment emits.  A lane keeps the frame of its
 // current emitter in registers and reloads it only when its photon index crosses into the
-// next emitter.
+// next emitter.  The hot loop only decides, with a conservative pre-test, which (photon,
+// telescope) pairs can be hits (~0.4 % of the photons) and pushes their 8-byte ids into a
+// per-warp queue; whenever 32 are queued the warp processes them with all lanes busy:
+// regenerate the photon from its counter-based random stream, exact sphere test, arrival
+// time, wavelength, weight, tally / record.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -22,8 +26,13 @@ namespace c8 {
 constexpr int kTile = 256;            // emitters per tile == threads per block
 constexpr int kWarps = kTile / 32;
 constexpr int kFrameStride = 36;      // floats per emitter frame in shared memory (144 B)
-constexpr int kTelSmemMax = 128;      // telescopes staged (and tallied) in shared memory
+constexpr int kTelSmemMax = 128;      // telescopes tallied in shared memory
+constexpr int kTelConstMax = 8;       // telescopes kept in the kernel-parameter constant bank
+constexpr int TEL_CONST = 0;          // brute force over <= kTelConstMax telescopes read from the constant bank
+constexpr int TEL_GRID = 1;           // candidate lookup in the ground-plane grid
+constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global memory (grid not buildable)
 constexpr int kMaxLayers = 8;
+constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
 constexpr int KIND_FL_ISO = 1;        // fluorescence, isotropic
@@ -50,9 +59,15 @@ struct KParams {
     int n_tel;
     const float4 *telA;            // device: (cx - x_ref, cy - y_ref, cz - z_ref, R^2)
     const float *telT;             // device: column depth T(c_z) [g/cm^2]
+    float4 tel_c[kTelConstMax];    // the same two tables in the constant bank when n_tel <= kTelConstMax
+    float telT_c[kTelConstMax];
     double x_ref, y_ref, z_ref;
+    // ground-plane candidate grid (n_tel > kTelConstMax): cell -> up to 4 telescope indices (0xffff = none)
+    const uint2 *grid;
+    int grid_nx, grid_ny;
+    float grid_x0, grid_y0, grid_inv_cell, grid_vzmin;
     // run
-    uint32_t key0, key1;
+    uint32_t rk0[10], rk1[10];     // Philox round keys: key + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t processes, n_procs;
     double c_ft;                   // 2 pi alpha (1/lam1 - 1/lam2) [1/m]  (R2)
     double bunch_size, fl_yield;
@@ -78,18 +93,47 @@ __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
 // a2: Philox4x32-10 (Salmon et al., SC'11), counter (j, S_lo, S_hi, tag), key = seed (R20).
 struct Rand4 { uint32_t r0, r1, r2, r3; };
 
-__device__ __forceinline__ Rand4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
-                                               uint32_t k0, uint32_t k1)
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u, kPhiloxM1 = 0xCD9E8D57u;
+
+__device__ __forceinline__ void philox_round(uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3, uint32_t k0, uint32_t k1)
+{
+    const unsigned long long pa = (unsigned long long)kPhiloxM0 * c0;
+    const unsigned long long pb = (unsigned long long)kPhiloxM1 * c2;
+    const uint32_t n0 = (uint32_t)(pb >> 32) ^ c1 ^ k0;
+    const uint32_t n2 = (uint32_t)(pa >> 32) ^ c3 ^ k1;
+    c1 = (uint32_t)pb; c3 = (uint32_t)pa; c0 = n0; c2 = n2;
+}
+
+__device__ __forceinline__ Rand4 philox4x32_10(const KParams &P, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3)
 {
 #pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const unsigned long long pa = (unsigned long long)0xD2511F53u * c0;
-        const unsigned long long pb = (unsigned long long)0xCD9E8D57u * c2;
-        const uint32_t n0 = (uint32_t)(pb >> 32) ^ c1 ^ k0;
-        const uint32_t n2 = (uint32_t)(pa >> 32) ^ c3 ^ k1;
-        c1 = (uint32_t)pb; c3 = (uint32_t)pa; c0 = n0; c2 = n2;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-    }
+    for (int r = 0; r < 10; ++r) philox_round(c0, c1, c2, c3, P.rk0[r], P.rk1[r]);
+    return Rand4{c0, c1, c2, c3};
+}
+
+// The counter is (j, S_lo, S_hi, tag): only word 0 changes from photon to photon of one emitter, so
+// the S-dependent halves of rounds 1 and 2 are computed once per emitter (3 words) and each photon
+// does 18 instead of 20 wide multiplies.  Same function, bit for bit.
+struct PhiloxEmitter { uint32_t C, D, E; };
+
+__device__ __forceinline__ PhiloxEmitter philox_emitter(const KParams &P, unsigned long long S)
+{
+    const unsigned long long pb = (unsigned long long)kPhiloxM1 * (uint32_t)(S >> 32);   // round 1, c2 = S_hi
+    const uint32_t A = (uint32_t)(pb >> 32) ^ (uint32_t)S ^ P.rk0[0];                    // c0 after round 1
+    const uint32_t B = (uint32_t)pb;                                                     // c1 after round 1
+    const unsigned long long pa = (unsigned long long)kPhiloxM0 * A;                     // round 2, c0 = A
+    return PhiloxEmitter{B ^ P.rk0[1], (uint32_t)(pa >> 32) ^ P.rk1[1], (uint32_t)pa};
+}
+
+__device__ __forceinline__ Rand4 philox_photon(const KParams &P, const PhiloxEmitter &pe, uint32_t j, uint32_t tag)
+{
+    const unsigned long long pa = (unsigned long long)kPhiloxM0 * j;                     // round 1, c0 = j
+    const uint32_t c2_1 = (uint32_t)(pa >> 32) ^ tag ^ P.rk1[0];
+    const uint32_t c3_1 = (uint32_t)pa;
+    const unsigned long long pb = (unsigned long long)kPhiloxM1 * c2_1;                  // round 2, c2
+    uint32_t c0 = (uint32_t)(pb >> 32) ^ pe.C, c1 = (uint32_t)pb, c2 = c3_1 ^ pe.D, c3 = pe.E;
+#pragma unroll
+    for (int r = 2; r < 10; ++r) philox_round(c0, c1, c2, c3, P.rk0[r], P.rk1[r]);
     return Rand4{c0, c1, c2, c3};
 }
 
@@ -107,11 +151,10 @@ struct TileSmem {
     uint8_t kind[kTile];
     uint8_t invalid[kTile];
     uint32_t warp_sum[kWarps];
-    float4 telA[kTelSmemMax];
-    float telT[kTelSmemMax];
     uint32_t t_hits[kTelSmemMax];
     double t_sw[kTelSmemMax], t_swt[kTelSmemMax];
     unsigned long long n_upward;
+    uint2 queue[kWarps][kQueue];                // per-warp ring of candidate (photon, telescope) pairs
 };
 
 // frame slots.  Axis-relative Cherenkov (KIND_CHER_AXIS):
@@ -267,138 +310,346 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
 }
 
 // ------------------------------------------------------------------------------------
-// a4/a5 rare path: a photon that passed the conservative pre-test for telescope k.
-//   ez    emission altitude above z_ref            (vx, vy, vz) unit direction, rv = 1 / vz
-//   gx,gy crossing of the plane z_ref relative to (x_ref, y_ref)
-//   s     distance of the emission point along the track, r2 the wavelength random word
-template <int MODE>
-__device__ __noinline__ void candidate(const KParams &P, TileSmem &sm, int k, int e, uint32_t j, unsigned long long S,
-                                       int tag, uint32_t r2, float s, float ez, float vx, float vy, float vz, float rv,
-                                       float gx, float gy)
+template <int TELSRC> __device__ __forceinline__ float4 tel_at(const KParams &P, int k)
 {
-    const float4 T = (P.n_tel <= kTelSmemMax) ? sm.telA[k] : P.telA[k];
-    const float qx = gx - T.x, qy = gy - T.y, qz = -T.z;
-    const float qv = fmaf(qx, vx, fmaf(qy, vy, qz * vz));
-    const float b2 = fmaf(qx, qx, fmaf(qy, qy, qz * qz)) - qv * qv;       // R10: distance^2 of the centre to the ray
-    const float hk = ez - T.z;                                             // emission height above the telescope plane
-    const float s_pl = -hk * rv;                                           // path length to that plane (R11)
-    const float s_c = (s_pl - T.z * rv) - qv;                              // closest approach along the forward ray
-    // (the point (gx, gy) is on the plane z_ref at path length -ez rv = s_pl - T.z rv)
-    if (!(b2 <= T.w) || !(hk > 0.0f) || !(s_c > 0.0f)) return;
-
-    const float *fr = &sm.frame[e * kFrameStride];
-    const float habs = (float)P.z_ref + ez;
-    // R8: arrival time = emission time + (geometric path + integral of eta dl) / c,
-    //     integral = kappa (T(c_z) - T(e_z)) / |v_z|
-    int li = 0;
-    for (int i = 1; i < P.n_layers; ++i) if (habs >= P.layerf[i].h_lo) li = i;
-    const LayerF lf = P.layerf[li];
-    const float Te = fmaf(lf.b, __expf(-habs * lf.inv_c), lf.a);
-    const float Tk = (P.n_tel <= kTelSmemMax) ? sm.telT[k] : P.telT[k];
-    const float excess = P.kappa_m * (Tk - Te) * fabsf(rv);
-    const float t = fmaf(s, fr[F_IBC], fr[F_T0]) + (s_pl + excess) * (1.0f / 0.299792458f);
-    // R4: wavelength
-    const float u3 = uniform01(r2);
-    const float lam = (tag == 0) ? __frcp_rn(fmaf(-u3, P.dinv_lam, P.inv_lam1)) : fmaf(u3, P.fl_dlam, P.fl_lam1);
-    // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
-    float w = fr[F_W0];
-    if (P.tau != nullptr) {
-        const int nh = P.tau_nh, nl = P.tau_nl;
-        float fh = (habs - P.tau_h0) * P.tau_inv_dh, fl = (lam - P.tau_l0) * P.tau_inv_dl;
-        fh = fminf(fmaxf(fh, 0.0f), (float)(nh - 1)); fl = fminf(fmaxf(fl, 0.0f), (float)(nl - 1));
-        int ih = min(max((int)floorf(fh), 0), max(nh - 2, 0)), il = min(max((int)floorf(fl), 0), max(nl - 2, 0));
-        const float th = fh - (float)ih, tl = fl - (float)il;
-        const int ih1 = (nh > 1) ? ih + 1 : ih, il1 = (nl > 1) ? il + 1 : il;
-        const float t00 = __ldg(&P.tau[ih * nl + il]), t01 = __ldg(&P.tau[ih * nl + il1]);
-        const float t10 = __ldg(&P.tau[ih1 * nl + il]), t11 = __ldg(&P.tau[ih1 * nl + il1]);
-        const float tau = (1.0f - th) * fmaf(tl, t01 - t00, t00) + th * fmaf(tl, t11 - t10, t10);
-        w *= __expf(-tau * fabsf(rv));
-    }
-    // a5: tally
-    if (P.n_tel <= kTelSmemMax) {
-        atomicAdd(&sm.t_hits[k], 1u);
-        atomicAdd(&sm.t_sw[k], (double)w);
-        atomicAdd(&sm.t_swt[k], (double)w * (double)t);
-    } else {
-        atomicAdd(&P.tallies[k].hits, 1ull);
-        atomicAdd(&P.tallies[k].sum_w, (double)w);
-        atomicAdd(&P.tallies[k].sum_wt, (double)w * (double)t);
-    }
-    if (MODE == 1) {
-        const unsigned long long slot = atomicAdd(&P.cursors[k], 1ull);
-        if (slot < P.tel_capacity[k]) {
-            const unsigned long long at = P.tel_offset[k] + slot;
-            float *rec = P.records + at * 7ull;
-            // position on the plane through the telescope centre, relative to the centre (R11)
-            rec[0] = fmaf(T.z * rv, vx, qx); rec[1] = fmaf(T.z * rv, vy, qy);
-            rec[2] = vx; rec[3] = vy; rec[4] = t; rec[5] = lam; rec[6] = w;
-            if (P.ids) P.ids[at] = (S << 25) | ((unsigned long long)tag << 24) | (unsigned long long)j;
-        }
-    }
+    if (TELSRC == TEL_CONST) return P.tel_c[k];
+    return __ldg(&P.telA[k]);
+}
+template <int TELSRC> __device__ __forceinline__ float telT_at(const KParams &P, int k)
+{
+    if (TELSRC == TEL_CONST) return P.telT_c[k];
+    return __ldg(&P.telT[k]);
 }
 
-// Conservative pre-test over all telescopes for a downward photon; calls candidate() for survivors.
-// For coplanar telescopes (q_z = 0): b^2 = |q|^2 - (q.v)^2 >= |q|^2 v_z^2, so |q|^2 v_z^2 > R^2 is a miss.
-template <bool COPLANAR, int MODE>
-__device__ __forceinline__ void test_telescopes(const KParams &P, TileSmem &sm, const float4 *__restrict__ tel,
-                                                int e, uint32_t j, unsigned long long S, int tag, uint32_t r2, float s,
-                                                float ez, float vx, float vy, float vz, float rv, float gx, float gy)
+__device__ __forceinline__ float rcp_approx(float x)
 {
-    const float vz2 = vz * vz;
-    for (int k = 0; k < P.n_tel; ++k) {
-        const float4 T = tel[k];
-        const float qx = gx - T.x, qy = gy - T.y;
-        bool cand;
-        if (COPLANAR) {
-            cand = fmaf(qy, qy, qx * qx) * vz2 <= T.w;
-        } else {
-            const float qv = fmaf(qx, vx, fmaf(qy, vy, -T.z * vz));
-            cand = fmaf(qx, qx, fmaf(qy, qy, T.z * T.z)) - qv * qv <= T.w * 1.0001f + 1e-3f;
-        }
-        if (cand) candidate<MODE>(P, sm, k, e, j, S, tag, r2, s, ez, vx, vy, vz, rv, gx, gy);
-    }
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 }
 
-// a3 + a4 for the generic kinds (isotropic / cone / generic Cherenkov).  Returns true if the photon goes upward.
-template <bool COPLANAR, int MODE>
-__device__ __noinline__ bool generic_photon(const KParams &P, TileSmem &sm, const float4 *__restrict__ tel, int kind,
-                                            int e, uint32_t j, unsigned long long S)
+// A photon ready for the exact test: emission point e relative to (x_ref, y_ref, z_ref) or, for the
+// axis kind, the crossing (gx, gy) of the plane z_ref; unit direction v; s = distance along the track.
+struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s; uint32_t r2; int tag; bool axis; };
+
+// a2 + a3 for photon j of emitter e, any kind (used by the queue drain and by the generic kinds' hot path).
+__device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S)
 {
     const float *fr = &sm.frame[e * kFrameStride];
-    const int tag = (kind == KIND_CHER_GEN) ? 0 : 1;
-    const Rand4 r = philox4x32_10(j, (uint32_t)S, (uint32_t)(S >> 32), (uint32_t)tag, P.key0, P.key1);
-    const float s = uniform01(r.r0) * fr[F_L];
-    const float ex = fmaf(s, fr[F_D0 + 0], fr[F_E0 + 0]), ey = fmaf(s, fr[F_D0 + 1], fr[F_E0 + 1]);
-    const float ez = fmaf(s, fr[F_D0 + 2], fr[F_E0 + 2]);
+    const int kind = sm.kind[e];
+    Photon ph;
+    ph.tag = (kind == KIND_CHER_AXIS || kind == KIND_CHER_GEN) ? 0 : 1;
+    ph.axis = (kind == KIND_CHER_AXIS);
+    const Rand4 r = philox4x32_10(P, j, (uint32_t)S, (uint32_t)(S >> 32), (uint32_t)ph.tag);
+    ph.r2 = r.r2;
+    if (kind == KIND_CHER_AXIS) {
+        const float w1 = one_two(r.r0);
+        const float sd = fmaf(w1, fr[F_NEGL], fr[F_K0C]);                            // K0 - u1 L
+        float sp, cp;
+        __sincosf(fmaf(one_two(r.r1), 6.2831853f, -9.42477760f), &sp, &cp);          // phi - pi, in [-pi, pi)
+        ph.vz = fmaf(cp, fr[F_AZ], fmaf(sp, fr[F_BZ], fr[F_CZ]));
+        ph.vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
+        ph.vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
+        const float rho = sd * rcp_approx(ph.vz);
+        ph.gx = fmaf(rho, fmaf(cp, fr[F_PX], sp * fr[F_QX]), fr[F_GX]);
+        ph.gy = fmaf(rho, fmaf(cp, fr[F_PY], sp * fr[F_QY]), fr[F_GY]);
+        ph.s = (w1 - kOneMinus) * fr[F_LEN];
+        ph.ez = -sd * fr[F_DZ];                                                      // emission altitude above z_ref
+        ph.ex = ph.ey = 0.0f;
+        return ph;
+    }
+    ph.s = uniform01(r.r0) * fr[F_L];
+    ph.ex = fmaf(ph.s, fr[F_D0 + 0], fr[F_E0 + 0]); ph.ey = fmaf(ph.s, fr[F_D0 + 1], fr[F_E0 + 1]);
+    ph.ez = fmaf(ph.s, fr[F_D0 + 2], fr[F_E0 + 2]);
     // sin', cos' of phi - pi = pi (2 u2 - 1); 2 u2 - 1 is exact in fp32 (R5)
     float sp, cp;
     sincospif(fmaf(2.0f, uniform01(r.r1), -1.0f), &sp, &cp);
-    float vx, vy, vz;
     if (kind == KIND_FL_ISO) {
         // R16: cos(theta) = 1 - 2 u4, v = (cos phi sin th, sin phi sin th, -cos th); cos phi = -cos'
         const float u4 = uniform01(r.r3);
         const float cth = fmaf(-2.0f, u4, 1.0f), sth = 2.0f * sqrtf(u4 * (1.0f - u4));
-        vx = -cp * sth; vy = -sp * sth; vz = -cth;
+        ph.vx = -cp * sth; ph.vy = -sp * sth; ph.vz = -cth;
     } else {
         float sth = 1.0f, cth = 1.0f;
         if (kind == KIND_CONE) {                      // R14: 1 - cos(theta') uniform in [0, 1 - cos(alpha_b)]
             const float t = uniform01(r.r3) * (float)P.omc;
             cth = 1.0f - t; sth = sqrtf(t * (2.0f - t));
         }
-        vx = fmaf(sth, fmaf(cp, fr[F_A0 + 0], sp * fr[F_B0 + 0]), cth * fr[F_C0 + 0]);
-        vy = fmaf(sth, fmaf(cp, fr[F_A0 + 1], sp * fr[F_B0 + 1]), cth * fr[F_C0 + 1]);
-        vz = fmaf(sth, fmaf(cp, fr[F_A0 + 2], sp * fr[F_B0 + 2]), cth * fr[F_C0 + 2]);
+        ph.vx = fmaf(sth, fmaf(cp, fr[F_A0 + 0], sp * fr[F_B0 + 0]), cth * fr[F_C0 + 0]);
+        ph.vy = fmaf(sth, fmaf(cp, fr[F_A0 + 1], sp * fr[F_B0 + 1]), cth * fr[F_C0 + 1]);
+        ph.vz = fmaf(sth, fmaf(cp, fr[F_A0 + 2], sp * fr[F_B0 + 2]), cth * fr[F_C0 + 2]);
     }
-    if (!(vz < 0.0f)) return true;
-    const float rv = 1.0f / vz;
-    const float spl = -ez * rv;
-    const float gx = fmaf(spl, vx, ex), gy = fmaf(spl, vy, ey);
-    test_telescopes<COPLANAR, MODE>(P, sm, tel, e, j, S, tag, r.r2, s, ez, vx, vy, vz, rv, gx, gy);
-    return false;
+    ph.gx = ph.gy = 0.0f;
+    return ph;
+}
+
+// One accepted (photon, telescope) pair, ready for the tally / record.
+struct Hit { float x, y, vx, vy, t, lam, w; int k; bool ok; };
+
+// a4 exact test (R10) + arrival time, wavelength, weight for photon `ph` against telescope k.
+template <int TELSRC>
+__device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &sm, int e, const Photon &ph, int k)
+{
+    Hit h;
+    h.k = k; h.vx = ph.vx; h.vy = ph.vy; h.ok = false;
+    h.x = h.y = h.t = h.lam = h.w = 0.0f;
+    if (!(ph.vz < 0.0f)) return h;
+    const float4 T = tel_at<TELSRC>(P, k);
+    const float rv = 1.0f / ph.vz;
+    float s_pl;
+    if (ph.axis) {
+        // q = g - c on the plane z_ref:  b^2 = |q|^2 - (q.v)^2,  the point g is at path length -ez / v_z
+        const float qx = ph.gx - T.x, qy = ph.gy - T.y, qz = -T.z;
+        const float qv = fmaf(qx, ph.vx, fmaf(qy, ph.vy, qz * ph.vz));
+        const float b2 = fmaf(qx, qx, fmaf(qy, qy, qz * qz)) - qv * qv;
+        const float hk = ph.ez - T.z;                                      // emission height above the telescope plane
+        s_pl = -hk * rv;
+        const float s_c = (s_pl - T.z * rv) - qv;
+        if (!(b2 <= T.w) || !(hk > 0.0f) || !(s_c > 0.0f)) return h;
+        h.x = fmaf(T.z * rv, ph.vx, qx); h.y = fmaf(T.z * rv, ph.vy, qy);  // on the plane z = c_z, relative to the centre (R11)
+    } else {
+        // no plane projection (ill-conditioned for |v_z| -> 0):  b = |m x v|,  m = c - e
+        const float mx = T.x - ph.ex, my = T.y - ph.ey, mz = T.z - ph.ez;
+        const float cx = fmaf(my, ph.vz, -(mz * ph.vy)), cy = fmaf(mz, ph.vx, -(mx * ph.vz)), cz = fmaf(mx, ph.vy, -(my * ph.vx));
+        const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+        const float s_c = fmaf(mx, ph.vx, fmaf(my, ph.vy, mz * ph.vz));
+        if (!(b2 <= T.w) || !(mz < 0.0f) || !(s_c > 0.0f)) return h;
+        s_pl = mz * rv;
+        h.x = fmaf(s_pl, ph.vx, -mx); h.y = fmaf(s_pl, ph.vy, -my);
+    }
+    const float *fr = &sm.frame[e * kFrameStride];
+    const float habs = (float)P.z_ref + ph.ez;
+    // R8: arrival time = emission time + (geometric path + integral of eta dl) / c,
+    //     integral = kappa (T(c_z) - T(e_z)) / |v_z|
+    int li = 0;
+    for (int i = 1; i < P.n_layers; ++i) if (habs >= P.layerf[i].h_lo) li = i;
+    const LayerF lf = P.layerf[li];
+    const float Te = fmaf(lf.b, __expf(-habs * lf.inv_c), lf.a);
+    const float excess = P.kappa_m * (telT_at<TELSRC>(P, k) - Te) * fabsf(rv);
+    h.t = fmaf(ph.s, fr[F_IBC], fr[F_T0]) + (s_pl + excess) * (1.0f / 0.299792458f);
+    // R4: wavelength
+    const float u3 = uniform01(ph.r2);
+    h.lam = (ph.tag == 0) ? __frcp_rn(fmaf(-u3, P.dinv_lam, P.inv_lam1)) : fmaf(u3, P.fl_dlam, P.fl_lam1);
+    // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
+    h.w = fr[F_W0];
+    if (P.tau != nullptr) {
+        const int nh = P.tau_nh, nl = P.tau_nl;
+        float fh = (habs - P.tau_h0) * P.tau_inv_dh, fl = (h.lam - P.tau_l0) * P.tau_inv_dl;
+        fh = fminf(fmaxf(fh, 0.0f), (float)(nh - 1)); fl = fminf(fmaxf(fl, 0.0f), (float)(nl - 1));
+        const int ih = min(max((int)floorf(fh), 0), max(nh - 2, 0)), il = min(max((int)floorf(fl), 0), max(nl - 2, 0));
+        const float th = fh - (float)ih, tl = fl - (float)il;
+        const int ih1 = (nh > 1) ? ih + 1 : ih, il1 = (nl > 1) ? il + 1 : il;
+        const float t00 = __ldg(&P.tau[ih * nl + il]), t01 = __ldg(&P.tau[ih * nl + il1]);
+        const float t10 = __ldg(&P.tau[ih1 * nl + il]), t11 = __ldg(&P.tau[ih1 * nl + il1]);
+        const float tau = (1.0f - th) * fmaf(tl, t01 - t00, t00) + th * fmaf(tl, t11 - t10, t10);
+        h.w *= __expf(-tau * fabsf(rv));
+    }
+    h.ok = true;
+    return h;
+}
+
+// a5 for one evaluated pair held by a single lane (slow paths): plain atomics.
+__device__ __forceinline__ void commit_one(const KParams &P, TileSmem &sm, const Hit &h, uint64_t id)
+{
+    const double w = (double)h.w, wt = (double)h.w * (double)h.t;
+    if (P.n_tel <= kTelSmemMax) { atomicAdd(&sm.t_hits[h.k], 1u); atomicAdd(&sm.t_sw[h.k], w); atomicAdd(&sm.t_swt[h.k], wt); }
+    else { atomicAdd(&P.tallies[h.k].hits, 1ull); atomicAdd(&P.tallies[h.k].sum_w, w); atomicAdd(&P.tallies[h.k].sum_wt, wt); }
+    if (P.records != nullptr) {
+        const unsigned long long slot = atomicAdd(&P.cursors[h.k], 1ull);
+        if (slot < P.tel_capacity[h.k]) {
+            const unsigned long long at = P.tel_offset[h.k] + slot;
+            float *rec = P.records + at * 7ull;
+            rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
+            if (P.ids) P.ids[at] = id;
+        }
+    }
+}
+
+// a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes
+// together.  Tally: one shared-memory atomic per (warp, telescope) when all hits of the warp are on one
+// telescope, else one per lane.  Photon output: the lanes of one telescope reserve their records with a
+// single bump of that telescope's cursor.
+__device__ __forceinline__ void commit_hits(const KParams &P, TileSmem &sm, const Hit &h, uint64_t id)
+{
+    constexpr uint32_t mask = 0xffffffffu;
+    const uint32_t lane = lane_id();
+    const uint32_t okm = __ballot_sync(mask, h.ok);
+    if (okm == 0u) return;
+    const int k0 = __shfl_sync(mask, h.k, __ffs(okm) - 1);
+    const bool one_tel = __all_sync(mask, !h.ok || h.k == k0);
+    const double w = h.ok ? (double)h.w : 0.0, wt = h.ok ? (double)h.w * (double)h.t : 0.0;
+    const bool in_smem = P.n_tel <= kTelSmemMax;
+    if (one_tel) {
+        double a = w, b = wt;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(mask, a, o); b += __shfl_xor_sync(mask, b, o); }
+        if (lane == 0u) {
+            if (in_smem) { atomicAdd(&sm.t_hits[k0], (uint32_t)__popc(okm)); atomicAdd(&sm.t_sw[k0], a); atomicAdd(&sm.t_swt[k0], b); }
+            else { atomicAdd(&P.tallies[k0].hits, (unsigned long long)__popc(okm)); atomicAdd(&P.tallies[k0].sum_w, a); atomicAdd(&P.tallies[k0].sum_wt, b); }
+        }
+    } else if (h.ok) {
+        if (in_smem) { atomicAdd(&sm.t_hits[h.k], 1u); atomicAdd(&sm.t_sw[h.k], w); atomicAdd(&sm.t_swt[h.k], wt); }
+        else { atomicAdd(&P.tallies[h.k].hits, 1ull); atomicAdd(&P.tallies[h.k].sum_w, w); atomicAdd(&P.tallies[h.k].sum_wt, wt); }
+    }
+    if (P.records != nullptr) {
+        // photon-output mode: per-telescope contiguous regions, warp-aggregated cursor bump
+        const uint32_t peers = __match_any_sync(mask, h.ok ? h.k : -1 - (int)lane);
+        if (h.ok) {
+            const int leader = __ffs(peers) - 1;
+            unsigned long long base = 0;
+            if ((int)lane == leader) base = atomicAdd(&P.cursors[h.k], (unsigned long long)__popc(peers));
+            base = __shfl_sync(peers, base, leader);
+            const unsigned long long slot = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
+            if (slot < P.tel_capacity[h.k]) {
+                const unsigned long long at = P.tel_offset[h.k] + slot;
+                float *rec = P.records + at * 7ull;
+                rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
+                if (P.ids) P.ids[at] = id;
+            }
+        }
+    }
+}
+
+// ---- the per-warp candidate queue.  Entry = (emitter, photon index, telescope) in 8 bytes:
+// x = j (24 bits) | e << 24,  y = telescope index.  The warp-uniform count lives in a register.
+__device__ __forceinline__ unsigned long long emitter_segment(const KParams &P, unsigned long long tile_first, int e)
+{
+    return tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
+}
+
+template <int TELSRC>
+__device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t head, uint32_t n)
+{
+    // lanes 0 .. n-1 take one entry each; the others only take part in the warp-wide commit
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    Hit h;
+    h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
+    uint64_t id = 0;
+    if (lane < n) {
+        const uint2 q = sm.queue[warp][(head + lane) & (kQueue - 1)];
+        const int e = (int)(q.x >> 24);
+        const uint32_t j = q.x & 0xffffffu;
+        const unsigned long long S = emitter_segment(P, tile_first, e);
+        const Photon ph = make_photon(P, sm, e, j, S);
+        h = evaluate_pair<TELSRC>(P, sm, e, ph, (int)q.y);
+        id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
+    }
+    __syncwarp();
+    commit_hits(P, sm, h, id);
+}
+
+// Push the candidates of this iteration (per lane: bit c of `cm` set = candidate number c, whose telescope
+// index is tel_of(c)) and drain 32 entries whenever that many are queued.  All 32 lanes call it together.
+template <int TELSRC, typename TelOf>
+__device__ __forceinline__ void push_candidates(const KParams &P, TileSmem &sm, unsigned long long tile_first,
+                                                uint32_t &q_head, uint32_t &q_count, uint32_t cm, int e, uint32_t j, TelOf tel_of)
+{
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    while (true) {
+        const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
+        if (have == 0u) break;
+        if (cm != 0u) {
+            const int c = __ffs(cm) - 1;
+            cm &= cm - 1u;
+            const uint32_t pos = q_head + q_count + (uint32_t)__popc(have & ((1u << lane) - 1u));
+            sm.queue[warp][pos & (kQueue - 1)] = make_uint2(j | ((uint32_t)e << 24), (uint32_t)tel_of(c));
+        }
+        q_count += (uint32_t)__popc(have);
+        __syncwarp();
+        if (q_count >= 32u) {
+            drain_queue<TELSRC>(P, sm, tile_first, q_head, 32u);
+            __syncwarp();
+            q_head = (q_head + 32u) & (kQueue - 1);
+            q_count -= 32u;
+        }
+    }
+}
+
+// ---- conservative pre-tests on the crossing (gx, gy) of the plane z_ref (valid while |v_z| is not tiny).
+// Coplanar telescopes (q_z = 0): b^2 >= |q|^2 v_z^2, so |q|^2 v_z^2 (1 - 1e-4) > R^2 is a miss.
+template <bool COPLANAR>
+__device__ __forceinline__ bool plane_pretest(const float4 T, float gx, float gy, float vx, float vy, float vz, float vz2s)
+{
+    const float qx = gx - T.x, qy = gy - T.y;
+    if (COPLANAR) return fmaf(qy, qy, qx * qx) * vz2s <= T.w;
+    const float qv = fmaf(qx, vx, fmaf(qy, vy, -T.z * vz));
+    const float qq = fmaf(qx, qx, fmaf(qy, qy, T.z * T.z));
+    return qq - qv * qv <= fmaf(qq, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f));        // slack for the fp32 cancellation
+}
+
+// Candidate mask of a photon over the telescopes reachable from its plane crossing.
+//  TEL_CONST: bit k = telescope k.   TEL_GRID: bit c = slot c of the photon's grid cell (returned in *cell).
+//  Photons flatter than the grid allows, and TEL_GLOBAL, return kAllTelescopes: the caller tests all of them.
+constexpr uint32_t kAllTelescopes = 0x80000000u;
+
+template <int TELSRC, bool COPLANAR, int NT>
+__device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
+{
+    const float vz2s = vz * vz * 0.9999f;
+    uint32_t cm = 0u;
+    if constexpr (TELSRC == TEL_CONST) {
+        // NT = n_tel rounded up to 1, 4 or 8; the unused slots hold R^2 = -1 (never a candidate).  Unrolled so that the
+        // telescope coordinates are constant-bank operands.
+#pragma unroll
+        for (int k = 0; k < NT; ++k)
+            if (plane_pretest<COPLANAR>(P.tel_c[k], gx, gy, vx, vy, vz, vz2s)) cm |= 1u << k;
+        return cm;
+    } else if constexpr (TELSRC == TEL_GRID) {
+        if (!(-vz >= P.grid_vzmin)) return kAllTelescopes;
+        const float fx = (gx - P.grid_x0) * P.grid_inv_cell, fy = (gy - P.grid_y0) * P.grid_inv_cell;
+        if (!(fx >= 0.0f && fy >= 0.0f && fx < (float)P.grid_nx && fy < (float)P.grid_ny)) return 0u;
+        const uint2 c = __ldg(&P.grid[(int)fy * P.grid_nx + (int)fx]);
+        *cell = c;
+        if (c.x == 0xffffffffu) return 0u;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const uint32_t k = ((i < 2 ? c.x : c.y) >> (16 * (i & 1))) & 0xffffu;
+            if (k != 0xffffu && plane_pretest<COPLANAR>(__ldg(&P.telA[k]), gx, gy, vx, vy, vz, vz2s)) cm |= 1u << i;
+        }
+        return cm;
+    } else {
+        return kAllTelescopes;
+    }
+}
+
+// Slow path for one lane: test every telescope exactly and commit its hits on the spot (flat photons under
+// TEL_GRID, everything under TEL_GLOBAL).
+template <int TELSRC>
+__device__ __noinline__ void all_telescopes(const KParams &P, TileSmem &sm, unsigned long long tile_first, int e, uint32_t j)
+{
+    const unsigned long long S = emitter_segment(P, tile_first, e);
+    const Photon ph = make_photon(P, sm, e, j, S);
+    for (int k = 0; k < P.n_tel; ++k) {
+        const Hit h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+        if (h.ok) commit_one(P, sm, h, (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j);
+    }
+}
+
+// a2-a4 of the hot loop for the generic kinds.  Returns the candidate mask (see plane_candidates); *upward is
+// set when the photon does not go down.  Photons flatter than |v_z| = 0.05 are tested against all telescopes.
+template <int TELSRC, bool COPLANAR, int NT>
+__device__ __noinline__ uint32_t generic_candidates(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S,
+                                                    uint2 *cell, bool *upward)
+{
+    const Photon ph = make_photon(P, sm, e, j, S);
+    *upward = !(ph.vz < 0.0f);
+    if (*upward) return 0u;
+    if (ph.vz > -0.05f) return kAllTelescopes;
+    const float spl = -ph.ez / ph.vz;
+    return plane_candidates<TELSRC, COPLANAR, NT>(P, fmaf(spl, ph.vx, ph.ex), fmaf(spl, ph.vy, ph.ey), ph.vx, ph.vy, ph.vz, cell);
 }
 
 // ------------------------------------------------------------------------------------
-template <bool COPLANAR, int MODE>
+struct AxisFrame { float negL, k0c, az, bz, cz, px, py, qx, qy, gx, gy; };
+
+__device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
+{
+    const float4 *fp = reinterpret_cast<const float4 *>(&sm.frame[e * kFrameStride]);
+    const float4 A = fp[0], B = fp[1], C = fp[2];
+    return AxisFrame{A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, C.y, C.z};
+}
+
+template <int TELSRC, bool COPLANAR, int NT>
 __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_constant__ KParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -406,14 +657,10 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int segs_per_tile = kTile / (int)P.n_procs;
 
-    // ---- stage telescopes, clear tile tallies
-    const bool tel_in_smem = P.n_tel <= kTelSmemMax;
-    if (tel_in_smem) {
-        for (int k = tid; k < P.n_tel; k += kTile) {
-            sm.telA[k] = P.telA[k]; sm.telT[k] = P.telT[k];
-            sm.t_hits[k] = 0u; sm.t_sw[k] = 0.0; sm.t_swt[k] = 0.0;
-        }
-    }
+    // ---- clear the tile tallies
+    const bool tally_in_smem = P.n_tel <= kTelSmemMax;
+    if (tally_in_smem)
+        for (int k = tid; k < P.n_tel; k += kTile) { sm.t_hits[k] = 0u; sm.t_sw[k] = 0.0; sm.t_swt[k] = 0.0; }
     if (tid == 0) sm.n_upward = 0ull;
     sm.invalid[tid] = 0;
     __syncthreads();
@@ -450,82 +697,80 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     // ---- phase 2: warp `warp` walks photons [lo, hi) of the tile's concatenated index space
     const uint32_t lo = (uint32_t)(((unsigned long long)total * (unsigned)warp) / kWarps);
     const uint32_t hi = (uint32_t)(((unsigned long long)total * (unsigned)(warp + 1)) / kWarps);
-    const float4 *tel = tel_in_smem ? sm.telA : P.telA;
     const unsigned long long tile_first = P.first_id + (unsigned long long)blockIdx.x * (unsigned)segs_per_tile;
-    uint32_t n_up = 0;
+    uint32_t n_up = 0, q_head = 0, q_count = 0;
 
     if (lo < hi) {
-        // emitter of this lane's first photon: the last e with prefix[e] <= g (skips empty emitters)
+        // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
         int e;
         {
-            const uint32_t g = min(lo + (uint32_t)lane, hi - 1u);
-            int a = 0, b = kTile;                 // invariant: prefix[a] <= g < prefix[b]
-            while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g) a = m; else b = m; }
+            const uint32_t g0 = min(lo + (uint32_t)lane, hi - 1u);
+            int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
+            while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
             e = a;
         }
         uint32_t start = sm.prefix[e], end = sm.prefix[e + 1];
         int kind = sm.kind[e];
-        unsigned long long S = tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
-        float f0, f1, f2, f3, f4, f5, f6, f7, f8, f9, f10;
-        {
-            const float4 *fp = reinterpret_cast<const float4 *>(&sm.frame[e * kFrameStride]);
-            const float4 A = fp[0], B = fp[1], C = fp[2];
-            f0 = A.x; f1 = A.y; f2 = A.z; f3 = A.w; f4 = B.x; f5 = B.y; f6 = B.z; f7 = B.w; f8 = C.x; f9 = C.y; f10 = C.z;
-        }
-        for (uint32_t base = lo; base < hi; base += 32u) {
-            const uint32_t g = base + (uint32_t)lane;
-            if (g >= hi) continue;
-            if (g >= end) {
-                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
-                start = sm.prefix[e];
-                kind = sm.kind[e];
-                S = tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
-                const float4 *fp = reinterpret_cast<const float4 *>(&sm.frame[e * kFrameStride]);
-                const float4 A = fp[0], B = fp[1], C = fp[2];
-                f0 = A.x; f1 = A.y; f2 = A.z; f3 = A.w; f4 = B.x; f5 = B.y; f6 = B.z; f7 = B.w; f8 = C.x; f9 = C.y; f10 = C.z;
-            }
-            const uint32_t j = g - start;
-            if (kind == KIND_CHER_AXIS) {
-                // a2
-                const Rand4 r = philox4x32_10(j, (uint32_t)S, (uint32_t)(S >> 32), 0u, P.key0, P.key1);
-                // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
-                const float w1 = one_two(r.r0);
-                const float sd = fmaf(w1, f0, f1);                              // K0 - u1 L
-                float sp, cp;
-                __sincosf(fmaf(one_two(r.r1), 6.2831853f, -9.42477760f), &sp, &cp);   // phi - pi, in [-pi, pi)
-                const float vz = fmaf(cp, f2, fmaf(sp, f3, f4));
-                if (!(vz < 0.0f)) { ++n_up; continue; }
-                // a4: ground = G + (sd / v_z) N,  N = cos' P + sin' Q
-                const float rv = __frcp_rn(vz);
-                const float rho = sd * rv;
-                const float gx = fmaf(rho, fmaf(cp, f5, sp * f7), f9);
-                const float gy = fmaf(rho, fmaf(cp, f6, sp * f8), f10);
-                const float vz2 = vz * vz;
-                for (int k = 0; k < P.n_tel; ++k) {
-                    const float4 T = tel[k];
-                    const float qx = gx - T.x, qy = gy - T.y;
-                    bool cand;
-                    const float *fr = &sm.frame[e * kFrameStride];
-                    if (COPLANAR) {
-                        cand = fmaf(qy, qy, qx * qx) * vz2 <= T.w;
-                    } else {
-                        const float vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
-                        const float vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
-                        const float qv = fmaf(qx, vx, fmaf(qy, vy, -T.z * vz));
-                        cand = fmaf(qx, qx, fmaf(qy, qy, T.z * T.z)) - qv * qv <= T.w * 1.0001f + 1e-3f;
-                    }
-                    if (cand) {
-                        const float vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
-                        const float vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
-                        const float s = (w1 - kOneMinus) * fr[F_LEN];
-                        const float ez = -sd * fr[F_DZ];
-                        candidate<MODE>(P, sm, k, e, j, S, 0, r.r2, s, ez, vx, vy, vz, rv, gx, gy);
-                    }
+        unsigned long long S = emitter_segment(P, tile_first, e);
+        PhiloxEmitter pe = philox_emitter(P, S);
+        AxisFrame f = load_axis_frame(sm, e);
+        uint32_t g = lo + (uint32_t)lane;
+        for (uint32_t left = hi - lo; ; g += 32u) {
+            // `left` = photons of the warp still to do (warp-uniform); the lanes >= left idle in the last round
+            const bool active = (uint32_t)lane < left;
+            uint32_t cm = 0u;
+            uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
+            uint32_t j = 0u;
+            if (active) {
+                if (g >= end) {
+                    do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+                    start = sm.prefix[e];
+                    kind = sm.kind[e];
+                    S = emitter_segment(P, tile_first, e);
+                    pe = philox_emitter(P, S);
+                    f = load_axis_frame(sm, e);
                 }
-            } else {
-                if (generic_photon<COPLANAR, MODE>(P, sm, tel, kind, e, j, S)) ++n_up;
+                j = g - start;
+                if (kind == KIND_CHER_AXIS) {
+                    const Rand4 r = philox_photon(P, pe, j, 0u);                                  // a2
+                    // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
+                    const float sd = fmaf(one_two(r.r0), f.negL, f.k0c);                          // K0 - u1 L
+                    float sp, cp;
+                    __sincosf(fmaf(one_two(r.r1), 6.2831853f, -9.42477760f), &sp, &cp);           // phi - pi, in [-pi, pi)
+                    const float vz = fmaf(cp, f.az, fmaf(sp, f.bz, f.cz));
+                    if (vz < 0.0f) {
+                        // a4: ground = G + (sd / v_z) N,  N = cos' P + sin' Q
+                        const float rho = sd * rcp_approx(vz);
+                        const float gx = fmaf(rho, fmaf(cp, f.px, sp * f.qx), f.gx);
+                        const float gy = fmaf(rho, fmaf(cp, f.py, sp * f.qy), f.gy);
+                        float vx = 0.0f, vy = 0.0f;
+                        if (!COPLANAR) {
+                            const float *fr = &sm.frame[e * kFrameStride];
+                            vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
+                            vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
+                        }
+                        cm = plane_candidates<TELSRC, COPLANAR, NT>(P, gx, gy, vx, vy, vz, &cell);
+                    } else {
+                        ++n_up;
+                    }
+                } else {
+                    bool up;
+                    cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, S, &cell, &up);
+                    if (up) ++n_up;
+                }
+                if (cm == kAllTelescopes) { all_telescopes<TELSRC>(P, sm, tile_first, e, j); cm = 0u; }
             }
+            if (__any_sync(0xffffffffu, cm != 0u)) {
+                if constexpr (TELSRC == TEL_GRID)
+                    push_candidates<TELSRC>(P, sm, tile_first, q_head, q_count, cm, e, j,
+                                            [&](int c) { return ((c < 2 ? cell.x : cell.y) >> (16 * (c & 1))) & 0xffffu; });
+                else
+                    push_candidates<TELSRC>(P, sm, tile_first, q_head, q_count, cm, e, j, [](int c) { return (uint32_t)c; });
+            }
+            if (left <= 32u) break;
+            left -= 32u;
         }
+        if (q_count) drain_queue<TELSRC>(P, sm, tile_first, q_head, q_count);
     }
 
     // ---- tile epilogue: counters and tallies
@@ -543,7 +788,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         nbad = __reduce_add_sync(0xffffffffu, nbad);
         if (lane == 0 && nbad) atomicAdd(&P.counters[6], (unsigned long long)nbad);
     }
-    if (tel_in_smem) {
+    if (tally_in_smem) {
         for (int k = tid; k < P.n_tel; k += kTile) {
             const uint32_t h = sm.t_hits[k];
             if (h) {

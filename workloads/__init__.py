@@ -244,24 +244,27 @@ def default_params(**kw) -> dict:
     return p
 
 
-def make_config(name: str, n_segments: int | None = None) -> dict:
+def make_config(name: str, n_segments: int | None = None, seed_offset: int = 0) -> dict:
     """Return dict(segments, telescopes, atmosphere, params, name) for
     'c1', 'c2', 'c3a', 'c3b', 'c4', 'c5', 'c5g' (BASELINE.json configs[0..4];
-    'c5g' is the accept-all variant SURVEY.md §8(d) adds)."""
+    'c5g' is the accept-all variant SURVEY.md §8(d) adds).  seed_offset != 0
+    draws a different, equally distributed segment set (one per rank when the
+    job is sharded); the Philox seed of the run is left unchanged."""
+    so = 7919 * int(seed_offset)
     if name == "c1":
         atm = atmosphere_single_layer()
-        seg = segments_config1(n_segments or 10_000, seed=1)
+        seg = segments_config1(n_segments or 10_000, seed=1 + so)
         tel = telescopes_single()
         par = default_params(seed=1)
     elif name in ("c2", "c5", "c5g"):
         atm = atmosphere_five_layer()
         n = n_segments or (1_000_000 if name == "c2" else 10_000_000)
-        seg = segments_shower(n, seed=2, atm=atm, xmax=350.0, lateral=(30.0,))
+        seg = segments_shower(n, seed=2 + so, atm=atm, xmax=350.0, lateral=(30.0,))
         tel = telescope_accept_all() if name == "c5g" else telescopes_square()
         par = default_params(seed=2, mode=MODE_TALLY if name == "c2" else MODE_OUTPUT)
     elif name in ("c3a", "c3b"):
         atm = atmosphere_five_layer()
-        seg = segments_shower(n_segments or 1_000_000, seed=3, atm=atm, xmax=700.0, lateral=(30.0,),
+        seg = segments_shower(n_segments or 1_000_000, seed=3 + so, atm=atm, xmax=700.0, lateral=(30.0,),
                               muon_fraction=0.0)
         seg["charge"] = -1.0
         tel = telescopes_far()
@@ -270,7 +273,7 @@ def make_config(name: str, n_segments: int | None = None) -> dict:
     elif name == "c4":
         tau = transmission_table(seed=4)
         atm = atmosphere_five_layer(tau=tau)
-        seg = segments_shower(n_segments or 10_000_000, seed=4, atm=atm, xmax=500.0, lateral=(20.0, 200.0))
+        seg = segments_shower(n_segments or 10_000_000, seed=4 + so, atm=atm, xmax=500.0, lateral=(20.0, 200.0))
         tel = telescopes_grid()
         par = default_params(seed=4, processes=PROC_CHERENKOV | PROC_FLUORESCENCE)
     else:
