@@ -40,8 +40,8 @@ struct c8opt_ctx {
     // ground-plane candidate grid (n_tel > kTelConstMax)
     int tel_src = c8::TEL_CONST;
     uint2 *d_grid = nullptr;
-    int grid_nx = 0, grid_ny = 0;
-    float grid_x0 = 0, grid_y0 = 0, grid_inv_cell = 0, grid_vzmin = 0;
+    int n_grid_levels = 0;
+    c8::GridLevel grid_lvl[c8::kGridLevels] = {};
     // results
     c8::Tally *d_tallies = nullptr;
     unsigned long long *d_counters = nullptr;   // [8]
@@ -110,11 +110,11 @@ kernel_t pick_kernel(int tel_src, bool coplanar, int nt)
 
 // Ground-plane candidate grid: a photon with |v_z| >= vzmin that hits telescope k crosses the
 // plane z_ref within rho_k = R / vzmin + |c_z - z_ref| sqrt(1 / vzmin^2 - 1) of (c_x, c_y).  Every cell lists the
-// telescopes whose disc (bounding square, plus slack for fp32 rounding) touches it; at most 4 per cell, else the
-// resolution is doubled, and if that does not help the grid is not used (brute force from global memory).
-bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
+// telescopes whose disc (plus slack for fp32 rounding) touches it; at most 4 per cell, else the resolution is
+// doubled, and if that does not help this level is not built.  The cells are appended to *cells.
+bool build_grid_level(c8opt_ctx *ctx, double vzmin, std::vector<uint2> *cells, c8::GridLevel *lvl)
 {
-    const double vzmin = 0.5, slack = 0.05;
+    const double slack = 0.05;
     const int n = ctx->n_tel_pending;
     std::vector<double> rho(n);
     double x_lo = INFINITY, x_hi = -INFINITY, y_lo = INFINITY, y_hi = -INFINITY, rho_max = 0;
@@ -136,12 +136,15 @@ bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
         std::vector<uint16_t> list((size_t)nx * ny * 4, 0xffffu);
         bool ok = true;
         for (int k = 0; k < n && ok; ++k) {
-            const int ix0 = std::max(0, (int)std::floor((ctx->h_telA[k].x - rho[k] - x_lo) / cell));
-            const int ix1 = std::min(nx - 1, (int)std::floor((ctx->h_telA[k].x + rho[k] - x_lo) / cell));
-            const int iy0 = std::max(0, (int)std::floor((ctx->h_telA[k].y - rho[k] - y_lo) / cell));
-            const int iy1 = std::min(ny - 1, (int)std::floor((ctx->h_telA[k].y + rho[k] - y_lo) / cell));
+            const double cx = ctx->h_telA[k].x - x_lo, cy = ctx->h_telA[k].y - y_lo;
+            const int ix0 = std::max(0, (int)std::floor((cx - rho[k]) / cell)), ix1 = std::min(nx - 1, (int)std::floor((cx + rho[k]) / cell));
+            const int iy0 = std::max(0, (int)std::floor((cy - rho[k]) / cell)), iy1 = std::min(ny - 1, (int)std::floor((cy + rho[k]) / cell));
             for (int iy = iy0; iy <= iy1 && ok; ++iy)
                 for (int ix = ix0; ix <= ix1; ++ix) {
+                    // distance from the disc centre to the cell rectangle (grown by 1e-3 cell against rounding of the lookup)
+                    const double gx0 = (ix - 1e-3) * cell, gx1 = (ix + 1 + 1e-3) * cell, gy0 = (iy - 1e-3) * cell, gy1 = (iy + 1 + 1e-3) * cell;
+                    const double ddx = std::fmax(0.0, std::fmax(gx0 - cx, cx - gx1)), ddy = std::fmax(0.0, std::fmax(gy0 - cy, cy - gy1));
+                    if (ddx * ddx + ddy * ddy > rho[k] * rho[k]) continue;
                     uint16_t *c = &list[((size_t)iy * nx + ix) * 4];
                     int slot = 0;
                     while (slot < 4 && c[slot] != 0xffffu) ++slot;
@@ -150,16 +153,29 @@ bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
                 }
         }
         if (!ok) continue;
-        cells->resize((size_t)nx * ny);
-        for (size_t i = 0; i < cells->size(); ++i)
-            (*cells)[i] = make_uint2((uint32_t)list[4 * i] | ((uint32_t)list[4 * i + 1] << 16),
-                                     (uint32_t)list[4 * i + 2] | ((uint32_t)list[4 * i + 3] << 16));
-        ctx->grid_nx = nx; ctx->grid_ny = ny;
-        ctx->grid_x0 = (float)x_lo; ctx->grid_y0 = (float)y_lo;
-        ctx->grid_inv_cell = (float)(1.0 / cell); ctx->grid_vzmin = (float)vzmin;
+        const size_t base = cells->size();
+        cells->resize(base + (size_t)nx * ny);
+        for (size_t i = 0; i < (size_t)nx * ny; ++i)
+            (*cells)[base + i] = make_uint2((uint32_t)list[4 * i] | ((uint32_t)list[4 * i + 1] << 16),
+                                            (uint32_t)list[4 * i + 2] | ((uint32_t)list[4 * i + 3] << 16));
+        lvl->nx = nx; lvl->ny = ny; lvl->base = (int)base;
+        lvl->x0 = (float)x_lo; lvl->y0 = (float)y_lo; lvl->inv_cell = (float)(1.0 / cell); lvl->vzmin = (float)vzmin;
         return true;
     }
     return false;
+}
+
+// Level 0 serves |v_z| >= 0.5 (Cherenkov light of a shower), level 1 the flatter photons down to |v_z| = 0.1
+// (isotropic fluorescence); what is flatter still, or has no grid, takes the kernel's wide test.
+bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
+{
+    const double vzmin[c8::kGridLevels] = {0.5, 0.1};
+    ctx->n_grid_levels = 0;
+    for (int l = 0; l < c8::kGridLevels; ++l) {
+        if (!build_grid_level(ctx, vzmin[l], cells, &ctx->grid_lvl[l])) break;
+        ctx->n_grid_levels = l + 1;
+    }
+    return ctx->n_grid_levels > 0;
 }
 
 // Validate params / outputs and fill the kernel parameter block (everything except seg / n / first_id).
@@ -201,8 +217,8 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
         for (int k = 0; k < c8::kTelConstMax; ++k) { P.tel_c[k] = make_float4(0.f, 0.f, 0.f, -1.f); P.telT_c[k] = 0.f; }   // R^2 = -1: never hit
         for (int k = 0; k < ctx->n_tel; ++k) { P.tel_c[k] = ctx->h_telA[k]; P.telT_c[k] = ctx->h_telT[k]; }
     }
-    P.grid = ctx->d_grid; P.grid_nx = ctx->grid_nx; P.grid_ny = ctx->grid_ny;
-    P.grid_x0 = ctx->grid_x0; P.grid_y0 = ctx->grid_y0; P.grid_inv_cell = ctx->grid_inv_cell; P.grid_vzmin = ctx->grid_vzmin;
+    P.grid = ctx->d_grid; P.n_grid_levels = ctx->n_grid_levels;
+    for (int l = 0; l < c8::kGridLevels; ++l) P.grid_lvl[l] = ctx->grid_lvl[l];
     P.x_ref = ctx->x_ref; P.y_ref = ctx->y_ref; P.z_ref = ctx->z_ref;
     for (int r = 0; r < 10; ++r) {
         P.rk0[r] = (uint32_t)rp->seed + (uint32_t)r * 0x9E3779B9u;

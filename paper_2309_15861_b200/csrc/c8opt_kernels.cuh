@@ -42,6 +42,9 @@ constexpr int KIND_CHER_GEN = 3;      // Cherenkov, generic projection (near-hor
 struct LayerD { double h_lo, a, b, c; };
 struct LayerF { float h_lo, a, b, inv_c; };
 
+struct GridLevel { int nx, ny, base; float x0, y0, inv_cell, vzmin; };
+constexpr int kGridLevels = 2;
+
 struct Tally { unsigned long long hits; double sum_w; double sum_wt; };
 
 // Everything the kernel needs, passed by value (constant bank).
@@ -62,10 +65,11 @@ struct KParams {
     float4 tel_c[kTelConstMax];    // the same two tables in the constant bank when n_tel <= kTelConstMax
     float telT_c[kTelConstMax];
     double x_ref, y_ref, z_ref;
-    // ground-plane candidate grid (n_tel > kTelConstMax): cell -> up to 4 telescope indices (0xffff = none)
+    // ground-plane candidate grids (n_tel > kTelConstMax): cell -> up to 4 telescope indices (0xffff = none).
+    // Level l serves photons with |v_z| >= grid_lvl[l].vzmin (level 0 the steep ones); n_grid_levels of them exist.
     const uint2 *grid;
-    int grid_nx, grid_ny;
-    float grid_x0, grid_y0, grid_inv_cell, grid_vzmin;
+    int n_grid_levels;
+    GridLevel grid_lvl[kGridLevels];
     // run
     uint32_t rk0[10], rk1[10];     // Philox round keys: key + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t processes, n_procs;
@@ -448,23 +452,6 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     return h;
 }
 
-// a5 for one evaluated pair held by a single lane (slow paths): plain atomics.
-__device__ __forceinline__ void commit_one(const KParams &P, TileSmem &sm, const Hit &h, uint64_t id)
-{
-    const double w = (double)h.w, wt = (double)h.w * (double)h.t;
-    if (P.n_tel <= kTelSmemMax) { atomicAdd(&sm.t_hits[h.k], 1u); atomicAdd(&sm.t_sw[h.k], w); atomicAdd(&sm.t_swt[h.k], wt); }
-    else { atomicAdd(&P.tallies[h.k].hits, 1ull); atomicAdd(&P.tallies[h.k].sum_w, w); atomicAdd(&P.tallies[h.k].sum_wt, wt); }
-    if (P.records != nullptr) {
-        const unsigned long long slot = atomicAdd(&P.cursors[h.k], 1ull);
-        if (slot < P.tel_capacity[h.k]) {
-            const unsigned long long at = P.tel_offset[h.k] + slot;
-            float *rec = P.records + at * 7ull;
-            rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
-            if (P.ids) P.ids[at] = id;
-        }
-    }
-}
-
 // a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes
 // together.  Tally: one shared-memory atomic per (warp, telescope) when all hits of the warp are on one
 // telescope, else one per lane.  Photon output: the lanes of one telescope reserve their records with a
@@ -595,10 +582,16 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
             if (plane_pretest<COPLANAR>(P.tel_c[k], gx, gy, vx, vy, vz, vz2s)) cm |= 1u << k;
         return cm;
     } else if constexpr (TELSRC == TEL_GRID) {
-        if (!(-vz >= P.grid_vzmin)) return kAllTelescopes;
-        const float fx = (gx - P.grid_x0) * P.grid_inv_cell, fy = (gy - P.grid_y0) * P.grid_inv_cell;
-        if (!(fx >= 0.0f && fy >= 0.0f && fx < (float)P.grid_nx && fy < (float)P.grid_ny)) return 0u;
-        const uint2 c = __ldg(&P.grid[(int)fy * P.grid_nx + (int)fx]);
+        // steep photons use level 0; flatter ones the coarser level 1 when it exists, else the wide test
+        int lvl = 0;
+        if (!(-vz >= P.grid_lvl[0].vzmin)) {
+            if (P.n_grid_levels < 2 || !(-vz >= P.grid_lvl[1].vzmin)) return kAllTelescopes;
+            lvl = 1;
+        }
+        const GridLevel &G = P.grid_lvl[lvl];
+        const float fx = (gx - G.x0) * G.inv_cell, fy = (gy - G.y0) * G.inv_cell;
+        if (!(fx >= 0.0f && fy >= 0.0f && fx < (float)G.nx && fy < (float)G.ny)) return 0u;
+        const uint2 c = __ldg(&P.grid[G.base + (int)fy * G.nx + (int)fx]);
         *cell = c;
         if (c.x == 0xffffffffu) return 0u;
 #pragma unroll
@@ -612,16 +605,41 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
     }
 }
 
-// Slow path for one lane: test every telescope exactly and commit its hits on the spot (flat photons under
-// TEL_GRID, everything under TEL_GLOBAL).
+// Wide test (photons flatter than the grids allow under TEL_GRID, every photon under TEL_GLOBAL).  `wide` = ballot of
+// the lanes holding such a photon.  One photon at a time: its (emitter, index) is broadcast, every lane rebuilds it
+// from the counter and tests the telescopes lane, lane + 32, ... with a conservative distance test (cross product,
+// no plane projection: valid for any v_z); the survivors go through the candidate queue like all others.
 template <int TELSRC>
-__device__ __noinline__ void all_telescopes(const KParams &P, TileSmem &sm, unsigned long long tile_first, int e, uint32_t j)
+__device__ __noinline__ void wide_test(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
+                                       uint32_t &q_count, uint32_t wide, int e, uint32_t j)
 {
-    const unsigned long long S = emitter_segment(P, tile_first, e);
-    const Photon ph = make_photon(P, sm, e, j, S);
-    for (int k = 0; k < P.n_tel; ++k) {
-        const Hit h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
-        if (h.ok) commit_one(P, sm, h, (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j);
+    const int lane = (int)lane_id();
+    while (wide) {
+        const int src = __ffs(wide) - 1;
+        wide &= wide - 1u;
+        const int eb = __shfl_sync(0xffffffffu, e, src);
+        const uint32_t jb = __shfl_sync(0xffffffffu, j, src);
+        const Photon ph = make_photon(P, sm, eb, jb, emitter_segment(P, tile_first, eb));
+        if (!(ph.vz < 0.0f)) continue;                                   // warp-uniform
+        // a point of the ray relative to (x_ref, y_ref, z_ref): the plane crossing (axis kind) or the emission point
+        const float px = ph.axis ? ph.gx : ph.ex, py = ph.axis ? ph.gy : ph.ey, pz = ph.axis ? 0.0f : ph.ez;
+        for (int k0 = 0; k0 < P.n_tel; k0 += 1024) {
+            uint32_t cm = 0u;
+            for (int c = 0; c < 32; ++c) {
+                const int k = k0 + c * 32 + lane;
+                if (k0 + c * 32 >= P.n_tel) break;                       // warp-uniform
+                if (k < P.n_tel) {
+                    const float4 T = __ldg(&P.telA[k]);
+                    const float mx = T.x - px, my = T.y - py, mz = T.z - pz;
+                    const float cx = fmaf(my, ph.vz, -(mz * ph.vy)), cy = fmaf(mz, ph.vx, -(mx * ph.vz)), cz = fmaf(mx, ph.vy, -(my * ph.vx));
+                    const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+                    const float mm = fmaf(mx, mx, fmaf(my, my, mz * mz));
+                    if (b2 <= fmaf(mm, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f))) cm |= 1u << c;
+                }
+            }
+            if (__any_sync(0xffffffffu, cm != 0u))
+                push_candidates<TELSRC>(P, sm, tile_first, q_head, q_count, cm, eb, jb, [&](int c) { return (uint32_t)(k0 + c * 32 + lane); });
+        }
     }
 }
 
@@ -758,7 +776,15 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
                     cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, S, &cell, &up);
                     if (up) ++n_up;
                 }
-                if (cm == kAllTelescopes) { all_telescopes<TELSRC>(P, sm, tile_first, e, j); cm = 0u; }
+            }
+            if constexpr (TELSRC == TEL_CONST) {
+                if (cm == kAllTelescopes) cm = (1u << NT) - 1u;          // flat photon: all slots go to the exact test
+            } else {
+                const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
+                if (wide) {
+                    wide_test<TELSRC>(P, sm, tile_first, q_head, q_count, wide, e, j);
+                    if (cm == kAllTelescopes) cm = 0u;
+                }
             }
             if (__any_sync(0xffffffffu, cm != 0u)) {
                 if constexpr (TELSRC == TEL_GRID)
