@@ -85,27 +85,28 @@ double host_depth(const c8opt_ctx *c, double h)
     return c->layer[i].a + c->layer[i].b * std::exp(-h / c->layer[i].c);
 }
 
-size_t smem_bytes() { return sizeof(c8::TileSmem); }
+size_t smem_bytes(bool out) { return sizeof(c8::TileSmem) + (out ? sizeof(c8::OutSmem) : 0); }
 
 typedef void (*kernel_t)(const c8::KParams);
 
-template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar)
+template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar, bool out)
 {
-    return coplanar ? c8::propagate_kernel<TELSRC, true, NT> : c8::propagate_kernel<TELSRC, false, NT>;
+    if (out) return coplanar ? c8::propagate_kernel<TELSRC, true, NT, true> : c8::propagate_kernel<TELSRC, false, NT, true>;
+    return coplanar ? c8::propagate_kernel<TELSRC, true, NT, false> : c8::propagate_kernel<TELSRC, false, NT, false>;
 }
 
 // nt = number of constant-bank telescope slots the hot loop tests (n_tel rounded up to 1, 4 or 8)
 int padded_count(int n_tel) { return n_tel <= 1 ? 1 : (n_tel <= 4 ? 4 : 8); }
 
-kernel_t pick_kernel(int tel_src, bool coplanar, int nt)
+kernel_t pick_kernel(int tel_src, bool coplanar, int nt, bool out)
 {
     if (tel_src == c8::TEL_CONST) {
-        if (nt == 1) return pick_kernel2<c8::TEL_CONST, 1>(coplanar);
-        if (nt == 4) return pick_kernel2<c8::TEL_CONST, 4>(coplanar);
-        return pick_kernel2<c8::TEL_CONST, 8>(coplanar);
+        if (nt == 1) return pick_kernel2<c8::TEL_CONST, 1>(coplanar, out);
+        if (nt == 4) return pick_kernel2<c8::TEL_CONST, 4>(coplanar, out);
+        return pick_kernel2<c8::TEL_CONST, 8>(coplanar, out);
     }
-    if (tel_src == c8::TEL_GRID) return pick_kernel2<c8::TEL_GRID, 0>(coplanar);
-    return pick_kernel2<c8::TEL_GLOBAL, 0>(coplanar);
+    if (tel_src == c8::TEL_GRID) return pick_kernel2<c8::TEL_GRID, 0>(coplanar, out);
+    return pick_kernel2<c8::TEL_GLOBAL, 0>(coplanar, out);
 }
 
 // Ground-plane candidate grid: a photon with |v_z| >= vzmin that hits telescope k crosses the
@@ -219,7 +220,8 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     }
     P.grid = ctx->d_grid; P.n_grid_levels = ctx->n_grid_levels;
     for (int l = 0; l < c8::kGridLevels; ++l) P.grid_lvl[l] = ctx->grid_lvl[l];
-    P.x_ref = ctx->x_ref; P.y_ref = ctx->y_ref; P.z_ref = ctx->z_ref;
+    P.x_ref = ctx->x_ref; P.y_ref = ctx->y_ref; P.z_ref = ctx->z_ref; P.z_ref_f = (float)ctx->z_ref;
+    for (int i = ctx->n_layers; i < c8::kMaxLayers; ++i) P.layerf[i].h_lo = INFINITY;   // never selected by the layer count
     for (int r = 0; r < 10; ++r) {
         P.rk0[r] = (uint32_t)rp->seed + (uint32_t)r * 0x9E3779B9u;
         P.rk1[r] = (uint32_t)(rp->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
@@ -261,8 +263,9 @@ int launch(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, const c8opt_segment *d
     const unsigned long long per_tile = c8::kTile / P.n_procs;
     const unsigned long long tiles = (n + per_tile - 1) / per_tile;
     if (tiles > 0x7fffffffull) return fail(ctx, C8OPT_ERR_ARGUMENT, "too many segments in one call");
-    kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel));
-    k<<<(unsigned)tiles, c8::kTile, smem_bytes(), st>>>(P);
+    const bool out = P.records != nullptr;
+    kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out);
+    k<<<(unsigned)tiles, c8::kTile, smem_bytes(out), st>>>(P);
     C8_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
     ctx->segments_total += n;
@@ -331,8 +334,9 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
     if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, 8 * sizeof(unsigned long long));
     for (int ts = 0; ts < 3 && e == cudaSuccess; ++ts)
         for (int nt = 1; nt <= 8 && e == cudaSuccess; nt *= (nt == 1 ? 4 : 2))
-            for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
-                e = cudaFuncSetAttribute(pick_kernel(ts, cp != 0, nt), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes());
+            for (int cp = 0; cp < 4 && e == cudaSuccess; ++cp)
+                e = cudaFuncSetAttribute(pick_kernel(ts, (cp & 1) != 0, nt, (cp & 2) != 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)smem_bytes((cp & 2) != 0));
     if (e != cudaSuccess) {
         fail(nullptr, C8OPT_ERR_CUDA, "context setup: %s", cudaGetErrorString(e));
         c8opt_destroy(ctx);

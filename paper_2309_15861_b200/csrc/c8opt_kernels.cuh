@@ -32,6 +32,10 @@ constexpr int TEL_CONST = 0;          // brute force over <= kTelConstMax telesc
 constexpr int TEL_GRID = 1;           // candidate lookup in the ground-plane grid
 constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global memory (grid not buildable)
 constexpr int kMaxLayers = 8;
+constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
+constexpr int kRound = 2;             // photon output: warp iterations per round (one cursor bump per tile and round)
+constexpr int kStageRecs = kRound * 32;           // records a warp can stage per round
+constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
@@ -65,6 +69,7 @@ struct KParams {
     float4 tel_c[kTelConstMax];    // the same two tables in the constant bank when n_tel <= kTelConstMax
     float telT_c[kTelConstMax];
     double x_ref, y_ref, z_ref;
+    float z_ref_f;                 // (float)z_ref
     // ground-plane candidate grids (n_tel > kTelConstMax): cell -> up to 4 telescope indices (0xffff = none).
     // Level l serves photons with |v_z| >= grid_lvl[l].vzmin (level 0 the steep ones); n_grid_levels of them exist.
     const uint2 *grid;
@@ -149,7 +154,7 @@ __device__ __forceinline__ float uniform01(uint32_t r) { return one_two(r) - kOn
 
 // ------------------------------------------------------------------------------------
 // shared-memory layout of one tile
-struct TileSmem {
+struct __align__(16) TileSmem {
     uint32_t prefix[kTile + 8];                 // exclusive scan of n_b; prefix[kTile] = total
     float frame[kTile * kFrameStride];          // fp32 frames, see frame slots below
     uint8_t kind[kTile];
@@ -159,7 +164,31 @@ struct TileSmem {
     double t_sw[kTelSmemMax], t_swt[kTelSmemMax];
     unsigned long long n_upward;
     uint2 queue[kWarps][kQueue];                // per-warp ring of candidate (photon, telescope) pairs
+    // per-thread tally accumulators (flushed into t_* when the telescope changes and at the end of the tile)
+    double acc_w[kTile], acc_wt[kTile];
+    uint32_t acc_n[kTile];
+    int acc_k[kTile];
 };
+
+// Photon-output kernels only (follows TileSmem in dynamic shared memory).  Records are staged per warp and leave the
+// tile once per round: the cursor of a telescope is bumped once per (tile, round, run of warps on that telescope)
+// instead of once per warp iteration, because same-address atomics serialise in L2 (~1 per clock).
+struct OutSmem {
+    __align__(16) float stage[kWarps][kStageRecs * kRecWords];
+    unsigned long long ids[kWarps][kStageRecs];
+    unsigned long long wbase[kWarps];            // first record slot of warp w's run in its telescope's region
+    int wk[kWarps];                              // telescope of the records warp w has staged this round
+    uint32_t wn[kWarps];                         // how many
+    int rounds;                                  // 1 while the tile runs in rounds (it saw staged records in round 0)
+    int staged_any;
+};
+
+template <bool OUT> __device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
+{
+    static_assert(OUT, "only photon-output kernels carry the staging area");
+    static_assert(sizeof(TileSmem) % 16 == 0, "OutSmem must stay 16-byte aligned");
+    return *reinterpret_cast<OutSmem *>(&sm + 1);
+}
 
 // frame slots.  Axis-relative Cherenkov (KIND_CHER_AXIS):
 //   F_NEGL   -L                      F_K0C  K0 + (1-2^-24) L,  K0 = -(z0 - z_ref)/d_z  (axis path length to the plane)
@@ -169,12 +198,13 @@ struct TileSmem {
 // Generic kinds: F_E0..2 start point relative to (x_ref, y_ref, z_ref), F_D0..2 direction, F_L,
 //   F_A0..C2 (7..15): v = sth (cos' A + sin' B) + cth C.
 // Hit-only slots (all kinds): F_W0 weight, F_T0 start time, F_IBC 1/(beta c), and for the axis kind
-//   F_DZ, F_AX..F_CY (v_x, v_y coefficients), F_LEN.
+//   F_DZ, F_AX..F_CY (v_x, v_y coefficients), F_LEN; F_LAYER = bits of the int index of the atmosphere layer that
+//   holds the whole segment, -1 if it crosses a layer boundary.
 enum {
     F_NEGL = 0, F_K0C = 1, F_AZ = 2, F_BZ = 3, F_CZ = 4, F_PX = 5, F_PY = 6, F_QX = 7, F_QY = 8, F_GX = 9, F_GY = 10,
     F_E0 = 0, F_D0 = 3, F_L = 6, F_A0 = 7, F_B0 = 10, F_C0 = 13,
     F_W0 = 16, F_T0 = 17, F_IBC = 18, F_DZ = 19, F_AX = 20, F_AY = 21, F_BX = 22, F_BY = 23, F_CX = 24, F_CY = 25,
-    F_LEN = 26
+    F_LEN = 26, F_LAYER = 27
 };
 
 // ------------------------------------------------------------------------------------
@@ -275,6 +305,14 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     if (kind == KIND_CONE) w0 *= 0.5 * P.omc;                    // R14: Omega / 4 pi
 
     fr[F_W0] = (float)w0; fr[F_T0] = s0.w; fr[F_IBC] = (float)ibc; fr[F_LEN] = (float)L;
+    {
+        // layer of both ends in fp32 altitudes as the photon loop sees them (1 m of margin against rounding)
+        const float za = (float)p0[2], zb = (float)(p0[2] + L * d[2]);
+        const float zlo = fminf(za, zb) - 1.0f, zhi = fmaxf(za, zb) + 1.0f;
+        int la = 0, lb = 0;
+        for (int i = 1; i < P.n_layers; ++i) { if (zlo >= P.layerf[i].h_lo) la = i; if (zhi >= P.layerf[i].h_lo) lb = i; }
+        fr[F_LAYER] = __int_as_float(la == lb ? la : -1);
+    }
     *kind_out = (uint8_t)kind;
     const double e0[3] = { p0[0] - P.x_ref, p0[1] - P.y_ref, p0[2] - P.z_ref };
     if (kind == KIND_FL_ISO) {
@@ -332,19 +370,25 @@ __device__ __forceinline__ float rcp_approx(float x)
     return r;
 }
 
+// 1/x to within 1 ulp for normal x: MUFU.RCP + one Newton step (3 instructions instead of the IEEE division's ~10)
+__device__ __forceinline__ float rcp_refined(float x)
+{
+    const float r = rcp_approx(x);
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
+
 // A photon ready for the exact test: emission point e relative to (x_ref, y_ref, z_ref) or, for the
 // axis kind, the crossing (gx, gy) of the plane z_ref; unit direction v; s = distance along the track.
 struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s; uint32_t r2; int tag; bool axis; };
 
-// a2 + a3 for photon j of emitter e, any kind (used by the queue drain and by the generic kinds' hot path).
-__device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S)
+// a3 for a photon of emitter e, any kind, from its four random words.
+__device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileSmem &sm, int e, const Rand4 r)
 {
     const float *fr = &sm.frame[e * kFrameStride];
     const int kind = sm.kind[e];
     Photon ph;
     ph.tag = (kind == KIND_CHER_AXIS || kind == KIND_CHER_GEN) ? 0 : 1;
     ph.axis = (kind == KIND_CHER_AXIS);
-    const Rand4 r = philox4x32_10(P, j, (uint32_t)S, (uint32_t)(S >> 32), (uint32_t)ph.tag);
     ph.r2 = r.r2;
     if (kind == KIND_CHER_AXIS) {
         const float w1 = one_two(r.r0);
@@ -387,6 +431,14 @@ __device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &
     return ph;
 }
 
+__device__ __forceinline__ uint32_t kind_tag(int kind) { return (kind == KIND_CHER_AXIS || kind == KIND_CHER_GEN) ? 0u : 1u; }
+
+// a2 + a3 for photon j of emitter e, any kind (used by the queue drain, the wide test and the generic kinds' hot path).
+__device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S)
+{
+    return photon_from_rand(P, sm, e, philox4x32_10(P, j, (uint32_t)S, (uint32_t)(S >> 32), kind_tag(sm.kind[e])));
+}
+
 // One accepted (photon, telescope) pair, ready for the tally / record.
 struct Hit { float x, y, vx, vy, t, lam, w; int k; bool ok; };
 
@@ -399,7 +451,7 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     h.x = h.y = h.t = h.lam = h.w = 0.0f;
     if (!(ph.vz < 0.0f)) return h;
     const float4 T = tel_at<TELSRC>(P, k);
-    const float rv = 1.0f / ph.vz;
+    const float rv = rcp_refined(ph.vz);
     float s_pl;
     if (ph.axis) {
         // q = g - c on the plane z_ref:  b^2 = |q|^2 - (q.v)^2,  the point g is at path length -ez / v_z
@@ -422,18 +474,24 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
         h.x = fmaf(s_pl, ph.vx, -mx); h.y = fmaf(s_pl, ph.vy, -my);
     }
     const float *fr = &sm.frame[e * kFrameStride];
-    const float habs = (float)P.z_ref + ph.ez;
+    const float habs = P.z_ref_f + ph.ez;
     // R8: arrival time = emission time + (geometric path + integral of eta dl) / c,
     //     integral = kappa (T(c_z) - T(e_z)) / |v_z|
-    int li = 0;
-    for (int i = 1; i < P.n_layers; ++i) if (habs >= P.layerf[i].h_lo) li = i;
+    // The layer of the emission altitude: the preamble left it in the frame when the whole segment lies in one
+    // layer (F_LAYER >= 0), else it is looked up (unused layers carry h_lo = +inf, so the count is the index).
+    int li = __float_as_int(fr[F_LAYER]);
+    if (li < 0) {
+        li = 0;
+#pragma unroll
+        for (int i = 1; i < kMaxLayers; ++i) li += (habs >= P.layerf[i].h_lo) ? 1 : 0;
+    }
     const LayerF lf = P.layerf[li];
     const float Te = fmaf(lf.b, __expf(-habs * lf.inv_c), lf.a);
     const float excess = P.kappa_m * (telT_at<TELSRC>(P, k) - Te) * fabsf(rv);
     h.t = fmaf(ph.s, fr[F_IBC], fr[F_T0]) + (s_pl + excess) * (1.0f / 0.299792458f);
     // R4: wavelength
     const float u3 = uniform01(ph.r2);
-    h.lam = (ph.tag == 0) ? __frcp_rn(fmaf(-u3, P.dinv_lam, P.inv_lam1)) : fmaf(u3, P.fl_dlam, P.fl_lam1);
+    h.lam = (ph.tag == 0) ? rcp_refined(fmaf(-u3, P.dinv_lam, P.inv_lam1)) : fmaf(u3, P.fl_dlam, P.fl_lam1);
     // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
     h.w = fr[F_W0];
     if (P.tau != nullptr) {
@@ -452,48 +510,141 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     return h;
 }
 
-// a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes
-// together.  Tally: one shared-memory atomic per (warp, telescope) when all hits of the warp are on one
-// telescope, else one per lane.  Photon output: the lanes of one telescope reserve their records with a
-// single bump of that telescope's cursor.
+// Photon output, hits on several telescopes: the lanes of one telescope reserve their records with a single bump of
+// that telescope's cursor.  Called by all 32 lanes.
+__device__ __forceinline__ void write_records_grouped(const KParams &P, const Hit &h, uint64_t id)
+{
+    const uint32_t lane = lane_id();
+    const uint32_t peers = __match_any_sync(0xffffffffu, h.ok ? h.k : -1 - (int)lane);
+    if (h.ok) {
+        const int leader = __ffs(peers) - 1;
+        unsigned long long base = 0;
+        if ((int)lane == leader) base = atomicAdd(&P.cursors[h.k], (unsigned long long)__popc(peers));
+        base = __shfl_sync(peers, base, leader);
+        const unsigned long long slot = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
+        if (slot < P.tel_capacity[h.k]) {
+            const unsigned long long at = P.tel_offset[h.k] + slot;
+            float *rec = P.records + at * (unsigned)kRecWords;
+            rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
+            if (P.ids) P.ids[at] = id;
+        }
+    }
+}
+
+// Tally: a thread adds its hits to its own accumulator in shared memory (no shuffles, no atomics)
+// and flushes it into the tile tallies when the telescope changes and at the end of the tile.
+__device__ __forceinline__ void flush_accumulator(const KParams &P, TileSmem &sm)
+{
+    const int t = threadIdx.x;
+    const uint32_t n = sm.acc_n[t];
+    if (n == 0u) return;
+    const int k = sm.acc_k[t];
+    if (P.n_tel <= kTelSmemMax) { atomicAdd(&sm.t_hits[k], n); atomicAdd(&sm.t_sw[k], sm.acc_w[t]); atomicAdd(&sm.t_swt[k], sm.acc_wt[t]); }
+    else { atomicAdd(&P.tallies[k].hits, (unsigned long long)n); atomicAdd(&P.tallies[k].sum_w, sm.acc_w[t]); atomicAdd(&P.tallies[k].sum_wt, sm.acc_wt[t]); }
+    sm.acc_n[t] = 0u; sm.acc_w[t] = 0.0; sm.acc_wt[t] = 0.0;
+}
+
+__device__ __forceinline__ void accumulate_hit(const KParams &P, TileSmem &sm, const Hit &h)
+{
+    const int t = threadIdx.x;
+    if (sm.acc_k[t] != h.k) { flush_accumulator(P, sm); sm.acc_k[t] = h.k; }
+    const double w = (double)h.w;
+    sm.acc_n[t] += 1u; sm.acc_w[t] += w; sm.acc_wt[t] += w * (double)h.t;
+}
+
+// Copy n staged records (7 n words at `st`) to record slots [first, first + n) of P.records: lane i takes words i,
+// i + 32, ..., so every store instruction of the warp covers 128 contiguous bytes (four full 32-byte sectors once the
+// run is past its first, possibly unaligned, sector).  Called by all 32 lanes.
+__device__ __forceinline__ void copy_records(const KParams &P, const float *st, const unsigned long long *sid,
+                                             unsigned long long first, uint32_t n)
+{
+    const uint32_t lane = lane_id(), nwords = n * kRecWords;
+    float *dst = P.records + first * (unsigned)kRecWords;
+#pragma unroll 4
+    for (uint32_t i = lane; i < nwords; i += 32u) dst[i] = st[i];
+    if (P.ids) for (uint32_t i = lane; i < n; i += 32u) P.ids[first + i] = sid[i];
+}
+
+// Photon output when all hits of the warp are on one telescope k0 (okm = the lanes holding one).  While the tile runs
+// in rounds the records are appended to the warp's staging area and leave at the end of the round (flush_round);
+// otherwise, or when the area is full or holds another telescope's records, the warp bumps the cursor itself.
+__device__ __forceinline__ void write_records_one_tel(const KParams &P, OutSmem &os, const Hit &h, uint64_t id, uint32_t okm, int k0)
+{
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    const uint32_t n = (uint32_t)__popc(okm), rank = (uint32_t)__popc(okm & ((1u << lane) - 1u));
+    __syncwarp();                                   // lane 0's update of wn / wk in the previous call
+    const uint32_t wn = os.wn[warp];
+    if (os.rounds && (wn == 0u || os.wk[warp] == k0) && wn + n <= (uint32_t)kStageRecs) {
+        if (h.ok) {
+            float *r = os.stage[warp] + (wn + rank) * kRecWords;
+            r[0] = h.x; r[1] = h.y; r[2] = h.vx; r[3] = h.vy; r[4] = h.t; r[5] = h.lam; r[6] = h.w;
+            if (P.ids) os.ids[warp][wn + rank] = id;
+        }
+        __syncwarp();                               // all lanes have read wn / wk
+        if (lane == 0u) { os.wk[warp] = k0; os.wn[warp] = wn + n; }
+        return;
+    }
+    unsigned long long base = 0;
+    if (lane == 0u) base = atomicAdd(&P.cursors[k0], (unsigned long long)n);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    const unsigned long long cap = P.tel_capacity[k0];
+    if (base >= cap) return;
+    if (h.ok && base + rank < cap) {
+        const unsigned long long at = P.tel_offset[k0] + base + rank;
+        float *rec = P.records + at * (unsigned)kRecWords;
+        rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
+        if (P.ids) P.ids[at] = id;
+    }
+}
+
+// End of a round, called by every thread of the tile: reserve the staged records of all warps (one cursor bump per
+// run of warps on the same telescope) and copy them out.  Returns whether anything was staged; if not and
+// `may_stop` is set, the tile leaves the rounds mode (os.rounds = 0, visible to all warps on return).
+__device__ __forceinline__ bool flush_round(const KParams &P, OutSmem &os, bool may_stop)
+{
+    const uint32_t warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int any = 0;
+        for (int w = 0; w < kWarps; ) {
+            if (os.wn[w] == 0u) { ++w; continue; }
+            any = 1;
+            const int k = os.wk[w];
+            uint32_t run = 0;
+            int w1 = w;
+            while (w1 < kWarps && (os.wn[w1] == 0u || os.wk[w1] == k)) { run += os.wn[w1]; ++w1; }
+            unsigned long long base = atomicAdd(&P.cursors[k], (unsigned long long)run);
+            for (int v = w; v < w1; ++v) { os.wbase[v] = base; base += os.wn[v]; }
+            w = w1;
+        }
+        os.staged_any = any;
+        if (may_stop && !any) os.rounds = 0;
+    }
+    __syncthreads();
+    const uint32_t n = os.wn[warp];
+    if (n) {
+        const int k = os.wk[warp];
+        const unsigned long long base = os.wbase[warp], cap = P.tel_capacity[k];
+        if (base < cap)
+            copy_records(P, os.stage[warp], os.ids[warp], P.tel_offset[k] + base, (uint32_t)min((unsigned long long)n, cap - base));
+    }
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) os.wn[warp] = 0u;
+    __syncwarp();
+    return os.staged_any != 0;
+}
+
+// a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes together.
+template <bool OUT>
 __device__ __forceinline__ void commit_hits(const KParams &P, TileSmem &sm, const Hit &h, uint64_t id)
 {
-    constexpr uint32_t mask = 0xffffffffu;
-    const uint32_t lane = lane_id();
-    const uint32_t okm = __ballot_sync(mask, h.ok);
+    const uint32_t okm = __ballot_sync(0xffffffffu, h.ok);
     if (okm == 0u) return;
-    const int k0 = __shfl_sync(mask, h.k, __ffs(okm) - 1);
-    const bool one_tel = __all_sync(mask, !h.ok || h.k == k0);
-    const double w = h.ok ? (double)h.w : 0.0, wt = h.ok ? (double)h.w * (double)h.t : 0.0;
-    const bool in_smem = P.n_tel <= kTelSmemMax;
-    if (one_tel) {
-        double a = w, b = wt;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(mask, a, o); b += __shfl_xor_sync(mask, b, o); }
-        if (lane == 0u) {
-            if (in_smem) { atomicAdd(&sm.t_hits[k0], (uint32_t)__popc(okm)); atomicAdd(&sm.t_sw[k0], a); atomicAdd(&sm.t_swt[k0], b); }
-            else { atomicAdd(&P.tallies[k0].hits, (unsigned long long)__popc(okm)); atomicAdd(&P.tallies[k0].sum_w, a); atomicAdd(&P.tallies[k0].sum_wt, b); }
-        }
-    } else if (h.ok) {
-        if (in_smem) { atomicAdd(&sm.t_hits[h.k], 1u); atomicAdd(&sm.t_sw[h.k], w); atomicAdd(&sm.t_swt[h.k], wt); }
-        else { atomicAdd(&P.tallies[h.k].hits, 1ull); atomicAdd(&P.tallies[h.k].sum_w, w); atomicAdd(&P.tallies[h.k].sum_wt, wt); }
-    }
-    if (P.records != nullptr) {
-        // photon-output mode: per-telescope contiguous regions, warp-aggregated cursor bump
-        const uint32_t peers = __match_any_sync(mask, h.ok ? h.k : -1 - (int)lane);
-        if (h.ok) {
-            const int leader = __ffs(peers) - 1;
-            unsigned long long base = 0;
-            if ((int)lane == leader) base = atomicAdd(&P.cursors[h.k], (unsigned long long)__popc(peers));
-            base = __shfl_sync(peers, base, leader);
-            const unsigned long long slot = base + (unsigned)__popc(peers & ((1u << lane) - 1u));
-            if (slot < P.tel_capacity[h.k]) {
-                const unsigned long long at = P.tel_offset[h.k] + slot;
-                float *rec = P.records + at * 7ull;
-                rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
-                if (P.ids) P.ids[at] = id;
-            }
-        }
+    if (h.ok) accumulate_hit(P, sm, h);
+    if constexpr (OUT) {
+        const int k0 = __shfl_sync(0xffffffffu, h.k, __ffs(okm) - 1);
+        if (__all_sync(0xffffffffu, !h.ok || h.k == k0)) write_records_one_tel(P, out_smem<OUT>(sm), h, id, okm, k0);
+        else write_records_grouped(P, h, id);
     }
 }
 
@@ -504,7 +655,7 @@ __device__ __forceinline__ unsigned long long emitter_segment(const KParams &P, 
     return tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
 }
 
-template <int TELSRC>
+template <int TELSRC, bool OUT>
 __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t head, uint32_t n)
 {
     // lanes 0 .. n-1 take one entry each; the others only take part in the warp-wide commit
@@ -522,12 +673,32 @@ __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigne
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
     __syncwarp();
-    commit_hits(P, sm, h, id);
+    commit_hits<OUT>(P, sm, h, id);
+}
+
+// Dense path: when at least kDenseMin lanes of a warp iteration hold a candidate, the pairs are evaluated on the spot
+// from the random words the lanes still hold (no queue; the axis kind also skips the second Philox, the generic kinds
+// redraw theirs).  `has` says which lanes take part; all 32 call.
+template <int TELSRC, bool OUT>
+__device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned long long tile_first, int e, uint32_t j,
+                                        uint32_t r0, uint32_t r1, uint32_t r2, int k, bool has)
+{
+    Hit h;
+    h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
+    uint64_t id = 0;
+    if (has) {
+        const unsigned long long S = emitter_segment(P, tile_first, e);
+        const Photon ph = (sm.kind[e] == KIND_CHER_AXIS) ? photon_from_rand(P, sm, e, Rand4{r0, r1, r2, 0u}) : make_photon(P, sm, e, j, S);
+        h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+        id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
+    }
+    __syncwarp();
+    commit_hits<OUT>(P, sm, h, id);
 }
 
 // Push the candidates of this iteration (per lane: bit c of `cm` set = candidate number c, whose telescope
 // index is tel_of(c)) and drain 32 entries whenever that many are queued.  All 32 lanes call it together.
-template <int TELSRC, typename TelOf>
+template <int TELSRC, bool OUT, typename TelOf>
 __device__ __forceinline__ void push_candidates(const KParams &P, TileSmem &sm, unsigned long long tile_first,
                                                 uint32_t &q_head, uint32_t &q_count, uint32_t cm, int e, uint32_t j, TelOf tel_of)
 {
@@ -544,7 +715,7 @@ __device__ __forceinline__ void push_candidates(const KParams &P, TileSmem &sm, 
         q_count += (uint32_t)__popc(have);
         __syncwarp();
         if (q_count >= 32u) {
-            drain_queue<TELSRC>(P, sm, tile_first, q_head, 32u);
+            drain_queue<TELSRC, OUT>(P, sm, tile_first, q_head, 32u);
             __syncwarp();
             q_head = (q_head + 32u) & (kQueue - 1);
             q_count -= 32u;
@@ -568,6 +739,13 @@ __device__ __forceinline__ bool plane_pretest(const float4 T, float gx, float gy
 //  TEL_CONST: bit k = telescope k.   TEL_GRID: bit c = slot c of the photon's grid cell (returned in *cell).
 //  Photons flatter than the grid allows, and TEL_GLOBAL, return kAllTelescopes: the caller tests all of them.
 constexpr uint32_t kAllTelescopes = 0x80000000u;
+
+// telescope index of candidate bit c
+template <int TELSRC> __device__ __forceinline__ uint32_t slot_telescope(const uint2 cell, int c)
+{
+    if (TELSRC == TEL_GRID) return ((c < 2 ? cell.x : cell.y) >> (16 * (c & 1))) & 0xffffu;
+    return (uint32_t)c;
+}
 
 template <int TELSRC, bool COPLANAR, int NT>
 __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
@@ -609,7 +787,7 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
 // the lanes holding such a photon.  One photon at a time: its (emitter, index) is broadcast, every lane rebuilds it
 // from the counter and tests the telescopes lane, lane + 32, ... with a conservative distance test (cross product,
 // no plane projection: valid for any v_z); the survivors go through the candidate queue like all others.
-template <int TELSRC>
+template <int TELSRC, bool OUT>
 __device__ __noinline__ void wide_test(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
                                        uint32_t &q_count, uint32_t wide, int e, uint32_t j)
 {
@@ -638,7 +816,7 @@ __device__ __noinline__ void wide_test(const KParams &P, TileSmem &sm, unsigned 
                 }
             }
             if (__any_sync(0xffffffffu, cm != 0u))
-                push_candidates<TELSRC>(P, sm, tile_first, q_head, q_count, cm, eb, jb, [&](int c) { return (uint32_t)(k0 + c * 32 + lane); });
+                push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, eb, jb, [&](int c) { return (uint32_t)(k0 + c * 32 + lane); });
         }
     }
 }
@@ -667,7 +845,7 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
     return AxisFrame{A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, C.y, C.z};
 }
 
-template <int TELSRC, bool COPLANAR, int NT>
+template <int TELSRC, bool COPLANAR, int NT, bool OUT>
 __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_constant__ KParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -681,6 +859,12 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         for (int k = tid; k < P.n_tel; k += kTile) { sm.t_hits[k] = 0u; sm.t_sw[k] = 0.0; sm.t_swt[k] = 0.0; }
     if (tid == 0) sm.n_upward = 0ull;
     sm.invalid[tid] = 0;
+    sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
+    if constexpr (OUT) {
+        OutSmem &os = out_smem<OUT>(sm);
+        if (tid < kWarps) { os.wn[tid] = 0u; os.wk[tid] = -1; }
+        if (tid == 0) { os.rounds = 1; os.staged_any = 0; }
+    }
     __syncthreads();
 
     // ---- phase 1: preamble of emitter tid (a1)
@@ -718,11 +902,14 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const unsigned long long tile_first = P.first_id + (unsigned long long)blockIdx.x * (unsigned)segs_per_tile;
     uint32_t n_up = 0, q_head = 0, q_count = 0;
 
-    if (lo < hi) {
+    // Every warp runs the same number of iterations (the ranges differ by at most one photon), so the photon-output
+    // kernels can close a round with a block-wide barrier every kRound iterations.
+    const uint32_t n_iter = ((total + kWarps - 1u) / kWarps + 31u) / 32u;
+    if (total) {
         // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
         int e;
         {
-            const uint32_t g0 = min(lo + (uint32_t)lane, hi - 1u);
+            const uint32_t g0 = min(lo + (uint32_t)lane, max(hi, 1u) - 1u);
             int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
             while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
             e = a;
@@ -732,13 +919,15 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         unsigned long long S = emitter_segment(P, tile_first, e);
         PhiloxEmitter pe = philox_emitter(P, S);
         AxisFrame f = load_axis_frame(sm, e);
-        uint32_t g = lo + (uint32_t)lane;
-        for (uint32_t left = hi - lo; ; g += 32u) {
+        uint32_t g = lo + (uint32_t)lane, left = hi - lo;
+        bool rounds = OUT;
+        for (uint32_t it = 0; it < n_iter; ++it, g += 32u) {
             // `left` = photons of the warp still to do (warp-uniform); the lanes >= left idle in the last round
             const bool active = (uint32_t)lane < left;
             uint32_t cm = 0u;
             uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
             uint32_t j = 0u;
+            Rand4 r = {0u, 0u, 0u, 0u};
             if (active) {
                 if (g >= end) {
                     do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
@@ -750,7 +939,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
                 }
                 j = g - start;
                 if (kind == KIND_CHER_AXIS) {
-                    const Rand4 r = philox_photon(P, pe, j, 0u);                                  // a2
+                    r = philox_photon(P, pe, j, 0u);                                              // a2
                     // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
                     const float sd = fmaf(one_two(r.r0), f.negL, f.k0c);                          // K0 - u1 L
                     float sp, cp;
@@ -782,21 +971,40 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             } else {
                 const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
                 if (wide) {
-                    wide_test<TELSRC>(P, sm, tile_first, q_head, q_count, wide, e, j);
+                    wide_test<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, wide, e, j);
                     if (cm == kAllTelescopes) cm = 0u;
                 }
             }
-            if (__any_sync(0xffffffffu, cm != 0u)) {
-                if constexpr (TELSRC == TEL_GRID)
-                    push_candidates<TELSRC>(P, sm, tile_first, q_head, q_count, cm, e, j,
-                                            [&](int c) { return ((c < 2 ? cell.x : cell.y) >> (16 * (c & 1))) & 0xffffu; });
-                else
-                    push_candidates<TELSRC>(P, sm, tile_first, q_head, q_count, cm, e, j, [](int c) { return (uint32_t)c; });
+            const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
+            if constexpr (OUT) {
+                if (__popc(have) >= kDenseMin) {
+                    // dense iteration: each lane's first candidate is evaluated on the spot, further ones are queued
+                    const bool has = cm != 0u;
+                    int k = 0;
+                    if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
+                    dense_eval<TELSRC, OUT>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, k, has);
+                }
+                if (__any_sync(0xffffffffu, cm != 0u))
+                    push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+                left = (left > 32u) ? left - 32u : 0u;
+                if (rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
+                    OutSmem &os = out_smem<OUT>(sm);
+                    // nothing staged in round 0: a sparse tile, which goes on without rounds (and barriers)
+                    const bool first = it < (uint32_t)kRound;
+                    if (!flush_round(P, os, first) && first) rounds = false;
+                }
+            } else {
+                if (have)
+                    push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+                left = (left > 32u) ? left - 32u : 0u;
             }
-            if (left <= 32u) break;
-            left -= 32u;
         }
-        if (q_count) drain_queue<TELSRC>(P, sm, tile_first, q_head, q_count);
+        if (q_count) drain_queue<TELSRC, OUT>(P, sm, tile_first, q_head, q_count);
+        if constexpr (OUT) {
+            // records the last drain staged (the tile is still in rounds mode): one more flush
+            if (rounds) flush_round(P, out_smem<OUT>(sm), false);
+        }
+        flush_accumulator(P, sm);
     }
 
     // ---- tile epilogue: counters and tallies

@@ -186,3 +186,36 @@ def test_accept_all_output(c8):
     rep = pu.compare(cfg, g, o)
     _report("c5g-3k", rep)
     assert rep["matched"] == rep["hits_oracle"] >= 0.999 * (g["counters"]["generated"] - g["counters"]["upward"])
+
+
+def test_dense_hits_several_telescopes_misaligned_regions(c8):
+    """Large overlapping spheres: most warp iterations are dense, the lanes of a warp hit different telescopes,
+    a photon hits several; odd capacities make every region start off a 16-byte boundary."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=3000)
+    cfg["telescopes"] = np.array([[0.0, 0.0, 2000.0, 300.0], [40.0, -30.0, 2000.0, 150.0],
+                                  [-60.0, 20.0, 2000.0, 80.0], [10.0, 90.0, 2000.0, 6.0]], dtype=np.float32)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=(1 << 20) + 3)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("dense-4tel", rep)
+    assert rep["matched"] > 0.5 * g["counters"]["generated"]
+    t = pu.gpu_run(cfg, c8.MODE_TALLY)
+    assert np.array_equal(t["tallies"]["hits"], g["tallies"]["hits"])
+
+
+def test_dense_output_capacity_overflow(c8):
+    """Accept-all output into a region that is too small: exactly `capacity` records, each a true hit, rest counted."""
+    import parity_util as pu
+    cfg = wl.make_config("c5g", n_segments=3000)
+    cap = 100_001
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=cap)
+    o = pu.oracle_run(cfg)
+    assert g["counters"]["records"] == cap == len(g["records"])
+    assert g["counters"]["dropped"] == g["counters"]["hits"] - cap > 0
+    ids = g["records"]["id"]
+    assert len(np.unique(ids)) == cap
+    pos = np.searchsorted(o["records"]["id"], ids)
+    assert np.array_equal(o["records"]["id"][pos], ids)
+    assert np.max(np.abs(o["records"]["x"][pos] - g["records"]["x"].astype(np.float64))) < pu.TOL_XY_M
+    assert np.max(np.abs(o["records"]["t"][pos] - g["records"]["t"].astype(np.float64))) < pu.TOL_T_NS
