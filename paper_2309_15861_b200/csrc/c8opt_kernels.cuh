@@ -36,6 +36,7 @@ constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, 
 constexpr int kRound = 2;             // photon output: warp iterations per round (one cursor bump per tile and round)
 constexpr int kStageRecs = kRound * 32;           // records a warp can stage per round
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
+constexpr int kGenericWeight = 3;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
@@ -160,6 +161,8 @@ struct __align__(16) TileSmem {
     uint8_t kind[kTile];
     uint8_t invalid[kTile];
     uint32_t warp_sum[kWarps];
+    unsigned long long warp_wsum[kWarps];
+    uint32_t bound[kWarps + 1];                 // photon ranges of the warps
     uint32_t t_hits[kTelSmemMax];
     double t_sw[kTelSmemMax], t_swt[kTelSmemMax];
     unsigned long long n_upward;
@@ -883,28 +886,56 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             if (P.n_procs == 1) P.counts[seg_i * 2ull + (unsigned)(tag ^ 1)] = 0u;
         }
     }
-    // ---- exclusive scan of nb over the tile
+    // ---- exclusive scan of nb over the tile, and of the cost-weighted counts that balance the warps: a photon of a
+    // generic kind (fluorescence, near-horizontal Cherenkov tracks) costs about kGenericWeight axis-kind photons.
+    const uint32_t weight = (nb != 0u && sm.kind[tid] != KIND_CHER_AXIS) ? (uint32_t)kGenericWeight : 1u;
+    const unsigned long long wnb = (unsigned long long)nb * weight;
     uint32_t inc = nb;
+    unsigned long long winc = wnb;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
-    if (lane == 31) sm.warp_sum[warp] = inc;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+        const unsigned long long wv = __shfl_up_sync(0xffffffffu, winc, o);
+        if (lane >= o) { inc += v; winc += wv; }
+    }
+    if (lane == 31) { sm.warp_sum[warp] = inc; sm.warp_wsum[warp] = winc; }
     __syncthreads();
     uint32_t woff = 0, total = 0;
+    unsigned long long wwoff = 0, wtotal = 0;
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) { const uint32_t v = sm.warp_sum[w]; if (w < warp) woff += v; total += v; }
-    sm.prefix[tid] = woff + inc - nb;
+    for (int w = 0; w < kWarps; ++w) {
+        const uint32_t v = sm.warp_sum[w];
+        const unsigned long long wv = sm.warp_wsum[w];
+        if (w < warp) { woff += v; wwoff += wv; }
+        total += v; wtotal += wv;
+    }
+    const uint32_t excl = woff + inc - nb;
+    sm.prefix[tid] = excl;
     if (tid < 8) sm.prefix[kTile + tid] = (tid == 0) ? total : 0xffffffffu;
+    // warp w walks photons [bound[w], bound[w + 1]): equal shares of the weighted index space.  The emitter that
+    // holds a share boundary converts it back to a photon index.
+    if (tid == 0) { sm.bound[0] = 0u; sm.bound[kWarps] = total; }
+    if (wnb) {
+        const unsigned long long wexcl = wwoff + winc - wnb;
+#pragma unroll
+        for (int w = 1; w < kWarps; ++w) {
+            const unsigned long long x = wtotal / kWarps * (unsigned)w + wtotal % kWarps * (unsigned)w / kWarps;   // floor(wtotal w / 8)
+            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = excl + (uint32_t)((x - wexcl) / weight);
+        }
+    }
     __syncthreads();
 
     // ---- phase 2: warp `warp` walks photons [lo, hi) of the tile's concatenated index space
-    const uint32_t lo = (uint32_t)(((unsigned long long)total * (unsigned)warp) / kWarps);
-    const uint32_t hi = (uint32_t)(((unsigned long long)total * (unsigned)(warp + 1)) / kWarps);
+    const uint32_t lo = sm.bound[warp], hi = sm.bound[warp + 1];
     const unsigned long long tile_first = P.first_id + (unsigned long long)blockIdx.x * (unsigned)segs_per_tile;
     uint32_t n_up = 0, q_head = 0, q_count = 0;
 
-    // Every warp runs the same number of iterations (the ranges differ by at most one photon), so the photon-output
-    // kernels can close a round with a block-wide barrier every kRound iterations.
-    const uint32_t n_iter = ((total + kWarps - 1u) / kWarps + 31u) / 32u;
+    // Every warp runs the same number of iterations (that of the longest range), so the photon-output kernels can
+    // close a round with a block-wide barrier every kRound iterations.
+    uint32_t max_len = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) max_len = max(max_len, sm.bound[w + 1] - sm.bound[w]);
+    const uint32_t n_iter = (max_len + 31u) / 32u;
     if (total) {
         // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
         int e;
