@@ -36,7 +36,7 @@ constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, 
 constexpr int kRound = 2;             // photon output: warp iterations per round (one cursor bump per tile and round)
 constexpr int kStageRecs = kRound * 32;           // records a warp can stage per round
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
-constexpr int kGenericWeight = 3;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
+constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
@@ -167,6 +167,8 @@ struct __align__(16) TileSmem {
     double t_sw[kTelSmemMax], t_swt[kTelSmemMax];
     unsigned long long n_upward;
     uint2 queue[kWarps][kQueue];                // per-warp ring of candidate (photon, telescope) pairs
+    uint32_t wide_list[kWarps][64];             // photons waiting for the wide test: j | e << 24
+    uint32_t wide_count[kWarps];
     // per-thread tally accumulators (flushed into t_* when the telescope changes and at the end of the tile)
     double acc_w[kTile], acc_wt[kTile];
     uint32_t acc_n[kTile];
@@ -380,6 +382,21 @@ __device__ __forceinline__ float rcp_refined(float x)
     return fmaf(r, fmaf(-x, r, 1.0f), r);
 }
 
+// sin(pi x), cos(pi x) for x in [-1, 1] to ~1e-7 absolute: quadrant reduction to |r| <= 1/4 (exact in fp32) and
+// Taylor polynomials in pi r (next terms < 3e-9).  About a third of sincospif's instructions, which also serves
+// arguments outside [-1, 1] and special values.
+__device__ __forceinline__ void sincospi_unit(float x, float *s, float *c)
+{
+    const float q = rintf(x + x);
+    const float r = fmaf(-0.5f, q, x), r2 = r * r;
+    const float sn = r * fmaf(r2, fmaf(r2, fmaf(r2, fmaf(r2, 0.0821458866f, -0.599264529f), 2.55016404f), -5.16771278f), 3.14159265f);
+    const float cs = fmaf(r2, fmaf(r2, fmaf(r2, fmaf(r2, fmaf(r2, -0.0258068913f, 0.235330630f), -1.33526277f), 4.05871213f), -4.93480220f), 1.0f);
+    const int qi = (int)q;
+    const float a = (qi & 1) ? cs : sn, b = (qi & 1) ? sn : cs;        // odd quadrant: sin <- cos, cos <- -sin
+    *s = (qi & 2) ? -a : a;
+    *c = ((qi + 1) & 2) ? -b : b;
+}
+
 // A photon ready for the exact test: emission point e relative to (x_ref, y_ref, z_ref) or, for the
 // axis kind, the crossing (gx, gy) of the plane z_ref; unit direction v; s = distance along the track.
 struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s; uint32_t r2; int tag; bool axis; };
@@ -414,7 +431,7 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
     ph.ez = fmaf(ph.s, fr[F_D0 + 2], fr[F_E0 + 2]);
     // sin', cos' of phi - pi = pi (2 u2 - 1); 2 u2 - 1 is exact in fp32 (R5)
     float sp, cp;
-    sincospif(fmaf(2.0f, uniform01(r.r1), -1.0f), &sp, &cp);
+    sincospi_unit(fmaf(2.0f, uniform01(r.r1), -1.0f), &sp, &cp);
     if (kind == KIND_FL_ISO) {
         // R16: cos(theta) = 1 - 2 u4, v = (cos phi sin th, sin phi sin th, -cos th); cos phi = -cos'
         const float u4 = uniform01(r.r3);
@@ -786,42 +803,67 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
     }
 }
 
-// Wide test (photons flatter than the grids allow under TEL_GRID, every photon under TEL_GLOBAL).  `wide` = ballot of
-// the lanes holding such a photon.  One photon at a time: its (emitter, index) is broadcast, every lane rebuilds it
-// from the counter and tests the telescopes lane, lane + 32, ... with a conservative distance test (cross product,
-// no plane projection: valid for any v_z); the survivors go through the candidate queue like all others.
+// Wide test (photons flatter than the grids allow under TEL_GRID, every photon under TEL_GLOBAL).  Such photons are
+// collected in a per-warp list; a batch of up to 32 is processed with one photon per lane: the lane rebuilds its
+// photon from the counter and tests every telescope (the table is read at warp-uniform addresses) with a
+// conservative distance test (cross product, no plane projection: valid for any v_z); the survivors go through the
+// candidate queue like all others.
 template <int TELSRC, bool OUT>
-__device__ __noinline__ void wide_test(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
-                                       uint32_t &q_count, uint32_t wide, int e, uint32_t j)
+__device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
+                                        uint32_t &q_count, uint32_t n)
 {
-    const int lane = (int)lane_id();
-    while (wide) {
-        const int src = __ffs(wide) - 1;
-        wide &= wide - 1u;
-        const int eb = __shfl_sync(0xffffffffu, e, src);
-        const uint32_t jb = __shfl_sync(0xffffffffu, j, src);
-        const Photon ph = make_photon(P, sm, eb, jb, emitter_segment(P, tile_first, eb));
-        if (!(ph.vz < 0.0f)) continue;                                   // warp-uniform
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    int e = 0;
+    uint32_t j = 0u;
+    bool live = false;
+    float px = 0.f, py = 0.f, pz = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
+    if (lane < n) {
+        const uint32_t q = sm.wide_list[warp][lane];
+        e = (int)(q >> 24); j = q & 0xffffffu;
+        const Photon ph = make_photon(P, sm, e, j, emitter_segment(P, tile_first, e));
+        live = ph.vz < 0.0f;
         // a point of the ray relative to (x_ref, y_ref, z_ref): the plane crossing (axis kind) or the emission point
-        const float px = ph.axis ? ph.gx : ph.ex, py = ph.axis ? ph.gy : ph.ey, pz = ph.axis ? 0.0f : ph.ez;
-        for (int k0 = 0; k0 < P.n_tel; k0 += 1024) {
-            uint32_t cm = 0u;
-            for (int c = 0; c < 32; ++c) {
-                const int k = k0 + c * 32 + lane;
-                if (k0 + c * 32 >= P.n_tel) break;                       // warp-uniform
-                if (k < P.n_tel) {
-                    const float4 T = __ldg(&P.telA[k]);
-                    const float mx = T.x - px, my = T.y - py, mz = T.z - pz;
-                    const float cx = fmaf(my, ph.vz, -(mz * ph.vy)), cy = fmaf(mz, ph.vx, -(mx * ph.vz)), cz = fmaf(mx, ph.vy, -(my * ph.vx));
-                    const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
-                    const float mm = fmaf(mx, mx, fmaf(my, my, mz * mz));
-                    if (b2 <= fmaf(mm, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f))) cm |= 1u << c;
-                }
-            }
-            if (__any_sync(0xffffffffu, cm != 0u))
-                push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, eb, jb, [&](int c) { return (uint32_t)(k0 + c * 32 + lane); });
-        }
+        px = ph.axis ? ph.gx : ph.ex; py = ph.axis ? ph.gy : ph.ey; pz = ph.axis ? 0.0f : ph.ez;
+        vx = ph.vx; vy = ph.vy; vz = ph.vz;
     }
+    for (int k0 = 0; k0 < P.n_tel; k0 += 32) {
+        uint32_t cm = 0u;
+        const int kn = min(32, P.n_tel - k0);
+        if (live) {
+            for (int c = 0; c < kn; ++c) {
+                const float4 T = __ldg(&P.telA[k0 + c]);
+                const float mx = T.x - px, my = T.y - py, mz = T.z - pz;
+                const float cx = fmaf(my, vz, -(mz * vy)), cy = fmaf(mz, vx, -(mx * vz)), cz = fmaf(mx, vy, -(my * vx));
+                const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+                const float mm = fmaf(mx, mx, fmaf(my, my, mz * mz));
+                if (b2 <= fmaf(mm, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f))) cm |= 1u << c;
+            }
+        }
+        if (__any_sync(0xffffffffu, cm != 0u))
+            push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return (uint32_t)(k0 + c); });
+    }
+}
+
+// Append the photons of the lanes in `wide` to the warp's list and process a batch when 32 are waiting.
+template <int TELSRC, bool OUT>
+__device__ __forceinline__ void wide_push(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
+                                          uint32_t &q_count, uint32_t wide, int e, uint32_t j)
+{
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    __syncwarp();
+    uint32_t n = sm.wide_count[warp];
+    if ((wide >> lane) & 1u) sm.wide_list[warp][n + (uint32_t)__popc(wide & ((1u << lane) - 1u))] = j | ((uint32_t)e << 24);
+    n += (uint32_t)__popc(wide);
+    __syncwarp();
+    if (n >= 32u) {
+        wide_batch<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, 32u);
+        __syncwarp();
+        const uint32_t moved = (lane < n - 32u) ? sm.wide_list[warp][32u + lane] : 0u;
+        __syncwarp();
+        if (lane < n - 32u) sm.wide_list[warp][lane] = moved;
+        n -= 32u;
+    }
+    if (lane == 0u) sm.wide_count[warp] = n;
 }
 
 // a2-a4 of the hot loop for the generic kinds.  Returns the candidate mask (see plane_candidates); *upward is
@@ -863,6 +905,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     if (tid == 0) sm.n_upward = 0ull;
     sm.invalid[tid] = 0;
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
+    if (tid < kWarps) sm.wide_count[tid] = 0u;
     if constexpr (OUT) {
         OutSmem &os = out_smem<OUT>(sm);
         if (tid < kWarps) { os.wn[tid] = 0u; os.wk[tid] = -1; }
@@ -1002,7 +1045,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             } else {
                 const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
                 if (wide) {
-                    wide_test<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, wide, e, j);
+                    wide_push<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, wide, e, j);
                     if (cm == kAllTelescopes) cm = 0u;
                 }
             }
@@ -1029,6 +1072,11 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
                     push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
                 left = (left > 32u) ? left - 32u : 0u;
             }
+        }
+        if constexpr (TELSRC != TEL_CONST) {
+            __syncwarp();
+            const uint32_t nw = sm.wide_count[warp];
+            if (nw) wide_batch<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, nw);
         }
         if (q_count) drain_queue<TELSRC, OUT>(P, sm, tile_first, q_head, q_count);
         if constexpr (OUT) {
