@@ -160,7 +160,8 @@ bool build_grid_level(c8opt_ctx *ctx, double vzmin, std::vector<uint2> *cells, c
             (*cells)[base + i] = make_uint2((uint32_t)list[4 * i] | ((uint32_t)list[4 * i + 1] << 16),
                                             (uint32_t)list[4 * i + 2] | ((uint32_t)list[4 * i + 3] << 16));
         lvl->nx = nx; lvl->ny = ny; lvl->base = (int)base;
-        lvl->x0 = (float)x_lo; lvl->y0 = (float)y_lo; lvl->inv_cell = (float)(1.0 / cell); lvl->vzmin = (float)vzmin;
+        lvl->inv_cell = (float)(1.0 / cell); lvl->vzmin = (float)vzmin;
+        lvl->ox = (float)(-x_lo * (double)lvl->inv_cell); lvl->oy = (float)(-y_lo * (double)lvl->inv_cell);
         return true;
     }
     return false;

@@ -47,7 +47,7 @@ constexpr int KIND_CHER_GEN = 3;      // Cherenkov, generic projection (near-hor
 struct LayerD { double h_lo, a, b, c; };
 struct LayerF { float h_lo, a, b, inv_c; };
 
-struct GridLevel { int nx, ny, base; float x0, y0, inv_cell, vzmin; };
+struct GridLevel { int nx, ny, base; float ox, oy, inv_cell, vzmin; };   // cell index = floor(x * inv_cell + ox)
 constexpr int kGridLevels = 2;
 
 struct Tally { unsigned long long hits; double sum_w; double sum_wt; };
@@ -767,12 +767,34 @@ template <int TELSRC> __device__ __forceinline__ uint32_t slot_telescope(const u
     return (uint32_t)c;
 }
 
+// Candidates of one grid level: cell of the plane crossing (most cells are empty: one load, one compare), then the
+// pre-test of the telescopes listed there (slots fill from 0, so the first empty slot ends the list).
+template <bool COPLANAR>
+__device__ __forceinline__ uint32_t grid_lookup(const KParams &P, const GridLevel &G, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
+{
+    const int ix = __float2int_rd(fmaf(gx, G.inv_cell, G.ox)), iy = __float2int_rd(fmaf(gy, G.inv_cell, G.oy));
+    if ((unsigned)ix >= (unsigned)G.nx || (unsigned)iy >= (unsigned)G.ny) return 0u;
+    const uint2 c = __ldg(&P.grid[G.base + iy * G.nx + ix]);
+    if (c.x == 0xffffffffu) return 0u;
+    *cell = c;
+    const float vz2s = vz * vz * 0.9999f;
+    uint32_t cm = plane_pretest<COPLANAR>(__ldg(&P.telA[c.x & 0xffffu]), gx, gy, vx, vy, vz, vz2s) ? 1u : 0u;
+    if ((c.x >> 16) != 0xffffu) {
+        if (plane_pretest<COPLANAR>(__ldg(&P.telA[c.x >> 16]), gx, gy, vx, vy, vz, vz2s)) cm |= 2u;
+        if (c.y != 0xffffffffu) {
+            if (plane_pretest<COPLANAR>(__ldg(&P.telA[c.y & 0xffffu]), gx, gy, vx, vy, vz, vz2s)) cm |= 4u;
+            if ((c.y >> 16) != 0xffffu && plane_pretest<COPLANAR>(__ldg(&P.telA[c.y >> 16]), gx, gy, vx, vy, vz, vz2s)) cm |= 8u;
+        }
+    }
+    return cm;
+}
+
 template <int TELSRC, bool COPLANAR, int NT>
 __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
 {
-    const float vz2s = vz * vz * 0.9999f;
-    uint32_t cm = 0u;
     if constexpr (TELSRC == TEL_CONST) {
+        const float vz2s = vz * vz * 0.9999f;
+        uint32_t cm = 0u;
         // NT = n_tel rounded up to 1, 4 or 8; the unused slots hold R^2 = -1 (never a candidate).  Unrolled so that the
         // telescope coordinates are constant-bank operands.
 #pragma unroll
@@ -780,24 +802,11 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
             if (plane_pretest<COPLANAR>(P.tel_c[k], gx, gy, vx, vy, vz, vz2s)) cm |= 1u << k;
         return cm;
     } else if constexpr (TELSRC == TEL_GRID) {
-        // steep photons use level 0; flatter ones the coarser level 1 when it exists, else the wide test
-        int lvl = 0;
-        if (!(-vz >= P.grid_lvl[0].vzmin)) {
-            if (P.n_grid_levels < 2 || !(-vz >= P.grid_lvl[1].vzmin)) return kAllTelescopes;
-            lvl = 1;
-        }
-        const GridLevel &G = P.grid_lvl[lvl];
-        const float fx = (gx - G.x0) * G.inv_cell, fy = (gy - G.y0) * G.inv_cell;
-        if (!(fx >= 0.0f && fy >= 0.0f && fx < (float)G.nx && fy < (float)G.ny)) return 0u;
-        const uint2 c = __ldg(&P.grid[G.base + (int)fy * G.nx + (int)fx]);
-        *cell = c;
-        if (c.x == 0xffffffffu) return 0u;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const uint32_t k = ((i < 2 ? c.x : c.y) >> (16 * (i & 1))) & 0xffffu;
-            if (k != 0xffffu && plane_pretest<COPLANAR>(__ldg(&P.telA[k]), gx, gy, vx, vy, vz, vz2s)) cm |= 1u << i;
-        }
-        return cm;
+        // steep photons use level 0; flatter ones the coarser level 1 when it exists, else the wide test.  One code
+        // path per level, so that the level's parameters are constant-bank operands.
+        if (-vz >= P.grid_lvl[0].vzmin) return grid_lookup<COPLANAR>(P, P.grid_lvl[0], gx, gy, vx, vy, vz, cell);
+        if (P.n_grid_levels > 1 && -vz >= P.grid_lvl[1].vzmin) return grid_lookup<COPLANAR>(P, P.grid_lvl[1], gx, gy, vx, vy, vz, cell);
+        return kAllTelescopes;
     } else {
         return kAllTelescopes;
     }
