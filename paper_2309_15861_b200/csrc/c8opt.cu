@@ -383,14 +383,15 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telA, A.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telT, T.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
     ctx->tel_src = c8::TEL_CONST;
-    if (n > c8::kTelConstMax) {
+    if (n >= c8::kTelGridMin) {
+        // the grid lookup costs about as much as two brute-force pre-tests, so it serves from 3 telescopes up
         std::vector<uint2> cells;
         ctx->n_tel_pending = n;
         if (build_grid(ctx, &cells)) {
             C8_CUDA(ctx, cudaMalloc(&ctx->d_grid, sizeof(uint2) * cells.size()));
             C8_CUDA(ctx, cudaMemcpy(ctx->d_grid, cells.data(), sizeof(uint2) * cells.size(), cudaMemcpyHostToDevice));
             ctx->tel_src = c8::TEL_GRID;
-        } else {
+        } else if (n > c8::kTelConstMax) {
             ctx->tel_src = c8::TEL_GLOBAL;
         }
     }

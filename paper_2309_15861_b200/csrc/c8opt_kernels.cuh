@@ -28,6 +28,7 @@ constexpr int kWarps = kTile / 32;
 constexpr int kFrameStride = 36;      // floats per emitter frame in shared memory (144 B)
 constexpr int kTelSmemMax = 128;      // telescopes tallied in shared memory
 constexpr int kTelConstMax = 8;       // telescopes kept in the kernel-parameter constant bank
+constexpr int kTelGridMin = 9;        // from this many telescopes on, the ground-plane grid replaces the brute-force pre-tests
 constexpr int TEL_CONST = 0;          // brute force over <= kTelConstMax telescopes read from the constant bank
 constexpr int TEL_GRID = 1;           // candidate lookup in the ground-plane grid
 constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global memory (grid not buildable)
@@ -997,31 +998,31 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
             e = a;
         }
-        uint32_t start = sm.prefix[e], end = sm.prefix[e + 1];
+        // Loop-carried per lane: photon index g, emitter e with its end, index j within the emitter, kind, the hoisted
+        // Philox words and (brute-force kernels only; the grid kernels are short of registers and reload it from
+        // shared memory every iteration) the axis frame.
+        constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
+        uint32_t end = sm.prefix[e + 1];
         int kind = sm.kind[e];
-        unsigned long long S = emitter_segment(P, tile_first, e);
-        PhiloxEmitter pe = philox_emitter(P, S);
-        AxisFrame f = load_axis_frame(sm, e);
-        uint32_t g = lo + (uint32_t)lane, left = hi - lo;
+        PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+        AxisFrame f_reg = load_axis_frame(sm, e);
+        uint32_t g = lo + (uint32_t)lane, j = g - sm.prefix[e];
         bool rounds = OUT;
-        for (uint32_t it = 0; it < n_iter; ++it, g += 32u) {
-            // `left` = photons of the warp still to do (warp-uniform); the lanes >= left idle in the last round
-            const bool active = (uint32_t)lane < left;
+        for (uint32_t it = 0; it < n_iter; ++it, g += 32u, j += 32u) {
+            const bool active = g < hi;                  // the lanes past the warp's range idle in its last iterations
             uint32_t cm = 0u;
             uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
-            uint32_t j = 0u;
             Rand4 r = {0u, 0u, 0u, 0u};
             if (active) {
                 if (g >= end) {
                     do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
-                    start = sm.prefix[e];
+                    j = g - sm.prefix[e];
                     kind = sm.kind[e];
-                    S = emitter_segment(P, tile_first, e);
-                    pe = philox_emitter(P, S);
-                    f = load_axis_frame(sm, e);
+                    pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+                    if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
                 }
-                j = g - start;
                 if (kind == KIND_CHER_AXIS) {
+                    const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
                     r = philox_photon(P, pe, j, 0u);                                              // a2
                     // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
                     const float sd = fmaf(one_two(r.r0), f.negL, f.k0c);                          // K0 - u1 L
@@ -1045,7 +1046,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
                     }
                 } else {
                     bool up;
-                    cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, S, &cell, &up);
+                    cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, emitter_segment(P, tile_first, e), &cell, &up);
                     if (up) ++n_up;
                 }
             }
@@ -1069,7 +1070,6 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
                 }
                 if (__any_sync(0xffffffffu, cm != 0u))
                     push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
-                left = (left > 32u) ? left - 32u : 0u;
                 if (rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
                     OutSmem &os = out_smem<OUT>(sm);
                     // nothing staged in round 0: a sparse tile, which goes on without rounds (and barriers)
@@ -1079,7 +1079,6 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             } else {
                 if (have)
                     push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
-                left = (left > 32u) ? left - 32u : 0u;
             }
         }
         if constexpr (TELSRC != TEL_CONST) {
