@@ -49,6 +49,12 @@ extern "C" {
 #define C8OPT_PROC_FLUORESCENCE  2u   /* bit 1 */
 #define C8OPT_MODE_TALLY   0u
 #define C8OPT_MODE_OUTPUT  1u
+/* c8opt_run_params.flags.  CULL: segment culling (Fig. 2 :63-65) in its exact, conservative form:
+ * a Cherenkov segment whose emission cone provably misses every telescope sphere -- for every telescope k,
+ * | angle(d, c_k - p_mid) - theta_c | > asin(R_k / D) + asin((L/2) / D), D = |c_k - p_mid| - L/2 -- skips the
+ * photon loop.  Tallies and records are identical with and without it; the skipped bunches still count as
+ * generated and are reported in counters[C8OPT_CNT_CULLED]; C8OPT_CNT_UPWARD then covers propagated bunches only. */
+#define C8OPT_FLAG_CULL    1u
 
 typedef struct c8opt_ctx c8opt_ctx;   /* opaque, owned by the library */
 
@@ -93,7 +99,7 @@ typedef struct {
     double   fl_yield_per_MeV;     /* constant fluorescence yield (R13)        */
     double   fl_lam1_nm, fl_lam2_nm;
     int32_t  fl_beam_telescope;    /* -1 isotropic, else beam toward this telescope (R14)   */
-    int32_t  reserved;
+    uint32_t flags;                /* C8OPT_FLAG_* bits                                     */
     double   fl_beam_halfangle_rad;
 } c8opt_run_params;
 
@@ -123,7 +129,7 @@ typedef struct { uint64_t hits; double sum_w; double sum_wt; } c8opt_tally;
 /* indices into the counters[8] array of c8opt_read_tallies */
 enum {
     C8OPT_CNT_SEGMENTS = 0, C8OPT_CNT_GENERATED = 1, C8OPT_CNT_UPWARD = 2, C8OPT_CNT_HITS = 3,
-    C8OPT_CNT_RECORDS = 4, C8OPT_CNT_DROPPED = 5, C8OPT_CNT_INVALID = 6, C8OPT_CNT_UNUSED = 7
+    C8OPT_CNT_RECORDS = 4, C8OPT_CNT_DROPPED = 5, C8OPT_CNT_INVALID = 6, C8OPT_CNT_CULLED = 7
 };
 
 /* Validate the descriptor, build the layer / transmission tables and upload

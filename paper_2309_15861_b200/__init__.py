@@ -25,7 +25,8 @@ from .build import LIB_PATH, build  # noqa: F401
 MAX_LAYERS = 8
 PROC_CHERENKOV, PROC_FLUORESCENCE = 1, 2
 MODE_TALLY, MODE_OUTPUT = 0, 1
-COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "unused")
+FLAG_CULL = 1
+COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "culled")
 TALLY_DTYPE = np.dtype([("hits", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
 RECORD_FLOATS = 7
 
@@ -56,7 +57,7 @@ class _RunParams(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("processes", C.c_uint32), ("mode", C.c_uint32),
                 ("lam1_nm", C.c_double), ("lam2_nm", C.c_double), ("bunch_size", C.c_double),
                 ("fl_yield_per_MeV", C.c_double), ("fl_lam1_nm", C.c_double), ("fl_lam2_nm", C.c_double),
-                ("fl_beam_telescope", C.c_int32), ("reserved", C.c_int32), ("fl_beam_halfangle_rad", C.c_double)]
+                ("fl_beam_telescope", C.c_int32), ("flags", C.c_uint32), ("fl_beam_halfangle_rad", C.c_double)]
 
 
 class _Output(C.Structure):
@@ -118,7 +119,7 @@ def make_run_params(p: dict) -> _RunParams:
     return _RunParams(int(p["seed"]), int(p["processes"]), int(p.get("mode", MODE_TALLY)),
                       float(p["lam1"]), float(p["lam2"]), float(p["bunch_size"]),
                       float(p["fl_yield"]), float(p["fl_lam1"]), float(p["fl_lam2"]),
-                      int(p["fl_beam_telescope"]), 0, float(p["fl_beam_halfangle"]))
+                      int(p["fl_beam_telescope"]), int(p.get("flags", 0)), float(p["fl_beam_halfangle"]))
 
 
 class Context:

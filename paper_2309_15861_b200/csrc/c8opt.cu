@@ -33,6 +33,7 @@ struct c8opt_ctx {
     bool coplanar = true;
     std::vector<double> tel_xyzr;          // absolute, as given (float -> double)
     double x_ref = 0, y_ref = 0, z_ref = 0;
+    float cull_Rb = 0;                 // radius about the reference point that holds every telescope sphere
     float4 *d_telA = nullptr;
     float *d_telT = nullptr;
     std::vector<float4> h_telA;
@@ -188,6 +189,7 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     const unsigned procs = rp->processes;
     if (procs == 0 || (procs & ~3u)) return fail(ctx, C8OPT_ERR_ARGUMENT, "processes must be a combination of bits 0 and 1");
     if (rp->mode > 1u) return fail(ctx, C8OPT_ERR_ARGUMENT, "mode must be 0 (tally) or 1 (photon output)");
+    if (rp->flags & ~C8OPT_FLAG_CULL) return fail(ctx, C8OPT_ERR_ARGUMENT, "unknown bit in flags");
     if (!(rp->bunch_size > 0.0) || !std::isfinite(rp->bunch_size)) return fail(ctx, C8OPT_ERR_ARGUMENT, "bunch_size must be > 0");
     if (procs & C8OPT_PROC_CHERENKOV)
         if (!(rp->lam1_nm > 0.0) || !(rp->lam2_nm > rp->lam1_nm)) return fail(ctx, C8OPT_ERR_ARGUMENT, "need 0 < lam1 < lam2");
@@ -228,6 +230,7 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
         P.rk1[r] = (uint32_t)(rp->seed >> 32) + (uint32_t)r * 0xBB67AE85u;
     }
     P.processes = procs; P.n_procs = (procs == 3u) ? 2u : 1u;
+    P.flags = rp->flags; P.cull_Rb = ctx->cull_Rb;
     if (procs & C8OPT_PROC_CHERENKOV) {
         // PAPER.md:45 prefactor: pi e^2 / (h eps0 c0) = 2 pi alpha; the lambda integral of lambda^-2 in closed form (R2)
         const double two_pi_alpha = 2.0 * 3.14159265358979323846 * 7.2973525693e-3;
@@ -376,6 +379,12 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
         A[k] = make_float4((float)(x - ctx->x_ref), (float)(y - ctx->y_ref), (float)(z - ctx->z_ref), (float)(r * r));
         T[k] = (float)host_depth(ctx, z);
     }
+    double rb = 0.0;
+    for (int k = 0; k < n; ++k) {
+        const double x = xyzr[4 * k] - ctx->x_ref, y = xyzr[4 * k + 1] - ctx->y_ref, z = xyzr[4 * k + 2] - ctx->z_ref;
+        rb = std::fmax(rb, std::sqrt(x * x + y * y + z * z) + xyzr[4 * k + 3]);
+    }
+    ctx->cull_Rb = (float)(rb * (1.0 + 1e-6));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telA, sizeof(float4) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telT, sizeof(float) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_tallies, sizeof(c8::Tally) * n));
@@ -494,7 +503,7 @@ int c8opt_read_tallies(c8opt_ctx *ctx, c8opt_tally *host_out, int32_t n_tel, uin
         counters[C8OPT_CNT_RECORDS] = stored;
         counters[C8OPT_CNT_DROPPED] = dropped;
         counters[C8OPT_CNT_INVALID] = cnt[6];
-        counters[C8OPT_CNT_UNUSED] = 0;
+        counters[C8OPT_CNT_CULLED] = cnt[7];
     }
     if (dropped) return fail(ctx, C8OPT_ERR_CAPACITY, "%llu photon records dropped: output capacity exceeded", dropped);
     return C8OPT_OK;

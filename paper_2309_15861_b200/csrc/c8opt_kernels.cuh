@@ -38,6 +38,8 @@ constexpr int kRound = 2;             // photon output: warp iterations per roun
 constexpr int kStageRecs = kRound * 32;           // records a warp can stage per round
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
 constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
+constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
+constexpr uint32_t kFlagCull = 1u;    // == C8OPT_FLAG_CULL
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
@@ -77,6 +79,9 @@ struct KParams {
     const uint2 *grid;
     int n_grid_levels;
     GridLevel grid_lvl[kGridLevels];
+    // segment culling (C8OPT_FLAG_CULL): bounding sphere of the telescope array about (x_ref, y_ref, z_ref)
+    uint32_t flags;
+    float cull_Rb;
     // run
     uint32_t rk0[10], rk1[10];     // Philox round keys: key + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t processes, n_procs;
@@ -166,7 +171,7 @@ struct __align__(16) TileSmem {
     uint32_t bound[kWarps + 1];                 // photon ranges of the warps
     uint32_t t_hits[kTelSmemMax];
     double t_sw[kTelSmemMax], t_swt[kTelSmemMax];
-    unsigned long long n_upward;
+    unsigned long long n_upward, n_culled;
     uint2 queue[kWarps][kQueue];                // per-warp ring of candidate (photon, telescope) pairs
     uint32_t wide_list[kWarps][64];             // photons waiting for the wide test: j | e << 24
     uint32_t wide_count[kWarps];
@@ -251,13 +256,49 @@ __device__ __forceinline__ void rodrigues_columns(const double dir[3], double m0
     m1[0] = 2.0 * Ax * Ay;                   m1[1] = 1.0 - 2.0 * Ax * Ax - 2.0 * Az * Az; m1[2] = 2.0 * Ay * Az;
 }
 
+// Segment culling, exact and conservative.  A photon leaves the track at angle theta_c to d, so it can
+// reach the sphere (c, R) from the emission point e only if |angle(d, c - e) - theta_c| <= asin(R / |c - e|).  Over
+// the segment (midpoint m, half length hl) the direction to c swings by at most asin(hl / D) and |c - e| >= D =
+// |c - m| - hl.  With a = (R + 1 cm) / D, b = hl / D and sin(asin a + asin b) <= a + b, the sphere is out of reach if
+// cos(psi - theta_c) <= 0 or |sin(psi - theta_c)| > a + b + 2e-5 (the slack covers the fp32 photon directions and
+// this test's own rounding).  Returns true when the sphere CAN be hit (or the test cannot tell).
+__device__ __forceinline__ bool cone_reaches(float ux, float uy, float uz, float R, float dx, float dy, float dz, float hl,
+                                             float sin_c, float cos_c)
+{
+    const float uu = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
+    const float inv = rsqrtf(uu), D = uu * inv - hl;
+    if (!(D > R + 0.01f)) return true;
+    const float sA = (R + 0.01f + hl) / D + 2e-5f;
+    if (!(sA < 1.0f)) return true;
+    const float cpsi = fmaf(dx, ux, fmaf(dy, uy, dz * uz)) * inv;
+    const float cx = fmaf(dy, uz, -(dz * uy)), cy = fmaf(dz, ux, -(dx * uz)), cz = fmaf(dx, uy, -(dy * ux));
+    const float spsi = sqrtf(fmaf(cx, cx, fmaf(cy, cy, cz * cz))) * inv;
+    const float s = fmaf(spsi, cos_c, -(cpsi * sin_c)), c = fmaf(cpsi, cos_c, spsi * sin_c);
+    return c > 0.0f && fabsf(s) <= sA;
+}
+
+// true = no photon of this Cherenkov emitter can hit any telescope.  m = segment midpoint relative to the reference
+// point; first the array's bounding sphere, then (small arrays) every telescope.
+__device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, float mz, float dx, float dy, float dz, float hl,
+                                          float sin_c, float cos_c)
+{
+    if (!cone_reaches(-mx, -my, -mz, P.cull_Rb, dx, dy, dz, hl, sin_c, cos_c)) return true;
+    if (P.n_tel > kCullTelMax) return false;
+    for (int k = 0; k < P.n_tel; ++k) {
+        const float4 T = __ldg(&P.telA[k]);
+        if (cone_reaches(T.x - mx, T.y - my, T.z - mz, sqrtf(T.w), dx, dy, dz, hl, sin_c, cos_c)) return false;
+    }
+    return true;
+}
+
 // Preamble of emitter (segment i, process tag).  Writes the frame, returns n_b.
 // *bad is set when the segment is invalid (non-finite field, gamma <= 1, L < 0, |d| off unity by > 1e-3,
 // or n_b >= 2^24).
 __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1, const float4 s2, int tag,
-                             float *__restrict__ fr, uint8_t *kind_out, bool *bad)
+                             float *__restrict__ fr, uint8_t *kind_out, bool *bad, bool *culled)
 {
     *bad = false;
+    *culled = false;
     const double L = (double)s1.w, gamma = (double)s2.x, zq = (double)s2.y, dE = (double)s2.z;
     const double dx = (double)s1.x, dy = (double)s1.y, dz = (double)s1.z;
     const double dn = sqrt(dadd(dadd(dmul(dx, dx), dmul(dy, dy)), dmul(dz, dz)));
@@ -309,6 +350,14 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     if (nb > 16777215.0) { *bad = true; return 0; }
     double w0 = ddiv(mu, nb);
     if (kind == KIND_CONE) w0 *= 0.5 * P.omc;                    // R14: Omega / 4 pi
+    if ((P.flags & kFlagCull) && tag == 0) {
+        const double hl = 0.5 * L;
+        if (cull_emitter(P, (float)(p0[0] + hl * d[0] - P.x_ref), (float)(p0[1] + hl * d[1] - P.y_ref), (float)(p0[2] + hl * d[2] - P.z_ref),
+                         (float)d[0], (float)d[1], (float)d[2], (float)hl, (float)sin_c, (float)cos_c)) {
+            *culled = true;
+            return (uint32_t)nb;
+        }
+    }
 
     fr[F_W0] = (float)w0; fr[F_T0] = s0.w; fr[F_IBC] = (float)ibc; fr[F_LEN] = (float)L;
     {
@@ -912,7 +961,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const bool tally_in_smem = P.n_tel <= kTelSmemMax;
     if (tally_in_smem)
         for (int k = tid; k < P.n_tel; k += kTile) { sm.t_hits[k] = 0u; sm.t_sw[k] = 0.0; sm.t_swt[k] = 0.0; }
-    if (tid == 0) sm.n_upward = 0ull;
+    if (tid == 0) { sm.n_upward = 0ull; sm.n_culled = 0ull; }
     sm.invalid[tid] = 0;
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
     if (tid < kWarps) sm.wide_count[tid] = 0u;
@@ -927,17 +976,24 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const int seg_local = (P.n_procs == 2) ? (tid & (kTile / 2 - 1)) : tid;
     const int tag = (P.n_procs == 2) ? (tid >> 7) : ((P.processes & 1u) ? 0 : 1);
     const unsigned long long seg_i = (unsigned long long)blockIdx.x * (unsigned)segs_per_tile + (unsigned)seg_local;
-    uint32_t nb = 0;
+    uint32_t nb = 0, n_culled = 0;
     if (seg_i < P.n_seg) {
         const float4 *sp = P.seg + seg_i * 3ull;
         const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
-        bool bad;
-        nb = preamble(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad);
+        bool bad, culled;
+        nb = preamble(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled);
         if (bad) sm.invalid[seg_local] = 1;
         if (P.counts) {
             P.counts[seg_i * 2ull + (unsigned)tag] = nb;
             if (P.n_procs == 1) P.counts[seg_i * 2ull + (unsigned)(tag ^ 1)] = 0u;
         }
+        if (culled) { n_culled = nb; nb = 0u; }           // generated, but provably no hit: not propagated
+    }
+    if (P.flags & kFlagCull) {
+        unsigned long long c = n_culled;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+        if (lane == 0 && c) atomicAdd(&sm.n_culled, c);
     }
     // ---- exclusive scan of nb over the tile, and of the cost-weighted counts that balance the warps: a photon of a
     // generic kind (fluorescence, near-horizontal Cherenkov tracks) costs about kGenericWeight axis-kind photons.
@@ -1100,8 +1156,9 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     if (lane == 0 && n_up) atomicAdd(&sm.n_upward, (unsigned long long)n_up);
     __syncthreads();
     if (tid == 0) {
-        if (total) atomicAdd(&P.counters[1], (unsigned long long)total);
+        if (total + sm.n_culled) atomicAdd(&P.counters[1], (unsigned long long)total + sm.n_culled);
         if (sm.n_upward) atomicAdd(&P.counters[2], sm.n_upward);
+        if (sm.n_culled) atomicAdd(&P.counters[7], sm.n_culled);
     }
     {
         // invalid segments of this tile (each counted once)

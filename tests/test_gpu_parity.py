@@ -219,3 +219,42 @@ def test_dense_output_capacity_overflow(c8):
     assert np.array_equal(o["records"]["id"][pos], ids)
     assert np.max(np.abs(o["records"]["x"][pos] - g["records"]["x"].astype(np.float64))) < pu.TOL_XY_M
     assert np.max(np.abs(o["records"]["t"][pos] - g["records"]["t"].astype(np.float64))) < pu.TOL_T_NS
+
+
+@pytest.mark.parametrize("name,n", [("c1", None), ("c2", 50_000), ("c4", 100_000), ("c3b", 50_000)])
+def test_segment_culling_changes_nothing(c8, name, n):
+    """C8OPT_FLAG_CULL (PAPER.md:57 in its exact form): the culled run must give the same records, bit for bit, and
+    the same tallies as the full run; only the work differs."""
+    import parity_util as pu
+    cfg = wl.make_config(name) if n is None else wl.make_config(name, n_segments=n)
+    a = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_CULL)
+    b = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    assert np.array_equal(a["counts"], b["counts"])
+    assert a["counters"]["generated"] == b["counters"]["generated"]
+    assert np.array_equal(a["tallies"]["hits"], b["tallies"]["hits"])
+    assert np.array_equal(a["records"]["id"], b["records"]["id"]) and np.array_equal(a["records"]["tel"], b["records"]["tel"])
+    for f in ("x", "y", "cx", "cy", "t", "lam", "w"):
+        assert np.array_equal(a["records"][f], b["records"][f])
+    assert np.allclose(a["tallies"]["sum_w"], b["tallies"]["sum_w"], rtol=1e-12)
+    assert a["counters"]["culled"] == 0
+    frac = b["counters"]["culled"] / max(1, b["counters"]["generated"])
+    print(f"[cull {name}] culled {b['counters']['culled']} of {b['counters']['generated']} bunches ({100 * frac:.1f} %)")
+    if name != "c3b":
+        assert frac > 0.2          # fluorescence (c3b) is never culled
+
+
+def test_segment_culling_non_coplanar_big_spheres(c8):
+    """Culling with telescopes of different sizes at different altitudes, against the oracle (which never culls)."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=30_000)
+    tel = cfg["telescopes"].copy()
+    tel[:, 2] += np.array([0.0, 35.0, -20.0, 60.0], dtype=np.float32)
+    tel[:, 3] = np.array([6.0, 12.0, 25.0, 40.0], dtype=np.float32)
+    cfg["telescopes"] = tel
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_CULL)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o, check_upward=False)
+    _report("cull-noncoplanar", rep)
+    assert g["counters"]["culled"] > 0 and rep["matched"] > 1000
