@@ -105,6 +105,21 @@ struct KParams {
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
 
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// 1/x to within 1 ulp for normal x: MUFU.RCP + one Newton step (3 instructions instead of the IEEE division's ~10)
+__device__ __forceinline__ float rcp_refined(float x)
+{
+    const float r = rcp_approx(x);
+    return fmaf(r, fmaf(-x, r, 1.0f), r);
+}
+
+
 // ------------------------------------------------------------------------------------
 // a2: Philox4x32-10 (Salmon et al., SC'11), counter (j, S_lo, S_hi, tag), key = seed (R20).
 struct Rand4 { uint32_t r0, r1, r2, r3; };
@@ -265,14 +280,16 @@ __device__ __forceinline__ void rodrigues_columns(const double dir[3], double m0
 __device__ __forceinline__ bool cone_reaches(float ux, float uy, float uz, float R, float dx, float dy, float dz, float hl,
                                              float sin_c, float cos_c)
 {
+    // MUFU-grade rsqrt / reciprocal (2 ulp) are ample against the 2e-5 slack
     const float uu = fmaf(ux, ux, fmaf(uy, uy, uz * uz));
-    const float inv = rsqrtf(uu), D = uu * inv - hl;
+    const float inv = rsqrtf(uu), D = fmaf(uu, inv, -hl);
     if (!(D > R + 0.01f)) return true;
-    const float sA = (R + 0.01f + hl) / D + 2e-5f;
+    const float sA = fmaf(R + 0.01f + hl, rcp_approx(D), 2e-5f);
     if (!(sA < 1.0f)) return true;
     const float cpsi = fmaf(dx, ux, fmaf(dy, uy, dz * uz)) * inv;
     const float cx = fmaf(dy, uz, -(dz * uy)), cy = fmaf(dz, ux, -(dx * uz)), cz = fmaf(dx, uy, -(dy * ux));
-    const float spsi = sqrtf(fmaf(cx, cx, fmaf(cy, cy, cz * cz))) * inv;
+    const float cc = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+    const float spsi = cc * rsqrtf(fmaxf(cc, 1e-30f)) * inv;
     const float s = fmaf(spsi, cos_c, -(cpsi * sin_c)), c = fmaf(cpsi, cos_c, spsi * sin_c);
     return c > 0.0f && fabsf(s) <= sA;
 }
@@ -286,7 +303,8 @@ __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, 
     if (P.n_tel > kCullTelMax) return false;
     for (int k = 0; k < P.n_tel; ++k) {
         const float4 T = __ldg(&P.telA[k]);
-        if (cone_reaches(T.x - mx, T.y - my, T.z - mz, sqrtf(T.w), dx, dy, dz, hl, sin_c, cos_c)) return false;
+        const float R = T.w * rsqrtf(fmaxf(T.w, 1e-30f));
+        if (cone_reaches(T.x - mx, T.y - my, T.z - mz, R, dx, dy, dz, hl, sin_c, cos_c)) return false;
     }
     return true;
 }
@@ -416,20 +434,6 @@ template <int TELSRC> __device__ __forceinline__ float telT_at(const KParams &P,
 {
     if (TELSRC == TEL_CONST) return P.telT_c[k];
     return __ldg(&P.telT[k]);
-}
-
-__device__ __forceinline__ float rcp_approx(float x)
-{
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-
-// 1/x to within 1 ulp for normal x: MUFU.RCP + one Newton step (3 instructions instead of the IEEE division's ~10)
-__device__ __forceinline__ float rcp_refined(float x)
-{
-    const float r = rcp_approx(x);
-    return fmaf(r, fmaf(-x, r, 1.0f), r);
 }
 
 // sin(pi x), cos(pi x) for x in [-1, 1] to ~1e-7 absolute: quadrant reduction to |r| <= 1/4 (exact in fp32) and
