@@ -254,3 +254,50 @@ def run(atmosphere: dict, telescopes, segments, params: dict, first_id: int = 0,
         counters += p[2]
     records = np.concatenate([p[3] for p in parts]) if record_capacity else None
     return dict(counts=counts, tallies=tallies, counters=counters, records=records)
+
+
+# ------------------------------------------------------------------ ground-plane radial profile
+HIST_DTYPE = np.dtype([("n", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
+
+
+def ground_histogram(atmosphere: dict, segments, params: dict, core_xy, r_max: float, n_bins: int,
+                     first_id: int = 0, threads: int = 1, record_capacity: int = 1 << 24) -> dict:
+    """Radial intensity and timing profile on the observation level (section 3.1, Fig. 3a/3b:
+    photon density and mean arrival time against the distance from the shower core; R26).
+
+    Definition written out: every bunch that crosses the plane z = h_obs going down (R10 with an accept-all
+    detector: a sphere of radius 1e9 m centred on the core at h_obs, so its record holds the crossing point
+    relative to the core, R11, the arrival time, R8, and the weight, R17) falls into the bin
+    floor(r / (r_max / n_bins)), r = sqrt(x^2 + y^2); bins hold {n, sum w, sum w t}; r >= r_max counts as overflow.
+    Density = sum_w / annulus area and mean time = sum_wt / sum_w are formed by `profile()`.
+    """
+    tel = np.array([[float(core_xy[0]), float(core_xy[1]), float(atmosphere["h_obs"]), 1.0e9]], dtype=np.float32)
+    res = run(atmosphere, tel, segments, params, first_id=first_id, want_counts=True,
+              record_capacity=record_capacity, threads=threads)
+    rec = res["records"]
+    assert int(res["counters"][COUNTER_NAMES.index("dropped")]) == 0, "record_capacity too small for the histogram"
+    r = np.sqrt(rec["x"].astype(np.float64) ** 2 + rec["y"].astype(np.float64) ** 2)
+    dr = float(r_max) / int(n_bins)
+    b = np.floor(r / dr).astype(np.int64)
+    inside = b < n_bins
+    hist = np.zeros(n_bins, dtype=HIST_DTYPE)
+    w = rec["w"].astype(np.float64)
+    t = rec["t"].astype(np.float64)
+    hist["n"] = np.bincount(b[inside], minlength=n_bins).astype(np.uint64)
+    hist["sum_w"] = np.bincount(b[inside], weights=w[inside], minlength=n_bins)
+    hist["sum_wt"] = np.bincount(b[inside], weights=(w * t)[inside], minlength=n_bins)
+    return dict(hist=hist, overflow=int(np.count_nonzero(~inside)), r=r, records=rec, counters=res["counters"],
+                counts=res["counts"])
+
+
+def profile(hist, r_max: float, min_photons: int = 50):
+    """Fig. 3a / 3b quantities: photon density [1/m^2] and mean arrival time [ns] per radial bin; bins with fewer than
+    `min_photons` bunches are masked (NaN), the paper's cut of at least 50 photons per bin."""
+    n_bins = len(hist)
+    edges = np.linspace(0.0, float(r_max), n_bins + 1)
+    area = np.pi * (edges[1:] ** 2 - edges[:-1] ** 2)
+    ok = hist["n"] >= min_photons
+    dens = np.where(ok, hist["sum_w"] / area, np.nan)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        mean_t = np.where(ok & (hist["sum_w"] > 0), hist["sum_wt"] / hist["sum_w"], np.nan)
+    return 0.5 * (edges[1:] + edges[:-1]), dens, mean_t

@@ -553,3 +553,72 @@ def test_tiny_case_against_pure_python_restatement():
         assert q["cx"] == pytest.approx(h[3], abs=1e-10) and q["cy"] == pytest.approx(h[4], abs=1e-10)
         assert q["t"] == pytest.approx(h[5], abs=1e-8) and q["lam"] == pytest.approx(h[6], rel=1e-12)
         assert q["w"] == pytest.approx(h[7], rel=1e-9)
+
+
+# ------------------------------------------------------------------ ground-plane radial profile
+def test_ground_histogram_vertical_track_closed_form():
+    """A vertical track above the core: a photon emitted at path length s lands at r = (z0 - s - h_obs) tan(theta_c),
+    uniform in s, so the radial histogram is flat between r(L) and r(0), empty elsewhere, holds all n_b bunches with
+    total weight mu, and the mean arrival time of a bin lies between the closed-form times of its two edges."""
+    z0, L, h_obs = 10000.0, 400.0, 2000.0
+    seg = one_segment(x0=30.0, y0=-40.0, z0=z0, length=L, gamma=1e6)
+    par = W.default_params(bunch_size=0.05, seed=11)
+    st, f = O.preamble(ATM1, par, seg[0], 0)
+    assert st == 0 and f.n_b > 100000
+    r_max, n_bins = 120.0, 240
+    res = O.ground_histogram(ATM1, seg, par, (30.0, -40.0), r_max, n_bins)
+    h = res["hist"]
+    tan_c = f.sin_c / f.cos_c
+    r_hi, r_lo = (z0 - h_obs) * tan_c, (z0 - L - h_obs) * tan_c
+    assert 95.0 < r_lo < r_hi < 110.0
+    assert int(h["n"].sum()) == f.n_b and res["overflow"] == 0
+    assert math.isclose(h["sum_w"].sum(), f.n_b * f.w0, rel_tol=1e-12)
+    dr = r_max / n_bins
+    edges = np.arange(n_bins + 1) * dr
+    overlap = np.clip(np.minimum(edges[1:], r_hi) - np.maximum(edges[:-1], r_lo), 0.0, None)
+    expect = f.n_b * overlap / (r_hi - r_lo)
+    assert np.all(h["n"][overlap == 0.0] == 0)
+    assert np.all(np.abs(h["n"].astype(np.float64) - expect) <= 5.0 * np.sqrt(expect) + 1.0)
+    beta = math.sqrt(1.0 - 1e-12)
+    kappa = 0.01 * ATM1["eta0"] / ATM1["rho0"]
+
+    def t_of_r(r):                       # closed form along the vertical track: emission height from the landing radius
+        hgt = r / tan_c + h_obs
+        s = z0 - hgt
+        return s / (beta * C) + ((hgt - h_obs) / f.cos_c + kappa * (O.depth(ATM1, h_obs) - O.depth(ATM1, hgt)) / f.cos_c) / C
+
+    for b in np.nonzero(overlap > 0.5 * dr)[0]:
+        ta, tb = t_of_r(max(edges[b], r_lo)), t_of_r(min(edges[b + 1], r_hi))
+        mean_t = h["sum_wt"][b] / h["sum_w"][b]
+        assert min(ta, tb) - 1e-9 <= mean_t <= max(ta, tb) + 1e-9
+
+
+def test_ground_histogram_overflow_core_offset_and_profile_cut():
+    seg = one_segment(z0=10000.0, length=10.0, gamma=1e6)
+    par = W.default_params(bunch_size=0.05, seed=5)
+    st, f = O.preamble(ATM1, par, seg[0], 0)
+    # the ring (radius ~106 m about (0, 0)) seen from a core 1 km away: everything overflows a 120 m histogram
+    far = O.ground_histogram(ATM1, seg, par, (1000.0, 0.0), 120.0, 24)
+    assert far["overflow"] == f.n_b and int(far["hist"]["n"].sum()) == 0
+    # seen from a core 50 m away the distances spread over |106 - 50| .. 106 + 50
+    off = O.ground_histogram(ATM1, seg, par, (50.0, 0.0), 200.0, 40)
+    lo, hi = np.nonzero(off["hist"]["n"])[0][[0, -1]]
+    tan_c = f.sin_c / f.cos_c
+    assert lo == int(((8000.0 - 10.0) * tan_c - 50.0) // 5.0) and hi == int((8000.0 * tan_c + 50.0) // 5.0)
+    # Fig. 3 quantities: density = sum_w / annulus area, mean time = sum_wt / sum_w, bins under 50 photons masked
+    hist = np.zeros(3, dtype=O.HIST_DTYPE)
+    hist["n"], hist["sum_w"], hist["sum_wt"] = [49, 50, 1000], [49.0, 100.0, 500.0], [490.0, 300.0, 2500.0]
+    rc, dens, mt = O.profile(hist, 30.0)
+    assert np.allclose(rc, [5.0, 15.0, 25.0])
+    assert np.isnan(dens[0]) and np.isnan(mt[0])
+    assert math.isclose(dens[1], 100.0 / (math.pi * (400.0 - 100.0))) and math.isclose(mt[1], 3.0)
+    assert math.isclose(dens[2], 500.0 / (math.pi * (900.0 - 400.0))) and math.isclose(mt[2], 5.0)
+
+
+def test_ground_histogram_counts_every_downward_bunch():
+    """Conservation on a shower-shaped sample: bins + overflow = generated - upward."""
+    cfg = W.make_config("c2", n_segments=300)
+    res = O.ground_histogram(cfg["atmosphere"], cfg["segments"], cfg["params"], (0.0, 0.0), 500.0, 100)
+    cnt = dict(zip(O.COUNTER_NAMES, (int(v) for v in res["counters"])))
+    assert int(res["hist"]["n"].sum()) + res["overflow"] == cnt["generated"] - cnt["upward"] > 10000
+    assert res["overflow"] > 0 and np.count_nonzero(res["hist"]["n"]) > 50
