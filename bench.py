@@ -155,6 +155,9 @@ def main():
     ap.add_argument("--segments", type=int, default=None, help="override the segment count of the workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ground-hist", action="store_true",
+                    help="ground-plane radial profile mode (C8OPT_MODE_GROUND_HIST, PAPER.md:85-89) on the workload's "
+                         "segments: 1000 bins of 1 m about the shower axis; telescopes are not consulted")
     ap.add_argument("--cull", action="store_true",
                     help="segment culling on (C8OPT_FLAG_CULL): same tallies, `value` then counts culled bunches too")
     args = ap.parse_args()
@@ -193,9 +196,21 @@ def main():
     par = dict(cfg["params"])
     if args.cull:
         par["flags"] = c8.FLAG_CULL
+    if args.ground_hist:
+        par["mode"] = c8.MODE_GROUND_HIST
+        par["fl_beam_telescope"] = -1
     output_mode = par["mode"] == c8.MODE_OUTPUT
     ctx = c8.Context(cfg["atmosphere"])
     ctx.add_telescopes(tel)
+    if args.ground_hist:
+        ctx.set_ground_histogram(0.0, 0.0, 1000.0, 1000)
+
+    def read_counters():
+        """Synchronise, read the step's result back (D2H) and return the counters."""
+        if args.ground_hist:
+            return ctx.read_ground_histogram()[2]
+        return ctx.read_tallies()[1]
+
     h_seg = torch.from_numpy(seg.view(np.uint8).reshape(n, 48).copy()).pin_memory()
     d_seg = h_seg.to(dev)
     kw = {}
@@ -224,7 +239,7 @@ def main():
 
     for _ in range(args.warmup):
         step()
-    tallies, counters, tel_count = ctx.read_tallies()
+    counters = read_counters()
     photons_per_step = counters["generated"]
     culled_per_step = counters["culled"]
     hits_per_step = counters["hits"]
@@ -265,7 +280,7 @@ def main():
         for _ in range(2):
             ctx.reset_tallies()
             ctx.propagate_segments_host(h_seg, par, n=n, first_segment_id=first_id, **kw)
-            ctx.read_tallies()
+            read_counters()
         ke = max(3, min(args.steps, 20))
         torch.cuda.synchronize()
         if world > 1:
@@ -274,14 +289,14 @@ def main():
         for _ in range(ke):
             ctx.reset_tallies()
             ctx.propagate_segments_host(h_seg, par, n=n, first_segment_id=first_id, **kw)
-            ctx.read_tallies()                          # synchronises + D2H
+            read_counters()                             # synchronises + D2H
         dt = time.perf_counter() - t0
         if world > 1:
             t = torch.tensor([dt], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
         e2e = {"value": photons_all * ke / dt, "unit": UNIT, "h2d_bytes_per_step": int(n * 48),
-               "d2h_bytes_per_step": int(n_tel * 24 + 8 * 8 + n_tel * 8), "steps": ke,
+               "d2h_bytes_per_step": int(1001 * 24 + 8 * 8) if args.ground_hist else int(n_tel * 24 + 8 * 8 + n_tel * 8), "steps": ke,
                "note": "c8opt_propagate_segments_host from pinned host memory (chunked H2D overlapped with the kernels) "
                        "+ c8opt_read_tallies; wall clock"}
 
@@ -298,7 +313,9 @@ def main():
         roofline = {"bound": "hbm", "achieved": bytes_per_launch / per_launch_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                     "traffic": None, "peak_source": peaks["source"], "bytes_per_photon": RECORD_BYTES}
     else:
-        instr = ALG_INSTR.get(args.workload, 122.0)
+        # ground histogram: no pre-tests (-24) but every downward bunch is carried to the plane: v_x, v_y, arrival time
+        # (exp), wavelength, radius, bin, three shared-memory atomics (+ ~90); DESIGN.md §7
+        instr = 190.0 if args.ground_hist else ALG_INSTR.get(args.workload, 122.0)
         peak = 148 * 4 * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12            # thread-instructions / s, issue-slot peak
         # culled bunches cost no photon-loop instructions: the roofline counts the propagated ones only
         roofline = {"bound": "alu", "achieved": instr * (photons_per_step - culled_per_step) / per_launch_s / 1e12, "peak": peak,
@@ -314,7 +331,7 @@ def main():
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": cfg["name"], "segments_per_gpu": n, "photons_per_step_per_gpu": photons_per_step,
-                   "hits_per_step_per_gpu": hits_per_step, "telescopes": n_tel, "mode": "output" if output_mode else "tally",
+                   "hits_per_step_per_gpu": hits_per_step, "telescopes": n_tel, "mode": "ground histogram (1000 x 1 m)" if args.ground_hist else "output" if output_mode else "tally",
                    "l2": "flushed between steps (256 MiB fill, untimed)", "timing": "sum of per-step CUDA-event times",
                    "parallelism": f"segments sharded over {world} GPU(s), no data-path collective",
                    "culling": (f"on: {culled_per_step} of the bunches per step are generated but provably miss every telescope "

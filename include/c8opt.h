@@ -49,6 +49,11 @@ extern "C" {
 #define C8OPT_PROC_FLUORESCENCE  2u   /* bit 1 */
 #define C8OPT_MODE_TALLY   0u
 #define C8OPT_MODE_OUTPUT  1u
+/* Ground-plane radial profile (section 3.1 "Intensity & Timing Profile", Fig. 3a / 3b): every bunch
+ * that crosses the observation level z = h_obs going down is binned by its distance r from the shower core
+ * (c8opt_set_ground_histogram); a bin holds {n, sum w, sum w t} with the arrival time of R8 on that plane and the
+ * transmission weight of R17.  Telescopes are not consulted and none are needed (R26). */
+#define C8OPT_MODE_GROUND_HIST 2u
 /* c8opt_run_params.flags.  CULL: segment culling (Fig. 2 :63-65) in its exact, conservative form:
  * a Cherenkov segment whose emission cone provably misses every telescope sphere -- for every telescope k,
  * | angle(d, c_k - p_mid) - theta_c | > asin(R_k / D) + asin((L/2) / D), D = |c_k - p_mid| - L/2 -- skips the
@@ -93,7 +98,7 @@ typedef struct {
 typedef struct {
     uint64_t seed;                 /* Philox key = (seed[31:0], seed[63:32])  (R20)        */
     uint32_t processes;            /* C8OPT_PROC_* bits                                     */
-    uint32_t mode;                 /* C8OPT_MODE_TALLY or C8OPT_MODE_OUTPUT                 */
+    uint32_t mode;                 /* C8OPT_MODE_TALLY, C8OPT_MODE_OUTPUT or C8OPT_MODE_GROUND_HIST */
     double   lam1_nm, lam2_nm;     /* Cherenkov band (PAPER.md:45 integral over lambda)     */
     double   bunch_size;           /* B: n_b = ceil(mu / B) bunches of weight mu / n_b (R1) */
     double   fl_yield_per_MeV;     /* constant fluorescence yield (R13)        */
@@ -125,6 +130,11 @@ typedef struct {
 } c8opt_output;
 
 typedef struct { uint64_t hits; double sum_w; double sum_wt; } c8opt_tally;
+
+/* One radial bin of the ground-plane profile: bunches, sum of weights, sum of weight x arrival time [ns].
+ * Photon density = sum_w / (pi (r_hi^2 - r_lo^2)); mean arrival time = sum_wt / sum_w; the paper masks bins with
+ * fewer than 50 photons -- left to the caller. */
+typedef struct { uint64_t n; double sum_w; double sum_wt; } c8opt_hist_bin;
 
 /* indices into the counters[8] array of c8opt_read_tallies */
 enum {
@@ -173,6 +183,17 @@ int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, ui
  * copied); ARGUMENT if n_tel differs from the telescope count. */
 int c8opt_read_tallies(c8opt_ctx *ctx, c8opt_tally *host_out, int32_t n_tel,
                        uint64_t *counters, uint64_t *host_tel_count);
+
+/* Configure (n_bins in 1 .. 1024) or drop (n_bins == 0) the ground-plane radial profile: n_bins equal bins of
+ * width r_max_m / n_bins about the core (core_x_m, core_y_m) on the observation level of the atmosphere; bunches
+ * landing at r >= r_max_m are counted as overflow.  Allocates n_bins + 1 device bins, zeroed (and zeroed again by
+ * c8opt_reset_tallies).  Synchronises the device.  Errors: ARGUMENT, CUDA. */
+int c8opt_set_ground_histogram(c8opt_ctx *ctx, double core_x_m, double core_y_m, double r_max_m, int32_t n_bins);
+
+/* Wait for the device and copy the profile accumulated by the C8OPT_MODE_GROUND_HIST calls since the last reset to
+ * HOST memory: host_out[n_bins]; *overflow (may be NULL) = bunches beyond r_max; counters[8] (may be NULL) as in
+ * c8opt_read_tallies with HITS = bunches that reached the plane.  Errors: ARGUMENT (n_bins mismatch), CUDA. */
+int c8opt_read_ground_histogram(c8opt_ctx *ctx, c8opt_hist_bin *host_out, int32_t n_bins, uint64_t *overflow, uint64_t *counters);
 
 /* Zero tallies, counters and the per-telescope record cursors (asynchronous
  * on `cuda_stream`). */

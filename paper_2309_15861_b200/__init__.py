@@ -24,15 +24,16 @@ from .build import LIB_PATH, build  # noqa: F401
 
 MAX_LAYERS = 8
 PROC_CHERENKOV, PROC_FLUORESCENCE = 1, 2
-MODE_TALLY, MODE_OUTPUT = 0, 1
+MODE_TALLY, MODE_OUTPUT, MODE_GROUND_HIST = 0, 1, 2
 FLAG_CULL = 1
 COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "culled")
 TALLY_DTYPE = np.dtype([("hits", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
+HIST_DTYPE = np.dtype([("n", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
 RECORD_FLOATS = 7
 
 EXPORTS = ("c8opt_create_atmosphere", "c8opt_add_telescopes", "c8opt_propagate_segments",
            "c8opt_propagate_segments_host", "c8opt_read_tallies", "c8opt_reset_tallies", "c8opt_destroy",
-           "c8opt_last_error", "c8opt_launch_count")
+           "c8opt_last_error", "c8opt_launch_count", "c8opt_set_ground_histogram", "c8opt_read_ground_histogram")
 
 
 class C8optError(RuntimeError):
@@ -89,7 +90,9 @@ def lib():
         L.c8opt_last_error.restype = C.c_char_p
         L.c8opt_launch_count.argtypes = [vp]
         L.c8opt_launch_count.restype = C.c_uint64
-        for name in EXPORTS[:6]:
+        L.c8opt_set_ground_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_int32]
+        L.c8opt_read_ground_histogram.argtypes = [vp, vp, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+        for name in EXPORTS[:6] + EXPORTS[9:]:
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -141,6 +144,7 @@ class Context:
             d.tau = tau.ctypes.data_as(C.POINTER(C.c_float))
         self._h = C.c_void_p()
         self.n_tel = 0
+        self.hist_bins = 0
         rc = lib().c8opt_create_atmosphere(C.byref(d), C.byref(self._h))
         if rc != 0:
             raise C8optError(rc, lib().c8opt_last_error(None).decode())
@@ -191,6 +195,19 @@ class Context:
                                              tel_count.ctypes.data_as(C.POINTER(C.c_uint64))),
                     allow=(-3,) if allow_overflow else ())
         return tallies, dict(zip(COUNTER_NAMES, (int(c) for c in counters))), tel_count
+
+    def set_ground_histogram(self, core_x: float, core_y: float, r_max: float, n_bins: int):
+        self._check(lib().c8opt_set_ground_histogram(self._h, float(core_x), float(core_y), float(r_max), int(n_bins)))
+        self.hist_bins = int(n_bins)
+
+    def read_ground_histogram(self):
+        """Synchronises; returns (bins[n_bins] of {n, sum_w, sum_wt}, overflow, counters dict)."""
+        bins = np.zeros(self.hist_bins, dtype=HIST_DTYPE)
+        over = C.c_uint64(0)
+        counters = np.zeros(8, dtype=np.uint64)
+        self._check(lib().c8opt_read_ground_histogram(self._h, bins.ctypes.data, self.hist_bins, C.byref(over),
+                                                      counters.ctypes.data_as(C.POINTER(C.c_uint64))))
+        return bins, int(over.value), dict(zip(COUNTER_NAMES, (int(c) for c in counters)))
 
     def reset_tallies(self, stream=None):
         self._check(lib().c8opt_reset_tallies(self._h, _stream(stream)))

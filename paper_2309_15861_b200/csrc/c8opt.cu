@@ -34,6 +34,10 @@ struct c8opt_ctx {
     std::vector<double> tel_xyzr;          // absolute, as given (float -> double)
     double x_ref = 0, y_ref = 0, z_ref = 0;
     float cull_Rb = 0;                 // radius about the reference point that holds every telescope sphere
+    // ground-plane radial profile (C8OPT_MODE_GROUND_HIST)
+    c8::Tally *d_hist = nullptr;       // [hist_bins + 1], the last one counts the overflow
+    int hist_bins = 0;
+    double hist_core_x = 0, hist_core_y = 0, hist_r_max = 0;
     float4 *d_telA = nullptr;
     float *d_telT = nullptr;
     std::vector<float4> h_telA;
@@ -86,14 +90,17 @@ double host_depth(const c8opt_ctx *c, double h)
     return c->layer[i].a + c->layer[i].b * std::exp(-h / c->layer[i].c);
 }
 
-size_t smem_bytes(bool out) { return sizeof(c8::TileSmem) + (out ? sizeof(c8::OutSmem) : 0); }
+size_t smem_bytes(int mode)
+{
+    return sizeof(c8::TileSmem) + (mode == c8::MODE_OUT ? sizeof(c8::OutSmem) : mode == c8::MODE_HIST ? sizeof(c8::HistSmem) : 0);
+}
 
 typedef void (*kernel_t)(const c8::KParams);
 
 template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar, bool out)
 {
-    if (out) return coplanar ? c8::propagate_kernel<TELSRC, true, NT, true> : c8::propagate_kernel<TELSRC, false, NT, true>;
-    return coplanar ? c8::propagate_kernel<TELSRC, true, NT, false> : c8::propagate_kernel<TELSRC, false, NT, false>;
+    if (out) return coplanar ? c8::propagate_kernel<TELSRC, true, NT, c8::MODE_OUT> : c8::propagate_kernel<TELSRC, false, NT, c8::MODE_OUT>;
+    return coplanar ? c8::propagate_kernel<TELSRC, true, NT, c8::MODE_TALLY> : c8::propagate_kernel<TELSRC, false, NT, c8::MODE_TALLY>;
 }
 
 // nt = number of constant-bank telescope slots the hot loop tests (n_tel rounded up to 1, 4 or 8)
@@ -185,10 +192,15 @@ bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
 int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *out, c8::KParams *kp)
 {
     if (!rp) return fail(ctx, C8OPT_ERR_ARGUMENT, "params is NULL");
-    if (ctx->n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no telescopes: call c8opt_add_telescopes first");
+    const bool hist = rp->mode == C8OPT_MODE_GROUND_HIST;
+    if (!hist && ctx->n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no telescopes: call c8opt_add_telescopes first");
+    if (hist && ctx->hist_bins < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no histogram: call c8opt_set_ground_histogram first");
+    if (hist && rp->flags) return fail(ctx, C8OPT_ERR_ARGUMENT, "flags must be 0 in ground-histogram mode (every bunch counts)");
+    if (hist && (rp->processes & C8OPT_PROC_FLUORESCENCE) && rp->fl_beam_telescope >= 0)
+        return fail(ctx, C8OPT_ERR_ARGUMENT, "ground-histogram mode has no telescope to beam at");
     const unsigned procs = rp->processes;
     if (procs == 0 || (procs & ~3u)) return fail(ctx, C8OPT_ERR_ARGUMENT, "processes must be a combination of bits 0 and 1");
-    if (rp->mode > 1u) return fail(ctx, C8OPT_ERR_ARGUMENT, "mode must be 0 (tally) or 1 (photon output)");
+    if (rp->mode > 2u) return fail(ctx, C8OPT_ERR_ARGUMENT, "mode must be 0 (tally), 1 (photon output) or 2 (ground histogram)");
     if (rp->flags & ~C8OPT_FLAG_CULL) return fail(ctx, C8OPT_ERR_ARGUMENT, "unknown bit in flags");
     if (!(rp->bunch_size > 0.0) || !std::isfinite(rp->bunch_size)) return fail(ctx, C8OPT_ERR_ARGUMENT, "bunch_size must be > 0");
     if (procs & C8OPT_PROC_CHERENKOV)
@@ -196,7 +208,7 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     if (procs & C8OPT_PROC_FLUORESCENCE) {
         if (!(rp->fl_yield_per_MeV >= 0.0) || !(rp->fl_lam1_nm > 0.0) || !(rp->fl_lam2_nm >= rp->fl_lam1_nm))
             return fail(ctx, C8OPT_ERR_ARGUMENT, "bad fluorescence yield / band");
-        if (rp->fl_beam_telescope >= ctx->n_tel) return fail(ctx, C8OPT_ERR_ARGUMENT, "fl_beam_telescope out of range");
+        if (!hist && rp->fl_beam_telescope >= ctx->n_tel) return fail(ctx, C8OPT_ERR_ARGUMENT, "fl_beam_telescope out of range");
         if (rp->fl_beam_telescope >= 0 && !(rp->fl_beam_halfangle_rad > 0.0 && rp->fl_beam_halfangle_rad <= 3.14159265358979323846))
             return fail(ctx, C8OPT_ERR_ARGUMENT, "fl_beam_halfangle_rad must be in (0, pi]");
     }
@@ -248,6 +260,17 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
         P.omc = 2.0 * sh * sh;
     }
     P.tallies = ctx->d_tallies; P.counters = ctx->d_counters; P.cursors = ctx->d_cursors;
+    if (hist) {
+        // R26: the profile is taken on the observation level about the core; the kernel sees one accept-all detector
+        // there (R^2 = 1e30), so a hit's (x, y) is the plane crossing relative to the core.
+        P.n_tel = 1; P.telA = nullptr; P.telT = nullptr; P.tallies = nullptr; P.cursors = nullptr;
+        for (int k = 0; k < c8::kTelConstMax; ++k) { P.tel_c[k] = make_float4(0.f, 0.f, 0.f, -1.f); P.telT_c[k] = 0.f; }
+        P.tel_c[0] = make_float4(0.f, 0.f, 0.f, 1e30f);
+        P.telT_c[0] = (float)host_depth(ctx, ctx->h_obs);
+        P.x_ref = ctx->hist_core_x; P.y_ref = ctx->hist_core_y; P.z_ref = ctx->h_obs; P.z_ref_f = (float)ctx->h_obs;
+        P.n_grid_levels = 0; P.grid = nullptr;
+        P.hist = ctx->d_hist; P.hist_bins = ctx->hist_bins; P.hist_inv_dr = (float)(ctx->hist_bins / ctx->hist_r_max);
+    }
     if (out) {
         if (rp->mode == C8OPT_MODE_OUTPUT) {
             P.records = out->records; P.tel_offset = (const unsigned long long *)out->tel_offset;
@@ -267,9 +290,14 @@ int launch(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, const c8opt_segment *d
     const unsigned long long per_tile = c8::kTile / P.n_procs;
     const unsigned long long tiles = (n + per_tile - 1) / per_tile;
     if (tiles > 0x7fffffffull) return fail(ctx, C8OPT_ERR_ARGUMENT, "too many segments in one call");
-    const bool out = P.records != nullptr;
-    kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out);
-    k<<<(unsigned)tiles, c8::kTile, smem_bytes(out), st>>>(P);
+    if (mode == C8OPT_MODE_GROUND_HIST) {
+        // one accept-all detector on the observation level: brute-force kernel with a single coplanar slot
+        c8::propagate_kernel<c8::TEL_CONST, true, 1, c8::MODE_HIST><<<(unsigned)tiles, c8::kTile, smem_bytes(c8::MODE_HIST), st>>>(P);
+    } else {
+        const bool out = P.records != nullptr;
+        kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out);
+        k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY), st>>>(P);
+    }
     C8_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
     ctx->segments_total += n;
@@ -340,7 +368,10 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
         for (int nt = 1; nt <= 8 && e == cudaSuccess; nt *= (nt == 1 ? 4 : 2))
             for (int cp = 0; cp < 4 && e == cudaSuccess; ++cp)
                 e = cudaFuncSetAttribute(pick_kernel(ts, (cp & 1) != 0, nt, (cp & 2) != 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)smem_bytes((cp & 2) != 0));
+                                         (int)smem_bytes((cp & 2) ? c8::MODE_OUT : c8::MODE_TALLY));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(c8::propagate_kernel<c8::TEL_CONST, true, 1, c8::MODE_HIST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)smem_bytes(c8::MODE_HIST));
     if (e != cudaSuccess) {
         fail(nullptr, C8OPT_ERR_CUDA, "context setup: %s", cudaGetErrorString(e));
         c8opt_destroy(ctx);
@@ -518,7 +549,54 @@ int c8opt_reset_tallies(c8opt_ctx *ctx, void *cuda_stream)
         C8_CUDA(ctx, cudaMemsetAsync(ctx->d_tallies, 0, sizeof(c8::Tally) * ctx->n_tel, st));
         C8_CUDA(ctx, cudaMemsetAsync(ctx->d_cursors, 0, sizeof(unsigned long long) * ctx->n_tel, st));
     }
+    if (ctx->d_hist) C8_CUDA(ctx, cudaMemsetAsync(ctx->d_hist, 0, sizeof(c8::Tally) * (ctx->hist_bins + 1), st));
     ctx->segments_total = 0;
+    return C8OPT_OK;
+}
+
+int c8opt_set_ground_histogram(c8opt_ctx *ctx, double core_x_m, double core_y_m, double r_max_m, int32_t n_bins)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    if (n_bins < 0 || n_bins > c8::kHistMax) return fail(ctx, C8OPT_ERR_ARGUMENT, "n_bins must be 0 .. %d", c8::kHistMax);
+    if (n_bins > 0 && (!std::isfinite(core_x_m) || !std::isfinite(core_y_m) || !(r_max_m > 0.0) || !std::isfinite(r_max_m)))
+        return fail(ctx, C8OPT_ERR_ARGUMENT, "need a finite core and r_max > 0");
+    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    C8_CUDA(ctx, cudaDeviceSynchronize());
+    cudaFree(ctx->d_hist);
+    ctx->d_hist = nullptr; ctx->hist_bins = 0;
+    if (n_bins == 0) return C8OPT_OK;
+    C8_CUDA(ctx, cudaMalloc(&ctx->d_hist, sizeof(c8::Tally) * (n_bins + 1)));
+    C8_CUDA(ctx, cudaMemset(ctx->d_hist, 0, sizeof(c8::Tally) * (n_bins + 1)));
+    ctx->hist_bins = n_bins; ctx->hist_core_x = core_x_m; ctx->hist_core_y = core_y_m; ctx->hist_r_max = r_max_m;
+    return C8OPT_OK;
+}
+
+int c8opt_read_ground_histogram(c8opt_ctx *ctx, c8opt_hist_bin *host_out, int32_t n_bins, uint64_t *overflow, uint64_t *counters)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    if (!host_out) return fail(ctx, C8OPT_ERR_ARGUMENT, "host_out is NULL");
+    if (n_bins != ctx->hist_bins || n_bins < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "n_bins = %d but the context has %d bins", n_bins, ctx->hist_bins);
+    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    C8_CUDA(ctx, cudaDeviceSynchronize());
+    static_assert(sizeof(c8opt_hist_bin) == sizeof(c8::Tally), "histogram bin layout");
+    C8_CUDA(ctx, cudaMemcpy(host_out, ctx->d_hist, sizeof(c8::Tally) * n_bins, cudaMemcpyDeviceToHost));
+    c8::Tally over;
+    C8_CUDA(ctx, cudaMemcpy(&over, ctx->d_hist + n_bins, sizeof(over), cudaMemcpyDeviceToHost));
+    if (overflow) *overflow = over.hits;
+    if (counters) {
+        unsigned long long cnt[8];
+        C8_CUDA(ctx, cudaMemcpy(cnt, ctx->d_counters, sizeof(cnt), cudaMemcpyDeviceToHost));
+        unsigned long long inside = 0;
+        for (int b = 0; b < n_bins; ++b) inside += host_out[b].n;
+        counters[C8OPT_CNT_SEGMENTS] = ctx->segments_total;
+        counters[C8OPT_CNT_GENERATED] = cnt[1];
+        counters[C8OPT_CNT_UPWARD] = cnt[2];
+        counters[C8OPT_CNT_HITS] = inside + over.hits;
+        counters[C8OPT_CNT_RECORDS] = 0;
+        counters[C8OPT_CNT_DROPPED] = 0;
+        counters[C8OPT_CNT_INVALID] = cnt[6];
+        counters[C8OPT_CNT_CULLED] = cnt[7];
+    }
     return C8OPT_OK;
 }
 
@@ -533,7 +611,7 @@ void c8opt_destroy(c8opt_ctx *ctx)
     }
     for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
     cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_grid);
-    cudaFree(ctx->d_tallies); cudaFree(ctx->d_counters); cudaFree(ctx->d_cursors);
+    cudaFree(ctx->d_tallies); cudaFree(ctx->d_counters); cudaFree(ctx->d_cursors); cudaFree(ctx->d_hist);
     cudaGetLastError();
     delete ctx;
 }

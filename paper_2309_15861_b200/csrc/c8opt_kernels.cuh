@@ -40,6 +40,8 @@ constexpr int kDenseMin = 16;         // candidates in one warp iteration from w
 constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
 constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
 constexpr uint32_t kFlagCull = 1u;    // == C8OPT_FLAG_CULL
+constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
+constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
@@ -101,6 +103,10 @@ struct KParams {
     unsigned long long *cursors;   // device [n_tel]  (photon-output mode)
     float *records; const unsigned long long *tel_offset, *tel_capacity;
     unsigned long long *ids; uint32_t *counts;
+    // ground-plane radial profile (MODE_HIST): bins [hist_bins] + one overflow bin, about (x_ref, y_ref) on z_ref = h_obs
+    Tally *hist;
+    int hist_bins;
+    float hist_inv_dr;
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
@@ -209,12 +215,20 @@ struct OutSmem {
     int staged_any;
 };
 
-template <bool OUT> __device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
+__device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
 {
-    static_assert(OUT, "only photon-output kernels carry the staging area");
     static_assert(sizeof(TileSmem) % 16 == 0, "OutSmem must stay 16-byte aligned");
     return *reinterpret_cast<OutSmem *>(&sm + 1);
 }
+
+// Ground-histogram kernel only (follows TileSmem in dynamic shared memory): the tile's private radial histogram.
+struct HistSmem {
+    uint32_t n[kHistMax];
+    float sw[kHistMax], swt[kHistMax];
+    uint32_t overflow;
+};
+
+__device__ __forceinline__ HistSmem &hist_smem(TileSmem &sm) { return *reinterpret_cast<HistSmem *>(&sm + 1); }
 
 // frame slots.  Axis-relative Cherenkov (KIND_CHER_AXIS):
 //   F_NEGL   -L                      F_K0C  K0 + (1-2^-24) L,  K0 = -(z0 - z_ref)/d_z  (axis path length to the plane)
@@ -709,15 +723,33 @@ __device__ __forceinline__ bool flush_round(const KParams &P, OutSmem &os, bool 
 }
 
 // a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes together.
-template <bool OUT>
+template <int MODE>
 __device__ __forceinline__ void commit_hits(const KParams &P, TileSmem &sm, const Hit &h, uint64_t id)
 {
     const uint32_t okm = __ballot_sync(0xffffffffu, h.ok);
     if (okm == 0u) return;
+    if constexpr (MODE == MODE_HIST) {
+        // ground-plane radial profile: h.x, h.y are relative to the core on the plane z = h_obs
+        HistSmem &hs = hist_smem(sm);
+        bool over = false;
+        if (h.ok) {
+            const float r2 = fmaf(h.x, h.x, h.y * h.y);
+            const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
+            const float fb = r * P.hist_inv_dr;
+            over = !(fb < (float)P.hist_bins);
+            if (!over) {
+                const int b = (int)fb;
+                atomicAdd(&hs.n[b], 1u); atomicAdd(&hs.sw[b], h.w); atomicAdd(&hs.swt[b], h.w * h.t);
+            }
+        }
+        const uint32_t om = __ballot_sync(0xffffffffu, over);
+        if (om && lane_id() == 0u) atomicAdd(&hs.overflow, (uint32_t)__popc(om));
+        return;
+    }
     if (h.ok) accumulate_hit(P, sm, h);
-    if constexpr (OUT) {
+    if constexpr (MODE == MODE_OUT) {
         const int k0 = __shfl_sync(0xffffffffu, h.k, __ffs(okm) - 1);
-        if (__all_sync(0xffffffffu, !h.ok || h.k == k0)) write_records_one_tel(P, out_smem<OUT>(sm), h, id, okm, k0);
+        if (__all_sync(0xffffffffu, !h.ok || h.k == k0)) write_records_one_tel(P, out_smem(sm), h, id, okm, k0);
         else write_records_grouped(P, h, id);
     }
 }
@@ -729,7 +761,7 @@ __device__ __forceinline__ unsigned long long emitter_segment(const KParams &P, 
     return tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
 }
 
-template <int TELSRC, bool OUT>
+template <int TELSRC, int MODE>
 __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t head, uint32_t n)
 {
     // lanes 0 .. n-1 take one entry each; the others only take part in the warp-wide commit
@@ -747,13 +779,13 @@ __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigne
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
     __syncwarp();
-    commit_hits<OUT>(P, sm, h, id);
+    commit_hits<MODE>(P, sm, h, id);
 }
 
 // Dense path: when at least kDenseMin lanes of a warp iteration hold a candidate, the pairs are evaluated on the spot
 // from the random words the lanes still hold (no queue; the axis kind also skips the second Philox, the generic kinds
 // redraw theirs).  `has` says which lanes take part; all 32 call.
-template <int TELSRC, bool OUT>
+template <int TELSRC, int MODE>
 __device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned long long tile_first, int e, uint32_t j,
                                         uint32_t r0, uint32_t r1, uint32_t r2, int k, bool has)
 {
@@ -767,12 +799,12 @@ __device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
     __syncwarp();
-    commit_hits<OUT>(P, sm, h, id);
+    commit_hits<MODE>(P, sm, h, id);
 }
 
 // Push the candidates of this iteration (per lane: bit c of `cm` set = candidate number c, whose telescope
 // index is tel_of(c)) and drain 32 entries whenever that many are queued.  All 32 lanes call it together.
-template <int TELSRC, bool OUT, typename TelOf>
+template <int TELSRC, int MODE, typename TelOf>
 __device__ __forceinline__ void push_candidates(const KParams &P, TileSmem &sm, unsigned long long tile_first,
                                                 uint32_t &q_head, uint32_t &q_count, uint32_t cm, int e, uint32_t j, TelOf tel_of)
 {
@@ -789,7 +821,7 @@ __device__ __forceinline__ void push_candidates(const KParams &P, TileSmem &sm, 
         q_count += (uint32_t)__popc(have);
         __syncwarp();
         if (q_count >= 32u) {
-            drain_queue<TELSRC, OUT>(P, sm, tile_first, q_head, 32u);
+            drain_queue<TELSRC, MODE>(P, sm, tile_first, q_head, 32u);
             __syncwarp();
             q_head = (q_head + 32u) & (kQueue - 1);
             q_count -= 32u;
@@ -871,7 +903,7 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
 // photon from the counter and tests every telescope (the table is read at warp-uniform addresses) with a
 // conservative distance test (cross product, no plane projection: valid for any v_z); the survivors go through the
 // candidate queue like all others.
-template <int TELSRC, bool OUT>
+template <int TELSRC, int MODE>
 __device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
                                         uint32_t &q_count, uint32_t n)
 {
@@ -903,12 +935,12 @@ __device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned
             }
         }
         if (__any_sync(0xffffffffu, cm != 0u))
-            push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return (uint32_t)(k0 + c); });
+            push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return (uint32_t)(k0 + c); });
     }
 }
 
 // Append the photons of the lanes in `wide` to the warp's list and process a batch when 32 are waiting.
-template <int TELSRC, bool OUT>
+template <int TELSRC, int MODE>
 __device__ __forceinline__ void wide_push(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t &q_head,
                                           uint32_t &q_count, uint32_t wide, int e, uint32_t j)
 {
@@ -919,7 +951,7 @@ __device__ __forceinline__ void wide_push(const KParams &P, TileSmem &sm, unsign
     n += (uint32_t)__popc(wide);
     __syncwarp();
     if (n >= 32u) {
-        wide_batch<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, 32u);
+        wide_batch<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, 32u);
         __syncwarp();
         const uint32_t moved = (lane < n - 32u) ? sm.wide_list[warp][32u + lane] : 0u;
         __syncwarp();
@@ -953,7 +985,7 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
     return AxisFrame{A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, C.y, C.z};
 }
 
-template <int TELSRC, bool COPLANAR, int NT, bool OUT>
+template <int TELSRC, bool COPLANAR, int NT, int MODE>
 __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_constant__ KParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -969,10 +1001,16 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     sm.invalid[tid] = 0;
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
     if (tid < kWarps) sm.wide_count[tid] = 0u;
+    constexpr bool OUT = (MODE == MODE_OUT);
     if constexpr (OUT) {
-        OutSmem &os = out_smem<OUT>(sm);
+        OutSmem &os = out_smem(sm);
         if (tid < kWarps) { os.wn[tid] = 0u; os.wk[tid] = -1; }
         if (tid == 0) { os.rounds = 1; os.staged_any = 0; }
+    }
+    if constexpr (MODE == MODE_HIST) {
+        HistSmem &hs = hist_smem(sm);
+        for (int b = tid; b < P.hist_bins; b += kTile) { hs.n[b] = 0u; hs.sw[b] = 0.0f; hs.swt[b] = 0.0f; }
+        if (tid == 0) hs.overflow = 0u;
     }
     __syncthreads();
 
@@ -1115,41 +1153,41 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             } else {
                 const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
                 if (wide) {
-                    wide_push<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, wide, e, j);
+                    wide_push<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, wide, e, j);
                     if (cm == kAllTelescopes) cm = 0u;
                 }
             }
             const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
-            if constexpr (OUT) {
+            if constexpr (MODE != MODE_TALLY) {
                 if (__popc(have) >= kDenseMin) {
                     // dense iteration: each lane's first candidate is evaluated on the spot, further ones are queued
                     const bool has = cm != 0u;
                     int k = 0;
                     if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
-                    dense_eval<TELSRC, OUT>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, k, has);
+                    dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, k, has);
                 }
                 if (__any_sync(0xffffffffu, cm != 0u))
-                    push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
-                if (rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
-                    OutSmem &os = out_smem<OUT>(sm);
+                    push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+                if (OUT && rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
+                    OutSmem &os = out_smem(sm);
                     // nothing staged in round 0: a sparse tile, which goes on without rounds (and barriers)
                     const bool first = it < (uint32_t)kRound;
                     if (!flush_round(P, os, first) && first) rounds = false;
                 }
             } else {
                 if (have)
-                    push_candidates<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+                    push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
             }
         }
         if constexpr (TELSRC != TEL_CONST) {
             __syncwarp();
             const uint32_t nw = sm.wide_count[warp];
-            if (nw) wide_batch<TELSRC, OUT>(P, sm, tile_first, q_head, q_count, nw);
+            if (nw) wide_batch<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, nw);
         }
-        if (q_count) drain_queue<TELSRC, OUT>(P, sm, tile_first, q_head, q_count);
+        if (q_count) drain_queue<TELSRC, MODE>(P, sm, tile_first, q_head, q_count);
         if constexpr (OUT) {
             // records the last drain staged (the tile is still in rounds mode): one more flush
-            if (rounds) flush_round(P, out_smem<OUT>(sm), false);
+            if (rounds) flush_round(P, out_smem(sm), false);
         }
         flush_accumulator(P, sm);
     }
@@ -1169,6 +1207,20 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         uint32_t nbad = (tid < segs_per_tile) ? sm.invalid[tid] : 0u;
         nbad = __reduce_add_sync(0xffffffffu, nbad);
         if (lane == 0 && nbad) atomicAdd(&P.counters[6], (unsigned long long)nbad);
+    }
+    if constexpr (MODE == MODE_HIST) {
+        // the tile's histogram into the global one (the barrier above ordered the warps' updates); bin hist_bins = overflow
+        HistSmem &hs = hist_smem(sm);
+        for (int b = tid; b < P.hist_bins; b += kTile) {
+            const uint32_t c = hs.n[b];
+            if (c) {
+                atomicAdd(&P.hist[b].hits, (unsigned long long)c);
+                atomicAdd(&P.hist[b].sum_w, (double)hs.sw[b]);
+                atomicAdd(&P.hist[b].sum_wt, (double)hs.swt[b]);
+            }
+        }
+        if (tid == 0 && hs.overflow) atomicAdd(&P.hist[P.hist_bins].hits, (unsigned long long)hs.overflow);
+        return;
     }
     if (tally_in_smem) {
         for (int k = tid; k < P.n_tel; k += kTile) {

@@ -185,3 +185,71 @@ def compare(cfg: dict, g: dict, o: dict, first_id: int = 0, check_records: bool 
             assert abs(tg - to) <= TOL_TALLY_REL * abs(to) + TOL_T_NS * abs(wo), f"(d) telescope {k} sum_wt: {tg} vs {to}"
     rep["flip_list"] = flips
     return rep
+
+
+def gpu_hist(cfg: dict, core, r_max: float, n_bins: int, first_id: int = 0, chunks: int = 1):
+    """Ground-plane radial profile of cfg through the CUDA path (C8OPT_MODE_GROUND_HIST)."""
+    import torch
+
+    import paper_2309_15861_b200 as c8
+
+    seg = cfg["segments"]
+    n = len(seg)
+    par = dict(cfg["params"])
+    par["mode"] = c8.MODE_GROUND_HIST
+    ctx = c8.Context(cfg["atmosphere"])
+    ctx.set_ground_histogram(core[0], core[1], r_max, n_bins)
+    dev = torch.device("cuda:0")
+    d_counts = torch.zeros((n, 2), dtype=torch.int32, device=dev)
+    d_seg = torch.from_numpy(seg.view(np.uint8).reshape(n, 48).copy()).to(dev)
+    bounds = [n * i // chunks for i in range(chunks + 1)]
+    for lo, hi in zip(bounds[:-1], bounds[1:]):
+        ctx.propagate_segments(d_seg[lo:], par, n=hi - lo, first_segment_id=first_id + lo, counts=d_counts[lo:])
+    bins, over, counters = ctx.read_ground_histogram()
+    out = dict(hist=bins, overflow=over, counters=counters, counts=d_counts.cpu().numpy().astype(np.uint32),
+               launches=ctx.launch_count)
+    ctx.close()
+    return out
+
+
+def compare_hist(g: dict, o: dict, r_max: float, n_bins: int, edge_m: float = 2e-3) -> dict:
+    """Per-bin parity of the radial profile.  A bunch within `edge_m` of a bin edge may fall on either side in fp32
+    (positions agree to well under a millimetre, criterion (c)); those are counted from the oracle's radii and bound
+    the per-bin difference.  Bins with at least 50 bunches (the paper's cut): sum of weights within 1e-3
+    relative beyond the edge bunches, mean arrival time within 0.1 ns (criterion (d))."""
+    assert np.array_equal(g["counts"], o["counts"]), "criterion (a): per-segment bunch counts differ"
+    gh, oh = g["hist"], o["hist"]
+    dr = r_max / n_bins
+    r = o["r"]
+    frac = r / dr - np.floor(r / dr)
+    near = (np.minimum(frac, 1.0 - frac) * dr <= edge_m)
+    b_lo = np.floor((r - edge_m) / dr).astype(np.int64)
+    b_hi = np.floor((r + edge_m) / dr).astype(np.int64)
+    slack = np.zeros(n_bins + 1, dtype=np.int64)
+    for b in (b_lo[near], b_hi[near]):
+        np.add.at(slack, np.clip(b, 0, n_bins), 1)
+    dn = np.abs(gh["n"].astype(np.int64) - oh["n"].astype(np.int64))
+    assert np.all(dn <= slack[:n_bins]), (np.nonzero(dn > slack[:n_bins])[0][:10], dn.max())
+    total_g, total_o = int(gh["n"].sum()) + g["overflow"], int(oh["n"].sum()) + o["overflow"]
+    assert abs(total_g - total_o) <= max(2, int(1e-5 * total_o)), (total_g, total_o)
+    assert abs(g["overflow"] - o["overflow"]) <= slack[n_bins] + max(2, int(1e-5 * total_o))
+    big = (oh["n"] >= 50) & (gh["n"] >= 50)
+    w_mean = oh["sum_w"][big] / oh["n"][big]
+    dw = np.abs(gh["sum_w"][big] - oh["sum_w"][big])
+    assert np.all(dw <= 1e-3 * oh["sum_w"][big] + 2.0 * slack[:n_bins][big] * w_mean)
+    # mean time: a bunch near an edge may sit in either bin, which moves that bin's mean by at most w |t - mean| / sum_w;
+    # beyond the sum of those (enumerated from the oracle's records) the means agree within 0.1 ns
+    rec = o["records"]
+    w_all, t_all = rec["w"].astype(np.float64), rec["t"].astype(np.float64)
+    mt_full = np.where(oh["sum_w"] > 0, oh["sum_wt"] / np.maximum(oh["sum_w"], 1e-300), 0.0)
+    infl = np.zeros(n_bins + 1)
+    for b in (b_lo[near], b_hi[near]):
+        bc = np.clip(b, 0, n_bins)
+        np.add.at(infl, bc, w_all[near] * np.abs(t_all[near] - np.append(mt_full, 0.0)[bc]))
+    mt_g, mt_o = gh["sum_wt"][big] / gh["sum_w"][big], oh["sum_wt"][big] / oh["sum_w"][big]
+    dt = np.abs(mt_g - mt_o) - 1.05 * infl[:n_bins][big] / oh["sum_w"][big]
+    assert np.all(dt <= TOL_T_NS), dt.max()
+    return dict(bunches=total_o, overflow_gpu=g["overflow"], overflow_oracle=o["overflow"], bins_ge50=int(big.sum()),
+                bins_differing=int(np.count_nonzero(dn)), max_dn=int(dn.max()), edge_bunches=int(near.sum()),
+                max_dmean_t_ns=float(dt.max()) if dt.size else 0.0,
+                max_dsumw_rel=float(np.max(dw / oh["sum_w"][big])) if dw.size else 0.0)

@@ -258,3 +258,45 @@ def test_segment_culling_non_coplanar_big_spheres(c8):
     rep = pu.compare(cfg, g, o, check_upward=False)
     _report("cull-noncoplanar", rep)
     assert g["counters"]["culled"] > 0 and rep["matched"] > 1000
+
+
+@pytest.mark.parametrize("name,n,r_max,n_bins,core", [("c2", 30_000, 500.0, 1000, (0.0, 0.0)),
+                                                      ("c4", 20_000, 2000.0, 500, (15.0, -25.0)),
+                                                      ("c1", 2_000, 300.0, 64, (0.0, 0.0)),
+                                                      ("c2", 1, 500.0, 1024, (0.0, 0.0))])
+def test_ground_histogram(c8, name, n, r_max, n_bins, core):
+    """C8OPT_MODE_GROUND_HIST (Fig. 3): radial photon density and arrival-time profile on the
+    observation level against the oracle's binning of the accept-all plane records."""
+    import oracle
+    import parity_util as pu
+    cfg = wl.make_config(name, n_segments=n)
+    g = pu.gpu_hist(cfg, core, r_max, n_bins, chunks=2 if n > 1 else 1)
+    o = oracle.ground_histogram(cfg["atmosphere"], cfg["segments"], cfg["params"], core, r_max, n_bins, threads=pu.n_threads())
+    rep = pu.compare_hist(g, o, r_max, n_bins)
+    print(f"[hist {name}-{n}] " + " ".join(f"{k}={v}" for k, v in rep.items()))
+    assert g["counters"]["generated"] == int(o["counts"].astype(np.uint64).sum())
+    if n > 1000:
+        assert rep["bins_ge50"] > 20
+
+
+def test_ground_histogram_needs_configuration_and_resets(c8):
+    import torch
+    cfg = wl.make_config("c1", n_segments=500)
+    par = dict(cfg["params"], mode=c8.MODE_GROUND_HIST)
+    ctx = c8.Context(cfg["atmosphere"])
+    d_seg = torch.from_numpy(cfg["segments"].view(np.uint8).reshape(-1, 48).copy()).to("cuda:0")
+    with pytest.raises(c8.C8optError):
+        ctx.propagate_segments(d_seg, par, n=500, first_segment_id=0)          # no histogram configured
+    ctx.set_ground_histogram(0.0, 0.0, 300.0, 30)
+    with pytest.raises(c8.C8optError):
+        ctx.propagate_segments(d_seg, dict(par, flags=c8.FLAG_CULL), n=500, first_segment_id=0)
+    ctx.propagate_segments(d_seg, par, n=500, first_segment_id=0)
+    a, over_a, cnt = ctx.read_ground_histogram()
+    assert int(a["n"].sum()) + over_a == cnt["generated"] - cnt["upward"] == cnt["hits"] > 1000
+    ctx.propagate_segments(d_seg, par, n=500, first_segment_id=0)                # accumulates
+    b, over_b, _ = ctx.read_ground_histogram()
+    assert np.array_equal(b["n"], 2 * a["n"]) and over_b == 2 * over_a
+    ctx.reset_tallies()
+    c, over_c, _ = ctx.read_ground_histogram()
+    assert int(c["n"].sum()) == 0 and over_c == 0
+    ctx.close()
