@@ -270,6 +270,7 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
         P.x_ref = ctx->hist_core_x; P.y_ref = ctx->hist_core_y; P.z_ref = ctx->h_obs; P.z_ref_f = (float)ctx->h_obs;
         P.n_grid_levels = 0; P.grid = nullptr;
         P.hist = ctx->d_hist; P.hist_bins = ctx->hist_bins; P.hist_inv_dr = (float)(ctx->hist_bins / ctx->hist_r_max);
+        P.hist_wscale = (float)(65536.0 / rp->bunch_size); P.hist_winv = 1.0 / (double)P.hist_wscale;
     }
     if (out) {
         if (rp->mode == C8OPT_MODE_OUTPUT) {
