@@ -36,6 +36,7 @@ constexpr int kMaxLayers = 8;
 constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
 constexpr int kRound = 2;             // photon output: warp iterations per round (one cursor bump per tile and round)
 constexpr int kStageRecs = kRound * 32;           // records a warp can stage per round
+constexpr int kDenseTile = 64;        // records a tile must stage in its first round (512 photons) to stay in the rounds mode
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
 constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
 constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
@@ -212,8 +213,7 @@ struct OutSmem {
     unsigned long long wbase[kWarps];            // first record slot of warp w's run in its telescope's region
     int wk[kWarps];                              // telescope of the records warp w has staged this round
     uint32_t wn[kWarps];                         // how many
-    int rounds;                                  // 1 while the tile runs in rounds (it saw staged records in round 0)
-    int staged_any;
+    int rounds;                                  // 1 while the tile runs in rounds (enough staged records in round 0)
 };
 
 __device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
@@ -692,17 +692,18 @@ __device__ __forceinline__ void write_records_one_tel(const KParams &P, OutSmem 
 }
 
 // End of a round, called by every thread of the tile: reserve the staged records of all warps (one cursor bump per
-// run of warps on the same telescope) and copy them out.  Returns whether anything was staged; if not and
-// `may_stop` is set, the tile leaves the rounds mode (os.rounds = 0, visible to all warps on return).
+// run of warps on the same telescope) and copy them out.  Returns whether the tile stays in the rounds mode: with
+// `may_stop` set (first round) it leaves it (os.rounds = 0, visible to all warps on return) unless at least
+// kDenseTile records were staged, i.e. unless a good part of its photons hit.
 __device__ __forceinline__ bool flush_round(const KParams &P, OutSmem &os, bool may_stop)
 {
     const uint32_t warp = threadIdx.x >> 5;
     __syncthreads();
     if (threadIdx.x == 0) {
-        int any = 0;
+        uint32_t staged = 0;
+        for (int w = 0; w < kWarps; ++w) staged += os.wn[w];
         for (int w = 0; w < kWarps; ) {
             if (os.wn[w] == 0u) { ++w; continue; }
-            any = 1;
             const int k = os.wk[w];
             uint32_t run = 0;
             int w1 = w;
@@ -711,8 +712,7 @@ __device__ __forceinline__ bool flush_round(const KParams &P, OutSmem &os, bool 
             for (int v = w; v < w1; ++v) { os.wbase[v] = base; base += os.wn[v]; }
             w = w1;
         }
-        os.staged_any = any;
-        if (may_stop && !any) os.rounds = 0;
+        if (may_stop && staged < (uint32_t)kDenseTile) os.rounds = 0;
     }
     __syncthreads();
     const uint32_t n = os.wn[warp];
@@ -725,7 +725,7 @@ __device__ __forceinline__ bool flush_round(const KParams &P, OutSmem &os, bool 
     __syncwarp();
     if ((threadIdx.x & 31) == 0) os.wn[warp] = 0u;
     __syncwarp();
-    return os.staged_any != 0;
+    return os.rounds != 0;
 }
 
 // a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes together.
@@ -998,6 +998,132 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
     return AxisFrame{A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, C.y, C.z};
 }
 
+// ------------------------------------------------------------------------------------
+// The lane's position in its warp's photon range and everything else the photon loop carries.
+struct WarpWalk {
+    int e, kind;                       // current emitter and its kind
+    uint32_t end, g, j;                // end of the emitter in the tile's index space, photon index, index within the emitter
+    PhiloxEmitter pe;
+    AxisFrame f_reg;
+    uint32_t n_up, q_head, q_count;
+};
+
+// Iterations [it0, it1) of the photon loop (phase 2).  INLINE: tiles in which most photons hit (ground histogram: all
+// tiles; photon output: while the tile runs in rounds) evaluate the first candidate of an axis-kind photon right in
+// the loop, from the values already in registers: no queue, no second Philox, no second sincos.  The sparse tiles of
+// the photon-output kernels run the instance without that code.  Returns whether the tile is (still) in rounds mode.
+template <int TELSRC, bool COPLANAR, int NT, int MODE, bool INLINE>
+__device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &ww, const uint32_t hi, const unsigned long long tile_first,
+                                     const uint32_t it0, const uint32_t it1, const uint32_t n_iter, bool rounds)
+{
+    constexpr bool OUT = (MODE == MODE_OUT);
+    constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
+    const int tid = threadIdx.x, lane = tid & 31;
+    int e = ww.e, kind = ww.kind;
+    uint32_t end = ww.end, g = ww.g, j = ww.j, n_up = ww.n_up, q_head = ww.q_head, q_count = ww.q_count;
+    PhiloxEmitter pe = ww.pe;
+    AxisFrame f_reg = ww.f_reg;
+    (void)tid; (void)lane;
+    for (uint32_t it = it0; it < it1; ++it, g += 32u, j += 32u) {
+        const bool active = g < hi;                  // the lanes past the warp's range idle in its last iterations
+        uint32_t cm = 0u;
+        uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
+        Rand4 r = {0u, 0u, 0u, 0u};
+        Hit h;
+        h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
+        if (active) {
+            if (g >= end) {
+                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+                j = g - sm.prefix[e];
+                kind = sm.kind[e];
+                pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+                if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
+            }
+            if (kind == KIND_CHER_AXIS) {
+                const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
+                r = philox_photon(P, pe, j, 0u);                                              // a2
+                // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
+                const float sd = fmaf(one_two(r.r0), f.negL, f.k0c);                          // K0 - u1 L
+                float sp, cp;
+                __sincosf(fmaf(one_two(r.r1), 6.2831853f, -9.42477760f), &sp, &cp);           // phi - pi, in [-pi, pi)
+                const float vz = fmaf(cp, f.az, fmaf(sp, f.bz, f.cz));
+                if (vz < 0.0f) {
+                    // a4: ground = G + (sd / v_z) N,  N = cos' P + sin' Q
+                    const float rho = sd * rcp_approx(vz);
+                    const float gx = fmaf(rho, fmaf(cp, f.px, sp * f.qx), f.gx);
+                    const float gy = fmaf(rho, fmaf(cp, f.py, sp * f.qy), f.gy);
+                    float vx = 0.0f, vy = 0.0f;
+                    if (!COPLANAR) {
+                        const float *fr = &sm.frame[e * kFrameStride];
+                        vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
+                        vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
+                    }
+                    cm = plane_candidates<TELSRC, COPLANAR, NT>(P, gx, gy, vx, vy, vz, &cell);
+                    if constexpr (MODE != MODE_TALLY) {
+                        if (INLINE && cm != 0u && cm != kAllTelescopes) {
+                            const float *fr = &sm.frame[e * kFrameStride];
+                            Photon ph;
+                            ph.axis = true; ph.tag = 0; ph.r2 = r.r2;
+                            ph.vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
+                            ph.vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
+                            ph.vz = vz; ph.gx = gx; ph.gy = gy;
+                            ph.s = (one_two(r.r0) - kOneMinus) * fr[F_LEN];
+                            ph.ez = -sd * fr[F_DZ];
+                            ph.ex = ph.ey = 0.0f;
+                            const int k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1);
+                            cm &= cm - 1u;
+                            h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+                        }
+                    }
+                } else {
+                    ++n_up;
+                }
+            } else {
+                bool up;
+                cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, emitter_segment(P, tile_first, e), &cell, &up);
+                if (up) ++n_up;
+            }
+        }
+        if constexpr (TELSRC == TEL_CONST) {
+            if (cm == kAllTelescopes) cm = (1u << NT) - 1u;          // flat photon: all slots go to the exact test
+        } else {
+            const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
+            if (wide) {
+                wide_push<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, wide, e, j);
+                if (cm == kAllTelescopes) cm = 0u;
+            }
+        }
+        if constexpr (MODE != MODE_TALLY) {
+            if (INLINE)           // the record id of an axis-kind photon: tag 0
+                commit_hits<MODE>(P, sm, h, (emitter_segment(P, tile_first, e) << 25) | (unsigned long long)j);
+        }
+        const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
+        if constexpr (MODE != MODE_TALLY) {
+            if (__popc(have) >= kDenseMin) {
+                // dense iteration: each lane's first candidate is evaluated on the spot, further ones are queued
+                const bool has = cm != 0u;
+                int k = 0;
+                if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
+                dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, k, has);
+            }
+            if (__any_sync(0xffffffffu, cm != 0u))
+                push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+            if (OUT && rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
+                OutSmem &os = out_smem(sm);
+                // nothing staged in round 0: a sparse tile, which goes on without rounds (and barriers)
+                const bool first = it < (uint32_t)kRound;
+                if (!flush_round(P, os, first) && first) rounds = false;
+            }
+        } else {
+            if (have)
+                push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+        }
+    }
+    ww.e = e; ww.kind = kind; ww.end = end; ww.g = g; ww.j = j; ww.n_up = n_up; ww.q_head = q_head; ww.q_count = q_count;
+    ww.pe = pe; ww.f_reg = f_reg;
+    return rounds;
+}
+
 template <int TELSRC, bool COPLANAR, int NT, int MODE>
 __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_constant__ KParams P)
 {
@@ -1018,7 +1144,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     if constexpr (OUT) {
         OutSmem &os = out_smem(sm);
         if (tid < kWarps) { os.wn[tid] = 0u; os.wk[tid] = -1; }
-        if (tid == 0) { os.rounds = 1; os.staged_any = 0; }
+        if (tid == 0) os.rounds = 1;
     }
     if constexpr (MODE == MODE_HIST) {
         HistSmem &hs = hist_smem(sm);
@@ -1092,7 +1218,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     // ---- phase 2: warp `warp` walks photons [lo, hi) of the tile's concatenated index space
     const uint32_t lo = sm.bound[warp], hi = sm.bound[warp + 1];
     const unsigned long long tile_first = P.first_id + (unsigned long long)blockIdx.x * (unsigned)segs_per_tile;
-    uint32_t n_up = 0, q_head = 0, q_count = 0;
+    uint32_t n_up = 0;
 
     // Every warp runs the same number of iterations (that of the longest range), so the photon-output kernels can
     // close a round with a block-wide barrier every kRound iterations.
@@ -1102,96 +1228,34 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const uint32_t n_iter = (max_len + 31u) / 32u;
     if (total) {
         // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
-        int e;
+        WarpWalk ww;
         {
             const uint32_t g0 = min(lo + (uint32_t)lane, max(hi, 1u) - 1u);
             int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
             while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
-            e = a;
+            ww.e = a;
         }
         // Loop-carried per lane: photon index g, emitter e with its end, index j within the emitter, kind, the hoisted
         // Philox words and (brute-force kernels only; the grid kernels are short of registers and reload it from
         // shared memory every iteration) the axis frame.
-        constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
-        uint32_t end = sm.prefix[e + 1];
-        int kind = sm.kind[e];
-        PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
-        AxisFrame f_reg = load_axis_frame(sm, e);
-        uint32_t g = lo + (uint32_t)lane, j = g - sm.prefix[e];
-        bool rounds = OUT;
-        for (uint32_t it = 0; it < n_iter; ++it, g += 32u, j += 32u) {
-            const bool active = g < hi;                  // the lanes past the warp's range idle in its last iterations
-            uint32_t cm = 0u;
-            uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
-            Rand4 r = {0u, 0u, 0u, 0u};
-            if (active) {
-                if (g >= end) {
-                    do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
-                    j = g - sm.prefix[e];
-                    kind = sm.kind[e];
-                    pe = philox_emitter(P, emitter_segment(P, tile_first, e));
-                    if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
-                }
-                if (kind == KIND_CHER_AXIS) {
-                    const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
-                    r = philox_photon(P, pe, j, 0u);                                              // a2
-                    // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
-                    const float sd = fmaf(one_two(r.r0), f.negL, f.k0c);                          // K0 - u1 L
-                    float sp, cp;
-                    __sincosf(fmaf(one_two(r.r1), 6.2831853f, -9.42477760f), &sp, &cp);           // phi - pi, in [-pi, pi)
-                    const float vz = fmaf(cp, f.az, fmaf(sp, f.bz, f.cz));
-                    if (vz < 0.0f) {
-                        // a4: ground = G + (sd / v_z) N,  N = cos' P + sin' Q
-                        const float rho = sd * rcp_approx(vz);
-                        const float gx = fmaf(rho, fmaf(cp, f.px, sp * f.qx), f.gx);
-                        const float gy = fmaf(rho, fmaf(cp, f.py, sp * f.qy), f.gy);
-                        float vx = 0.0f, vy = 0.0f;
-                        if (!COPLANAR) {
-                            const float *fr = &sm.frame[e * kFrameStride];
-                            vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
-                            vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
-                        }
-                        cm = plane_candidates<TELSRC, COPLANAR, NT>(P, gx, gy, vx, vy, vz, &cell);
-                    } else {
-                        ++n_up;
-                    }
-                } else {
-                    bool up;
-                    cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, emitter_segment(P, tile_first, e), &cell, &up);
-                    if (up) ++n_up;
-                }
-            }
-            if constexpr (TELSRC == TEL_CONST) {
-                if (cm == kAllTelescopes) cm = (1u << NT) - 1u;          // flat photon: all slots go to the exact test
-            } else {
-                const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
-                if (wide) {
-                    wide_push<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, wide, e, j);
-                    if (cm == kAllTelescopes) cm = 0u;
-                }
-            }
-            const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
-            if constexpr (MODE != MODE_TALLY) {
-                if (__popc(have) >= kDenseMin) {
-                    // dense iteration: each lane's first candidate is evaluated on the spot, further ones are queued
-                    const bool has = cm != 0u;
-                    int k = 0;
-                    if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
-                    dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, k, has);
-                }
-                if (__any_sync(0xffffffffu, cm != 0u))
-                    push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
-                if (OUT && rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
-                    OutSmem &os = out_smem(sm);
-                    // nothing staged in round 0: a sparse tile, which goes on without rounds (and barriers)
-                    const bool first = it < (uint32_t)kRound;
-                    if (!flush_round(P, os, first) && first) rounds = false;
-                }
-            } else {
-                if (have)
-                    push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
-            }
+        ww.end = sm.prefix[ww.e + 1];
+        ww.kind = sm.kind[ww.e];
+        ww.pe = philox_emitter(P, emitter_segment(P, tile_first, ww.e));
+        ww.f_reg = load_axis_frame(sm, ww.e);
+        ww.g = lo + (uint32_t)lane; ww.j = ww.g - sm.prefix[ww.e];
+        ww.n_up = 0u; ww.q_head = 0u; ww.q_count = 0u;
+        bool rounds = false;
+        if constexpr (OUT) {
+            // round 0 decides whether the tile is dense (stays in rounds mode, inline evaluation) or sparse
+            const uint32_t it1 = min((uint32_t)kRound, n_iter);
+            rounds = walk<TELSRC, COPLANAR, NT, MODE, true>(P, sm, ww, hi, tile_first, 0u, it1, n_iter, true);
+            if (rounds) walk<TELSRC, COPLANAR, NT, MODE, true>(P, sm, ww, hi, tile_first, it1, n_iter, n_iter, true);
+            else walk<TELSRC, COPLANAR, NT, MODE, false>(P, sm, ww, hi, tile_first, it1, n_iter, n_iter, false);
+        } else {
+            walk<TELSRC, COPLANAR, NT, MODE, MODE == MODE_HIST>(P, sm, ww, hi, tile_first, 0u, n_iter, n_iter, false);
         }
+        n_up = ww.n_up;
+        uint32_t q_head = ww.q_head, q_count = ww.q_count;
         if constexpr (TELSRC != TEL_CONST) {
             __syncwarp();
             const uint32_t nw = sm.wide_count[warp];
