@@ -300,3 +300,75 @@ def test_ground_histogram_needs_configuration_and_resets(c8):
     c, over_c, _ = ctx.read_ground_histogram()
     assert int(c["n"].sum()) == 0 and over_c == 0
     ctx.close()
+
+
+def test_no_grid_possible_many_overlapping_spheres(c8):
+    """12 large overlapping spheres: more than 4 reach discs cover every cell, no grid can be built, and every photon
+    takes the wide test (TEL_GLOBAL), one photon per lane against all telescopes."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=1500)
+    rng = np.random.Generator(np.random.PCG64(5))
+    tel = np.zeros((12, 4), dtype=np.float32)
+    tel[:, 0] = rng.uniform(-40, 40, 12); tel[:, 1] = rng.uniform(-40, 40, 12)
+    tel[:, 2] = 2000.0 + rng.uniform(-10, 10, 12); tel[:, 3] = rng.uniform(30, 60, 12)
+    cfg["telescopes"] = tel
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("no-grid-12tel", rep)
+    assert rep["matched"] > 10000
+
+
+def test_large_array_1600_telescopes(c8):
+    """A 40 x 40 array (more than the 128 telescopes tallied in shared memory, more than culling tests one by one):
+    global-memory tallies, grid lookup, bounding-sphere culling only."""
+    import parity_util as pu
+    cfg = wl.make_config("c4", n_segments=3000)
+    cfg["telescopes"] = wl.telescopes_grid(n=40, spacing=35.0, r=6.0)
+    a = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=1 << 15)
+    o = pu.oracle_run(cfg, record_capacity=1 << 23)
+    rep = pu.compare(cfg, a, o)
+    _report("grid-1600tel", rep)
+    assert rep["matched"] > 10000
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_CULL)
+    b = pu.gpu_run(cfg, c8.MODE_TALLY)
+    assert np.array_equal(a["tallies"]["hits"], b["tallies"]["hits"])
+
+
+def test_eight_layers_and_segments_across_layer_boundaries(c8):
+    """8 atmosphere layers (the maximum) with long segments, so that many tracks cross a layer boundary and the
+    photons' layer is looked up per photon instead of taken from the frame."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=1500)
+    l5 = cfg["atmosphere"]["layers"]
+    # split the three lowest layers in two: same coefficients on both sides, so T(h) is unchanged but the index is not
+    layers = [l5[0], (2000.5, l5[0][1], l5[0][2], l5[0][3]), l5[1], (7000.0, l5[1][1], l5[1][2], l5[1][3]),
+              l5[2], (25000.0, l5[2][1], l5[2][2], l5[2][3]), l5[3], l5[4]]
+    cfg["atmosphere"] = dict(cfg["atmosphere"], layers=layers)
+    seg = cfg["segments"]
+    seg["length"] = np.minimum(seg["length"] * 40.0, (seg["z0"] - 2000.0) / np.maximum(-seg["dz"], 0.05) * 0.999).astype(np.float32)
+    cfg["telescopes"] = np.array([[0.0, 0.0, 2000.0, 25.0], [80.0, -40.0, 2000.0, 12.0]], dtype=np.float32)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("8-layers", rep)
+    assert rep["matched"] > 5000
+
+
+def test_one_segment_with_a_million_bunches(c8):
+    """The photon index of one emitter far beyond a tile's usual size (n_b ~ 1.5e6 < 2^24): index arithmetic, the
+    24-bit photon index of the record id, one warp share spanning a single emitter."""
+    import parity_util as pu
+    cfg = wl.make_config("c1", n_segments=3)
+    seg = cfg["segments"]
+    seg["x0"], seg["y0"], seg["z0"] = 0.0, 0.0, 9000.0
+    seg["dx"], seg["dy"], seg["dz"] = 0.0, 0.0, -1.0
+    seg["length"], seg["gamma"] = np.float32(50.0), np.float32(1e5)
+    seg["t0"] = -(seg["z0"] - 2000.0) / 0.299792458
+    cfg["params"] = dict(cfg["params"], bunch_size=5e-4)
+    cfg["telescopes"] = np.array([[70.0, 60.0, 2000.0, 8.0]], dtype=np.float32)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("1e6-bunches", rep)
+    assert g["counts"][:, 0].max() > 1_000_000 and rep["matched"] > 1000
