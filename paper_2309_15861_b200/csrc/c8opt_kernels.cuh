@@ -509,13 +509,13 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
     if (kind == KIND_FL_ISO) {
         // R16: cos(theta) = 1 - 2 u4, v = (cos phi sin th, sin phi sin th, -cos th); cos phi = -cos'
         const float u4 = uniform01(r.r3);
-        const float cth = fmaf(-2.0f, u4, 1.0f), sth = 2.0f * sqrtf(u4 * (1.0f - u4));
+        const float cth = fmaf(-2.0f, u4, 1.0f), uu = u4 * (1.0f - u4), sth = 2.0f * uu * rsqrtf(uu);   // u4 in (0, 1): uu > 0
         ph.vx = -cp * sth; ph.vy = -sp * sth; ph.vz = -cth;
     } else {
         float sth = 1.0f, cth = 1.0f;
         if (kind == KIND_CONE) {                      // R14: 1 - cos(theta') uniform in [0, 1 - cos(alpha_b)]
             const float t = uniform01(r.r3) * (float)P.omc;
-            cth = 1.0f - t; sth = sqrtf(t * (2.0f - t));
+            cth = 1.0f - t; sth = sqrtf(t * (2.0f - t));     // beamed: sin(theta') sets the aim at 10 km, keep the IEEE root
         }
         ph.vx = fmaf(sth, fmaf(cp, fr[F_A0 + 0], sp * fr[F_B0 + 0]), cth * fr[F_C0 + 0]);
         ph.vy = fmaf(sth, fmaf(cp, fr[F_A0 + 1], sp * fr[F_B0 + 1]), cth * fr[F_C0 + 1]);
@@ -796,18 +796,17 @@ __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigne
 }
 
 // Dense path: when at least kDenseMin lanes of a warp iteration hold a candidate, the pairs are evaluated on the spot
-// from the random words the lanes still hold (no queue; the axis kind also skips the second Philox, the generic kinds
-// redraw theirs).  `has` says which lanes take part; all 32 call.
+// from the random words the lanes still hold (no queue, no second Philox).  `has` says which lanes take part; all 32 call.
 template <int TELSRC, int MODE>
 __device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned long long tile_first, int e, uint32_t j,
-                                        uint32_t r0, uint32_t r1, uint32_t r2, int k, bool has)
+                                        uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3, int k, bool has)
 {
     Hit h;
     h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
     uint64_t id = 0;
     if (has) {
         const unsigned long long S = emitter_segment(P, tile_first, e);
-        const Photon ph = (sm.kind[e] == KIND_CHER_AXIS) ? photon_from_rand(P, sm, e, Rand4{r0, r1, r2, 0u}) : make_photon(P, sm, e, j, S);
+        const Photon ph = photon_from_rand(P, sm, e, Rand4{r0, r1, r2, r3});
         h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
@@ -977,14 +976,14 @@ __device__ __forceinline__ void wide_push(const KParams &P, TileSmem &sm, unsign
 // a2-a4 of the hot loop for the generic kinds.  Returns the candidate mask (see plane_candidates); *upward is
 // set when the photon does not go down.  Photons flatter than |v_z| = 0.05 are tested against all telescopes.
 template <int TELSRC, bool COPLANAR, int NT>
-__device__ __noinline__ uint32_t generic_candidates(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S,
-                                                    uint2 *cell, bool *upward)
+__device__ __noinline__ uint32_t generic_candidates(const KParams &P, const TileSmem &sm, int e, uint32_t r0, uint32_t r1, uint32_t r2,
+                                                    uint32_t r3, uint2 *cell, bool *upward)
 {
-    const Photon ph = make_photon(P, sm, e, j, S);
+    const Photon ph = photon_from_rand(P, sm, e, Rand4{r0, r1, r2, r3});
     *upward = !(ph.vz < 0.0f);
     if (*upward) return 0u;
     if (ph.vz > -0.05f) return kAllTelescopes;
-    const float spl = -ph.ez / ph.vz;
+    const float spl = -ph.ez * rcp_approx(ph.vz);          // candidate search only: the pre-tests carry slack
     return plane_candidates<TELSRC, COPLANAR, NT>(P, fmaf(spl, ph.vx, ph.ex), fmaf(spl, ph.vy, ph.ey), ph.vx, ph.vy, ph.vz, cell);
 }
 
@@ -1079,8 +1078,10 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                     ++n_up;
                 }
             } else {
+                // the same hoisted Philox as the axis kind (the process tag is counter word 3)
+                r = philox_photon(P, pe, j, kind_tag(kind));
                 bool up;
-                cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, j, emitter_segment(P, tile_first, e), &cell, &up);
+                cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, r.r0, r.r1, r.r2, r.r3, &cell, &up);
                 if (up) ++n_up;
             }
         }
@@ -1104,7 +1105,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 const bool has = cm != 0u;
                 int k = 0;
                 if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
-                dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, k, has);
+                dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, r.r3, k, has);
             }
             if (__any_sync(0xffffffffu, cm != 0u))
                 push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
