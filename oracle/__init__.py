@@ -48,7 +48,10 @@ class Params(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("processes", C.c_uint32),
                 ("lam1", C.c_double), ("lam2", C.c_double), ("bunch_size", C.c_double),
                 ("fl_yield", C.c_double), ("fl_lam1", C.c_double), ("fl_lam2", C.c_double),
-                ("fl_beam_telescope", C.c_int), ("fl_beam_halfangle", C.c_double)]
+                ("fl_beam_telescope", C.c_int), ("fl_beam_halfangle", C.c_double), ("refract", C.c_int)]
+
+
+FLAG_REFRACT = 2      # the bit of params["flags"] that asks for the refraction corrections (R27)
 
 
 class Frame(C.Structure):
@@ -96,6 +99,9 @@ def lib():
         L.orc_optical_depth.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double]
         L.orc_optical_depth.restype = C.c_double
         L.orc_transmission.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double, C.c_double]
+        L.orc_refraction.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double, C.c_double,
+                                     C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_refraction.restype = None
         L.orc_transmission.restype = C.c_double
         L.orc_run.argtypes = [C.POINTER(Atmosphere), dp, C.c_int, C.c_void_p, C.c_uint64, C.c_uint64,
                               C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64,
@@ -129,7 +135,8 @@ def make_atmosphere(atm: dict) -> Atmosphere:
 
 def make_params(p: dict) -> Params:
     return Params(int(p["seed"]), int(p["processes"]), p["lam1"], p["lam2"], p["bunch_size"],
-                  p["fl_yield"], p["fl_lam1"], p["fl_lam2"], int(p["fl_beam_telescope"]), p["fl_beam_halfangle"])
+                  p["fl_yield"], p["fl_lam1"], p["fl_lam2"], int(p["fl_beam_telescope"]), p["fl_beam_halfangle"],
+                  1 if (int(p.get("flags", 0)) & FLAG_REFRACT) else 0)
 
 
 def _dp(a):
@@ -190,6 +197,13 @@ def intersect(e, v, tel):
 
 def arrival_time(atm: dict, e_z, c_z, v_z, s_pl, t_e) -> float:
     return lib().orc_arrival_time(C.byref(make_atmosphere(atm)), e_z, c_z, v_z, s_pl, t_e)
+
+
+def refraction(atm: dict, e_z, c_z, v_z):
+    """(dr [m], dtheta [rad]) of R27 for a ray from altitude e_z down to c_z with direction cosine v_z < 0."""
+    dr, dth = C.c_double(0.0), C.c_double(0.0)
+    lib().orc_refraction(C.byref(make_atmosphere(atm)), float(e_z), float(c_z), float(v_z), C.byref(dr), C.byref(dth))
+    return dr.value, dth.value
 
 
 def optical_depth(atm: dict, h, lam) -> float:

@@ -58,6 +58,7 @@ typedef struct {
     double fl_yield, fl_lam1, fl_lam2; /* photons / MeV, fluorescence band (nm) */
     int fl_beam_telescope;             /* -1 = isotropic */
     double fl_beam_halfangle;          /* rad */
+    int refract;                       /* R27: apply the refraction corrections of PAPER.md:77 to position and angle */
 } orc_params;
 
 /* one fp32 segment record, 12 x 4 bytes (flags is a uint32 in the same slot) */
@@ -312,6 +313,55 @@ double orc_arrival_time(const orc_atmosphere *atm, double e_z, double c_z, doubl
     return t_e + (s_pl + excess_m) / ORC_C_M_PER_NS;
 }
 
+/* R27 ("straight line propagation followed by the application of correction factors which changes
+ * the arrival angle, position, and timing to comply with atmospheric refraction"; the formulas are in the paper's
+ * ref. [7], not available, so this is the first-order planar-Snell reading): n(z) sin(theta(z)) is constant along the
+ * ray, theta from the vertical.  To first order in eta = n - 1, for a ray leaving e_z at theta0 and reaching c_z < e_z:
+ *   theta(z) - theta0 = tan(theta0) (eta(e_z) - eta(z))
+ *   horizontal displacement beyond the straight line,
+ *   dr = int (tan theta(z) - tan theta0) dz = tan(theta0) / cos^2(theta0) * [ eta(e_z) (e_z - c_z) - int_{c_z}^{e_z} eta dz ],
+ *   int eta dz = 0.01 (eta0 / rho0) (T(c_z) - T(e_z))  [m]   (the same column integral as the delay of R8)
+ *   dtheta = tan(theta0) (eta(e_z) - eta(c_z)).
+ * Both are negative going down (the air gets denser: the ray bends towards the vertical).  The optical path changes
+ * only to second order (Fermat), so the arrival time of R8 stands. */
+void orc_refraction(const orc_atmosphere *atm, double e_z, double c_z, double v_z, double *dr, double *dtheta)
+{
+    double cos0 = fabs(v_z), sin0 = sqrt(fmax(0.0, 1.0 - v_z * v_z)), tan0 = sin0 / cos0;
+    double eta_e = orc_refractivity(atm, e_z), eta_c = orc_refractivity(atm, c_z);
+    double col = 0.01 * (atm->eta0 / atm->rho0) * (orc_depth(atm, c_z) - orc_depth(atm, e_z));
+    *dr = tan0 / (cos0 * cos0) * (eta_e * (e_z - c_z) - col);
+    *dtheta = tan0 * (eta_e - eta_c);
+}
+
+/* R10 / R11 with the corrections of R27 applied on the plane z = c_z: the arrival point moves by dr along the
+ * horizontal direction of flight, the direction turns by dtheta in the vertical plane of flight; the sphere test
+ * uses the corrected point and direction (q = corrected plane point - centre, q_z = 0):
+ *   b^2 = |q|^2 - (q . v')^2,  closest approach at s_pl - q . v' along the path. */
+int orc_intersect_refracted(const orc_atmosphere *atm, const double e[3], const double v[3], const double tel[4],
+                            double *b2, double *s_c, double *s_pl, double xy[2], double vout[3])
+{
+    vout[0] = v[0]; vout[1] = v[1]; vout[2] = v[2];
+    *b2 = 0.0; *s_c = 0.0; *s_pl = 0.0; xy[0] = xy[1] = 0.0;
+    if (!(v[2] < 0.0) || !(e[2] > tel[2])) return 0;
+    double sp = (tel[2] - e[2]) / v[2];
+    double x = e[0] + sp * v[0] - tel[0], y = e[1] + sp * v[1] - tel[1];
+    double sin0 = sqrt(v[0] * v[0] + v[1] * v[1]);
+    if (sin0 > 0.0) {
+        double dr, dth;
+        orc_refraction(atm, e[2], tel[2], v[2], &dr, &dth);
+        double hx = v[0] / sin0, hy = v[1] / sin0;
+        double th = atan2(sin0, -v[2]) + dth;
+        x += dr * hx; y += dr * hy;
+        vout[0] = sin(th) * hx; vout[1] = sin(th) * hy; vout[2] = -cos(th);
+    }
+    double qv = x * vout[0] + y * vout[1];
+    *b2 = x * x + y * y - qv * qv;
+    *s_c = sp - qv;
+    *s_pl = sp;
+    xy[0] = x; xy[1] = y;
+    return (*b2 <= tel[3] * tel[3]) && (*s_c > 0.0);
+}
+
 /* R17: tau(h, lambda) bilinear in the table, clamped at the edges; survival
  * exp(-tau / |v_z|) applied as a weight factor. */
 double orc_optical_depth(const orc_atmosphere *atm, double h, double lam)
@@ -370,8 +420,10 @@ void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
                 counters[1] += 1;
                 if (!(ph.v[2] < 0.0)) { counters[2] += 1; continue; }
                 for (int k = 0; k < n_tel; ++k) {
-                    double b2, s_c, s_pl, xy[2];
-                    if (!orc_intersect(ph.e, ph.v, &tel[4 * k], &b2, &s_c, &s_pl, xy)) continue;
+                    double b2, s_c, s_pl, xy[2], va[3] = { ph.v[0], ph.v[1], ph.v[2] };
+                    if (par->refract) {
+                        if (!orc_intersect_refracted(atm, ph.e, ph.v, &tel[4 * k], &b2, &s_c, &s_pl, xy, va)) continue;
+                    } else if (!orc_intersect(ph.e, ph.v, &tel[4 * k], &b2, &s_c, &s_pl, xy)) continue;
                     double t = orc_arrival_time(atm, ph.e[2], tel[4 * k + 2], ph.v[2], s_pl, ph.t_e);
                     double w = ph.w * orc_transmission(atm, ph.e[2], ph.lam, ph.v[2]);
                     tallies[k].hits += 1;
@@ -381,7 +433,7 @@ void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
                     if (records) {
                         if (*n_rec < cap) {
                             orc_record *r = &records[*n_rec];
-                            r->x = xy[0]; r->y = xy[1]; r->cx = ph.v[0]; r->cy = ph.v[1];
+                            r->x = xy[0]; r->y = xy[1]; r->cx = va[0]; r->cy = va[1];
                             r->t = t; r->lam = ph.lam; r->w = w;
                             r->id = (S << 25) | ((uint64_t)tag << 24) | (uint64_t)j;
                             r->tel = k; r->pad = 0;

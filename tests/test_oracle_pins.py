@@ -622,3 +622,69 @@ def test_ground_histogram_counts_every_downward_bunch():
     cnt = dict(zip(O.COUNTER_NAMES, (int(v) for v in res["counters"])))
     assert int(res["hist"]["n"].sum()) + res["overflow"] == cnt["generated"] - cnt["upward"] > 10000
     assert res["overflow"] > 0 and np.count_nonzero(res["hist"]["n"]) > 50
+
+
+# ------------------------------------------------------------------ refraction corrections (R27)
+def _snell_ray(atm, e_z, c_z, theta0, n_steps=200000):
+    """Numerically integrated planar Snell ray: n(z) sin(theta(z)) = const, dx = tan(theta) dz (midpoint rule)."""
+    edges = np.linspace(e_z, c_z, n_steps + 1)
+    zm = 0.5 * (edges[1:] + edges[:-1])
+    layers = atm["layers"]
+
+    def eta(z):
+        z = np.atleast_1d(np.asarray(z, dtype=np.float64))
+        out = np.empty_like(z)
+        for i, (h_lo, a, b, c) in enumerate(layers):
+            h_hi = layers[i + 1][0] if i + 1 < len(layers) else np.inf
+            m = (z >= h_lo) & (z < h_hi) if i else (z < h_hi)
+            out[m] = atm["eta0"] * ((b / c) * np.exp(-z[m] / c) / 100.0) / atm["rho0"]
+        return out
+
+    k = (1.0 + eta(e_z)[0]) * math.sin(theta0)
+    sin_t = k / (1.0 + eta(zm))
+    x = np.sum(sin_t / np.sqrt(1.0 - sin_t ** 2)) * (e_z - c_z) / n_steps
+    theta1 = math.asin(k / (1.0 + eta(c_z)[0]))
+    return x - (e_z - c_z) * math.tan(theta0), theta1 - theta0
+
+
+@pytest.mark.parametrize("atm", [ATM1, ATM5], ids=["one-layer", "five-layer"])
+@pytest.mark.parametrize("theta_deg,e_z", [(4.0, 10000.0), (20.0, 6000.0), (45.0, 12000.0), (1.0, 3000.0)])
+def test_refraction_corrections_against_integrated_snell_ray(atm, theta_deg, e_z):
+    """R27's closed forms against a ray traced through the same n(z) in 2e5 altitude steps: they are first order in
+    eta (3e-4 at most), so the agreement is to a few 1e-3 relative; both are negative (bending towards the vertical)."""
+    th = math.radians(theta_deg)
+    dr, dth = O.refraction(atm, e_z, 2000.0, -math.cos(th))
+    dr_num, dth_num = _snell_ray(atm, e_z, 2000.0, th)
+    assert dr < 0.0 and dth < 0.0
+    assert math.isclose(dr, dr_num, rel_tol=3e-3), (dr, dr_num)
+    assert math.isclose(dth, dth_num, rel_tol=3e-3), (dth, dth_num)
+
+
+def test_refraction_magnitude_and_vertical_ray():
+    """SURVEY.md §8(f) quotes ~3 cm and ~7e-6 rad at 4 degrees from 8 km above the plane; a vertical ray is not moved."""
+    dr, dth = O.refraction(ATM1, 10000.0, 2000.0, -math.cos(math.radians(4.0)))
+    assert 0.01 < -dr < 0.06 and 3e-6 < -dth < 1.5e-5
+    dr0, dth0 = O.refraction(ATM1, 10000.0, 2000.0, -1.0)
+    assert dr0 == 0.0 and dth0 == 0.0
+
+
+def test_refracted_records_move_by_the_corrections():
+    """Whole path with the flag: every record of an accept-all plane detector is the unrefracted record moved by dr
+    along the horizontal flight direction and turned by dtheta; times, wavelengths and weights are unchanged."""
+    seg = one_segment(z0=9000.0, d=(0.3, -0.1, -1.0), length=5.0, gamma=1e6)
+    par = W.default_params(bunch_size=0.5, seed=9)
+    tel = W.telescope_accept_all()
+    a = O.run(ATM5, tel, seg, par, record_capacity=10000)["records"]
+    b = O.run(ATM5, tel, seg, dict(par, flags=O.FLAG_REFRACT), record_capacity=10000)["records"]
+    assert len(a) == len(b) > 100 and np.array_equal(a["id"], b["id"])
+    assert np.array_equal(a["t"], b["t"]) and np.array_equal(a["lam"], b["lam"]) and np.array_equal(a["w"], b["w"])
+    for ra, rb in zip(a[:50], b[:50]):
+        vz = -math.sqrt(1.0 - ra["cx"] ** 2 - ra["cy"] ** 2)
+        sin0 = math.hypot(ra["cx"], ra["cy"])
+        st, f = O.preamble(ATM5, par, seg[0], 0)
+        ph = O.make_photon(f, par, 0, int(ra["id"]) & 0xFFFFFF, 0)
+        dr, dth = O.refraction(ATM5, ph.e[2], 2000.0, vz)
+        assert math.isclose(rb["x"] - ra["x"], dr * ra["cx"] / sin0, rel_tol=1e-6, abs_tol=1e-9)
+        assert math.isclose(rb["y"] - ra["y"], dr * ra["cy"] / sin0, rel_tol=1e-6, abs_tol=1e-9)
+        th_b = math.asin(math.hypot(rb["cx"], rb["cy"]))
+        assert math.isclose(th_b - math.asin(sin0), dth, rel_tol=1e-5, abs_tol=1e-12)
