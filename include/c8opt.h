@@ -60,6 +60,13 @@ extern "C" {
  * photon loop.  Tallies and records are identical with and without it; the skipped bunches still count as
  * generated and are reported in counters[C8OPT_CNT_CULLED]; C8OPT_CNT_UPWARD then covers propagated bunches only. */
 #define C8OPT_FLAG_CULL    1u
+/* REFRACT: the refraction corrections of PAPER.md:77 ("straight line propagation followed by the application of
+ * correction factors which changes the arrival angle, position, and timing") in the first-order planar-Snell reading
+ * DESIGN.md R27: on the plane of the telescope centre the arrival point moves by
+ *   dr = tan(theta0) / cos^2(theta0) [eta(e_z) (e_z - c_z) - kappa (T(c_z) - T(e_z))]   along the horizontal flight
+ * direction and the direction turns by dtheta = tan(theta0) (eta(e_z) - eta(c_z)); the sphere test and the record
+ * use the corrected point and direction; the arrival time (optical path, R8) changes only to second order and stands. */
+#define C8OPT_FLAG_REFRACT 2u
 
 typedef struct c8opt_ctx c8opt_ctx;   /* opaque, owned by the library */
 

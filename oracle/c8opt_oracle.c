@@ -346,7 +346,9 @@ int orc_intersect_refracted(const orc_atmosphere *atm, const double e[3], const 
     double sp = (tel[2] - e[2]) / v[2];
     double x = e[0] + sp * v[0] - tel[0], y = e[1] + sp * v[1] - tel[1];
     double sin0 = sqrt(v[0] * v[0] + v[1] * v[1]);
-    if (sin0 > 0.0) {
+    /* the planar first-order forms are for rays well away from the horizontal (the Cherenkov light of a shower):
+     * beyond a zenith angle of 60 degrees, |v_z| < 0.5, the straight line is kept (R27) */
+    if (sin0 > 0.0 && v[2] <= -0.5) {
         double dr, dth;
         orc_refraction(atm, e[2], tel[2], v[2], &dr, &dth);
         double hx = v[0] / sin0, hy = v[1] / sin0;

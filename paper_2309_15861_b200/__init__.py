@@ -26,6 +26,7 @@ MAX_LAYERS = 8
 PROC_CHERENKOV, PROC_FLUORESCENCE = 1, 2
 MODE_TALLY, MODE_OUTPUT, MODE_GROUND_HIST = 0, 1, 2
 FLAG_CULL = 1
+FLAG_REFRACT = 2
 COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "culled")
 TALLY_DTYPE = np.dtype([("hits", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
 HIST_DTYPE = np.dtype([("n", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])

@@ -40,13 +40,17 @@ struct c8opt_ctx {
     double hist_core_x = 0, hist_core_y = 0, hist_r_max = 0;
     float4 *d_telA = nullptr;
     float *d_telT = nullptr;
+    float *d_telEta = nullptr;
+    std::vector<float> h_telEta;
     std::vector<float4> h_telA;
     std::vector<float> h_telT;
     // ground-plane candidate grid (n_tel > kTelConstMax)
     int tel_src = c8::TEL_CONST;
     uint2 *d_grid = nullptr;
     int n_grid_levels = 0;
-    c8::GridLevel grid_lvl[c8::kGridLevels] = {};
+    c8::GridLevel grid_lvl[c8::kGridLevels + 1] = {};
+    bool have_refract_grid = false;
+    double refr_cmax = 0, r_max = 0;   // kappa T(lowest telescope) [m]; largest telescope radius
     // results
     c8::Tally *d_tallies = nullptr;
     unsigned long long *d_counters = nullptr;   // [8]
@@ -90,6 +94,14 @@ double host_depth(const c8opt_ctx *c, double h)
     return c->layer[i].a + c->layer[i].b * std::exp(-h / c->layer[i].c);
 }
 
+// refractivity eta(h) = eta0 rho(h) / rho0, rho = -dT/dh = (b / c) exp(-h / c) / 100 [g/cm^3] (host, fp64)
+double host_refractivity(const c8opt_ctx *c, double h)
+{
+    int i = 0;
+    for (int k = 1; k < c->n_layers; ++k) if (h >= c->layer[k].h_lo) i = k;
+    return c->eta0 * (c->layer[i].b / c->layer[i].c * std::exp(-h / c->layer[i].c) / 100.0) / c->rho0;
+}
+
 size_t smem_bytes(int mode)
 {
     return sizeof(c8::TileSmem) + (mode == c8::MODE_OUT ? sizeof(c8::OutSmem) : mode == c8::MODE_HIST ? sizeof(c8::HistSmem) : 0);
@@ -121,9 +133,9 @@ kernel_t pick_kernel(int tel_src, bool coplanar, int nt, bool out)
 // plane z_ref within rho_k = R / vzmin + |c_z - z_ref| sqrt(1 / vzmin^2 - 1) of (c_x, c_y).  Every cell lists the
 // telescopes whose disc (plus slack for fp32 rounding) touches it; at most 4 per cell, else the resolution is
 // doubled, and if that does not help this level is not built.  The cells are appended to *cells.
-bool build_grid_level(c8opt_ctx *ctx, double vzmin, std::vector<uint2> *cells, c8::GridLevel *lvl)
+bool build_grid_level(c8opt_ctx *ctx, double vzmin, double extra_reach, std::vector<uint2> *cells, c8::GridLevel *lvl)
 {
-    const double slack = 0.05;
+    const double slack = 0.05 + extra_reach;
     const int n = ctx->n_tel_pending;
     std::vector<double> rho(n);
     double x_lo = INFINITY, x_hi = -INFINITY, y_lo = INFINITY, y_hi = -INFINITY, rho_max = 0;
@@ -182,9 +194,13 @@ bool build_grid(c8opt_ctx *ctx, std::vector<uint2> *cells)
     const double vzmin[c8::kGridLevels] = {0.5, 0.1};
     ctx->n_grid_levels = 0;
     for (int l = 0; l < c8::kGridLevels; ++l) {
-        if (!build_grid_level(ctx, vzmin[l], cells, &ctx->grid_lvl[l])) break;
+        if (!build_grid_level(ctx, vzmin[l], 0.0, cells, &ctx->grid_lvl[l])) break;
         ctx->n_grid_levels = l + 1;
     }
+    // level 0 again for C8OPT_FLAG_REFRACT: the corrections move a photon with |v_z| >= 0.5 by up to
+    // refr_cmax sin / cos^3 <= 6.93 refr_cmax in the plane (R27); if that grid cannot be built the flag is refused
+    ctx->have_refract_grid = ctx->n_grid_levels > 0 &&
+                             build_grid_level(ctx, vzmin[0], 7.0 * ctx->refr_cmax, cells, &ctx->grid_lvl[c8::kGridLevels]);
     return ctx->n_grid_levels > 0;
 }
 
@@ -195,13 +211,13 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     const bool hist = rp->mode == C8OPT_MODE_GROUND_HIST;
     if (!hist && ctx->n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no telescopes: call c8opt_add_telescopes first");
     if (hist && ctx->hist_bins < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no histogram: call c8opt_set_ground_histogram first");
-    if (hist && rp->flags) return fail(ctx, C8OPT_ERR_ARGUMENT, "flags must be 0 in ground-histogram mode (every bunch counts)");
+    if (hist && (rp->flags & C8OPT_FLAG_CULL)) return fail(ctx, C8OPT_ERR_ARGUMENT, "no culling in ground-histogram mode (every bunch counts)");
     if (hist && (rp->processes & C8OPT_PROC_FLUORESCENCE) && rp->fl_beam_telescope >= 0)
         return fail(ctx, C8OPT_ERR_ARGUMENT, "ground-histogram mode has no telescope to beam at");
     const unsigned procs = rp->processes;
     if (procs == 0 || (procs & ~3u)) return fail(ctx, C8OPT_ERR_ARGUMENT, "processes must be a combination of bits 0 and 1");
     if (rp->mode > 2u) return fail(ctx, C8OPT_ERR_ARGUMENT, "mode must be 0 (tally), 1 (photon output) or 2 (ground histogram)");
-    if (rp->flags & ~C8OPT_FLAG_CULL) return fail(ctx, C8OPT_ERR_ARGUMENT, "unknown bit in flags");
+    if (rp->flags & ~(C8OPT_FLAG_CULL | C8OPT_FLAG_REFRACT)) return fail(ctx, C8OPT_ERR_ARGUMENT, "unknown bit in flags");
     if (!(rp->bunch_size > 0.0) || !std::isfinite(rp->bunch_size)) return fail(ctx, C8OPT_ERR_ARGUMENT, "bunch_size must be > 0");
     if (procs & C8OPT_PROC_CHERENKOV)
         if (!(rp->lam1_nm > 0.0) || !(rp->lam2_nm > rp->lam1_nm)) return fail(ctx, C8OPT_ERR_ARGUMENT, "need 0 < lam1 < lam2");
@@ -228,13 +244,13 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     P.tau = ctx->d_tau; P.tau_nh = ctx->tau_nh; P.tau_nl = ctx->tau_nl;
     P.tau_h0 = (float)ctx->tau_h0; P.tau_inv_dh = (float)(1.0 / ctx->tau_dh);
     P.tau_l0 = (float)ctx->tau_l0; P.tau_inv_dl = (float)(1.0 / ctx->tau_dl);
-    P.n_tel = ctx->n_tel; P.telA = ctx->d_telA; P.telT = ctx->d_telT;
+    P.n_tel = ctx->n_tel; P.telA = ctx->d_telA; P.telT = ctx->d_telT; P.telEta = ctx->d_telEta;
     if (ctx->tel_src == c8::TEL_CONST) {
         for (int k = 0; k < c8::kTelConstMax; ++k) { P.tel_c[k] = make_float4(0.f, 0.f, 0.f, -1.f); P.telT_c[k] = 0.f; }   // R^2 = -1: never hit
-        for (int k = 0; k < ctx->n_tel; ++k) { P.tel_c[k] = ctx->h_telA[k]; P.telT_c[k] = ctx->h_telT[k]; }
+        for (int k = 0; k < ctx->n_tel; ++k) { P.tel_c[k] = ctx->h_telA[k]; P.telT_c[k] = ctx->h_telT[k]; P.telEta_c[k] = ctx->h_telEta[k]; }
     }
     P.grid = ctx->d_grid; P.n_grid_levels = ctx->n_grid_levels;
-    for (int l = 0; l < c8::kGridLevels; ++l) P.grid_lvl[l] = ctx->grid_lvl[l];
+    for (int l = 0; l <= c8::kGridLevels; ++l) P.grid_lvl[l] = ctx->grid_lvl[l];
     P.x_ref = ctx->x_ref; P.y_ref = ctx->y_ref; P.z_ref = ctx->z_ref; P.z_ref_f = (float)ctx->z_ref;
     for (int i = ctx->n_layers; i < c8::kMaxLayers; ++i) P.layerf[i].h_lo = INFINITY;   // never selected by the layer count
     for (int r = 0; r < 10; ++r) {
@@ -243,6 +259,11 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     }
     P.processes = procs; P.n_procs = (procs == 3u) ? 2u : 1u;
     P.flags = rp->flags; P.cull_Rb = ctx->cull_Rb;
+    if (rp->flags & C8OPT_FLAG_REFRACT) {
+        if (ctx->tel_src == c8::TEL_GRID && !ctx->have_refract_grid && !hist)
+            return fail(ctx, C8OPT_ERR_ARGUMENT, "C8OPT_FLAG_REFRACT: no candidate grid with the refraction reach can be built for this array");
+        P.refr_cmax = (float)ctx->refr_cmax; P.refr_two_rmax = (float)(2.0 * ctx->r_max);
+    }
     if (procs & C8OPT_PROC_CHERENKOV) {
         // PAPER.md:45 prefactor: pi e^2 / (h eps0 c0) = 2 pi alpha; the lambda integral of lambda^-2 in closed form (R2)
         const double two_pi_alpha = 2.0 * 3.14159265358979323846 * 7.2973525693e-3;
@@ -267,8 +288,10 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
         for (int k = 0; k < c8::kTelConstMax; ++k) { P.tel_c[k] = make_float4(0.f, 0.f, 0.f, -1.f); P.telT_c[k] = 0.f; }
         P.tel_c[0] = make_float4(0.f, 0.f, 0.f, 1e30f);
         P.telT_c[0] = (float)host_depth(ctx, ctx->h_obs);
+        P.telEta_c[0] = (float)host_refractivity(ctx, ctx->h_obs); P.telEta = nullptr;
         P.x_ref = ctx->hist_core_x; P.y_ref = ctx->hist_core_y; P.z_ref = ctx->h_obs; P.z_ref_f = (float)ctx->h_obs;
         P.n_grid_levels = 0; P.grid = nullptr;
+        if (rp->flags & C8OPT_FLAG_REFRACT) P.refr_cmax = (float)(0.01 * ctx->eta0 / ctx->rho0 * host_depth(ctx, ctx->h_obs));
         P.hist = ctx->d_hist; P.hist_bins = ctx->hist_bins; P.hist_inv_dr = (float)(ctx->hist_bins / ctx->hist_r_max);
         P.hist_wscale = (float)(65536.0 / rp->bunch_size); P.hist_winv = 1.0 / (double)P.hist_wscale;
     }
@@ -397,8 +420,8 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     C8_CUDA(ctx, cudaSetDevice(ctx->device));
     C8_CUDA(ctx, cudaDeviceSynchronize());
     ctx->n_tel = 0;
-    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_tallies); cudaFree(ctx->d_cursors); cudaFree(ctx->d_grid);
-    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_tallies = nullptr; ctx->d_cursors = nullptr; ctx->d_grid = nullptr;
+    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_tallies); cudaFree(ctx->d_cursors); cudaFree(ctx->d_grid);
+    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_telEta = nullptr; ctx->d_tallies = nullptr; ctx->d_cursors = nullptr; ctx->d_grid = nullptr;
     ctx->tel_xyzr.assign(xyzr, xyzr + 4 * (size_t)n);
     // reference point: centre of the bounding box; all device coordinates are relative to it
     ctx->x_ref = 0.5 * (lo[0] + hi[0]); ctx->y_ref = 0.5 * (lo[1] + hi[1]); ctx->z_ref = 0.5 * (lo[2] + hi[2]);
@@ -411,6 +434,14 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
         A[k] = make_float4((float)(x - ctx->x_ref), (float)(y - ctx->y_ref), (float)(z - ctx->z_ref), (float)(r * r));
         T[k] = (float)host_depth(ctx, z);
     }
+    {
+        double z_low = INFINITY;
+        ctx->r_max = 0.0;
+        for (int k = 0; k < n; ++k) { z_low = std::fmin(z_low, xyzr[4 * k + 2]); ctx->r_max = std::fmax(ctx->r_max, xyzr[4 * k + 3]); }
+        ctx->refr_cmax = 0.01 * ctx->eta0 / ctx->rho0 * host_depth(ctx, z_low);
+    }
+    ctx->h_telEta.resize(n);
+    for (int k = 0; k < n; ++k) ctx->h_telEta[k] = (float)host_refractivity(ctx, xyzr[4 * k + 2]);
     double rb = 0.0;
     for (int k = 0; k < n; ++k) {
         const double x = xyzr[4 * k] - ctx->x_ref, y = xyzr[4 * k + 1] - ctx->y_ref, z = xyzr[4 * k + 2] - ctx->z_ref;
@@ -419,10 +450,12 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     ctx->cull_Rb = (float)(rb * (1.0 + 1e-6));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telA, sizeof(float4) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telT, sizeof(float) * n));
+    C8_CUDA(ctx, cudaMalloc(&ctx->d_telEta, sizeof(float) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_tallies, sizeof(c8::Tally) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_cursors, sizeof(unsigned long long) * n));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telA, A.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telT, T.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
+    C8_CUDA(ctx, cudaMemcpy(ctx->d_telEta, ctx->h_telEta.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
     ctx->tel_src = c8::TEL_CONST;
     if (n >= c8::kTelGridMin) {
         // the grid lookup costs about as much as two brute-force pre-tests, so it serves from 3 telescopes up
@@ -611,7 +644,7 @@ void c8opt_destroy(c8opt_ctx *ctx)
         cudaFree(ctx->d_stage[i]);
     }
     for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
-    cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_grid);
+    cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid);
     cudaFree(ctx->d_tallies); cudaFree(ctx->d_counters); cudaFree(ctx->d_cursors); cudaFree(ctx->d_hist);
     cudaGetLastError();
     delete ctx;

@@ -41,6 +41,7 @@ constexpr int kDenseMin = 16;         // candidates in one warp iteration from w
 constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
 constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
 constexpr uint32_t kFlagCull = 1u;    // == C8OPT_FLAG_CULL
+constexpr uint32_t kFlagRefract = 2u; // == C8OPT_FLAG_REFRACT
 constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
 constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
@@ -54,7 +55,7 @@ struct LayerD { double h_lo, a, b, c; };
 struct LayerF { float h_lo, a, b, inv_c; };
 
 struct GridLevel { int nx, ny, base; float ox, oy, inv_cell, vzmin; };   // cell index = floor(x * inv_cell + ox)
-constexpr int kGridLevels = 2;
+constexpr int kGridLevels = 2;        // |v_z| >= 0.5 and >= 0.1; slot kGridLevels holds level 0 with the refraction slack (R27)
 
 struct Tally { unsigned long long hits; double sum_w; double sum_wt; };
 
@@ -73,18 +74,23 @@ struct KParams {
     int n_tel;
     const float4 *telA;            // device: (cx - x_ref, cy - y_ref, cz - z_ref, R^2)
     const float *telT;             // device: column depth T(c_z) [g/cm^2]
+    const float *telEta;           // device: refractivity eta(c_z)  (C8OPT_FLAG_REFRACT)
     float4 tel_c[kTelConstMax];    // the same two tables in the constant bank when n_tel <= kTelConstMax
     float telT_c[kTelConstMax];
+    float telEta_c[kTelConstMax];
     double x_ref, y_ref, z_ref;
     float z_ref_f;                 // (float)z_ref
     // ground-plane candidate grids (n_tel > kTelConstMax): cell -> up to 4 telescope indices (0xffff = none).
     // Level l serves photons with |v_z| >= grid_lvl[l].vzmin (level 0 the steep ones); n_grid_levels of them exist.
     const uint2 *grid;
     int n_grid_levels;
-    GridLevel grid_lvl[kGridLevels];
+    GridLevel grid_lvl[kGridLevels + 1];
     // segment culling (C8OPT_FLAG_CULL): bounding sphere of the telescope array about (x_ref, y_ref, z_ref)
     uint32_t flags;
     float cull_Rb;
+    // C8OPT_FLAG_REFRACT: kappa T(lowest telescope) [m] bounds |eta(e_z) (e_z - c_z) - kappa (T(c_z) - T(e_z))|, so a
+    // photon's arrival point moves by at most refr_cmax sin(theta0) / cos^3(theta0); 0 without the flag
+    float refr_cmax, refr_two_rmax;
     // run
     uint32_t rk0[10], rk1[10];     // Philox round keys: key + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t processes, n_procs;
@@ -319,11 +325,13 @@ __device__ __forceinline__ bool cone_reaches(float ux, float uy, float uz, float
 __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, float mz, float dx, float dy, float dz, float hl,
                                           float sin_c, float cos_c)
 {
-    if (!cone_reaches(-mx, -my, -mz, P.cull_Rb, dx, dy, dz, hl, sin_c, cos_c)) return true;
+    // with the refraction corrections a photon may land up to 6.93 refr_cmax off its straight line (|v_z| >= 0.5)
+    const float grow = (P.flags & kFlagRefract) ? 7.0f * P.refr_cmax : 0.0f;
+    if (!cone_reaches(-mx, -my, -mz, P.cull_Rb + grow, dx, dy, dz, hl, sin_c, cos_c)) return true;
     if (P.n_tel > kCullTelMax) return false;
     for (int k = 0; k < P.n_tel; ++k) {
         const float4 T = __ldg(&P.telA[k]);
-        const float R = T.w * rsqrtf(fmaxf(T.w, 1e-30f));
+        const float R = T.w * rsqrtf(fmaxf(T.w, 1e-30f)) + grow;
         if (cone_reaches(T.x - mx, T.y - my, T.z - mz, R, dx, dy, dz, hl, sin_c, cos_c)) return false;
     }
     return true;
@@ -455,6 +463,11 @@ template <int TELSRC> __device__ __forceinline__ float telT_at(const KParams &P,
     if (TELSRC == TEL_CONST) return P.telT_c[k];
     return __ldg(&P.telT[k]);
 }
+template <int TELSRC> __device__ __forceinline__ float telEta_at(const KParams &P, int k)
+{
+    if (TELSRC == TEL_CONST) return P.telEta_c[k];
+    return __ldg(&P.telEta[k]);
+}
 
 // sin(pi x), cos(pi x) for x in [-1, 1] to ~1e-7 absolute: quadrant reduction to |r| <= 1/4 (exact in fp32) and
 // Taylor polynomials in pi r (next terms < 3e-9).  About a third of sincospif's instructions, which also serves
@@ -546,41 +559,77 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     if (!(ph.vz < 0.0f)) return h;
     const float4 T = tel_at<TELSRC>(P, k);
     const float rv = rcp_refined(ph.vz);
-    float s_pl;
-    if (ph.axis) {
-        // q = g - c on the plane z_ref:  b^2 = |q|^2 - (q.v)^2,  the point g is at path length -ez / v_z
-        const float qx = ph.gx - T.x, qy = ph.gy - T.y, qz = -T.z;
-        const float qv = fmaf(qx, ph.vx, fmaf(qy, ph.vy, qz * ph.vz));
-        const float b2 = fmaf(qx, qx, fmaf(qy, qy, qz * qz)) - qv * qv;
-        const float hk = ph.ez - T.z;                                      // emission height above the telescope plane
-        s_pl = -hk * rv;
-        const float s_c = (s_pl - T.z * rv) - qv;
-        if (!(b2 <= T.w) || !(hk > 0.0f) || !(s_c > 0.0f)) return h;
-        h.x = fmaf(T.z * rv, ph.vx, qx); h.y = fmaf(T.z * rv, ph.vy, qy);  // on the plane z = c_z, relative to the centre (R11)
-    } else {
-        // no plane projection (ill-conditioned for |v_z| -> 0):  b = |m x v|,  m = c - e
-        const float mx = T.x - ph.ex, my = T.y - ph.ey, mz = T.z - ph.ez;
-        const float cx = fmaf(my, ph.vz, -(mz * ph.vy)), cy = fmaf(mz, ph.vx, -(mx * ph.vz)), cz = fmaf(mx, ph.vy, -(my * ph.vx));
-        const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
-        const float s_c = fmaf(mx, ph.vx, fmaf(my, ph.vy, mz * ph.vz));
-        if (!(b2 <= T.w) || !(mz < 0.0f) || !(s_c > 0.0f)) return h;
-        s_pl = mz * rv;
-        h.x = fmaf(s_pl, ph.vx, -mx); h.y = fmaf(s_pl, ph.vy, -my);
-    }
     const float *fr = &sm.frame[e * kFrameStride];
     const float habs = P.z_ref_f + ph.ez;
+    // Column depth T(e_z) of the emission altitude (R8) and, for R27, the refractivity there.  The layer: the preamble
+    // left it in the frame when the whole segment lies in one layer (F_LAYER >= 0), else it is looked up (unused
+    // layers carry h_lo = +inf, so the count is the index).
+    float Te, eta_e;
+    auto atmosphere_at_emission = [&]() {
+        int li = __float_as_int(fr[F_LAYER]);
+        if (li < 0) {
+            li = 0;
+#pragma unroll
+            for (int i = 1; i < kMaxLayers; ++i) li += (habs >= P.layerf[i].h_lo) ? 1 : 0;
+        }
+        const LayerF lf = P.layerf[li];
+        const float E = __expf(-habs * lf.inv_c);
+        Te = fmaf(lf.b, E, lf.a);
+        eta_e = P.kappa_m * lf.b * lf.inv_c * E;             // eta0 rho(h) / rho0, rho = (b / c) exp(-h / c) / 100
+    };
+    float s_pl;
+    if ((P.flags & kFlagRefract) && ph.vz <= -0.5f) {
+        // R27: point and direction on the plane z = c_z corrected for refraction to first order, then
+        // the sphere test on the corrected values.  (x, y) = straight-line plane point relative to the centre.
+        float x, y, hk;
+        if (ph.axis) {
+            hk = ph.ez - T.z;
+            x = fmaf(T.z * rv, ph.vx, ph.gx - T.x); y = fmaf(T.z * rv, ph.vy, ph.gy - T.y);
+        } else {
+            const float mx = T.x - ph.ex, my = T.y - ph.ey, mz = T.z - ph.ez;
+            hk = -mz;
+            x = fmaf(mz * rv, ph.vx, -mx); y = fmaf(mz * rv, ph.vy, -my);
+        }
+        if (!(hk > 0.0f)) return h;
+        s_pl = -hk * rv;
+        atmosphere_at_emission();
+        const float arv = fabsf(rv);
+        // dr along the horizontal flight direction: (v_x, v_y) / sin(theta0) * tan(theta0) / cos^2(theta0) [...]
+        const float G = (eta_e * hk - P.kappa_m * (telT_at<TELSRC>(P, k) - Te)) * arv * arv * arv;
+        x = fmaf(ph.vx, G, x); y = fmaf(ph.vy, G, y);
+        // dtheta = tan(theta0) f, f = eta(e_z) - eta(c_z):  sin(theta0 + dtheta) = sin(theta0) (1 + f),
+        // -cos(theta0 + dtheta) = v_z + sin^2(theta0) f / |v_z|   (second order ~1e-11 dropped)
+        const float f = eta_e - telEta_at<TELSRC>(P, k);
+        const float vx = fmaf(ph.vx, f, ph.vx), vy = fmaf(ph.vy, f, ph.vy);
+        const float qv = fmaf(x, vx, y * vy);
+        const float b2 = fmaf(x, x, y * y) - qv * qv;
+        if (!(b2 <= T.w) || !(s_pl - qv > 0.0f)) return h;
+        h.x = x; h.y = y; h.vx = vx; h.vy = vy;
+    } else {
+        if (ph.axis) {
+            // q = g - c on the plane z_ref:  b^2 = |q|^2 - (q.v)^2,  the point g is at path length -ez / v_z
+            const float qx = ph.gx - T.x, qy = ph.gy - T.y, qz = -T.z;
+            const float qv = fmaf(qx, ph.vx, fmaf(qy, ph.vy, qz * ph.vz));
+            const float b2 = fmaf(qx, qx, fmaf(qy, qy, qz * qz)) - qv * qv;
+            const float hk = ph.ez - T.z;                                      // emission height above the telescope plane
+            s_pl = -hk * rv;
+            const float s_c = (s_pl - T.z * rv) - qv;
+            if (!(b2 <= T.w) || !(hk > 0.0f) || !(s_c > 0.0f)) return h;
+            h.x = fmaf(T.z * rv, ph.vx, qx); h.y = fmaf(T.z * rv, ph.vy, qy);  // on the plane z = c_z, relative to the centre (R11)
+        } else {
+            // no plane projection (ill-conditioned for |v_z| -> 0):  b = |m x v|,  m = c - e
+            const float mx = T.x - ph.ex, my = T.y - ph.ey, mz = T.z - ph.ez;
+            const float cx = fmaf(my, ph.vz, -(mz * ph.vy)), cy = fmaf(mz, ph.vx, -(mx * ph.vz)), cz = fmaf(mx, ph.vy, -(my * ph.vx));
+            const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+            const float s_c = fmaf(mx, ph.vx, fmaf(my, ph.vy, mz * ph.vz));
+            if (!(b2 <= T.w) || !(mz < 0.0f) || !(s_c > 0.0f)) return h;
+            s_pl = mz * rv;
+            h.x = fmaf(s_pl, ph.vx, -mx); h.y = fmaf(s_pl, ph.vy, -my);
+        }
+        atmosphere_at_emission();
+    }
     // R8: arrival time = emission time + (geometric path + integral of eta dl) / c,
     //     integral = kappa (T(c_z) - T(e_z)) / |v_z|
-    // The layer of the emission altitude: the preamble left it in the frame when the whole segment lies in one
-    // layer (F_LAYER >= 0), else it is looked up (unused layers carry h_lo = +inf, so the count is the index).
-    int li = __float_as_int(fr[F_LAYER]);
-    if (li < 0) {
-        li = 0;
-#pragma unroll
-        for (int i = 1; i < kMaxLayers; ++i) li += (habs >= P.layerf[i].h_lo) ? 1 : 0;
-    }
-    const LayerF lf = P.layerf[li];
-    const float Te = fmaf(lf.b, __expf(-habs * lf.inv_c), lf.a);
     const float excess = P.kappa_m * (telT_at<TELSRC>(P, k) - Te) * fabsf(rv);
     h.t = fmaf(ph.s, fr[F_IBC], fr[F_T0]) + (s_pl + excess) * (1.0f / 0.299792458f);
     // R4: wavelength
@@ -843,14 +892,25 @@ __device__ __forceinline__ void push_candidates(const KParams &P, TileSmem &sm, 
 
 // ---- conservative pre-tests on the crossing (gx, gy) of the plane z_ref (valid while |v_z| is not tiny).
 // Coplanar telescopes (q_z = 0): b^2 >= |q|^2 v_z^2, so |q|^2 v_z^2 (1 - 1e-4) > R^2 is a miss.
+// `add` widens the test for the refraction corrections (R27): a point that moves by at most d in the plane can be hit
+// if |q| |v_z| <= R + x, x = d |v_z|, and (R + x)^2 <= R^2 + x (2 R_max + x) = R^2 + add.  0 without the flag.
 template <bool COPLANAR>
-__device__ __forceinline__ bool plane_pretest(const float4 T, float gx, float gy, float vx, float vy, float vz, float vz2s)
+__device__ __forceinline__ bool plane_pretest(const float4 T, float gx, float gy, float vx, float vy, float vz, float vz2s, float add)
 {
     const float qx = gx - T.x, qy = gy - T.y;
-    if (COPLANAR) return fmaf(qy, qy, qx * qx) * vz2s <= T.w;
+    if (COPLANAR) return fmaf(fmaf(qy, qy, qx * qx), vz2s, -add) <= T.w;
     const float qv = fmaf(qx, vx, fmaf(qy, vy, -T.z * vz));
     const float qq = fmaf(qx, qx, fmaf(qy, qy, T.z * T.z));
-    return qq - qv * qv <= fmaf(qq, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f));        // slack for the fp32 cancellation
+    return qq - qv * qv - add <= fmaf(qq, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f));   // slack for the fp32 cancellation
+}
+
+// Slack of the pre-tests for a photon whose arrival point the refraction corrections may move (|v_z| >= 0.5 only).
+__device__ __forceinline__ float refraction_slack(const KParams &P, float vz)
+{
+    if (!(vz <= -0.5f)) return 0.0f;
+    const float rv = rcp_approx(vz), s2 = fmaf(-vz, vz, 1.0f);
+    const float x = 1.01f * P.refr_cmax * sqrtf(fmaxf(s2, 0.0f)) * rv * rv;      // d |v_z| = cmax sin / cos^2
+    return x * (P.refr_two_rmax + x);
 }
 
 // Candidate mask of a photon over the telescopes reachable from its plane crossing.
@@ -868,7 +928,8 @@ template <int TELSRC> __device__ __forceinline__ uint32_t slot_telescope(const u
 // Candidates of one grid level: cell of the plane crossing (most cells are empty: one load, one compare), then the
 // pre-test of the telescopes listed there (slots fill from 0, so the first empty slot ends the list).
 template <bool COPLANAR>
-__device__ __forceinline__ uint32_t grid_lookup(const KParams &P, const GridLevel &G, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
+__device__ __forceinline__ uint32_t grid_lookup(const KParams &P, const GridLevel &G, float gx, float gy, float vx, float vy, float vz, uint2 *cell,
+                                                float add)
 {
     const int ix = __float2int_rd(fmaf(gx, G.inv_cell, G.ox)), iy = __float2int_rd(fmaf(gy, G.inv_cell, G.oy));
     if ((unsigned)ix >= (unsigned)G.nx || (unsigned)iy >= (unsigned)G.ny) return 0u;
@@ -876,34 +937,38 @@ __device__ __forceinline__ uint32_t grid_lookup(const KParams &P, const GridLeve
     if (c.x == 0xffffffffu) return 0u;
     *cell = c;
     const float vz2s = vz * vz * 0.9999f;
-    uint32_t cm = plane_pretest<COPLANAR>(__ldg(&P.telA[c.x & 0xffffu]), gx, gy, vx, vy, vz, vz2s) ? 1u : 0u;
+    uint32_t cm = plane_pretest<COPLANAR>(__ldg(&P.telA[c.x & 0xffffu]), gx, gy, vx, vy, vz, vz2s, add) ? 1u : 0u;
     if ((c.x >> 16) != 0xffffu) {
-        if (plane_pretest<COPLANAR>(__ldg(&P.telA[c.x >> 16]), gx, gy, vx, vy, vz, vz2s)) cm |= 2u;
+        if (plane_pretest<COPLANAR>(__ldg(&P.telA[c.x >> 16]), gx, gy, vx, vy, vz, vz2s, add)) cm |= 2u;
         if (c.y != 0xffffffffu) {
-            if (plane_pretest<COPLANAR>(__ldg(&P.telA[c.y & 0xffffu]), gx, gy, vx, vy, vz, vz2s)) cm |= 4u;
-            if ((c.y >> 16) != 0xffffu && plane_pretest<COPLANAR>(__ldg(&P.telA[c.y >> 16]), gx, gy, vx, vy, vz, vz2s)) cm |= 8u;
+            if (plane_pretest<COPLANAR>(__ldg(&P.telA[c.y & 0xffffu]), gx, gy, vx, vy, vz, vz2s, add)) cm |= 4u;
+            if ((c.y >> 16) != 0xffffu && plane_pretest<COPLANAR>(__ldg(&P.telA[c.y >> 16]), gx, gy, vx, vy, vz, vz2s, add)) cm |= 8u;
         }
     }
     return cm;
 }
 
-template <int TELSRC, bool COPLANAR, int NT>
+template <int TELSRC, bool COPLANAR, int NT, bool REFR>
 __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
 {
     if constexpr (TELSRC == TEL_CONST) {
-        const float vz2s = vz * vz * 0.9999f;
+        const float vz2s = vz * vz * 0.9999f, add = REFR ? refraction_slack(P, vz) : 0.0f;
         uint32_t cm = 0u;
         // NT = n_tel rounded up to 1, 4 or 8; the unused slots hold R^2 = -1 (never a candidate).  Unrolled so that the
         // telescope coordinates are constant-bank operands.
 #pragma unroll
         for (int k = 0; k < NT; ++k)
-            if (plane_pretest<COPLANAR>(P.tel_c[k], gx, gy, vx, vy, vz, vz2s)) cm |= 1u << k;
+            if (plane_pretest<COPLANAR>(P.tel_c[k], gx, gy, vx, vy, vz, vz2s, add)) cm |= 1u << k;
         return cm;
     } else if constexpr (TELSRC == TEL_GRID) {
         // steep photons use level 0; flatter ones the coarser level 1 when it exists, else the wide test.  One code
         // path per level, so that the level's parameters are constant-bank operands.
-        if (-vz >= P.grid_lvl[0].vzmin) return grid_lookup<COPLANAR>(P, P.grid_lvl[0], gx, gy, vx, vy, vz, cell);
-        if (P.n_grid_levels > 1 && -vz >= P.grid_lvl[1].vzmin) return grid_lookup<COPLANAR>(P, P.grid_lvl[1], gx, gy, vx, vy, vz, cell);
+        if (-vz >= P.grid_lvl[0].vzmin) {
+            // with the refraction corrections the steep photons use the copy of level 0 whose discs carry their reach
+            if (REFR) return grid_lookup<COPLANAR>(P, P.grid_lvl[kGridLevels], gx, gy, vx, vy, vz, cell, refraction_slack(P, vz));
+            return grid_lookup<COPLANAR>(P, P.grid_lvl[0], gx, gy, vx, vy, vz, cell, 0.0f);
+        }
+        if (P.n_grid_levels > 1 && -vz >= P.grid_lvl[1].vzmin) return grid_lookup<COPLANAR>(P, P.grid_lvl[1], gx, gy, vx, vy, vz, cell, 0.0f);
         return kAllTelescopes;
     } else {
         return kAllTelescopes;
@@ -975,7 +1040,7 @@ __device__ __forceinline__ void wide_push(const KParams &P, TileSmem &sm, unsign
 
 // a2-a4 of the hot loop for the generic kinds.  Returns the candidate mask (see plane_candidates); *upward is
 // set when the photon does not go down.  Photons flatter than |v_z| = 0.05 are tested against all telescopes.
-template <int TELSRC, bool COPLANAR, int NT>
+template <int TELSRC, bool COPLANAR, int NT, bool REFR>
 __device__ __noinline__ uint32_t generic_candidates(const KParams &P, const TileSmem &sm, int e, uint32_t r0, uint32_t r1, uint32_t r2,
                                                     uint32_t r3, uint2 *cell, bool *upward)
 {
@@ -984,7 +1049,7 @@ __device__ __noinline__ uint32_t generic_candidates(const KParams &P, const Tile
     if (*upward) return 0u;
     if (ph.vz > -0.05f) return kAllTelescopes;
     const float spl = -ph.ez * rcp_approx(ph.vz);          // candidate search only: the pre-tests carry slack
-    return plane_candidates<TELSRC, COPLANAR, NT>(P, fmaf(spl, ph.vx, ph.ex), fmaf(spl, ph.vy, ph.ey), ph.vx, ph.vy, ph.vz, cell);
+    return plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, fmaf(spl, ph.vx, ph.ex), fmaf(spl, ph.vy, ph.ey), ph.vx, ph.vy, ph.vz, cell);
 }
 
 // ------------------------------------------------------------------------------------
@@ -1011,7 +1076,7 @@ struct WarpWalk {
 // tiles; photon output: while the tile runs in rounds) evaluate the first candidate of an axis-kind photon right in
 // the loop, from the values already in registers: no queue, no second Philox, no second sincos.  The sparse tiles of
 // the photon-output kernels run the instance without that code.  Returns whether the tile is (still) in rounds mode.
-template <int TELSRC, bool COPLANAR, int NT, int MODE, bool INLINE>
+template <int TELSRC, bool COPLANAR, int NT, int MODE, bool INLINE, bool REFR, bool FIRST>
 __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &ww, const uint32_t hi, const unsigned long long tile_first,
                                      const uint32_t it0, const uint32_t it1, const uint32_t n_iter, bool rounds)
 {
@@ -1057,7 +1122,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                         vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
                         vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
                     }
-                    cm = plane_candidates<TELSRC, COPLANAR, NT>(P, gx, gy, vx, vy, vz, &cell);
+                    cm = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gx, gy, vx, vy, vz, &cell);
                     if constexpr (MODE != MODE_TALLY) {
                         if (INLINE && cm != 0u && cm != kAllTelescopes) {
                             const float *fr = &sm.frame[e * kFrameStride];
@@ -1081,7 +1146,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 // the same hoisted Philox as the axis kind (the process tag is counter word 3)
                 r = philox_photon(P, pe, j, kind_tag(kind));
                 bool up;
-                cm = generic_candidates<TELSRC, COPLANAR, NT>(P, sm, e, r.r0, r.r1, r.r2, r.r3, &cell, &up);
+                cm = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, r.r0, r.r1, r.r2, r.r3, &cell, &up);
                 if (up) ++n_up;
             }
         }
@@ -1110,10 +1175,10 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
             if (__any_sync(0xffffffffu, cm != 0u))
                 push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
             if (OUT && rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
-                OutSmem &os = out_smem(sm);
-                // nothing staged in round 0: a sparse tile, which goes on without rounds (and barriers)
-                const bool first = it < (uint32_t)kRound;
-                if (!flush_round(P, os, first) && first) rounds = false;
+                // FIRST = the instance that runs round 0: too little staged there means a sparse tile, which goes on
+                // without rounds (and barriers).  In the other instances `rounds` is a constant.
+                if constexpr (FIRST) { if (!flush_round(P, out_smem(sm), true)) rounds = false; }
+                else flush_round(P, out_smem(sm), false);
             }
         } else {
             if (have)
@@ -1245,16 +1310,22 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         ww.f_reg = load_axis_frame(sm, ww.e);
         ww.g = lo + (uint32_t)lane; ww.j = ww.g - sm.prefix[ww.e];
         ww.n_up = 0u; ww.q_head = 0u; ww.q_count = 0u;
+        // One instance of the loop per (inline evaluation, refraction slack in the pre-tests): both are uniform over the
+        // tile, and a photon of the default path pays for neither.
         bool rounds = false;
+#define C8_WALK(INL, FIRST, IT0, IT1, RND)                                                                                       \
+    ((P.flags & kFlagRefract) ? walk<TELSRC, COPLANAR, NT, MODE, INL, true, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND) \
+                              : walk<TELSRC, COPLANAR, NT, MODE, INL, false, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND))
         if constexpr (OUT) {
             // round 0 decides whether the tile is dense (stays in rounds mode, inline evaluation) or sparse
             const uint32_t it1 = min((uint32_t)kRound, n_iter);
-            rounds = walk<TELSRC, COPLANAR, NT, MODE, true>(P, sm, ww, hi, tile_first, 0u, it1, n_iter, true);
-            if (rounds) walk<TELSRC, COPLANAR, NT, MODE, true>(P, sm, ww, hi, tile_first, it1, n_iter, n_iter, true);
-            else walk<TELSRC, COPLANAR, NT, MODE, false>(P, sm, ww, hi, tile_first, it1, n_iter, n_iter, false);
+            rounds = C8_WALK(true, true, 0u, it1, true);
+            if (rounds) C8_WALK(true, false, it1, n_iter, true);
+            else C8_WALK(false, false, it1, n_iter, false);
         } else {
-            walk<TELSRC, COPLANAR, NT, MODE, MODE == MODE_HIST>(P, sm, ww, hi, tile_first, 0u, n_iter, n_iter, false);
+            C8_WALK((MODE == MODE_HIST), false, 0u, n_iter, false);
         }
+#undef C8_WALK
         n_up = ww.n_up;
         uint32_t q_head = ww.q_head, q_count = ww.q_count;
         if constexpr (TELSRC != TEL_CONST) {

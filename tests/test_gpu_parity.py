@@ -372,3 +372,49 @@ def test_one_segment_with_a_million_bunches(c8):
     rep = pu.compare(cfg, g, o)
     _report("1e6-bunches", rep)
     assert g["counts"][:, 0].max() > 1_000_000 and rep["matched"] > 1000
+
+
+@pytest.mark.parametrize("name,n", [("c1", None), ("c2", 50_000), ("c4", 60_000)])
+def test_refraction_corrections(c8, name, n):
+    """C8OPT_FLAG_REFRACT (R27): arrival point and direction corrected to first order on the GPU against
+    the oracle with the same flag; the corrections are visible (the records differ from the straight-line run)."""
+    import parity_util as pu
+    cfg = wl.make_config(name) if n is None else wl.make_config(name, n_segments=n)
+    plain = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_REFRACT)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report(f"refract-{name}", rep)
+    assert rep["matched"] > 100
+    common, ia, ib = np.intersect1d(plain["records"]["id"] * 4096 + plain["records"]["tel"],
+                                    g["records"]["id"] * 4096 + g["records"]["tel"], return_indices=True)
+    shift = np.hypot(plain["records"]["x"][ia] - g["records"]["x"][ib], plain["records"]["y"][ia] - g["records"]["y"][ib])
+    assert len(common) > 0.9 * len(g["records"]) and 1e-3 < np.median(shift) < 1.0
+
+
+def test_refraction_with_culling_non_coplanar(c8):
+    """Both flags, spheres of different sizes at different altitudes: the culling test carries the refraction reach."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=30_000)
+    tel = cfg["telescopes"].copy()
+    tel[:, 2] += np.array([0.0, 35.0, -20.0, 60.0], dtype=np.float32)
+    tel[:, 3] = np.array([6.0, 12.0, 25.0, 40.0], dtype=np.float32)
+    cfg["telescopes"] = tel
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_REFRACT | c8.FLAG_CULL)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o, check_upward=False)
+    _report("refract-cull-noncoplanar", rep)
+    assert g["counters"]["culled"] > 0 and rep["matched"] > 1000
+
+
+def test_refraction_in_ground_histogram(c8):
+    import oracle
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=20_000)
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_REFRACT)
+    g = pu.gpu_hist(cfg, (0.0, 0.0), 500.0, 500)
+    o = oracle.ground_histogram(cfg["atmosphere"], cfg["segments"], cfg["params"], (0.0, 0.0), 500.0, 500, threads=pu.n_threads())
+    rep = pu.compare_hist(g, o, 500.0, 500)
+    print("[hist refract] " + " ".join(f"{k}={v}" for k, v in rep.items()))
