@@ -390,6 +390,7 @@ def test_refraction_corrections(c8, name, n):
     common, ia, ib = np.intersect1d(plain["records"]["id"] * 4096 + plain["records"]["tel"],
                                     g["records"]["id"] * 4096 + g["records"]["tel"], return_indices=True)
     shift = np.hypot(plain["records"]["x"][ia] - g["records"]["x"][ib], plain["records"]["y"][ia] - g["records"]["y"][ib])
+    print(f"[refract-{name}] median shift of the arrival point {np.median(shift):.4f} m, max {shift.max():.3f} m")
     assert len(common) > 0.9 * len(g["records"]) and 1e-3 < np.median(shift) < 1.0
 
 
