@@ -102,6 +102,8 @@ def lib():
         L.orc_refraction.argtypes = [C.POINTER(Atmosphere), C.c_double, C.c_double, C.c_double,
                                      C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_refraction.restype = None
+        L.orc_array_sphere.argtypes = [C.POINTER(C.c_double), C.c_int, C.POINTER(C.c_double)]
+        L.orc_array_sphere.restype = None
         L.orc_transmission.restype = C.c_double
         L.orc_run.argtypes = [C.POINTER(Atmosphere), dp, C.c_int, C.c_void_p, C.c_uint64, C.c_uint64,
                               C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64,
@@ -176,6 +178,17 @@ def preamble(atm: dict, params: dict, segment, tag: int, beam_tel=None):
     st = lib().orc_preamble(C.byref(make_atmosphere(atm)), C.byref(make_params(params)),
                             seg.ctypes.data, int(tag), _dp(bt), C.byref(f))
     return st, f
+
+
+BEAM_ARRAY = -2       # params["fl_beam_telescope"]: one emission cone around the whole array, photon number scaled (R28)
+
+
+def array_sphere(telescopes) -> np.ndarray:
+    """(centre_x, centre_y, centre_z, R_b) of R28: the sphere that holds every telescope sphere."""
+    tel64 = np.ascontiguousarray(np.asarray(telescopes, dtype=np.float32).astype(np.float64).reshape(-1))
+    out = np.zeros(4)
+    lib().orc_array_sphere(_dp(tel64), len(tel64) // 4, _dp(out))
+    return out
 
 
 def make_photon(frame: Frame, params: dict, S: int, j: int, tag: int) -> Photon:

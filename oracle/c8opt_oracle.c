@@ -222,7 +222,30 @@ int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_seg
         orc_rodrigues(f->d, f->A, f->M);
     } else {
         mu = par->fl_yield * (double)s->dE;               /* constant yield x total energy loss */
-        if (par->fl_beam_telescope >= 0) {
+        if (par->fl_beam_telescope == -2) {
+            /* R28 ("an opening angle and pointing depending on the telescope distance ... From the
+             * resulting solid angle, the required scaling factor is calculated and applied to the total number of
+             * photons ... for multiple telescopes, an emission area is defined which includes all telescopes"):
+             * beam_tel_xyz = (centre, R_b) of a sphere that holds every telescope sphere.  Seen from the segment
+             * midpoint m at distance D, every direction from any point of the track to any point of that sphere lies
+             * within alpha of the line m -> centre, sin(alpha) = (R_b + L/2) / D.  The emission is uniform in that cone
+             * and the NUMBER of photons is scaled by Omega / 4 pi = (1 - cos alpha) / 2 (weights stay mu'/n_b).
+             * D <= R_b + L/2 (inside the array): isotropic, unscaled. */
+            double u[3];
+            for (int i = 0; i < 3; ++i) u[i] = beam_tel_xyz[i] - (f->p0[i] + (0.5 * L) * f->d[i]);
+            double D = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+            double sa = (beam_tel_xyz[3] + 0.5 * L) / D;
+            if (sa < 1.0) {
+                f->kind = 2;
+                for (int i = 0; i < 3; ++i) u[i] /= D;
+                orc_rodrigues(u, f->A, f->M);
+                double ca = sqrt(1.0 - sa * sa);
+                f->one_minus_cos_ab = (sa * sa) / (1.0 + ca);    /* 1 - cos(alpha) without cancellation */
+                mu = mu * (0.5 * f->one_minus_cos_ab);
+            } else {
+                f->kind = 1;
+            }
+        } else if (par->fl_beam_telescope >= 0) {
             f->kind = 2;
             double los[3];
             for (int i = 0; i < 3; ++i) los[i] = beam_tel_xyz[i] - (f->p0[i] + 0.5 * L * f->d[i]);
@@ -241,7 +264,8 @@ int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_seg
     f->mu = mu;
     f->n_b = (uint32_t)nb;
     f->w0 = mu / nb;
-    if (f->kind == 2) f->w0 *= f->one_minus_cos_ab * 0.5; /* Omega / 4 pi = (1 - cos alpha_b) / 2 */
+    if (f->kind == 2 && par->fl_beam_telescope >= 0)
+        f->w0 *= f->one_minus_cos_ab * 0.5;              /* R14 (weight form): Omega / 4 pi = (1 - cos alpha_b) / 2 */
     return 0;
 }
 
@@ -400,11 +424,29 @@ double orc_transmission(const orc_atmosphere *atm, double h, double lam, double 
  *   records  : NULL or orc_record[cap]; *n_rec is advanced
  * Brute force over ALL telescopes; a photon may hit several; no shadowing (R10).
  */
+/* R28: the sphere that holds every telescope sphere: centre = centre of the bounding box of the telescope centres,
+ * R_b = max_k (|c_k - centre| + R_k). */
+void orc_array_sphere(const double *tel, int n_tel, double out[4])
+{
+    double lo[3] = { INFINITY, INFINITY, INFINITY }, hi[3] = { -INFINITY, -INFINITY, -INFINITY };
+    for (int k = 0; k < n_tel; ++k)
+        for (int i = 0; i < 3; ++i) { lo[i] = fmin(lo[i], tel[4 * k + i]); hi[i] = fmax(hi[i], tel[4 * k + i]); }
+    for (int i = 0; i < 3; ++i) out[i] = 0.5 * (lo[i] + hi[i]);
+    double rb = 0.0;
+    for (int k = 0; k < n_tel; ++k) {
+        double x = tel[4 * k] - out[0], y = tel[4 * k + 1] - out[1], z = tel[4 * k + 2] - out[2];
+        rb = fmax(rb, sqrt(x * x + y * y + z * z) + tel[4 * k + 3]);
+    }
+    out[3] = rb;
+}
+
 void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
              const orc_segment *seg, uint64_t n, uint64_t first_id, const orc_params *par,
              uint32_t *counts, orc_tally *tallies, uint64_t *counters,
              orc_record *records, uint64_t cap, uint64_t *n_rec)
 {
+    double array[4];
+    orc_array_sphere(tel, n_tel, array);
     for (uint64_t i = 0; i < n; ++i) {
         uint64_t S = first_id + i;
         counters[0] += 1;
@@ -413,7 +455,8 @@ void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
             if (counts) counts[2 * i + tag] = 0;
             if (!((par->processes >> tag) & 1u)) continue;
             orc_frame f;
-            const double *bt = (tag == 1 && par->fl_beam_telescope >= 0) ? &tel[4 * par->fl_beam_telescope] : NULL;
+            const double *bt = (tag == 1 && par->fl_beam_telescope >= 0) ? &tel[4 * par->fl_beam_telescope]
+                             : (tag == 1 && par->fl_beam_telescope == -2) ? array : NULL;
             if (orc_preamble(atm, par, &seg[i], tag, bt, &f) != 0) { invalid = 1; continue; }
             if (counts) counts[2 * i + tag] = f.n_b;
             for (uint32_t j = 0; j < f.n_b; ++j) {

@@ -688,3 +688,72 @@ def test_refracted_records_move_by_the_corrections():
         assert math.isclose(rb["y"] - ra["y"], dr * ra["cy"] / sin0, rel_tol=1e-6, abs_tol=1e-9)
         th_b = math.asin(math.hypot(rb["cx"], rb["cy"]))
         assert math.isclose(th_b - math.asin(sin0), dth, rel_tol=1e-5, abs_tol=1e-12)
+
+
+# ------------------------------------------------------------------ beaming at the whole array (R28)
+def test_array_beaming_solid_angle_and_photon_number():
+    """Cone around the whole array with the paper's scaling of the photon NUMBER: closed-form solid angle, n_b and
+    weight; inside the array (D <= R_b + L/2) the emission stays isotropic and unscaled."""
+    tel = W.telescopes_square()                                     # (+-50, +-50, 2000), R = 6
+    sph = O.array_sphere(tel)
+    assert np.allclose(sph[:3], [0.0, 0.0, 2000.0]) and math.isclose(sph[3], math.hypot(50.0, 50.0) + 6.0, rel_tol=1e-12)
+    par = W.default_params(processes=W.PROC_FLUORESCENCE, fl_beam_telescope=O.BEAM_ARRAY, bunch_size=1.0)
+    seg = one_segment(x0=3000.0, y0=4000.0, z0=2000.0 + 12000.0, d=(0.0, 0.6, -0.8), length=20.0, dE=2.5e6)   # mu = 1e7
+    st, f = O.preamble(ATM5, par, seg[0], 1, beam_tel=sph)
+    mid = np.array([3000.0, 4000.0, 14000.0]) + 10.0 * np.array([0.0, 0.6, -0.8])
+    D = np.linalg.norm(sph[:3] - mid)
+    alpha = math.asin((sph[3] + 10.0) / D)
+    frac = (1.0 - math.cos(alpha)) / 2.0
+    assert st == 0 and f.kind == 2
+    assert math.isclose(f.one_minus_cos_ab, 1.0 - math.cos(alpha), rel_tol=1e-9)
+    mu = 4.0 * 2.5e6
+    assert f.n_b == math.ceil(mu * frac / 1.0) and math.isclose(f.w0, mu * frac / f.n_b, rel_tol=1e-9)
+    assert 0.5 < f.w0 <= 1.0 and f.n_b < 1e-4 * mu                   # the gain: far fewer bunches of about unit weight
+    # inside the array: isotropic, unscaled
+    seg_in = one_segment(x0=10.0, y0=0.0, z0=2030.0, length=5.0, dE=250.0)
+    st, fi = O.preamble(ATM5, par, seg_in[0], 1, beam_tel=sph)
+    assert st == 0 and fi.kind == 1 and fi.n_b == 1000 and fi.w0 == 1.0
+
+
+def test_array_beaming_cone_holds_every_ray_to_every_telescope():
+    """Brute force: from random points of the track to random points of every telescope sphere, the direction lies in
+    the emission cone; and every emitted photon lies in it too."""
+    tel = W.telescopes_grid(n=3, spacing=120.0)
+    sph = O.array_sphere(tel)
+    par = W.default_params(processes=W.PROC_FLUORESCENCE, fl_beam_telescope=O.BEAM_ARRAY, bunch_size=1.0, seed=21)
+    seg = one_segment(x0=-900.0, y0=400.0, z0=4500.0, d=(0.5, 0.1, -0.86), length=300.0, dE=1e6)
+    st, f = O.preamble(ATM5, par, seg[0], 1, beam_tel=sph)
+    assert st == 0 and f.kind == 2
+    p0, d, L = np.array(list(f.p0)), np.array(list(f.d)), f.L
+    axis = sph[:3] - (p0 + 0.5 * L * d)
+    axis /= np.linalg.norm(axis)
+    cos_a = 1.0 - f.one_minus_cos_ab
+    rng = np.random.Generator(np.random.PCG64(3))
+    for k in range(len(tel)):
+        c, R = tel[k, :3].astype(np.float64), float(tel[k, 3])
+        for _ in range(200):
+            e = p0 + rng.uniform(0.0, L) * d
+            n = rng.normal(size=3)
+            pt = c + R * rng.uniform(0.0, 1.0) ** (1 / 3) * n / np.linalg.norm(n)
+            u = (pt - e) / np.linalg.norm(pt - e)
+            assert u @ axis >= cos_a - 1e-12
+    for j in range(0, f.n_b, max(1, f.n_b // 300)):
+        v = np.array(list(O.make_photon(f, par, 0, j, 1).v))
+        assert v @ axis >= cos_a - 1e-12
+
+
+def test_array_beaming_keeps_the_expected_tally():
+    """The scaled number of photons in the cone gives the same expected weighted tally as isotropic emission."""
+    tel = np.array([[0.0, 0.0, 2000.0, 300.0], [500.0, 0.0, 2000.0, 200.0]], dtype=np.float32)
+    seg = one_segment(x0=100.0, y0=50.0, z0=5000.0, length=1e-3, gamma=100.0, dE=2.5e5)      # mu = 1e6 at one point
+    par_i = W.default_params(processes=W.PROC_FLUORESCENCE, seed=5)
+    par_a = W.default_params(processes=W.PROC_FLUORESCENCE, seed=6, fl_beam_telescope=O.BEAM_ARRAY)
+    ri = O.run(ATM5, tel, seg, par_i)
+    ra = O.run(ATM5, tel, seg, par_a)
+    assert int(ra["counters"][1]) < 0.1 * int(ri["counters"][1])      # far fewer photons generated
+    for k in range(2):
+        # isotropic: binomial with p_k = hits / n; the beamed run has the same expectation n p_k with unit-ish weights
+        n_i = int(ri["counters"][1]); h_i = int(ri["tallies"]["hits"][k])
+        sig = math.sqrt(h_i) + math.sqrt(ra["tallies"]["sum_w"][k])
+        assert abs(ri["tallies"]["sum_w"][k] - ra["tallies"]["sum_w"][k]) < 5.0 * sig, (k, ri["tallies"][k], ra["tallies"][k])
+        assert h_i > 500
