@@ -59,6 +59,14 @@ extern "C" {
  * | angle(d, c_k - p_mid) - theta_c | > asin(R_k / D) + asin((L/2) / D), D = |c_k - p_mid| - L/2 -- skips the
  * photon loop.  Tallies and records are identical with and without it; the skipped bunches still count as
  * generated and are reported in counters[C8OPT_CNT_CULLED]; C8OPT_CNT_UPWARD then covers propagated bunches only. */
+/* c8opt_run_params.fl_beam_telescope = C8OPT_BEAM_ARRAY: PAPER.md:39 for several telescopes ("an emission area is
+ * defined which includes all telescopes involved"; "the required scaling factor is calculated and applied to the total
+ * number of photons").  Per segment, the emission is uniform in the cone about the line from the segment midpoint to
+ * the centre of the sphere holding every telescope sphere (centre of the bounding box of the telescope centres,
+ * R_b = max |c_k - centre| + R_k), sin(alpha) = (R_b + L/2) / D; the photon NUMBER is mu (1 - cos alpha) / 2 and the
+ * bunches keep weight mu'/n_b; segments inside that sphere emit isotropically, unscaled.  fl_beam_halfangle_rad is
+ * not used (R28). */
+#define C8OPT_BEAM_ARRAY   (-2)
 #define C8OPT_FLAG_CULL    1u
 /* REFRACT: the refraction corrections of PAPER.md:77 ("straight line propagation followed by the application of
  * correction factors which changes the arrival angle, position, and timing") in the first-order planar-Snell reading
@@ -110,7 +118,8 @@ typedef struct {
     double   bunch_size;           /* B: n_b = ceil(mu / B) bunches of weight mu / n_b (R1) */
     double   fl_yield_per_MeV;     /* constant fluorescence yield (R13)        */
     double   fl_lam1_nm, fl_lam2_nm;
-    int32_t  fl_beam_telescope;    /* -1 isotropic, else beam toward this telescope (R14)   */
+    int32_t  fl_beam_telescope;    /* -1 isotropic; k >= 0 beam toward telescope k (R14);
+                                      C8OPT_BEAM_ARRAY beam at the whole array (R28)        */
     uint32_t flags;                /* C8OPT_FLAG_* bits                                     */
     double   fl_beam_halfangle_rad;
 } c8opt_run_params;

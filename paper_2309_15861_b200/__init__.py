@@ -25,6 +25,7 @@ from .build import LIB_PATH, build  # noqa: F401
 MAX_LAYERS = 8
 PROC_CHERENKOV, PROC_FLUORESCENCE = 1, 2
 MODE_TALLY, MODE_OUTPUT, MODE_GROUND_HIST = 0, 1, 2
+BEAM_ARRAY = -2
 FLAG_CULL = 1
 FLAG_REFRACT = 2
 COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "culled")

@@ -33,6 +33,7 @@ struct c8opt_ctx {
     bool coplanar = true;
     std::vector<double> tel_xyzr;          // absolute, as given (float -> double)
     double x_ref = 0, y_ref = 0, z_ref = 0;
+    double array_rb = 0;               // the same radius, exact (fluorescence beamed at the array, R28)
     float cull_Rb = 0;                 // radius about the reference point that holds every telescope sphere
     // ground-plane radial profile (C8OPT_MODE_GROUND_HIST)
     c8::Tally *d_hist = nullptr;       // [hist_bins + 1], the last one counts the overflow
@@ -212,7 +213,7 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     if (!hist && ctx->n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no telescopes: call c8opt_add_telescopes first");
     if (hist && ctx->hist_bins < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "no histogram: call c8opt_set_ground_histogram first");
     if (hist && (rp->flags & C8OPT_FLAG_CULL)) return fail(ctx, C8OPT_ERR_ARGUMENT, "no culling in ground-histogram mode (every bunch counts)");
-    if (hist && (rp->processes & C8OPT_PROC_FLUORESCENCE) && rp->fl_beam_telescope >= 0)
+    if (hist && (rp->processes & C8OPT_PROC_FLUORESCENCE) && rp->fl_beam_telescope != -1)
         return fail(ctx, C8OPT_ERR_ARGUMENT, "ground-histogram mode has no telescope to beam at");
     const unsigned procs = rp->processes;
     if (procs == 0 || (procs & ~3u)) return fail(ctx, C8OPT_ERR_ARGUMENT, "processes must be a combination of bits 0 and 1");
@@ -274,6 +275,10 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     P.bunch_size = rp->bunch_size; P.fl_yield = rp->fl_yield_per_MeV;
     P.fl_lam1 = (float)rp->fl_lam1_nm; P.fl_dlam = (float)(rp->fl_lam2_nm - rp->fl_lam1_nm);
     P.beam_tel = (procs & C8OPT_PROC_FLUORESCENCE) ? rp->fl_beam_telescope : -1;
+    if (P.beam_tel < -2) return fail(ctx, C8OPT_ERR_ARGUMENT, "fl_beam_telescope must be >= -2");
+    if (P.beam_tel == C8OPT_BEAM_ARRAY) {
+        P.beam_x = ctx->x_ref; P.beam_y = ctx->y_ref; P.beam_z = ctx->z_ref; P.beam_rb = ctx->array_rb;
+    }
     if (P.beam_tel >= 0) {
         P.beam_x = ctx->tel_xyzr[4 * P.beam_tel + 0]; P.beam_y = ctx->tel_xyzr[4 * P.beam_tel + 1];
         P.beam_z = ctx->tel_xyzr[4 * P.beam_tel + 2];
@@ -448,6 +453,7 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
         rb = std::fmax(rb, std::sqrt(x * x + y * y + z * z) + xyzr[4 * k + 3]);
     }
     ctx->cull_Rb = (float)(rb * (1.0 + 1e-6));
+    ctx->array_rb = rb;
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telA, sizeof(float4) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telT, sizeof(float) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telEta, sizeof(float) * n));

@@ -99,7 +99,8 @@ struct KParams {
     float inv_lam1, dinv_lam;      // Cherenkov: 1/lam = inv_lam1 - u3 * dinv_lam (R4)
     float fl_lam1, fl_dlam;
     int beam_tel;
-    double beam_x, beam_y, beam_z; // centre of the beam telescope (absolute)
+    double beam_x, beam_y, beam_z; // centre of the beam telescope, or (beam_tel == -2) of the array's sphere (absolute)
+    double beam_rb;                // radius of the sphere that holds every telescope sphere (beam_tel == -2, R28)
     double omc;                    // 1 - cos(alpha_b) (R14)
     // work
     const float4 *seg;             // device, 3 x float4 per segment
@@ -251,12 +252,12 @@ __device__ __forceinline__ HistSmem &hist_smem(TileSmem &sm) { return *reinterpr
 //   F_A0..C2 (7..15): v = sth (cos' A + sin' B) + cth C.
 // Hit-only slots (all kinds): F_W0 weight, F_T0 start time, F_IBC 1/(beta c), and for the axis kind
 //   F_DZ, F_AX..F_CY (v_x, v_y coefficients), F_LEN; F_LAYER = bits of the int index of the atmosphere layer that
-//   holds the whole segment, -1 if it crosses a layer boundary.
+//   holds the whole segment, -1 if it crosses a layer boundary; F_OMC = 1 - cos(half-angle) of a beamed emitter's cone.
 enum {
     F_NEGL = 0, F_K0C = 1, F_AZ = 2, F_BZ = 3, F_CZ = 4, F_PX = 5, F_PY = 6, F_QX = 7, F_QY = 8, F_GX = 9, F_GY = 10,
     F_E0 = 0, F_D0 = 3, F_L = 6, F_A0 = 7, F_B0 = 10, F_C0 = 13,
     F_W0 = 16, F_T0 = 17, F_IBC = 18, F_DZ = 19, F_AX = 20, F_AY = 21, F_BX = 22, F_BY = 23, F_CX = 24, F_CY = 25,
-    F_LEN = 26, F_LAYER = 27
+    F_LEN = 26, F_LAYER = 27, F_OMC = 28
 };
 
 // ------------------------------------------------------------------------------------
@@ -357,7 +358,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     const double beta = sqrt(dsub(1.0, ig2));
     const double ibc = 1.0 / (beta * 0.299792458);        // R7: the particle moves at beta c  [ns/m]
 
-    double mu, sin_c = 0.0, cos_c = 1.0;
+    double mu, sin_c = 0.0, cos_c = 1.0, omc_e = P.omc;      // omc_e = 1 - cos(alpha) of this emitter's cone
     int kind;
     double axis[3];
     if (tag == 0) {
@@ -378,7 +379,26 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     } else {
         // constant yield x total energy loss over the track (R13).
         mu = dmul(P.fl_yield, dE);
-        if (P.beam_tel >= 0) {
+        if (P.beam_tel == -2) {
+            // PAPER.md:39, R28: one emission cone around the sphere (beam_x/y/z, beam_rb) that holds every telescope,
+            // sin(alpha) = (R_b + L/2) / D from the segment midpoint, and the NUMBER of photons scaled by
+            // Omega / 4 pi = (1 - cos alpha) / 2.  Operation order as in the oracle (feeds n_b).  Inside the array:
+            // isotropic, unscaled.
+            const double bt[3] = { P.beam_x, P.beam_y, P.beam_z };
+            for (int i = 0; i < 3; ++i) axis[i] = dsub(bt[i], dadd(p0[i], dmul(dmul(0.5, L), d[i])));
+            const double D = sqrt(dadd(dadd(dmul(axis[0], axis[0]), dmul(axis[1], axis[1])), dmul(axis[2], axis[2])));
+            const double sa = ddiv(dadd(P.beam_rb, dmul(0.5, L)), D);
+            if (sa < 1.0) {
+                kind = KIND_CONE;
+                for (int i = 0; i < 3; ++i) axis[i] = ddiv(axis[i], D);
+                const double ca = sqrt(dsub(1.0, dmul(sa, sa)));
+                omc_e = ddiv(dmul(sa, sa), dadd(1.0, ca));
+                mu = dmul(mu, dmul(0.5, omc_e));
+            } else {
+                kind = KIND_FL_ISO;
+                axis[0] = axis[1] = 0.0; axis[2] = -1.0;
+            }
+        } else if (P.beam_tel >= 0) {
             // PAPER.md:39, R15: line of sight from the segment midpoint to the telescope centre.
             const double bt[3] = { P.beam_x, P.beam_y, P.beam_z };
             double ln = 0.0;
@@ -395,7 +415,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     const double nb = ceil(ddiv(mu, P.bunch_size));              // R1: deterministic bunches
     if (nb > 16777215.0) { *bad = true; return 0; }
     double w0 = ddiv(mu, nb);
-    if (kind == KIND_CONE) w0 *= 0.5 * P.omc;                    // R14: Omega / 4 pi
+    if (kind == KIND_CONE && P.beam_tel >= 0) w0 *= 0.5 * P.omc;  // R14 (weight form): Omega / 4 pi
     if ((P.flags & kFlagCull) && tag == 0) {
         const double hl = 0.5 * L;
         if (cull_emitter(P, (float)(p0[0] + hl * d[0] - P.x_ref), (float)(p0[1] + hl * d[1] - P.y_ref), (float)(p0[2] + hl * d[2] - P.z_ref),
@@ -405,7 +425,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
         }
     }
 
-    fr[F_W0] = (float)w0; fr[F_T0] = s0.w; fr[F_IBC] = (float)ibc; fr[F_LEN] = (float)L;
+    fr[F_W0] = (float)w0; fr[F_T0] = s0.w; fr[F_IBC] = (float)ibc; fr[F_LEN] = (float)L; fr[F_OMC] = (float)omc_e;
     {
         // layer of both ends in fp32 altitudes as the photon loop sees them (1 m of margin against rounding)
         const float za = (float)p0[2], zb = (float)(p0[2] + L * d[2]);
@@ -527,7 +547,7 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
     } else {
         float sth = 1.0f, cth = 1.0f;
         if (kind == KIND_CONE) {                      // R14: 1 - cos(theta') uniform in [0, 1 - cos(alpha_b)]
-            const float t = uniform01(r.r3) * (float)P.omc;
+            const float t = uniform01(r.r3) * fr[F_OMC];
             cth = 1.0f - t; sth = sqrtf(t * (2.0f - t));     // beamed: sin(theta') sets the aim at 10 km, keep the IEEE root
         }
         ph.vx = fmaf(sth, fmaf(cp, fr[F_A0 + 0], sp * fr[F_B0 + 0]), cth * fr[F_C0 + 0]);

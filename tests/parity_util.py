@@ -103,6 +103,8 @@ def oracle_impact(cfg: dict, rid: int, k: int, first_id: int = 0):
     tel = np.asarray(cfg["telescopes"], dtype=np.float32).astype(np.float64)
     par = cfg["params"]
     bt = tel[par["fl_beam_telescope"]] if (tag == 1 and par["fl_beam_telescope"] >= 0) else None
+    if tag == 1 and par["fl_beam_telescope"] == oracle.BEAM_ARRAY:
+        bt = oracle.array_sphere(cfg["telescopes"])
     st, fr = oracle.preamble(cfg["atmosphere"], par, seg, tag, bt)
     assert st == 0 and j < fr.n_b
     ph = oracle.make_photon(fr, par, S, j, tag)

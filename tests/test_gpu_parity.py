@@ -419,3 +419,35 @@ def test_refraction_in_ground_histogram(c8):
     o = oracle.ground_histogram(cfg["atmosphere"], cfg["segments"], cfg["params"], (0.0, 0.0), 500.0, 500, threads=pu.n_threads())
     rep = pu.compare_hist(g, o, 500.0, 500)
     print("[hist refract] " + " ".join(f"{k}={v}" for k, v in rep.items()))
+
+
+def test_fluorescence_beamed_at_the_array(c8):
+    """fl_beam_telescope = C8OPT_BEAM_ARRAY (R28): per-segment cone around the whole array with the photon
+    number scaled; counts bit-exact against the oracle, records compared; far array (every segment beamed) and the
+    c4 array (segments inside the array's sphere stay isotropic)."""
+    import parity_util as pu
+    cfg = wl.make_config("c3a", n_segments=100_000)
+    tel = wl.telescopes_square().copy()
+    tel[:, 0] += 2500.0; tel[:, 1] -= 1500.0        # 2.9 km off the shower axis
+    tel[:, 3] = 12.0
+    cfg["telescopes"] = tel
+    cfg["params"] = dict(cfg["params"], fl_beam_telescope=c8.BEAM_ARRAY, fl_yield=4000.0)
+    # tracks a few metres above the telescopes' plane would reach them 2.9 km away along nearly horizontal rays
+    # (v_z ~ 0.003, t ~ 2e5 ns), beyond what fp32 positions and times can hold to 1 cm / 0.1 ns: keep the others
+    cfg["segments"] = cfg["segments"][cfg["segments"]["z0"] > 3000.0]
+    iso_generated = int(np.ceil(4000.0 * cfg["segments"]["dE"].astype(np.float64)).sum())
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("beam-array-far", rep)
+    assert rep["matched"] > 300 and g["counters"]["upward"] == 0
+    assert g["counters"]["generated"] < 1e-3 * iso_generated          # the paper's gain: the number of photons
+
+    cfg = wl.make_config("c4", n_segments=20_000)
+    cfg["params"] = dict(cfg["params"], fl_beam_telescope=c8.BEAM_ARRAY, fl_yield=400.0)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("beam-array-c4", rep)
+    fl = rep  # both processes: compare() has already checked the per-process counts
+    assert rep["matched"] > 20000
