@@ -34,6 +34,7 @@ struct c8opt_ctx {
     std::vector<double> tel_xyzr;          // absolute, as given (float -> double)
     double x_ref = 0, y_ref = 0, z_ref = 0;
     double array_rb = 0;               // the same radius, exact (fluorescence beamed at the array, R28)
+    int n_sm = 148;
     float cull_Rb = 0;                 // radius about the reference point that holds every telescope sphere
     // ground-plane radial profile (C8OPT_MODE_GROUND_HIST)
     c8::Tally *d_hist = nullptr;       // [hist_bins + 1], the last one counts the overflow
@@ -316,7 +317,13 @@ int launch(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, const c8opt_segment *d
     if (n == 0) return C8OPT_OK;
     P.seg = reinterpret_cast<const float4 *>(d_seg);
     P.n_seg = n; P.first_id = first_id; P.counts = counts;
-    const unsigned long long per_tile = c8::kTile / P.n_procs;
+    // Full tiles for large inputs; small inputs are cut into about one wave of tiles (3 CTAs on each of the SMs), at
+    // least 8 segments each, so that 10^4 segments do not run on a quarter of the GPU.
+    const unsigned long long per_tile_max = c8::kTile / P.n_procs;
+    const unsigned long long one_wave = 3ull * (unsigned long long)ctx->n_sm;
+    unsigned long long per_tile = (n + one_wave - 1) / one_wave;
+    per_tile = std::min(per_tile_max, std::max(8ull, per_tile));
+    P.tile_segs = (int)per_tile;
     const unsigned long long tiles = (n + per_tile - 1) / per_tile;
     if (tiles > 0x7fffffffull) return fail(ctx, C8OPT_ERR_ARGUMENT, "too many segments in one call");
     if (mode == C8OPT_MODE_GROUND_HIST) {
@@ -379,6 +386,7 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
     c8opt_ctx *ctx = new (std::nothrow) c8opt_ctx();
     if (!ctx) return fail(nullptr, C8OPT_ERR_ARGUMENT, "out of host memory");
     ctx->device = dev;
+    ctx->n_sm = prop.multiProcessorCount > 0 ? prop.multiProcessorCount : 148;
     ctx->n_layers = desc->n_layers;
     for (int i = 0; i < desc->n_layers; ++i)
         ctx->layer[i] = HostLayer{desc->layers[i].h_lo_m, desc->layers[i].a_gcm2, desc->layers[i].b_gcm2, desc->layers[i].c_m};

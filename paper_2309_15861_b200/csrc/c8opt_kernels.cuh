@@ -94,6 +94,7 @@ struct KParams {
     // run
     uint32_t rk0[10], rk1[10];     // Philox round keys: key + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t processes, n_procs;
+    int tile_segs;                 // segments per tile, <= kTile / n_procs
     double c_ft;                   // 2 pi alpha (1/lam1 - 1/lam2) [1/m]  (R2)
     double bunch_size, fl_yield;
     float inv_lam1, dinv_lam;      // Cherenkov: 1/lam = inv_lam1 - u3 * dinv_lam (R4)
@@ -1216,7 +1217,9 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem &sm = *reinterpret_cast<TileSmem *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int segs_per_tile = kTile / (int)P.n_procs;
+    // segments per tile: kTile / n_procs for large inputs; fewer for small ones, so that the tiles still fill the GPU
+    // (the emitter slots keep their places: Cherenkov from 0, fluorescence from kTile / 2 when both run)
+    const int segs_per_tile = P.tile_segs;
 
     // ---- clear the tile tallies
     const bool tally_in_smem = P.n_tel <= kTelSmemMax;
@@ -1244,7 +1247,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const int tag = (P.n_procs == 2) ? (tid >> 7) : ((P.processes & 1u) ? 0 : 1);
     const unsigned long long seg_i = (unsigned long long)blockIdx.x * (unsigned)segs_per_tile + (unsigned)seg_local;
     uint32_t nb = 0, n_culled = 0;
-    if (seg_i < P.n_seg) {
+    if (seg_local < segs_per_tile && seg_i < P.n_seg) {
         const float4 *sp = P.seg + seg_i * 3ull;
         const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
         bool bad, culled;
@@ -1373,7 +1376,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     }
     {
         // invalid segments of this tile (each counted once)
-        uint32_t nbad = (tid < segs_per_tile) ? sm.invalid[tid] : 0u;
+        uint32_t nbad = (tid < kTile / (int)P.n_procs) ? sm.invalid[tid] : 0u;
         nbad = __reduce_add_sync(0xffffffffu, nbad);
         if (lane == 0 && nbad) atomicAdd(&P.counters[6], (unsigned long long)nbad);
     }
