@@ -32,6 +32,14 @@ UNIT = "photons/s"
 # uniforms/generation/projection 40 + 8 per telescope tested + loop 10
 ALG_INSTR = {"c1": 98.0, "c2": 122.0, "c5": 122.0, "c3a": 110.0, "c3b": 120.0, "c4": 130.0}
 RECORD_BYTES = 28.0
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the round's `ncu --set full` captures under
+# profiles/, per 10^6 segments (they scale with the segment count); None = not captured for this workload.
+NCU_TRAFFIC_PER_1E6_SEGMENTS = {
+    ("c2", "tally"): 48.07e6,        # profiles/ncu_c2_tally_r01.md: the 48 MB segment table once
+    ("c4", "tally"): 48.58e6,        # profiles/ncu_c4_tally_r01.md
+    ("c5g", "output"): 5.071e9,      # profiles/ncu_c5g_output_r01.md: 5.022 GB written + 48.75 MB read
+    ("c2", "hist"): 48.09e6,         # profiles/ncu_c2_groundhist_r01.md
+}
 
 
 def load_peaks():
@@ -322,6 +330,11 @@ def main():
                     "unit": "Tinstr/s", "traffic": None, "peak_source": "148 SM x 4 schedulers x 32 lanes x sm_max_mhz "
                     f"({peaks['source']})", "alg_instr_per_photon": instr,
                     "hbm_achieved_gbs": (48.0 * n + RECORD_BYTES * (hits_per_step if output_mode else 0)) / per_launch_s / 1e9}
+    mode_key = "hist" if args.ground_hist else ("output" if output_mode else "tally")
+    traffic = NCU_TRAFFIC_PER_1E6_SEGMENTS.get((args.workload, mode_key))
+    if traffic is not None and not args.cull:
+        roofline["traffic"] = traffic * n / 1e6
+        roofline["traffic_source"] = "ncu --set full capture of this round (profiles/), scaled to this segment count"
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
     roofline["kernel"] = "c8::propagate_kernel"
     roofline["kernel_ms"] = per_launch_s * 1e3
