@@ -197,7 +197,8 @@ struct __align__(16) TileSmem {
     float frame[kTile * kFrameStride];          // fp32 frames, see frame slots below
     uint8_t kind[kTile];
     uint8_t invalid[kTile];
-    uint32_t warp_sum[kWarps];
+    uint32_t warp_sum[kWarps], warp_pad[kWarps];
+    uint8_t odd[kTile + 8];                     // 1 = the emitter's count is odd: its last slot of the index space is empty
     unsigned long long warp_wsum[kWarps];
     uint32_t bound[kWarps + 1];                 // photon ranges of the warps
     uint32_t t_hits[kTelSmemMax];
@@ -1110,7 +1111,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
     AxisFrame f_reg = ww.f_reg;
     (void)tid; (void)lane;
     for (uint32_t it = it0; it < it1; ++it, g += 32u, j += 32u) {
-        const bool active = g < hi;                  // the lanes past the warp's range idle in its last iterations
+        bool active = g < hi;                        // the lanes past the warp's range idle in its last iterations
         uint32_t cm = 0u;
         uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
         Rand4 r = {0u, 0u, 0u, 0u};
@@ -1124,6 +1125,9 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 pe = philox_emitter(P, emitter_segment(P, tile_first, e));
                 if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
             }
+            if (g + 1u == end && sm.odd[e]) active = false;      // the empty slot after an odd count
+        }
+        if (active) {
             if (kind == KIND_CHER_AXIS) {
                 const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
                 r = philox_photon(P, pe, j, 0u);                                              // a2
@@ -1211,6 +1215,116 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
     return rounds;
 }
 
+// The pair loop (tally kernels, and the sparse tiles of the photon-output kernels after round 0): a lane takes the two
+// adjacent slots g, g + 1 (g even) of the index space per trip, a warp 64.  Both photons belong to the same emitter
+// (the index space is padded to even counts), so one emitter state serves both; their Philox chains and geometry are
+// independent and interleave, which halves the dependent-issue stalls per photon, and the round keys / telescope
+// constants are fetched once for two photons.  Walks the warp's photons [base, hi), base even.
+template <int TELSRC, bool COPLANAR, int NT, int MODE, bool REFR>
+__device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const uint32_t base, const uint32_t hi,
+                                           const unsigned long long tile_first, uint32_t &n_up_out, uint32_t &q_head, uint32_t &q_count)
+{
+    constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
+    const int lane = threadIdx.x & 31;
+    if (base >= hi) return;
+    uint32_t g = base + 2u * (uint32_t)lane;
+    int e;
+    {
+        const uint32_t g0 = min(g, hi - 2u);
+        int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
+        while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
+        e = a;
+    }
+    uint32_t end = sm.prefix[e + 1], rend = end - sm.odd[e], j = g - sm.prefix[e], n_up = 0u;
+    int kind = sm.kind[e];
+    PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+    AxisFrame f_reg = load_axis_frame(sm, e);
+    for (uint32_t b0 = base; b0 < hi; b0 += 64u, g += 64u, j += 64u) {
+        const bool active = g < hi;
+        uint32_t cmA = 0u, cmB = 0u;
+        uint2 cellA = make_uint2(0xffffffffu, 0xffffffffu), cellB = cellA;
+        Rand4 rA = {0u, 0u, 0u, 0u}, rB = rA;
+        if (active) {
+            if (g >= end) {
+                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+                rend = end - sm.odd[e];
+                j = g - sm.prefix[e];
+                kind = sm.kind[e];
+                pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+                if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
+            }
+            const bool hasB = g + 1u < rend;                     // slot g + 1 is empty after an odd count
+            if (kind == KIND_CHER_AXIS) {
+                const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
+                rA = philox_photon(P, pe, j, 0u);                                                 // a2, twice
+                rB = philox_photon(P, pe, j + 1u, 0u);
+                // a3 / a4 as in walk(), for both photons
+                const float sdA = fmaf(one_two(rA.r0), f.negL, f.k0c), sdB = fmaf(one_two(rB.r0), f.negL, f.k0c);
+                float spA, cpA, spB, cpB;
+                __sincosf(fmaf(one_two(rA.r1), 6.2831853f, -9.42477760f), &spA, &cpA);
+                __sincosf(fmaf(one_two(rB.r1), 6.2831853f, -9.42477760f), &spB, &cpB);
+                const float vzA = fmaf(cpA, f.az, fmaf(spA, f.bz, f.cz)), vzB = fmaf(cpB, f.az, fmaf(spB, f.bz, f.cz));
+                const float rhoA = sdA * rcp_approx(vzA), rhoB = sdB * rcp_approx(vzB);
+                const float gxA = fmaf(rhoA, fmaf(cpA, f.px, spA * f.qx), f.gx), gyA = fmaf(rhoA, fmaf(cpA, f.py, spA * f.qy), f.gy);
+                const float gxB = fmaf(rhoB, fmaf(cpB, f.px, spB * f.qx), f.gx), gyB = fmaf(rhoB, fmaf(cpB, f.py, spB * f.qy), f.gy);
+                float vxA = 0.0f, vyA = 0.0f, vxB = 0.0f, vyB = 0.0f;
+                if (!COPLANAR) {
+                    const float *fr = &sm.frame[e * kFrameStride];
+                    vxA = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); vyA = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
+                    vxB = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); vyB = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
+                }
+                if (vzA < 0.0f) cmA = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxA, gyA, vxA, vyA, vzA, &cellA); else ++n_up;
+                if (hasB) {
+                    if (vzB < 0.0f) cmB = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cellB); else ++n_up;
+                }
+            } else {
+                const uint32_t tag = kind_tag(kind);
+                bool up;
+                rA = philox_photon(P, pe, j, tag);
+                cmA = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rA.r0, rA.r1, rA.r2, rA.r3, &cellA, &up);
+                if (up) ++n_up;
+                if (hasB) {
+                    rB = philox_photon(P, pe, j + 1u, tag);
+                    cmB = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rB.r0, rB.r1, rB.r2, rB.r3, &cellB, &up);
+                    if (up) ++n_up;
+                }
+            }
+        }
+        // candidates of slot A, then of slot B: wide test / on-the-spot evaluation / queue, as in walk()
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            uint32_t cm = s ? cmB : cmA;
+            const uint2 cell = s ? cellB : cellA;
+            const Rand4 r = s ? rB : rA;
+            const uint32_t jj = j + (uint32_t)s;
+            if constexpr (TELSRC == TEL_CONST) {
+                if (cm == kAllTelescopes) cm = (1u << NT) - 1u;
+            } else {
+                const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
+                if (wide) {
+                    wide_push<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, wide, e, jj);
+                    if (cm == kAllTelescopes) cm = 0u;
+                }
+            }
+            const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
+            if constexpr (MODE != MODE_TALLY) {
+                if (__popc(have) >= kDenseMin) {
+                    const bool has = cm != 0u;
+                    int k = 0;
+                    if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
+                    dense_eval<TELSRC, MODE>(P, sm, tile_first, e, jj, r.r0, r.r1, r.r2, r.r3, k, has);
+                }
+                if (__any_sync(0xffffffffu, cm != 0u))
+                    push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, jj, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+            } else {
+                if (have)
+                    push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, jj, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+            }
+        }
+    }
+    n_up_out += n_up;
+}
+
 template <int TELSRC, bool COPLANAR, int NT, int MODE>
 __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_constant__ KParams P)
 {
@@ -1267,9 +1381,14 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     }
     // ---- exclusive scan of nb over the tile, and of the cost-weighted counts that balance the warps: a photon of a
     // generic kind (fluorescence, near-horizontal Cherenkov tracks) costs about kGenericWeight axis-kind photons.
+    // Every emitter takes an even number of slots of the index space (one empty slot after an odd count), so that the
+    // pairs (g, g + 1), g even, which a lane of the pair loop takes, never straddle two emitters or two warps.
+    const uint32_t nbp = nb + (nb & 1u);
+    sm.odd[tid] = (uint8_t)(nb & 1u);
+    const uint32_t n_pad_w = (uint32_t)__popc(__ballot_sync(0xffffffffu, (nb & 1u) != 0u));
     const uint32_t weight = (nb != 0u && sm.kind[tid] != KIND_CHER_AXIS) ? (uint32_t)kGenericWeight : 1u;
-    const unsigned long long wnb = (unsigned long long)nb * weight;
-    uint32_t inc = nb;
+    const unsigned long long wnb = (unsigned long long)nbp * weight;
+    uint32_t inc = nbp;
     unsigned long long winc = wnb;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -1277,18 +1396,18 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         const unsigned long long wv = __shfl_up_sync(0xffffffffu, winc, o);
         if (lane >= o) { inc += v; winc += wv; }
     }
-    if (lane == 31) { sm.warp_sum[warp] = inc; sm.warp_wsum[warp] = winc; }
+    if (lane == 31) { sm.warp_sum[warp] = inc; sm.warp_wsum[warp] = winc; sm.warp_pad[warp] = n_pad_w; }
     __syncthreads();
-    uint32_t woff = 0, total = 0;
+    uint32_t woff = 0, total = 0, n_pad = 0;
     unsigned long long wwoff = 0, wtotal = 0;
 #pragma unroll
     for (int w = 0; w < kWarps; ++w) {
         const uint32_t v = sm.warp_sum[w];
         const unsigned long long wv = sm.warp_wsum[w];
         if (w < warp) { woff += v; wwoff += wv; }
-        total += v; wtotal += wv;
+        total += v; wtotal += wv; n_pad += sm.warp_pad[w];
     }
-    const uint32_t excl = woff + inc - nb;
+    const uint32_t excl = woff + inc - nbp;
     sm.prefix[tid] = excl;
     if (tid < 8) sm.prefix[kTile + tid] = (tid == 0) ? total : 0xffffffffu;
     // warp w walks photons [bound[w], bound[w + 1]): equal shares of the weighted index space.  The emitter that
@@ -1299,7 +1418,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
 #pragma unroll
         for (int w = 1; w < kWarps; ++w) {
             const unsigned long long x = wtotal / kWarps * (unsigned)w + wtotal % kWarps * (unsigned)w / kWarps;   // floor(wtotal w / 8)
-            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = excl + (uint32_t)((x - wexcl) / weight);
+            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & ~1u;
         }
     }
     __syncthreads();
@@ -1339,16 +1458,24 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
 #define C8_WALK(INL, FIRST, IT0, IT1, RND)                                                                                       \
     ((P.flags & kFlagRefract) ? walk<TELSRC, COPLANAR, NT, MODE, INL, true, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND) \
                               : walk<TELSRC, COPLANAR, NT, MODE, INL, false, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND))
+#define C8_WALK_PAIRS(BASE)                                                                                                    \
+    do {                                                                                                                       \
+        if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count); \
+        else walk_pairs<TELSRC, COPLANAR, NT, MODE, false>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count);     \
+    } while (0)
         if constexpr (OUT) {
-            // round 0 decides whether the tile is dense (stays in rounds mode, inline evaluation) or sparse
+            // round 0 decides whether the tile is dense (stays in rounds mode, inline evaluation) or sparse (pair loop)
             const uint32_t it1 = min((uint32_t)kRound, n_iter);
             rounds = C8_WALK(true, true, 0u, it1, true);
             if (rounds) C8_WALK(true, false, it1, n_iter, true);
-            else C8_WALK(false, false, it1, n_iter, false);
+            else C8_WALK_PAIRS(min(lo + 32u * it1, hi));
+        } else if constexpr (MODE == MODE_HIST) {
+            C8_WALK(true, false, 0u, n_iter, false);
         } else {
-            C8_WALK((MODE == MODE_HIST), false, 0u, n_iter, false);
+            C8_WALK_PAIRS(lo);
         }
 #undef C8_WALK
+#undef C8_WALK_PAIRS
         n_up = ww.n_up;
         uint32_t q_head = ww.q_head, q_count = ww.q_count;
         if constexpr (TELSRC != TEL_CONST) {
@@ -1370,7 +1497,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     if (lane == 0 && n_up) atomicAdd(&sm.n_upward, (unsigned long long)n_up);
     __syncthreads();
     if (tid == 0) {
-        if (total + sm.n_culled) atomicAdd(&P.counters[1], (unsigned long long)total + sm.n_culled);
+        if (total - n_pad + sm.n_culled) atomicAdd(&P.counters[1], (unsigned long long)(total - n_pad) + sm.n_culled);
         if (sm.n_upward) atomicAdd(&P.counters[2], sm.n_upward);
         if (sm.n_culled) atomicAdd(&P.counters[7], sm.n_culled);
     }
