@@ -1088,7 +1088,7 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
 // The lane's position in its warp's photon range and everything else the photon loop carries.
 struct WarpWalk {
     int e, kind;                       // current emitter and its kind
-    uint32_t end, g, j;                // end of the emitter in the tile's index space, photon index, index within the emitter
+    uint32_t end, g, j;                // real end of the emitter in the tile's index space, photon index, index within the emitter
     PhiloxEmitter pe;
     AxisFrame f_reg;
     uint32_t n_up, q_head, q_count;
@@ -1118,14 +1118,17 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
         Hit h;
         h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
         if (active) {
-            if (g >= end) {
-                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+            // `end` holds the emitter's real end (its padded end less the empty slot after an odd count)
+            if (g >= ((end + 1u) & ~1u)) {
+                uint32_t pend;
+                do { ++e; pend = sm.prefix[e + 1]; } while (g >= pend);
+                end = pend - sm.odd[e];
                 j = g - sm.prefix[e];
                 kind = sm.kind[e];
                 pe = philox_emitter(P, emitter_segment(P, tile_first, e));
                 if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
             }
-            if (g + 1u == end && sm.odd[e]) active = false;      // the empty slot after an odd count
+            if (g >= end) active = false;                        // the empty slot
         }
         if (active) {
             if (kind == KIND_CHER_AXIS) {
@@ -1446,7 +1449,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         // Loop-carried per lane: photon index g, emitter e with its end, index j within the emitter, kind, the hoisted
         // Philox words and (brute-force kernels only; the grid kernels are short of registers and reload it from
         // shared memory every iteration) the axis frame.
-        ww.end = sm.prefix[ww.e + 1];
+        ww.end = sm.prefix[ww.e + 1] - sm.odd[ww.e];
         ww.kind = sm.kind[ww.e];
         ww.pe = philox_emitter(P, emitter_segment(P, tile_first, ww.e));
         ww.f_reg = load_axis_frame(sm, ww.e);
@@ -1468,11 +1471,14 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             const uint32_t it1 = min((uint32_t)kRound, n_iter);
             rounds = C8_WALK(true, true, 0u, it1, true);
             if (rounds) C8_WALK(true, false, it1, n_iter, true);
-            else C8_WALK_PAIRS(min(lo + 32u * it1, hi));
+            else if constexpr (TELSRC == TEL_CONST) C8_WALK_PAIRS(min(lo + 32u * it1, hi));
+            else C8_WALK(false, false, it1, n_iter, false);
         } else if constexpr (MODE == MODE_HIST) {
             C8_WALK(true, false, 0u, n_iter, false);
+        } else if constexpr (TELSRC == TEL_CONST) {
+            C8_WALK_PAIRS(lo);            // the grid kernels are short of registers for two photons per lane
         } else {
-            C8_WALK_PAIRS(lo);
+            C8_WALK(false, false, 0u, n_iter, false);
         }
 #undef C8_WALK
 #undef C8_WALK_PAIRS
