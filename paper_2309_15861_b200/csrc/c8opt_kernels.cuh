@@ -1084,6 +1084,12 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
     return AxisFrame{A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, C.y, C.z};
 }
 
+// The kernels that run the pair loop (walk_pairs) pad every emitter to an even number of slots of the index space.
+template <int TELSRC, int MODE> __device__ __forceinline__ constexpr bool index_space_is_padded()
+{
+    return TELSRC == TEL_CONST && MODE != MODE_HIST;
+}
+
 // ------------------------------------------------------------------------------------
 // The lane's position in its warp's photon range and everything else the photon loop carries.
 struct WarpWalk {
@@ -1118,17 +1124,18 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
         Hit h;
         h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
         if (active) {
-            // `end` holds the emitter's real end (its padded end less the empty slot after an odd count)
-            if (g >= ((end + 1u) & ~1u)) {
+            // padded kernels: `end` holds the emitter's real end (its padded end less the empty slot after an odd count)
+            constexpr bool kPadded = index_space_is_padded<TELSRC, MODE>();
+            if (g >= (kPadded ? ((end + 1u) & ~1u) : end)) {
                 uint32_t pend;
                 do { ++e; pend = sm.prefix[e + 1]; } while (g >= pend);
-                end = pend - sm.odd[e];
+                end = kPadded ? pend - sm.odd[e] : pend;
                 j = g - sm.prefix[e];
                 kind = sm.kind[e];
                 pe = philox_emitter(P, emitter_segment(P, tile_first, e));
                 if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
             }
-            if (g >= end) active = false;                        // the empty slot
+            if (kPadded && g >= end) active = false;             // the empty slot
         }
         if (active) {
             if (kind == KIND_CHER_AXIS) {
@@ -1386,9 +1393,12 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     // generic kind (fluorescence, near-horizontal Cherenkov tracks) costs about kGenericWeight axis-kind photons.
     // Every emitter takes an even number of slots of the index space (one empty slot after an odd count), so that the
     // pairs (g, g + 1), g even, which a lane of the pair loop takes, never straddle two emitters or two warps.
-    const uint32_t nbp = nb + (nb & 1u);
-    sm.odd[tid] = (uint8_t)(nb & 1u);
-    const uint32_t n_pad_w = (uint32_t)__popc(__ballot_sync(0xffffffffu, (nb & 1u) != 0u));
+    // Only the kernels that run the pair loop pad (the brute-force tally and output kernels).
+    constexpr bool kPadded = index_space_is_padded<TELSRC, MODE>();
+    const uint32_t odd = kPadded ? (nb & 1u) : 0u;
+    const uint32_t nbp = nb + odd;
+    sm.odd[tid] = (uint8_t)odd;
+    const uint32_t n_pad_w = (uint32_t)__popc(__ballot_sync(0xffffffffu, odd != 0u));
     const uint32_t weight = (nb != 0u && sm.kind[tid] != KIND_CHER_AXIS) ? (uint32_t)kGenericWeight : 1u;
     const unsigned long long wnb = (unsigned long long)nbp * weight;
     uint32_t inc = nbp;
@@ -1421,7 +1431,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
 #pragma unroll
         for (int w = 1; w < kWarps; ++w) {
             const unsigned long long x = wtotal / kWarps * (unsigned)w + wtotal % kWarps * (unsigned)w / kWarps;   // floor(wtotal w / 8)
-            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & ~1u;
+            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & (kPadded ? ~1u : ~0u);
         }
     }
     __syncthreads();
