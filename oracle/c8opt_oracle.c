@@ -276,11 +276,24 @@ int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_seg
  * PAPER.md:61 (photon vector), PAPER.md:69-71 (matrix). */
 void orc_make_photon(const orc_frame *f, const orc_params *par, uint64_t S, uint32_t j, int tag, orc_photon *ph)
 {
-    uint32_t ctr[4] = { j, (uint32_t)S, (uint32_t)(S >> 32), (uint32_t)tag };
+    /* R20: fluorescence (tag 1) draws one Philox block per photon, counter (j, S_lo, S_hi, 1), words -> u1..u4.
+     * Cherenkov (tag 0) needs a position, an azimuth and a wavelength: one block, counter (j >> 1, S_lo, S_hi, 0),
+     * serves the two photons 2k and 2k + 1: words (a, b) = (r0, r1) for the even one, (r2, r3) for the odd one;
+     * u1 = U(a), u2 = U(b) from their upper 23 bits (R19), and the wavelength uniform from the 9 + 9 lower bits
+     * those leave over: u3 = ((a & 511) 2^9 + (b & 511) + 1/2) 2^-18. */
+    uint32_t ctr[4] = { tag == 0 ? (j >> 1) : j, (uint32_t)S, (uint32_t)(S >> 32), (uint32_t)tag };
     uint32_t key[2] = { (uint32_t)par->seed, (uint32_t)(par->seed >> 32) };
     uint32_t r[4];
     orc_philox4x32_10(ctr, key, r);
-    double u1 = orc_uniform(r[0]), u2 = orc_uniform(r[1]), u3 = orc_uniform(r[2]), u4 = orc_uniform(r[3]);
+    double u1, u2, u3, u4;
+    if (tag == 0) {
+        uint32_t a = r[2 * (j & 1u)], b = r[2 * (j & 1u) + 1];
+        u1 = orc_uniform(a); u2 = orc_uniform(b);
+        u3 = ((double)(((a & 511u) << 9) | (b & 511u)) + 0.5) / 262144.0;
+        u4 = 0.0;
+    } else {
+        u1 = orc_uniform(r[0]); u2 = orc_uniform(r[1]); u3 = orc_uniform(r[2]); u4 = orc_uniform(r[3]);
+    }
 
     double s = u1 * f->L;                                  /* "randomly distributed along the track" PAPER.md:35 */
     for (int i = 0; i < 3; ++i) ph->e[i] = f->p0[i] + s * f->d[i];

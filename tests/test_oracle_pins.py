@@ -532,8 +532,9 @@ def test_tiny_case_against_pure_python_restatement():
     S = (1 << 33) + 5
     hits = []
     for j in range(nb):
-        rr = philox([j, S & 0xFFFFFFFF, S >> 32, 0], [12345, 7])
-        u = [((x >> 9) + 0.5) / 2 ** 23 for x in rr]
+        rr = philox([j >> 1, S & 0xFFFFFFFF, S >> 32, 0], [12345, 7])       # R20: one block for the photons 2k, 2k + 1
+        a, b = rr[2 * (j & 1)], rr[2 * (j & 1) + 1]
+        u = [((a >> 9) + 0.5) / 2 ** 23, ((b >> 9) + 0.5) / 2 ** 23, ((((a & 511) << 9) | (b & 511)) + 0.5) / 2 ** 18]
         e = p0 + u[0] * L * d
         phi = 2 * math.pi * u[1]
         p = np.array([math.cos(phi) * math.sin(theta), math.sin(phi) * math.sin(theta), -math.cos(theta)])
@@ -757,3 +758,35 @@ def test_array_beaming_keeps_the_expected_tally():
         sig = math.sqrt(h_i) + math.sqrt(ra["tallies"]["sum_w"][k])
         assert abs(ri["tallies"]["sum_w"][k] - ra["tallies"]["sum_w"][k]) < 5.0 * sig, (k, ri["tallies"][k], ra["tallies"][k])
         assert h_i > 500
+
+
+def test_cherenkov_pair_shares_one_philox_block_R20():
+    """R20: photons 2k and 2k + 1 of a Cherenkov emitter take the two halves of one Philox block; position and azimuth
+    use the upper 23 bits of their two words, the wavelength the 18 lower bits left over.  Checked word by word on a
+    few photons, and statistically: the three uniforms are uniform and mutually uncorrelated."""
+    seg = one_segment(z0=9000.0, length=100.0, gamma=1e5)
+    par = W.default_params(seed=(3 << 32) | 99, bunch_size=0.05)
+    st, f = O.preamble(ATM1, par, seg[0], 0)
+    S = 1234567
+    inv1, inv2 = 1.0 / par["lam1"], 1.0 / par["lam2"]
+    for j in (0, 1, 2, 7, 1000, 1001):
+        ph = O.make_photon(f, par, S, j, 0)
+        r = O.philox4x32_10([j >> 1, S & 0xFFFFFFFF, S >> 32, 0], [99, 3])
+        a, b = int(r[2 * (j & 1)]), int(r[2 * (j & 1) + 1])
+        u1 = ((a >> 9) + 0.5) / 2 ** 23
+        u3 = ((((a & 511) << 9) | (b & 511)) + 0.5) / 2 ** 18
+        assert math.isclose(ph.e[2], 9000.0 - u1 * 100.0, rel_tol=0, abs_tol=1e-9)
+        assert math.isclose(ph.lam, 1.0 / (inv1 - u3 * (inv1 - inv2)), rel_tol=1e-13)
+    n = min(f.n_b, 40000) & ~1
+    u = np.empty((n, 3))
+    for j in range(n):
+        ph = O.make_photon(f, par, S, j, 0)
+        u[j, 0] = (9000.0 - ph.e[2]) / 100.0
+        u[j, 1] = (math.atan2(ph.v[1], ph.v[0]) / (2 * math.pi)) % 1.0
+        u[j, 2] = (inv1 - 1.0 / ph.lam) / (inv1 - inv2)
+    assert np.all(np.abs(u.mean(axis=0) - 0.5) < 5 * math.sqrt(1 / 12 / n))
+    assert np.all(np.abs(u.var(axis=0) - 1 / 12) < 0.005)
+    c = np.corrcoef(u.T)
+    assert abs(c[0, 1]) < 0.03 and abs(c[0, 2]) < 0.03 and abs(c[1, 2]) < 0.03
+    # neighbours 2k, 2k + 1 are as independent as any other two photons
+    assert abs(np.corrcoef(u[0::2, 0], u[1::2, 0])[0, 1]) < 0.03 and abs(np.corrcoef(u[0::2, 2], u[1::2, 2])[0, 1]) < 0.03
