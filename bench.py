@@ -28,9 +28,10 @@ import workloads as wl  # noqa: E402
 
 METRIC = "photons generated+propagated per second"
 UNIT = "photons/s"
-# algorithmic thread-instructions per photon: Philox 40 +
-# uniforms/generation/projection 40 + 8 per telescope tested + loop 10
-ALG_INSTR = {"c1": 98.0, "c2": 122.0, "c5": 122.0, "c3a": 110.0, "c3b": 120.0, "c4": 130.0}
+# algorithmic thread-instructions per photon: Philox 42 per block -- one block per
+# fluorescence photon, one per TWO Cherenkov photons (R20) -- + uniforms/generation/projection 40 + 6 per telescope
+# tested + loop 10
+ALG_INSTR = {"c1": 77.0, "c2": 101.0, "c5": 101.0, "c3a": 110.0, "c3b": 120.0, "c4": 110.0}
 RECORD_BYTES = 28.0
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the round's `ncu --set full` captures under
 # profiles/, per 10^6 segments (they scale with the segment count); None = not captured for this workload.
@@ -322,8 +323,8 @@ def main():
                     "traffic": None, "peak_source": peaks["source"], "bytes_per_photon": RECORD_BYTES}
     else:
         # ground histogram: no pre-tests (-24) but every downward bunch is carried to the plane: v_x, v_y, arrival time
-        # (exp), wavelength, radius, bin, three shared-memory atomics (+ ~90); DESIGN.md §7
-        instr = 190.0 if args.ground_hist else ALG_INSTR.get(args.workload, 122.0)
+        # (exp), wavelength, radius, bin, three shared-memory atomics (+ ~90): 101 - 24 + 92; DESIGN.md §7
+        instr = 169.0 if args.ground_hist else ALG_INSTR.get(args.workload, 101.0)
         peak = 148 * 4 * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12            # thread-instructions / s, issue-slot peak
         # culled bunches cost no photon-loop instructions: the roofline counts the propagated ones only
         roofline = {"bound": "alu", "achieved": instr * (photons_per_step - culled_per_step) / per_launch_s / 1e12, "peak": peak,

@@ -190,6 +190,18 @@ __device__ __forceinline__ float one_two(uint32_t r) { return __uint_as_float(0x
 constexpr float kOneMinus = 0.99999994f;   // 1 - 2^-24 = 0x3f7fffff
 __device__ __forceinline__ float uniform01(uint32_t r) { return one_two(r) - kOneMinus; }
 
+// R20: one Philox block, counter (j >> 1, S, tag 0), serves the Cherenkov photons 2k and 2k + 1: the even one takes the
+// words (r0, r1), the odd one (r2, r3).  Position and azimuth use the upper 23 bits of the photon's two words (R19); the
+// wavelength uniform is built from the 9 + 9 lower bits they leave over: ((a & 511) 2^9 + (b & 511) + 1/2) 2^-18.
+__device__ __forceinline__ Rand4 cherenkov_words(const Rand4 blk, uint32_t j)
+{
+    return (j & 1u) ? Rand4{blk.r2, blk.r3, 0u, 0u} : Rand4{blk.r0, blk.r1, 0u, 0u};
+}
+__device__ __forceinline__ float cherenkov_u3(uint32_t a, uint32_t b)
+{
+    return fmaf((float)(((a & 511u) << 9) | (b & 511u)), 3.814697265625e-06f, 1.9073486328125e-06f);   // exact: 18 bits
+}
+
 // ------------------------------------------------------------------------------------
 // shared-memory layout of one tile
 struct __align__(16) TileSmem {
@@ -508,7 +520,7 @@ __device__ __forceinline__ void sincospi_unit(float x, float *s, float *c)
 
 // A photon ready for the exact test: emission point e relative to (x_ref, y_ref, z_ref) or, for the
 // axis kind, the crossing (gx, gy) of the plane z_ref; unit direction v; s = distance along the track.
-struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s; uint32_t r2; int tag; bool axis; };
+struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s, u3; int tag; bool axis; };   // u3 = the wavelength uniform
 
 // a3 for a photon of emitter e, any kind, from its four random words.
 __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileSmem &sm, int e, const Rand4 r)
@@ -518,7 +530,8 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
     Photon ph;
     ph.tag = (kind == KIND_CHER_AXIS || kind == KIND_CHER_GEN) ? 0 : 1;
     ph.axis = (kind == KIND_CHER_AXIS);
-    ph.r2 = r.r2;
+    // Cherenkov kinds: r holds the photon's two words (cherenkov_words); fluorescence: the four words of its own block
+    ph.u3 = (ph.tag == 0) ? cherenkov_u3(r.r0, r.r1) : uniform01(r.r2);
     if (kind == KIND_CHER_AXIS) {
         const float w1 = one_two(r.r0);
         const float sd = fmaf(w1, fr[F_NEGL], fr[F_K0C]);                            // K0 - u1 L
@@ -565,7 +578,9 @@ __device__ __forceinline__ uint32_t kind_tag(int kind) { return (kind == KIND_CH
 // a2 + a3 for photon j of emitter e, any kind (used by the queue drain, the wide test and the generic kinds' hot path).
 __device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S)
 {
-    return photon_from_rand(P, sm, e, philox4x32_10(P, j, (uint32_t)S, (uint32_t)(S >> 32), kind_tag(sm.kind[e])));
+    const uint32_t tag = kind_tag(sm.kind[e]);
+    const Rand4 blk = philox4x32_10(P, tag ? j : (j >> 1), (uint32_t)S, (uint32_t)(S >> 32), tag);
+    return photon_from_rand(P, sm, e, tag ? blk : cherenkov_words(blk, j));
 }
 
 // One accepted (photon, telescope) pair, ready for the tally / record.
@@ -655,7 +670,7 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     const float excess = P.kappa_m * (telT_at<TELSRC>(P, k) - Te) * fabsf(rv);
     h.t = fmaf(ph.s, fr[F_IBC], fr[F_T0]) + (s_pl + excess) * (1.0f / 0.299792458f);
     // R4: wavelength
-    const float u3 = uniform01(ph.r2);
+    const float u3 = ph.u3;
     h.lam = (ph.tag == 0) ? rcp_refined(fmaf(-u3, P.dinv_lam, P.inv_lam1)) : fmaf(u3, P.fl_dlam, P.fl_lam1);
     // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
     h.w = fr[F_W0];
@@ -1140,7 +1155,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
         if (active) {
             if (kind == KIND_CHER_AXIS) {
                 const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
-                r = philox_photon(P, pe, j, 0u);                                              // a2
+                r = cherenkov_words(philox_photon(P, pe, j >> 1, 0u), j);                      // a2 (R20)
                 // a3: remaining axis path length to the plane, azimuth (PAPER.md:61 c_rng, R5)
                 const float sd = fmaf(one_two(r.r0), f.negL, f.k0c);                          // K0 - u1 L
                 float sp, cp;
@@ -1162,7 +1177,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                         if (INLINE && cm != 0u && cm != kAllTelescopes) {
                             const float *fr = &sm.frame[e * kFrameStride];
                             Photon ph;
-                            ph.axis = true; ph.tag = 0; ph.r2 = r.r2;
+                            ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(r.r0, r.r1);
                             ph.vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
                             ph.vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
                             ph.vz = vz; ph.gx = gx; ph.gy = gy;
@@ -1179,7 +1194,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 }
             } else {
                 // the same hoisted Philox as the axis kind (the process tag is counter word 3)
-                r = philox_photon(P, pe, j, kind_tag(kind));
+                r = kind_tag(kind) ? philox_photon(P, pe, j, 1u) : cherenkov_words(philox_photon(P, pe, j >> 1, 0u), j);
                 bool up;
                 cm = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, r.r0, r.r1, r.r2, r.r3, &cell, &up);
                 if (up) ++n_up;
@@ -1266,8 +1281,9 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
             const bool hasB = g + 1u < rend;                     // slot g + 1 is empty after an odd count
             if (kind == KIND_CHER_AXIS) {
                 const AxisFrame f = kFrameInRegs ? f_reg : load_axis_frame(sm, e);
-                rA = philox_photon(P, pe, j, 0u);                                                 // a2, twice
-                rB = philox_photon(P, pe, j + 1u, 0u);
+                const Rand4 blk = philox_photon(P, pe, j >> 1, 0u);                               // a2: one block, two photons (R20; j is even)
+                rA = Rand4{blk.r0, blk.r1, 0u, 0u};
+                rB = Rand4{blk.r2, blk.r3, 0u, 0u};
                 // a3 / a4 as in walk(), for both photons
                 const float sdA = fmaf(one_two(rA.r0), f.negL, f.k0c), sdB = fmaf(one_two(rB.r0), f.negL, f.k0c);
                 float spA, cpA, spB, cpB;
@@ -1290,11 +1306,12 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
             } else {
                 const uint32_t tag = kind_tag(kind);
                 bool up;
-                rA = philox_photon(P, pe, j, tag);
+                const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
+                rA = tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u};
                 cmA = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rA.r0, rA.r1, rA.r2, rA.r3, &cellA, &up);
                 if (up) ++n_up;
                 if (hasB) {
-                    rB = philox_photon(P, pe, j + 1u, tag);
+                    rB = tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u};
                     cmB = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rB.r0, rB.r1, rB.r2, rB.r3, &cellB, &up);
                     if (up) ++n_up;
                 }
