@@ -1102,7 +1102,7 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
 // The kernels that run the pair loop (walk_pairs) pad every emitter to an even number of slots of the index space.
 template <int TELSRC, int MODE> __device__ __forceinline__ constexpr bool index_space_is_padded()
 {
-    return TELSRC == TEL_CONST && MODE != MODE_HIST;
+    return MODE == MODE_TALLY || (TELSRC == TEL_CONST && MODE != MODE_HIST);
 }
 
 // ------------------------------------------------------------------------------------
@@ -1502,10 +1502,8 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             else C8_WALK(false, false, it1, n_iter, false);
         } else if constexpr (MODE == MODE_HIST) {
             C8_WALK(true, false, 0u, n_iter, false);
-        } else if constexpr (TELSRC == TEL_CONST) {
-            C8_WALK_PAIRS(lo);            // the grid kernels are short of registers for two photons per lane
         } else {
-            C8_WALK(false, false, 0u, n_iter, false);
+            C8_WALK_PAIRS(lo);
         }
 #undef C8_WALK
 #undef C8_WALK_PAIRS
