@@ -451,3 +451,22 @@ def test_fluorescence_beamed_at_the_array(c8):
     _report("beam-array-c4", rep)
     fl = rep  # both processes: compare() has already checked the per-process counts
     assert rep["matched"] > 20000
+
+
+@pytest.mark.parametrize("name,n,mode_out", [("c2", 40_000, True), ("c4", 30_000, True), ("c5g", 2_000, True), ("c4", 30_000, False)])
+def test_runs_are_repeatable(c8, name, n, mode_out):
+    """Three runs of the same input: identical hit counts and (after sorting by id) bit-identical records -- the queues,
+    staging areas and round flushes leave no room for a race to change a result; only the fp64 sums may differ in
+    their last bits (atomic order)."""
+    import parity_util as pu
+    cfg = wl.make_config(name, n_segments=n)
+    mode = c8.MODE_OUTPUT if mode_out else c8.MODE_TALLY
+    runs = [pu.gpu_run(cfg, mode, capacity_per_tel=1 << 20) for _ in range(3)]
+    for other in runs[1:]:
+        assert np.array_equal(runs[0]["tallies"]["hits"], other["tallies"]["hits"])
+        assert np.array_equal(runs[0]["counts"], other["counts"])
+        assert runs[0]["counters"] == other["counters"]
+        assert np.allclose(runs[0]["tallies"]["sum_w"], other["tallies"]["sum_w"], rtol=1e-12)
+        if mode_out:
+            for f in ("id", "tel", "x", "y", "cx", "cy", "t", "lam", "w"):
+                assert np.array_equal(runs[0]["records"][f], other["records"][f])
