@@ -1102,7 +1102,7 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
 // The kernels that run the pair loop (walk_pairs) pad every emitter to an even number of slots of the index space.
 template <int TELSRC, int MODE> __device__ __forceinline__ constexpr bool index_space_is_padded()
 {
-    return MODE == MODE_TALLY || (TELSRC == TEL_CONST && MODE != MODE_HIST);
+    return true;
 }
 
 // ------------------------------------------------------------------------------------
@@ -1245,7 +1245,7 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
 // (the index space is padded to even counts), so one emitter state serves both; their Philox chains and geometry are
 // independent and interleave, which halves the dependent-issue stalls per photon, and the round keys / telescope
 // constants are fetched once for two photons.  Walks the warp's photons [base, hi), base even.
-template <int TELSRC, bool COPLANAR, int NT, int MODE, bool REFR>
+template <int TELSRC, bool COPLANAR, int NT, int MODE, bool REFR, bool INLINE>
 __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const uint32_t base, const uint32_t hi,
                                            const unsigned long long tile_first, uint32_t &n_up_out, uint32_t &q_head, uint32_t &q_count)
 {
@@ -1269,6 +1269,9 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
         uint32_t cmA = 0u, cmB = 0u;
         uint2 cellA = make_uint2(0xffffffffu, 0xffffffffu), cellB = cellA;
         Rand4 rA = {0u, 0u, 0u, 0u}, rB = rA;
+        Hit hA, hB;                                   // INLINE (ground histogram): both photons evaluated on the spot
+        hA.ok = false; hA.k = 0; hA.x = hA.y = hA.vx = hA.vy = hA.t = hA.lam = hA.w = 0.0f;
+        hB = hA;
         if (active) {
             if (g >= end) {
                 do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
@@ -1303,6 +1306,29 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                 if (hasB) {
                     if (vzB < 0.0f) cmB = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cellB); else ++n_up;
                 }
+                if constexpr (INLINE) {
+                    const float *fr = &sm.frame[e * kFrameStride];
+                    if (cmA != 0u && cmA != kAllTelescopes) {
+                        Photon ph;
+                        ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(rA.r0, rA.r1);
+                        ph.vx = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); ph.vy = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
+                        ph.vz = vzA; ph.gx = gxA; ph.gy = gyA; ph.s = (one_two(rA.r0) - kOneMinus) * fr[F_LEN]; ph.ez = -sdA * fr[F_DZ];
+                        ph.ex = ph.ey = 0.0f;
+                        const int k = (int)slot_telescope<TELSRC>(cellA, __ffs(cmA) - 1);
+                        cmA &= cmA - 1u;
+                        hA = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+                    }
+                    if (cmB != 0u && cmB != kAllTelescopes) {
+                        Photon ph;
+                        ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(rB.r0, rB.r1);
+                        ph.vx = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); ph.vy = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
+                        ph.vz = vzB; ph.gx = gxB; ph.gy = gyB; ph.s = (one_two(rB.r0) - kOneMinus) * fr[F_LEN]; ph.ez = -sdB * fr[F_DZ];
+                        ph.ex = ph.ey = 0.0f;
+                        const int k = (int)slot_telescope<TELSRC>(cellB, __ffs(cmB) - 1);
+                        cmB &= cmB - 1u;
+                        hB = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+                    }
+                }
             } else {
                 const uint32_t tag = kind_tag(kind);
                 bool up;
@@ -1316,6 +1342,11 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                     if (up) ++n_up;
                 }
             }
+        }
+        if constexpr (INLINE) {
+            const unsigned long long id0 = (emitter_segment(P, tile_first, e) << 25) | (unsigned long long)j;
+            commit_hits<MODE>(P, sm, hA, id0);
+            commit_hits<MODE>(P, sm, hB, id0 + 1ull);
         }
         // candidates of slot A, then of slot B: wide test / on-the-spot evaluation / queue, as in walk()
 #pragma unroll
@@ -1490,8 +1521,8 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
                               : walk<TELSRC, COPLANAR, NT, MODE, INL, false, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND))
 #define C8_WALK_PAIRS(BASE)                                                                                                    \
     do {                                                                                                                       \
-        if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count); \
-        else walk_pairs<TELSRC, COPLANAR, NT, MODE, false>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count);     \
+        if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true, MODE == MODE_HIST>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count); \
+        else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count);     \
     } while (0)
         if constexpr (OUT) {
             // round 0 decides whether the tile is dense (stays in rounds mode, inline evaluation) or sparse (pair loop)
@@ -1500,10 +1531,8 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
             if (rounds) C8_WALK(true, false, it1, n_iter, true);
             else if constexpr (TELSRC == TEL_CONST) C8_WALK_PAIRS(min(lo + 32u * it1, hi));
             else C8_WALK(false, false, it1, n_iter, false);
-        } else if constexpr (MODE == MODE_HIST) {
-            C8_WALK(true, false, 0u, n_iter, false);
         } else {
-            C8_WALK_PAIRS(lo);
+            C8_WALK_PAIRS(lo);            // tally: candidates to the queue; ground histogram: both photons evaluated inline
         }
 #undef C8_WALK
 #undef C8_WALK_PAIRS
