@@ -95,6 +95,8 @@ struct KParams {
     uint32_t rk0[10], rk1[10];     // Philox round keys: key + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t processes, n_procs;
     int tile_segs;                 // segments per tile, <= kTile / n_procs
+    int split_part;                // 0: this launch runs every requested process; 1 / 2: first / second launch of a
+                                   // two-process request (Cherenkov, then fluorescence): see launch() in c8opt.cu
     double c_ft;                   // 2 pi alpha (1/lam1 - 1/lam2) [1/m]  (R2)
     double bunch_size, fl_yield;
     float inv_lam1, dinv_lam;      // Cherenkov: 1/lam = inv_lam1 - u3 * dinv_lam (R4)
@@ -1427,7 +1429,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         if (bad) sm.invalid[seg_local] = 1;
         if (P.counts) {
             P.counts[seg_i * 2ull + (unsigned)tag] = nb;
-            if (P.n_procs == 1) P.counts[seg_i * 2ull + (unsigned)(tag ^ 1)] = 0u;
+            if (P.n_procs == 1 && P.split_part == 0) P.counts[seg_i * 2ull + (unsigned)(tag ^ 1)] = 0u;
         }
         if (culled) { n_culled = nb; nb = 0u; }           // generated, but provably no hit: not propagated
     }
@@ -1565,7 +1567,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
         // invalid segments of this tile (each counted once)
         uint32_t nbad = (tid < kTile / (int)P.n_procs) ? sm.invalid[tid] : 0u;
         nbad = __reduce_add_sync(0xffffffffu, nbad);
-        if (lane == 0 && nbad) atomicAdd(&P.counters[6], (unsigned long long)nbad);
+        if (lane == 0 && nbad && P.split_part != 2) atomicAdd(&P.counters[6], (unsigned long long)nbad);   // once per segment
     }
     if constexpr (MODE == MODE_HIST) {
         // the tile's histogram into the global one (the barrier above ordered the warps' updates); bin hist_bins = overflow
