@@ -37,7 +37,7 @@ RECORD_BYTES = 28.0
 # profiles/, per 10^6 segments (they scale with the segment count); None = not captured for this workload.
 NCU_TRAFFIC_PER_1E6_SEGMENTS = {
     ("c2", "tally"): 48.07e6,        # profiles/ncu_c2_tally_r01.md: the 48 MB segment table once
-    ("c4", "tally"): 49.97e6,        # profiles/ncu_c4_tally_r01.md (48.37 MB read + 1.6 MB of spills written)
+    ("c4", "tally"): 99.13e6,        # profiles/ncu_c4_tally_r01.md: two passes over the segment table + 2.4 MB of spills
     ("c5g", "output"): 5.084e9,      # profiles/ncu_c5g_output_r01.md: 5.035 GB written + 49.7 MB read
     ("c2", "hist"): 48.11e6,         # profiles/ncu_c2_groundhist_r01.md
 }
