@@ -470,3 +470,35 @@ def test_runs_are_repeatable(c8, name, n, mode_out):
         if mode_out:
             for f in ("id", "tel", "x", "y", "cx", "cy", "t", "lam", "w"):
                 assert np.array_equal(runs[0]["records"][f], other["records"][f])
+
+
+def test_config5_full_size_one_percent_block(c8):
+    """configs[4] at its full size (10^7 segments, photon-output mode, the launch bench.py times): the records of a
+    contiguous 1 % block of segments, found by their ids among the 6.7e6 records of the run, against the oracle run on
+    that block alone (its random streams are keyed by the global segment ids)."""
+    import parity_util as pu
+    cfg = wl.make_config("c5")
+    lo, n_blk = 5_000_000, 100_000
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=2_500_000)
+    assert g["counters"]["dropped"] == 0 and g["counters"]["records"] == g["counters"]["hits"] > 6_000_000
+    import oracle
+    o = oracle.run(cfg["atmosphere"], cfg["telescopes"], cfg["segments"][lo:lo + n_blk], cfg["params"], first_id=lo,
+                   want_counts=True, record_capacity=1 << 20, threads=pu.n_threads())
+    assert np.array_equal(g["counts"][lo:lo + n_blk], o["counts"])                      # (a) bit-exact counts
+    gr = g["records"]
+    seg_of = gr["id"] >> 25
+    gb = gr[(seg_of >= lo) & (seg_of < lo + n_blk)]
+    orr = o["records"]
+    orr = orr[np.lexsort((orr["tel"], orr["id"]))]
+    gk = gb["id"].astype(np.uint64) * 16 + gb["tel"].astype(np.uint64)
+    ok = orr["id"].astype(np.uint64) * 16 + orr["tel"].astype(np.uint64)
+    common, ia, ib = np.intersect1d(gk, ok, return_indices=True)
+    assert len(gk) + len(ok) - 2 * len(common) <= 3 and len(common) > 50_000             # (b) at most a few edge flips
+    a, b = gb[ia], orr[ib]
+    assert np.max(np.abs(a["x"] - b["x"])) <= pu.TOL_XY_M and np.max(np.abs(a["y"] - b["y"])) <= pu.TOL_XY_M      # (c)
+    assert np.max(np.abs(a["cx"] - b["cx"])) <= 1e-5 and np.max(np.abs(a["cy"] - b["cy"])) <= 1e-5
+    assert np.max(np.abs(a["t"] - b["t"])) <= pu.TOL_T_NS                                                        # (d)
+    assert np.max(np.abs(a["lam"] - b["lam"]) / b["lam"]) <= pu.TOL_LAM_REL
+    print(f"[parity c5-full-1pct] records_total={len(gr)} block_gpu={len(gk)} block_oracle={len(ok)} matched={len(common)} "
+          f"max_dxy_m={max(np.max(np.abs(a['x'] - b['x'])), np.max(np.abs(a['y'] - b['y']))):.3e} "
+          f"max_dt_ns={np.max(np.abs(a['t'] - b['t'])):.3e}")
