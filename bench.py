@@ -187,6 +187,8 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the photon path has no CPU fallback")
+    from paper_2309_15861_b200.build import build as build_cuda
+    build_cuda()      # in-tree nvcc build if libc8opt.so is missing or older than its sources (atomic replace)
     c8.lib()
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)

@@ -16,6 +16,8 @@ pytestmark = pytest.mark.gpu
 def c8():
     import torch
     assert torch.cuda.is_available(), "these tests need the B200"
+    from paper_2309_15861_b200.build import build
+    build()           # compiles libc8opt.so in-tree if it is missing or older than its sources (nvcc, sm_100a)
     import paper_2309_15861_b200 as c8
     c8.lib()          # fail loudly if the CUDA extension is missing
     return c8
