@@ -23,12 +23,13 @@ def shard_first_id(rank: int, n_per_rank: int) -> int:
     return int(rank) * int(n_per_rank)
 
 
-def pack_results(tallies: np.ndarray, counters: dict) -> np.ndarray:
-    """Flatten (tallies, counters) into one float64/uint64-safe vector pair for a sum all-reduce.
-    Returns an int64 vector (hits, counters) and a float64 vector (sum_w, sum_wt)."""
+def pack_results(tallies: np.ndarray, counters: dict):
+    """Flatten (tallies, counters) into two vectors for a sum all-reduce: an int64 vector (per-telescope hits, then
+    the eight counters in the order of paper_2309_15861_b200.COUNTER_NAMES, the keys Context.read_tallies() returns)
+    and a float64 vector (sum_w, sum_wt)."""
+    from . import COUNTER_NAMES
     ints = np.concatenate([tallies["hits"].astype(np.int64),
-                           np.array([counters[k] for k in ("segments", "generated", "upward", "hits", "records",
-                                                           "dropped", "invalid", "unused")], dtype=np.int64)])
+                           np.array([counters[k] for k in COUNTER_NAMES], dtype=np.int64)])
     flts = np.concatenate([tallies["sum_w"], tallies["sum_wt"]]).astype(np.float64)
     return ints, flts
 

@@ -18,13 +18,16 @@ def _free_port():
 def _worker(rank, world, port, q):
     import torch.distributed as dist
     import oracle
+    import paper_2309_15861_b200 as c8
     from paper_2309_15861_b200.sharding import all_reduce_results, shard_range
     os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     cfg = wl.make_config("c2", n_segments=3001)
     lo, hi = shard_range(len(cfg["segments"]), rank, world)
     r = oracle.run(cfg["atmosphere"], cfg["telescopes"], cfg["segments"][lo:hi], cfg["params"], first_id=lo)
-    counters = dict(zip(oracle.COUNTER_NAMES, (int(v) for v in r["counters"])))
+    # keyed exactly like Context.read_tallies() of the product (the oracle only supplies the per-shard numbers)
+    counters = dict(zip(c8.COUNTER_NAMES, (int(v) for v in r["counters"])))
+    counters["culled"] = 5 + rank                      # a value the reduction must carry
     t, c = all_reduce_results(r["tallies"], counters)
     if rank == 0:
         q.put((t, c))
@@ -50,6 +53,19 @@ def test_two_rank_partition_matches_single_run():
     assert np.allclose(t["sum_w"], full["tallies"]["sum_w"], rtol=1e-12)
     assert np.allclose(t["sum_wt"], full["tallies"]["sum_wt"], rtol=1e-9)
     assert c["generated"] == int(full["counters"][1]) and c["segments"] == 3001
+    assert c["culled"] == 5 + 6 and set(c) == set(__import__("paper_2309_15861_b200").COUNTER_NAMES)
+
+
+def test_pack_unpack_round_trip_with_the_product_counter_names():
+    """pack_results / unpack_results take and return the dict Context.read_tallies() returns ('unused')."""
+    import paper_2309_15861_b200 as c8
+    from paper_2309_15861_b200.sharding import pack_results, unpack_results
+    t = np.zeros(3, dtype=c8.TALLY_DTYPE)
+    t["hits"], t["sum_w"], t["sum_wt"] = [1, 2, 3], [0.5, 1.5, 2.5], [-1.0, 0.0, 7.0]
+    counters = {name: 10 + i for i, name in enumerate(c8.COUNTER_NAMES)}
+    ints, flts = pack_results(t, counters)
+    t2, c2 = unpack_results(ints, flts, 3)
+    assert c2 == counters and t2.tobytes() == t.tobytes()
 
 
 def test_shard_ranges_cover_exactly():
