@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -104,9 +105,13 @@ double host_refractivity(const c8opt_ctx *c, double h)
     return c->eta0 * (c->layer[i].b / c->layer[i].c * std::exp(-h / c->layer[i].c) / 100.0) / c->rho0;
 }
 
-size_t smem_bytes(int mode)
+// dynamic shared memory of a launch: the tile, plus the staging buffers of the brute-force photon-output kernels
+// (the id staging only when the caller wants ids), or the private histogram
+size_t smem_bytes(int mode, bool staging = true, bool ids = true)
 {
-    return sizeof(c8::TileSmem) + (mode == c8::MODE_OUT ? sizeof(c8::OutSmem) : mode == c8::MODE_HIST ? sizeof(c8::HistSmem) : 0);
+    if (mode == c8::MODE_HIST) return sizeof(c8::TileSmem) + sizeof(c8::HistSmem);
+    if (mode != c8::MODE_OUT || !staging) return sizeof(c8::TileSmem);
+    return sizeof(c8::TileSmem) + (ids ? sizeof(c8::OutSmem) : offsetof(c8::OutSmem, ids));
 }
 
 typedef void (*kernel_t)(const c8::KParams);
@@ -239,7 +244,7 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     for (int i = 0; i < ctx->n_layers; ++i) {
         P.layer[i] = c8::LayerD{ctx->layer[i].h_lo, ctx->layer[i].a, ctx->layer[i].b, ctx->layer[i].c};
         P.layerf[i] = c8::LayerF{(float)ctx->layer[i].h_lo, (float)ctx->layer[i].a, (float)ctx->layer[i].b,
-                                 (float)(1.0 / ctx->layer[i].c)};
+                                 (float)(1.4426950408889634 / ctx->layer[i].c)};
     }
     P.eta0 = ctx->eta0; P.rho0 = ctx->rho0;
     P.kappa_m = (float)(0.01 * ctx->eta0 / ctx->rho0);
@@ -328,7 +333,7 @@ int launch_one(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, unsigned long long
     } else {
         const bool out = P.records != nullptr;
         kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out);
-        k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY), st>>>(P);
+        k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, ctx->tel_src == c8::TEL_CONST, P.ids != nullptr), st>>>(P);
     }
     C8_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;

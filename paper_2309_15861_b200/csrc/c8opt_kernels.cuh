@@ -34,9 +34,10 @@ constexpr int TEL_GRID = 1;           // candidate lookup in the ground-plane gr
 constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global memory (grid not buildable)
 constexpr int kMaxLayers = 8;
 constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
-constexpr int kRound = 2;             // photon output: warp iterations per round (one cursor bump per tile and round)
-constexpr int kStageRecs = kRound * 32;           // records a warp can stage per round
-constexpr int kDenseTile = 64;        // records a tile must stage in its first round (512 photons) to stay in the rounds mode
+constexpr int kBlockRecs = 64;        // photon output, dense tiles: records a warp stages per trip of the dense loop (2 per lane)
+constexpr int kStageBufs = 3;         // staging buffers per warp (a block waits two trips for its slots, see walk_dense)
+constexpr int kRoundSlots = 4;        // reservation rounds in flight per tile (power of two > the two a warp may lag)
+constexpr int kProbeDense = 32;       // candidates among the kTile sampled photons from which a tile takes the dense loop (12.5 %)
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
 constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
 constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
@@ -45,6 +46,7 @@ constexpr uint32_t kFlagRefract = 2u; // == C8OPT_FLAG_REFRACT
 constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
 constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
+constexpr int kOutCtasPerSm = 2;       // resident CTAs per SM the brute-force photon-output kernels are compiled for (register budget)
 
 constexpr int KIND_CHER_AXIS = 0;     // Cherenkov, axis-relative projection (|d_z| large)
 constexpr int KIND_FL_ISO = 1;        // fluorescence, isotropic
@@ -52,7 +54,7 @@ constexpr int KIND_CONE = 2;          // fluorescence beamed (random polar angle
 constexpr int KIND_CHER_GEN = 3;      // Cherenkov, generic projection (near-horizontal / upward track)
 
 struct LayerD { double h_lo, a, b, c; };
-struct LayerF { float h_lo, a, b, inv_c; };
+struct LayerF { float h_lo, a, b, k2; };      // T(h) = a + b 2^(-h k2), k2 = log2(e) / c
 
 struct GridLevel { int nx, ny, base; float ox, oy, inv_cell, vzmin; };   // cell index = floor(x * inv_cell + ox)
 constexpr int kGridLevels = 2;        // |v_z| >= 0.5 and >= 0.1; slot kGridLevels holds level 0 with the refraction slack (R27)
@@ -227,16 +229,22 @@ struct __align__(16) TileSmem {
     int acc_k[kTile];
 };
 
-// Photon-output kernels only (follows TileSmem in dynamic shared memory).  Records are staged per warp and leave the
-// tile once per round: the cursor of a telescope is bumped once per (tile, round, run of warps on that telescope)
-// instead of once per warp iteration, because same-address atomics serialise in L2 (~1 per clock).
+// Photon-output kernels only (follows TileSmem in dynamic shared memory).  Dense tiles (most photons hit one telescope:
+// c5g) stage the records of a trip per warp and reserve their slots once per (tile, trip): same-address atomics
+// serialise in L2 (~1 per clock), so the cursor of a telescope must not be bumped once per warp and trip.  The
+// reservation is a split arrive / wait without a block barrier (walk_dense): a warp adds its record count to agg[r & 3]
+// (bits 8.. = records so far = the warp's offset in the round, bits 0..7 = warps arrived); the last of the kWarps
+// arrivals bumps the cursor by the round's total and publishes the base in rbase[r & 3], rflag[r & 3] = r + 1; a warp
+// picks the base up two trips later and sends its block out with one bulk copy (shared -> global, TMA).
 struct OutSmem {
-    __align__(16) float stage[kWarps][kStageRecs * kRecWords];
-    unsigned long long ids[kWarps][kStageRecs];
-    unsigned long long wbase[kWarps];            // first record slot of warp w's run in its telescope's region
-    int wk[kWarps];                              // telescope of the records warp w has staged this round
-    uint32_t wn[kWarps];                         // how many
-    int rounds;                                  // 1 while the tile runs in rounds (enough staged records in round 0)
+    unsigned long long rbase[kRoundSlots];       // first record slot of round r in the dense telescope's region
+    uint32_t agg[kRoundSlots];                   // see above
+    uint32_t rflag[kRoundSlots];
+    uint32_t probe[kTelConstMax];                // candidates per telescope among the sampled photons (probe_density)
+    // kStageBufs blocks per warp: block r is staged in buffer r % 3 while the bulk copies of blocks r - 1, r - 2 may
+    // still be reading theirs
+    __align__(16) float stage[kWarps][kStageBufs][kBlockRecs * kRecWords];
+    unsigned long long ids[kWarps][kStageBufs][kBlockRecs];     // last: not allocated when the caller wants no ids
 };
 
 __device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
@@ -522,7 +530,7 @@ __device__ __forceinline__ void sincospi_unit(float x, float *s, float *c)
 
 // A photon ready for the exact test: emission point e relative to (x_ref, y_ref, z_ref) or, for the
 // axis kind, the crossing (gx, gy) of the plane z_ref; unit direction v; s = distance along the track.
-struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s, u3; int tag; bool axis; };   // u3 = the wavelength uniform
+struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s, u3, rva; int tag; bool axis; };   // u3 = the wavelength uniform; rva = MUFU.RCP(v_z), axis kind
 
 // a3 for a photon of emitter e, any kind, from its four random words.
 __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileSmem &sm, int e, const Rand4 r)
@@ -542,7 +550,8 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
         ph.vz = fmaf(cp, fr[F_AZ], fmaf(sp, fr[F_BZ], fr[F_CZ]));
         ph.vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
         ph.vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
-        const float rho = sd * rcp_approx(ph.vz);
+        ph.rva = rcp_approx(ph.vz);
+        const float rho = sd * ph.rva;
         ph.gx = fmaf(rho, fmaf(cp, fr[F_PX], sp * fr[F_QX]), fr[F_GX]);
         ph.gy = fmaf(rho, fmaf(cp, fr[F_PY], sp * fr[F_QY]), fr[F_GY]);
         ph.s = (w1 - kOneMinus) * fr[F_LEN];
@@ -571,7 +580,7 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
         ph.vy = fmaf(sth, fmaf(cp, fr[F_A0 + 1], sp * fr[F_B0 + 1]), cth * fr[F_C0 + 1]);
         ph.vz = fmaf(sth, fmaf(cp, fr[F_A0 + 2], sp * fr[F_B0 + 2]), cth * fr[F_C0 + 2]);
     }
-    ph.gx = ph.gy = 0.0f;
+    ph.gx = ph.gy = ph.rva = 0.0f;
     return ph;
 }
 
@@ -588,16 +597,72 @@ __device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &
 // One accepted (photon, telescope) pair, ready for the tally / record.
 struct Hit { float x, y, vx, vy, t, lam, w; int k; bool ok; };
 
-// a4 exact test (R10) + arrival time, wavelength, weight for photon `ph` against telescope k.
-template <int TELSRC>
+// 2^x, MUFU.EX2 alone (flush-to-zero: the arguments here are -h / c log2(e), far from the denormal range)
+__device__ __forceinline__ float ex2_approx(float x)
+{
+    float r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// The pieces of the exact evaluation that evaluate_pair and the dense loop's fast path share.  Every multiply-add is
+// an explicit fmaf, so that both callers compile to the same arithmetic and a photon's record does not depend on the
+// path that produced it.
+//
+// Index of the atmosphere layer at altitude habs: from the frame when the whole segment lies in one layer, else looked
+// up (unused layers carry h_lo = +inf, so the count is the index).
+__device__ __forceinline__ int emission_layer(const KParams &P, int li_frame, float habs)
+{
+    int li = li_frame;
+    if (li < 0) {
+        li = 0;
+#pragma unroll
+        for (int i = 1; i < kMaxLayers; ++i) li += (habs >= P.layerf[i].h_lo) ? 1 : 0;
+    }
+    return li;
+}
+
+// Column depth T(h) = a + b exp(-h / c) of layer lf [g/cm^2]; *E = exp(-h / c)
+__device__ __forceinline__ float depth_at(const LayerF lf, float habs, float *E)
+{
+    *E = ex2_approx(-habs * lf.k2);
+    return fmaf(lf.b, *E, lf.a);
+}
+
+// R8: arrival time = emission time + (geometric path + integral of eta dl) / c,  integral = kappa (T(c_z) - T(e_z)) / |v_z|
+__device__ __forceinline__ float arrival_time(const KParams &P, float s, float ibc, float t0, float s_pl, float telT, float Te, float rv)
+{
+    const float excess = (P.kappa_m * (telT - Te)) * fabsf(rv);
+    return fmaf(s_pl + excess, 1.0f / 0.299792458f, fmaf(s, ibc, t0));
+}
+
+// R4: Cherenkov wavelength, 1 / lambda uniform
+__device__ __forceinline__ float cherenkov_lambda(const KParams &P, float u3) { return rcp_refined(fmaf(-u3, P.dinv_lam, P.inv_lam1)); }
+
+// R10 for an axis-kind photon and coplanar telescopes: q = g - c on the plane z_ref, b^2 = |q|^2 - (q.v)^2, emission
+// above the plane, closest approach ahead.
+__device__ __forceinline__ bool axis_test_coplanar(float qx, float qy, float vx, float vy, float ez, float rv, float R2, float *s_pl)
+{
+    const float qv = fmaf(qx, vx, qy * vy);
+    const float b2 = fmaf(-qv, qv, fmaf(qx, qx, qy * qy));
+    *s_pl = -ez * rv;
+    return (b2 <= R2) && (ez > 0.0f) && (*s_pl - qv > 0.0f);
+}
+
+// a4 exact test (R10) + arrival time, wavelength, weight for photon `ph` against telescope k.  Only h.ok and h.k are
+// defined when the pair is no hit.  COPLANAR (every telescope centre on the plane z_ref: T.z = 0) drops the terms
+// that vanish; the values are the same, bit for bit, as those of the general form (x + 0 = x), so a photon's record
+// does not depend on which instance evaluated it.
+template <int TELSRC, bool COPLANAR = false>
 __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &sm, int e, const Photon &ph, int k)
 {
     Hit h;
     h.k = k; h.vx = ph.vx; h.vy = ph.vy; h.ok = false;
-    h.x = h.y = h.t = h.lam = h.w = 0.0f;
     if (!(ph.vz < 0.0f)) return h;
     const float4 T = tel_at<TELSRC>(P, k);
-    const float rv = rcp_refined(ph.vz);
+    // 1 / v_z to 1 ulp: Newton step on MUFU.RCP (the axis kind brings the MUFU value it projected with)
+    const float r0 = ph.axis ? ph.rva : rcp_approx(ph.vz);
+    const float rv = fmaf(r0, fmaf(-ph.vz, r0, 1.0f), r0);
     const float *fr = &sm.frame[e * kFrameStride];
     const float habs = P.z_ref_f + ph.ez;
     // Column depth T(e_z) of the emission altitude (R8) and, for R27, the refractivity there.  The layer: the preamble
@@ -605,16 +670,10 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     // layers carry h_lo = +inf, so the count is the index).
     float Te, eta_e;
     auto atmosphere_at_emission = [&]() {
-        int li = __float_as_int(fr[F_LAYER]);
-        if (li < 0) {
-            li = 0;
-#pragma unroll
-            for (int i = 1; i < kMaxLayers; ++i) li += (habs >= P.layerf[i].h_lo) ? 1 : 0;
-        }
-        const LayerF lf = P.layerf[li];
-        const float E = __expf(-habs * lf.inv_c);
-        Te = fmaf(lf.b, E, lf.a);
-        eta_e = P.kappa_m * lf.b * lf.inv_c * E;             // eta0 rho(h) / rho0, rho = (b / c) exp(-h / c) / 100
+        const LayerF lf = P.layerf[emission_layer(P, __float_as_int(fr[F_LAYER]), habs)];
+        float E;
+        Te = depth_at(lf, habs, &E);
+        eta_e = P.kappa_m * lf.b * (lf.k2 * 0.693147181f) * E;   // eta0 rho(h) / rho0, rho = (b / c) exp(-h / c) / 100
     };
     float s_pl;
     if ((P.flags & kFlagRefract) && ph.vz <= -0.5f) {
@@ -647,14 +706,20 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     } else {
         if (ph.axis) {
             // q = g - c on the plane z_ref:  b^2 = |q|^2 - (q.v)^2,  the point g is at path length -ez / v_z
-            const float qx = ph.gx - T.x, qy = ph.gy - T.y, qz = -T.z;
-            const float qv = fmaf(qx, ph.vx, fmaf(qy, ph.vy, qz * ph.vz));
-            const float b2 = fmaf(qx, qx, fmaf(qy, qy, qz * qz)) - qv * qv;
-            const float hk = ph.ez - T.z;                                      // emission height above the telescope plane
-            s_pl = -hk * rv;
-            const float s_c = (s_pl - T.z * rv) - qv;
-            if (!(b2 <= T.w) || !(hk > 0.0f) || !(s_c > 0.0f)) return h;
-            h.x = fmaf(T.z * rv, ph.vx, qx); h.y = fmaf(T.z * rv, ph.vy, qy);  // on the plane z = c_z, relative to the centre (R11)
+            const float qx = ph.gx - T.x, qy = ph.gy - T.y;
+            if constexpr (COPLANAR) {
+                if (!axis_test_coplanar(qx, qy, ph.vx, ph.vy, ph.ez, rv, T.w, &s_pl)) return h;
+                h.x = qx; h.y = qy;
+            } else {
+                const float qz = -T.z;
+                const float qv = fmaf(qx, ph.vx, fmaf(qy, ph.vy, qz * ph.vz));
+                const float b2 = fmaf(-qv, qv, fmaf(qx, qx, fmaf(qy, qy, qz * qz)));
+                const float hk = ph.ez - T.z;                                      // emission height above the telescope plane
+                s_pl = -hk * rv;
+                const float s_c = (s_pl - T.z * rv) - qv;
+                if (!(b2 <= T.w) || !(hk > 0.0f) || !(s_c > 0.0f)) return h;
+                h.x = fmaf(T.z * rv, ph.vx, qx); h.y = fmaf(T.z * rv, ph.vy, qy);  // on the plane z = c_z, relative to the centre (R11)
+            }
         } else {
             // no plane projection (ill-conditioned for |v_z| -> 0):  b = |m x v|,  m = c - e
             const float mx = T.x - ph.ex, my = T.y - ph.ey, mz = T.z - ph.ez;
@@ -667,13 +732,10 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
         }
         atmosphere_at_emission();
     }
-    // R8: arrival time = emission time + (geometric path + integral of eta dl) / c,
-    //     integral = kappa (T(c_z) - T(e_z)) / |v_z|
-    const float excess = P.kappa_m * (telT_at<TELSRC>(P, k) - Te) * fabsf(rv);
-    h.t = fmaf(ph.s, fr[F_IBC], fr[F_T0]) + (s_pl + excess) * (1.0f / 0.299792458f);
+    h.t = arrival_time(P, ph.s, fr[F_IBC], fr[F_T0], s_pl, telT_at<TELSRC>(P, k), Te, rv);
     // R4: wavelength
     const float u3 = ph.u3;
-    h.lam = (ph.tag == 0) ? rcp_refined(fmaf(-u3, P.dinv_lam, P.inv_lam1)) : fmaf(u3, P.fl_dlam, P.fl_lam1);
+    h.lam = (ph.tag == 0) ? cherenkov_lambda(P, u3) : fmaf(u3, P.fl_dlam, P.fl_lam1);
     // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
     h.w = fr[F_W0];
     if (P.tau != nullptr) {
@@ -734,38 +796,12 @@ __device__ __forceinline__ void accumulate_hit(const KParams &P, TileSmem &sm, c
     sm.acc_n[t] += 1u; sm.acc_w[t] += w; sm.acc_wt[t] += w * (double)h.t;
 }
 
-// Copy n staged records (7 n words at `st`) to record slots [first, first + n) of P.records: lane i takes words i,
-// i + 32, ..., so every store instruction of the warp covers 128 contiguous bytes (four full 32-byte sectors once the
-// run is past its first, possibly unaligned, sector).  Called by all 32 lanes.
-__device__ __forceinline__ void copy_records(const KParams &P, const float *st, const unsigned long long *sid,
-                                             unsigned long long first, uint32_t n)
+// Photon output when all hits of the warp are on one telescope k0 (okm = the lanes holding one): one bump of that
+// telescope's cursor for the warp (sparse tiles, queue drains, telescopes other than a dense tile's own).
+__device__ __forceinline__ void write_records_one_tel(const KParams &P, const Hit &h, uint64_t id, uint32_t okm, int k0)
 {
-    const uint32_t lane = lane_id(), nwords = n * kRecWords;
-    float *dst = P.records + first * (unsigned)kRecWords;
-#pragma unroll 4
-    for (uint32_t i = lane; i < nwords; i += 32u) dst[i] = st[i];
-    if (P.ids) for (uint32_t i = lane; i < n; i += 32u) P.ids[first + i] = sid[i];
-}
-
-// Photon output when all hits of the warp are on one telescope k0 (okm = the lanes holding one).  While the tile runs
-// in rounds the records are appended to the warp's staging area and leave at the end of the round (flush_round);
-// otherwise, or when the area is full or holds another telescope's records, the warp bumps the cursor itself.
-__device__ __forceinline__ void write_records_one_tel(const KParams &P, OutSmem &os, const Hit &h, uint64_t id, uint32_t okm, int k0)
-{
-    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    const uint32_t lane = lane_id();
     const uint32_t n = (uint32_t)__popc(okm), rank = (uint32_t)__popc(okm & ((1u << lane) - 1u));
-    __syncwarp();                                   // lane 0's update of wn / wk in the previous call
-    const uint32_t wn = os.wn[warp];
-    if (os.rounds && (wn == 0u || os.wk[warp] == k0) && wn + n <= (uint32_t)kStageRecs) {
-        if (h.ok) {
-            float *r = os.stage[warp] + (wn + rank) * kRecWords;
-            r[0] = h.x; r[1] = h.y; r[2] = h.vx; r[3] = h.vy; r[4] = h.t; r[5] = h.lam; r[6] = h.w;
-            if (P.ids) os.ids[warp][wn + rank] = id;
-        }
-        __syncwarp();                               // all lanes have read wn / wk
-        if (lane == 0u) { os.wk[warp] = k0; os.wn[warp] = wn + n; }
-        return;
-    }
     unsigned long long base = 0;
     if (lane == 0u) base = atomicAdd(&P.cursors[k0], (unsigned long long)n);
     base = __shfl_sync(0xffffffffu, base, 0);
@@ -779,41 +815,72 @@ __device__ __forceinline__ void write_records_one_tel(const KParams &P, OutSmem 
     }
 }
 
-// End of a round, called by every thread of the tile: reserve the staged records of all warps (one cursor bump per
-// run of warps on the same telescope) and copy them out.  Returns whether the tile stays in the rounds mode: with
-// `may_stop` set (first round) it leaves it (os.rounds = 0, visible to all warps on return) unless at least
-// kDenseTile records were staged, i.e. unless a good part of its photons hit.
-__device__ __forceinline__ bool flush_round(const KParams &P, OutSmem &os, bool may_stop)
+// Bulk asynchronous copy shared -> global (TMA, cp.async.bulk): 16-byte aligned addresses, size a multiple of 16.
+__device__ __forceinline__ void bulk_store(void *gdst, const void *ssrc, uint32_t bytes)
 {
-    const uint32_t warp = threadIdx.x >> 5;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        uint32_t staged = 0;
-        for (int w = 0; w < kWarps; ++w) staged += os.wn[w];
-        for (int w = 0; w < kWarps; ) {
-            if (os.wn[w] == 0u) { ++w; continue; }
-            const int k = os.wk[w];
-            uint32_t run = 0;
-            int w1 = w;
-            while (w1 < kWarps && (os.wn[w1] == 0u || os.wk[w1] == k)) { run += os.wn[w1]; ++w1; }
-            unsigned long long base = atomicAdd(&P.cursors[k], (unsigned long long)run);
-            for (int v = w; v < w1; ++v) { os.wbase[v] = base; base += os.wn[v]; }
-            w = w1;
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 :: "l"(gdst), "r"((uint32_t)__cvta_generic_to_shared(ssrc)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all but the N most recent bulk groups of this thread have finished READING their shared-memory source
+template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" :: "n"(N) : "memory"); }
+// orders this thread's shared-memory writes before later async-proxy (bulk copy) reads of them
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Dense tiles: send the block of n records a warp staged in round r (words [0, 7 n) of staging buffer r % 3) to the
+// slots the round reserved for it, [base_r + off, base_r + off + n) of telescope kd's region.  Waits (lane 0 spins on
+// the flag in shared memory) until the last arrival of round r has published base_r; two trips of arithmetic lie
+// between the warp's own arrival and this call, so the wait is normally over.  Called by all 32 lanes, every round,
+// also with n == 0: the wait is what keeps a warp from running more than kRoundSlots - 1 rounds ahead of the others.
+//
+// 16-byte alignment: record slot s starts at word 7 s, so the words of a shared-memory slot and of a global slot are
+// in the same position within a 16-byte vector iff the two slot numbers agree modulo 4.  The order of the records
+// within a region is free (R22), so the block is rotated by rho = (-G) mod 4 slots, G = first global slot: staged
+// slot s goes to global slot G + rho + s, whose address is a multiple of 16 bytes for s = 0 -- the body leaves with
+// ONE bulk copy issued by lane 0 -- and the last rho (<= 3) staged records wrap around to global slots
+// G .. G + rho - 1 as scalar words, together with the <= 3 words the 16-byte body leaves over.
+template <bool IDS>
+__device__ __forceinline__ void copy_block(const KParams &P, OutSmem &os, const int kd, const uint32_t n, const uint32_t off,
+                                           const uint32_t r)
+{
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
+    unsigned long long b = 0;
+    if (lane == 0u) {
+        volatile uint32_t *flag = &os.rflag[r & (kRoundSlots - 1)];
+        while (*flag != r + 1u) __nanosleep(64);
+        __threadfence_block();
+        b = *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)];
+    }
+    __syncwarp();
+    b = __shfl_sync(0xffffffffu, b, 0);
+    if (n == 0u) return;
+    const unsigned long long cap = P.tel_capacity[kd], first = b + off;
+    if (first >= cap) return;
+    const uint32_t m = (uint32_t)min((unsigned long long)n, cap - first);
+    const unsigned long long G = P.tel_offset[kd] + first;
+    const float *st = os.stage[warp][r % kStageBufs];
+    float *dst = P.records + G * (unsigned)kRecWords;
+    if ((reinterpret_cast<uintptr_t>(P.records) & 15u) == 0u) {
+        const uint32_t rho = min((0u - (uint32_t)G) & 3u, m), body = (m - rho) * kRecWords, nb16 = body & ~3u, rest = body & 3u;
+        if (lane == 0u && nb16) bulk_store(dst + rho * kRecWords, st, nb16 * 4u);
+        // lanes 0 .. 7 rho - 1: the wrapped records; the next `rest` lanes: the words the 16-byte body left over
+        const uint32_t nwrap = rho * kRecWords;
+        if (lane < nwrap) dst[lane] = st[body + lane];
+        else if (lane < nwrap + rest) dst[nwrap + nb16 + (lane - nwrap)] = st[nb16 + (lane - nwrap)];
+        if constexpr (IDS) {
+            const unsigned long long *sid = os.ids[warp][r % kStageBufs];
+            for (uint32_t s = lane; s < m; s += 32u) P.ids[(s < m - rho) ? G + rho + s : G + s - (m - rho)] = sid[s];
         }
-        if (may_stop && staged < (uint32_t)kDenseTile) os.rounds = 0;
+    } else {
+        const uint32_t nwords = m * kRecWords;
+#pragma unroll 4
+        for (uint32_t i = lane; i < nwords; i += 32u) dst[i] = st[i];
+        if constexpr (IDS) {
+            const unsigned long long *sid = os.ids[warp][r % kStageBufs];
+            for (uint32_t s = lane; s < m; s += 32u) P.ids[G + s] = sid[s];
+        }
     }
-    __syncthreads();
-    const uint32_t n = os.wn[warp];
-    if (n) {
-        const int k = os.wk[warp];
-        const unsigned long long base = os.wbase[warp], cap = P.tel_capacity[k];
-        if (base < cap)
-            copy_records(P, os.stage[warp], os.ids[warp], P.tel_offset[k] + base, (uint32_t)min((unsigned long long)n, cap - base));
-    }
-    __syncwarp();
-    if ((threadIdx.x & 31) == 0) os.wn[warp] = 0u;
-    __syncwarp();
-    return os.rounds != 0;
 }
 
 // a5 for up to 32 evaluated pairs, one per lane (h.ok says which lanes hold a hit).  Called by all 32 lanes together.
@@ -850,7 +917,7 @@ __device__ __forceinline__ void commit_hits(const KParams &P, TileSmem &sm, cons
     if (h.ok) accumulate_hit(P, sm, h);
     if constexpr (MODE == MODE_OUT) {
         const int k0 = __shfl_sync(0xffffffffu, h.k, __ffs(okm) - 1);
-        if (__all_sync(0xffffffffu, !h.ok || h.k == k0)) write_records_one_tel(P, out_smem(sm), h, id, okm, k0);
+        if (__all_sync(0xffffffffu, !h.ok || h.k == k0)) write_records_one_tel(P, h, id, okm, k0);
         else write_records_grouped(P, h, id);
     }
 }
@@ -1101,12 +1168,6 @@ __device__ __forceinline__ AxisFrame load_axis_frame(const TileSmem &sm, int e)
     return AxisFrame{A.x, A.y, A.z, A.w, B.x, B.y, B.z, B.w, C.x, C.y, C.z};
 }
 
-// The kernels that run the pair loop (walk_pairs) pad every emitter to an even number of slots of the index space.
-template <int TELSRC, int MODE> __device__ __forceinline__ constexpr bool index_space_is_padded()
-{
-    return true;
-}
-
 // ------------------------------------------------------------------------------------
 // The lane's position in its warp's photon range and everything else the photon loop carries.
 struct WarpWalk {
@@ -1117,42 +1178,35 @@ struct WarpWalk {
     uint32_t n_up, q_head, q_count;
 };
 
-// Iterations [it0, it1) of the photon loop (phase 2).  INLINE: tiles in which most photons hit (ground histogram: all
-// tiles; photon output: while the tile runs in rounds) evaluate the first candidate of an axis-kind photon right in
-// the loop, from the values already in registers: no queue, no second Philox, no second sincos.  The sparse tiles of
-// the photon-output kernels run the instance without that code.  Returns whether the tile is (still) in rounds mode.
-template <int TELSRC, bool COPLANAR, int NT, int MODE, bool INLINE, bool REFR, bool FIRST>
-__device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &ww, const uint32_t hi, const unsigned long long tile_first,
-                                     const uint32_t it0, const uint32_t it1, const uint32_t n_iter, bool rounds)
+// The photon loop of the grid / global-table photon-output kernels (phase 2): one photon per lane and iteration, its
+// half of the Philox block selected by the photon index; candidates go to the queue, or are evaluated on the spot when
+// at least kDenseMin lanes hold one.
+template <int TELSRC, bool COPLANAR, int NT, int MODE, bool REFR>
+__device__ __forceinline__ void walk(const KParams &P, TileSmem &sm, WarpWalk &ww, const uint32_t hi, const unsigned long long tile_first,
+                                     const uint32_t n_iter)
 {
-    constexpr bool OUT = (MODE == MODE_OUT);
     constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
-    const int tid = threadIdx.x, lane = tid & 31;
     int e = ww.e, kind = ww.kind;
     uint32_t end = ww.end, g = ww.g, j = ww.j, n_up = ww.n_up, q_head = ww.q_head, q_count = ww.q_count;
     PhiloxEmitter pe = ww.pe;
     AxisFrame f_reg = ww.f_reg;
-    (void)tid; (void)lane;
-    for (uint32_t it = it0; it < it1; ++it, g += 32u, j += 32u) {
+    for (uint32_t it = 0; it < n_iter; ++it, g += 32u, j += 32u) {
         bool active = g < hi;                        // the lanes past the warp's range idle in its last iterations
         uint32_t cm = 0u;
         uint2 cell = make_uint2(0xffffffffu, 0xffffffffu);
         Rand4 r = {0u, 0u, 0u, 0u};
-        Hit h;
-        h.ok = false; h.k = 0; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
         if (active) {
-            // padded kernels: `end` holds the emitter's real end (its padded end less the empty slot after an odd count)
-            constexpr bool kPadded = index_space_is_padded<TELSRC, MODE>();
-            if (g >= (kPadded ? ((end + 1u) & ~1u) : end)) {
+            // `end` holds the emitter's real end (its padded end less the empty slot after an odd count)
+            if (g >= ((end + 1u) & ~1u)) {
                 uint32_t pend;
                 do { ++e; pend = sm.prefix[e + 1]; } while (g >= pend);
-                end = kPadded ? pend - sm.odd[e] : pend;
+                end = pend - sm.odd[e];
                 j = g - sm.prefix[e];
                 kind = sm.kind[e];
                 pe = philox_emitter(P, emitter_segment(P, tile_first, e));
                 if (kFrameInRegs) f_reg = load_axis_frame(sm, e);
             }
-            if (kPadded && g >= end) active = false;             // the empty slot
+            if (g >= end) active = false;             // the empty slot
         }
         if (active) {
             if (kind == KIND_CHER_AXIS) {
@@ -1175,22 +1229,6 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                         vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
                     }
                     cm = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gx, gy, vx, vy, vz, &cell);
-                    if constexpr (MODE != MODE_TALLY) {
-                        if (INLINE && cm != 0u && cm != kAllTelescopes) {
-                            const float *fr = &sm.frame[e * kFrameStride];
-                            Photon ph;
-                            ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(r.r0, r.r1);
-                            ph.vx = fmaf(cp, fr[F_AX], fmaf(sp, fr[F_BX], fr[F_CX]));
-                            ph.vy = fmaf(cp, fr[F_AY], fmaf(sp, fr[F_BY], fr[F_CY]));
-                            ph.vz = vz; ph.gx = gx; ph.gy = gy;
-                            ph.s = (one_two(r.r0) - kOneMinus) * fr[F_LEN];
-                            ph.ez = -sd * fr[F_DZ];
-                            ph.ex = ph.ey = 0.0f;
-                            const int k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1);
-                            cm &= cm - 1u;
-                            h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
-                        }
-                    }
                 } else {
                     ++n_up;
                 }
@@ -1211,35 +1249,19 @@ __device__ __forceinline__ bool walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 if (cm == kAllTelescopes) cm = 0u;
             }
         }
-        if constexpr (MODE != MODE_TALLY) {
-            if (INLINE)           // the record id of an axis-kind photon: tag 0
-                commit_hits<MODE>(P, sm, h, (emitter_segment(P, tile_first, e) << 25) | (unsigned long long)j);
-        }
         const uint32_t have = __ballot_sync(0xffffffffu, cm != 0u);
-        if constexpr (MODE != MODE_TALLY) {
-            if (__popc(have) >= kDenseMin) {
-                // dense iteration: each lane's first candidate is evaluated on the spot, further ones are queued
-                const bool has = cm != 0u;
-                int k = 0;
-                if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
-                dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, r.r3, k, has);
-            }
-            if (__any_sync(0xffffffffu, cm != 0u))
-                push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
-            if (OUT && rounds && ((it % kRound) == kRound - 1 || it + 1 == n_iter)) {
-                // FIRST = the instance that runs round 0: too little staged there means a sparse tile, which goes on
-                // without rounds (and barriers).  In the other instances `rounds` is a constant.
-                if constexpr (FIRST) { if (!flush_round(P, out_smem(sm), true)) rounds = false; }
-                else flush_round(P, out_smem(sm), false);
-            }
-        } else {
-            if (have)
-                push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
+        if (__popc(have) >= kDenseMin) {
+            // dense iteration: each lane's first candidate is evaluated on the spot, further ones are queued
+            const bool has = cm != 0u;
+            int k = 0;
+            if (has) { k = (int)slot_telescope<TELSRC>(cell, __ffs(cm) - 1); cm &= cm - 1u; }
+            dense_eval<TELSRC, MODE>(P, sm, tile_first, e, j, r.r0, r.r1, r.r2, r.r3, k, has);
         }
+        if (__any_sync(0xffffffffu, cm != 0u))
+            push_candidates<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, cm, e, j, [&](int c) { return slot_telescope<TELSRC>(cell, c); });
     }
     ww.e = e; ww.kind = kind; ww.end = end; ww.g = g; ww.j = j; ww.n_up = n_up; ww.q_head = q_head; ww.q_count = q_count;
     ww.pe = pe; ww.f_reg = f_reg;
-    return rounds;
 }
 
 // The pair loop (tally kernels, and the sparse tiles of the photon-output kernels after round 0): a lane takes the two
@@ -1315,20 +1337,20 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                         ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(rA.r0, rA.r1);
                         ph.vx = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); ph.vy = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
                         ph.vz = vzA; ph.gx = gxA; ph.gy = gyA; ph.s = (one_two(rA.r0) - kOneMinus) * fr[F_LEN]; ph.ez = -sdA * fr[F_DZ];
-                        ph.ex = ph.ey = 0.0f;
+                        ph.ex = ph.ey = 0.0f; ph.rva = rcp_approx(vzA);
                         const int k = (int)slot_telescope<TELSRC>(cellA, __ffs(cmA) - 1);
                         cmA &= cmA - 1u;
-                        hA = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+                        hA = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
                     }
                     if (cmB != 0u && cmB != kAllTelescopes) {
                         Photon ph;
                         ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(rB.r0, rB.r1);
                         ph.vx = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); ph.vy = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
                         ph.vz = vzB; ph.gx = gxB; ph.gy = gyB; ph.s = (one_two(rB.r0) - kOneMinus) * fr[F_LEN]; ph.ez = -sdB * fr[F_DZ];
-                        ph.ex = ph.ey = 0.0f;
+                        ph.ex = ph.ey = 0.0f; ph.rva = rcp_approx(vzB);
                         const int k = (int)slot_telescope<TELSRC>(cellB, __ffs(cmB) - 1);
                         cmB &= cmB - 1u;
-                        hB = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+                        hB = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
                     }
                 }
             } else {
@@ -1385,8 +1407,302 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
     n_up_out += n_up;
 }
 
+// Dense tiles, generic kinds (and the probe): a3 + a4 of one photon out of line -- photon in the global frame, the
+// conservative pre-tests over the NT constant-bank telescopes, the exact test of the first candidate.  *cm_left = the
+// further candidates (bit k = telescope k), *upward = the photon does not go down.
+template <bool COPLANAR, int NT, bool REFR>
+__device__ __forceinline__ uint32_t const_candidates(const KParams &P, const Photon &ph)
+{
+    if (ph.vz > -0.05f) return (1u << NT) - 1u;                      // flat photon: every slot goes to the exact test
+    uint2 cell;
+    if (ph.axis) return plane_candidates<TEL_CONST, COPLANAR, NT, REFR>(P, ph.gx, ph.gy, ph.vx, ph.vy, ph.vz, &cell);
+    const float spl = -ph.ez * rcp_approx(ph.vz);                    // candidate search only: the pre-tests carry slack
+    return plane_candidates<TEL_CONST, COPLANAR, NT, REFR>(P, fmaf(spl, ph.vx, ph.ex), fmaf(spl, ph.vy, ph.ey), ph.vx, ph.vy, ph.vz, &cell);
+}
+
+struct GenericHit { Hit h; uint32_t cm_left; bool upward; };
+
+template <bool COPLANAR, int NT, bool REFR>
+__device__ __noinline__ GenericHit generic_hit(const KParams &P, const TileSmem &sm, int e, const Rand4 r)
+{
+    GenericHit g;
+    g.h.ok = false; g.h.k = 0; g.h.x = g.h.y = g.h.vx = g.h.vy = g.h.t = g.h.lam = g.h.w = 0.0f;
+    g.cm_left = 0u;
+    const Photon ph = photon_from_rand(P, sm, e, r);
+    g.upward = !(ph.vz < 0.0f);
+    if (g.upward) return g;
+    uint32_t cm = const_candidates<COPLANAR, NT, REFR>(P, ph);
+    if (cm != 0u) {
+        const int k = __ffs(cm) - 1;
+        cm &= cm - 1u;
+        g.h = evaluate_pair<TEL_CONST, COPLANAR>(P, sm, e, ph, k);
+    }
+    g.cm_left = cm;
+    return g;
+}
+
+// ------------------------------------------------------------------------------------
+// Photon output, brute-force kernels: is this tile dense (a good part of its photons hit one telescope: c5g, a detector
+// that covers the light pool) or sparse (c5: 0.4 % hit)?  Every lane takes one photon of its warp's range, evenly
+// spread over it (even slots always hold a photon), draws it and runs the conservative pre-test only; the candidates
+// are counted per telescope in os.probe.  Nothing is tallied or written: the loops start from the beginning afterwards.
+template <bool COPLANAR, int NT, bool REFR>
+__device__ __noinline__ void probe_density(const KParams &P, TileSmem &sm, OutSmem &os, const uint32_t lo, const uint32_t hi,
+                                           const unsigned long long tile_first)
+{
+    const uint32_t lane = lane_id();
+    uint32_t cm = 0u;
+    if (lo < hi) {
+        const uint32_t stride = max(2u, ((hi - lo) >> 5) & ~1u), g = lo + stride * lane;
+        if (g < hi) {
+            int a = 0, b = kTile;                 // invariant: prefix[a] <= g < prefix[b]
+            while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g) a = m; else b = m; }
+            const int e = a;
+            const uint32_t j = g - sm.prefix[e];
+            const unsigned long long S = emitter_segment(P, tile_first, e);
+            const uint32_t tag = kind_tag(sm.kind[e]);
+            const Rand4 blk = philox4x32_10(P, tag ? j : (j >> 1), (uint32_t)S, (uint32_t)(S >> 32), tag);
+            const Rand4 r = tag ? blk : cherenkov_words(blk, j);
+            const Photon ph = photon_from_rand(P, sm, e, r);
+            if (ph.vz <= -0.05f) cm = const_candidates<COPLANAR, NT, REFR>(P, ph);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NT; ++k) {
+        const uint32_t c = (uint32_t)__popc(__ballot_sync(0xffffffffu, (cm >> k) & 1u));
+        if (c && lane == 0u) atomicAdd(&os.probe[k], c);
+    }
+}
+
+// The photon loop of a dense tile (photon output, brute-force kernels).  The pair loop of walk_pairs -- a lane takes
+// the adjacent slots g, g + 1 per trip, one Philox block for both (R20) -- with every candidate evaluated on the spot
+// from the values in registers, the records of the trip staged per warp (<= 64) and their slots reserved once per
+// tile and trip (OutSmem).  Per trip r:  arithmetic of trip r  ->  pick up the base of round r - 2 and send that block
+// out (copy_block: one bulk copy)  ->  stage block r  ->  arrive at round r.  The global atomic of a round, its latency
+// and the spread between the warps of the tile are thus covered by two trips of arithmetic, and there is no block
+// barrier.  Every warp of the tile runs all n_trips trips (it arrives with 0 records once its range is finished).
+// kd = the tile's dense telescope; hits on other telescopes, further candidates of a photon and the generic kinds
+// take the paths of the sparse loop (queue / direct cursor bump).
+// FAST: one coplanar telescope, no refraction corrections, no transmission table, no id side buffer (the launch that
+// is measured against the HBM roofline): the exact evaluation of an axis-kind photon written out on the values the
+// loop holds, built from the same pieces as evaluate_pair (bit-identical records).
+template <bool COPLANAR, int NT, bool REFR, bool FAST>
+__device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSmem &os, const uint32_t base, const uint32_t hi,
+                                           const unsigned long long tile_first, const uint32_t n_trips, const int kd,
+                                           uint32_t &n_up_out, uint32_t &q_head, uint32_t &q_count)
+{
+    constexpr int TELSRC = TEL_CONST;
+    static_assert(!FAST || (NT == 1 && COPLANAR && !REFR), "fast path: one coplanar telescope, straight lines");
+    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5, lt = (1u << lane) - 1u;
+    const bool want_ids = !FAST && P.ids != nullptr;
+    uint32_t g = base + 2u * lane;
+    int e;
+    {
+        const uint32_t g0 = (base < hi) ? min(g, hi - 2u) : 0u;
+        int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
+        while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
+        e = a;
+    }
+    uint32_t end = sm.prefix[e + 1], rend = end - sm.odd[e], j = g - sm.prefix[e], n_up = 0u;
+    int kind = sm.kind[e];
+    PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+    AxisFrame f = load_axis_frame(sm, e);
+    uint32_t n_1 = 0u, off_1 = 0u, n_2 = 0u, off_2 = 0u;      // the blocks staged one and two trips ago
+    // this thread's tally of hits on kd: fp32 partial sums over kTallyTrips trips (<= 2 kTallyTrips terms), then fp64
+    constexpr uint32_t kTallyTrips = 32u;
+    uint32_t acc_n = 0u;
+    float part_w = 0.0f, part_wt = 0.0f;
+    double acc_w = 0.0, acc_wt = 0.0;
+    for (uint32_t r = 0; r < n_trips; ++r, g += 64u, j += 64u) {
+        const bool active = g < hi;
+        uint32_t cmA = 0u, cmB = 0u;
+        Hit hA, hB;
+        hA.ok = false; hB.ok = false;
+        if (active) {
+            if (g >= end) {
+                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+                rend = end - sm.odd[e];
+                j = g - sm.prefix[e];
+                kind = sm.kind[e];
+                pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+                f = load_axis_frame(sm, e);
+            }
+            const bool hasB = g + 1u < rend;                     // slot g + 1 is empty after an odd count
+            if (kind == KIND_CHER_AXIS) {
+                const Rand4 blk = philox_photon(P, pe, j >> 1, 0u);                               // a2: one block, two photons (R20; j is even)
+                // a3 / a4 as in walk_pairs, for both photons
+                const float w1A = one_two(blk.r0), w1B = one_two(blk.r2);
+                const float sdA = fmaf(w1A, f.negL, f.k0c), sdB = fmaf(w1B, f.negL, f.k0c);
+                float spA, cpA, spB, cpB;
+                __sincosf(fmaf(one_two(blk.r1), 6.2831853f, -9.42477760f), &spA, &cpA);
+                __sincosf(fmaf(one_two(blk.r3), 6.2831853f, -9.42477760f), &spB, &cpB);
+                const float vzA = fmaf(cpA, f.az, fmaf(spA, f.bz, f.cz)), vzB = fmaf(cpB, f.az, fmaf(spB, f.bz, f.cz));
+                const float rvA = rcp_approx(vzA), rvB = rcp_approx(vzB);
+                const float rhoA = sdA * rvA, rhoB = sdB * rvB;
+                const float gxA = fmaf(rhoA, fmaf(cpA, f.px, spA * f.qx), f.gx), gyA = fmaf(rhoA, fmaf(cpA, f.py, spA * f.qy), f.gy);
+                const float gxB = fmaf(rhoB, fmaf(cpB, f.px, spB * f.qx), f.gx), gyB = fmaf(rhoB, fmaf(cpB, f.py, spB * f.qy), f.gy);
+                const float *fr = &sm.frame[e * kFrameStride];
+                const float4 vc0 = *reinterpret_cast<const float4 *>(fr + F_AX);      // AX, AY, BX, BY
+                const float4 vc1 = *reinterpret_cast<const float4 *>(fr + F_CX);      // CX, CY, LEN, LAYER
+                const float4 hs = *reinterpret_cast<const float4 *>(fr + F_W0);       // W0, T0, IBC, DZ
+                const float vxA = fmaf(cpA, vc0.x, fmaf(spA, vc0.z, vc1.x)), vyA = fmaf(cpA, vc0.y, fmaf(spA, vc0.w, vc1.y));
+                const float vxB = fmaf(cpB, vc0.x, fmaf(spB, vc0.z, vc1.x)), vyB = fmaf(cpB, vc0.y, fmaf(spB, vc0.w, vc1.y));
+                if constexpr (FAST) {
+                    // evaluate_pair<TEL_CONST, true> for telescope 0, straight lines, no transmission table
+                    const float4 T = P.tel_c[0];
+                    const float telT = P.telT_c[0];
+                    const int li_frame = __float_as_int(vc1.w);
+                    {
+                        const float rv = fmaf(rvA, fmaf(-vzA, rvA, 1.0f), rvA), ez = -sdA * hs.w;
+                        float s_pl;
+                        hA.x = gxA - T.x; hA.y = gyA - T.y;
+                        const bool ok = axis_test_coplanar(hA.x, hA.y, vxA, vyA, ez, rv, T.w, &s_pl);
+                        if (!(vzA < 0.0f)) ++n_up;
+                        hA.ok = ok && (vzA < 0.0f);
+                        const float habs = P.z_ref_f + ez;
+                        float E;
+                        const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
+                        hA.t = arrival_time(P, (w1A - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
+                        hA.lam = cherenkov_lambda(P, cherenkov_u3(blk.r0, blk.r1));
+                        hA.vx = vxA; hA.vy = vyA; hA.w = hs.x;
+                    }
+                    if (hasB) {
+                        const float rv = fmaf(rvB, fmaf(-vzB, rvB, 1.0f), rvB), ez = -sdB * hs.w;
+                        float s_pl;
+                        hB.x = gxB - T.x; hB.y = gyB - T.y;
+                        const bool ok = axis_test_coplanar(hB.x, hB.y, vxB, vyB, ez, rv, T.w, &s_pl);
+                        if (!(vzB < 0.0f)) ++n_up;
+                        hB.ok = ok && (vzB < 0.0f);
+                        const float habs = P.z_ref_f + ez;
+                        float E;
+                        const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
+                        hB.t = arrival_time(P, (w1B - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
+                        hB.lam = cherenkov_lambda(P, cherenkov_u3(blk.r2, blk.r3));
+                        hB.vx = vxB; hB.vy = vyB; hB.w = hs.x;
+                    }
+                } else {
+                    // one telescope: the exact test decides; several: the conservative pre-tests pick the candidates
+                    uint2 cell;
+                    if (vzA < 0.0f) cmA = (NT == 1) ? 1u : plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxA, gyA, vxA, vyA, vzA, &cell); else ++n_up;
+                    if (hasB) {
+                        if (vzB < 0.0f) cmB = (NT == 1) ? 1u : plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cell); else ++n_up;
+                    }
+                    if (cmA != 0u) {
+                        Photon ph;
+                        ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(blk.r0, blk.r1);
+                        ph.vx = vxA; ph.vy = vyA; ph.vz = vzA; ph.gx = gxA; ph.gy = gyA; ph.rva = rvA;
+                        ph.s = (w1A - kOneMinus) * vc1.z; ph.ez = -sdA * hs.w;
+                        ph.ex = ph.ey = 0.0f;
+                        const int k = (NT == 1) ? 0 : __ffs(cmA) - 1;
+                        cmA &= cmA - 1u;
+                        hA = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
+                    }
+                    if (cmB != 0u) {
+                        Photon ph;
+                        ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(blk.r2, blk.r3);
+                        ph.vx = vxB; ph.vy = vyB; ph.vz = vzB; ph.gx = gxB; ph.gy = gyB; ph.rva = rvB;
+                        ph.s = (w1B - kOneMinus) * vc1.z; ph.ez = -sdB * hs.w;
+                        ph.ex = ph.ey = 0.0f;
+                        const int k = (NT == 1) ? 0 : __ffs(cmB) - 1;
+                        cmB &= cmB - 1u;
+                        hB = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
+                    }
+                }
+            } else {
+                // generic kinds: out of line (photon in the global frame, pre-tests, exact test of the first candidate)
+                const uint32_t tag = kind_tag(kind);
+                const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
+                const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u});
+                hA = ga.h; cmA = ga.cm_left;
+                if (ga.upward) ++n_up;
+                if (hasB) {
+                    const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u});
+                    hB = gb.h; cmB = gb.cm_left;
+                    if (gb.upward) ++n_up;
+                }
+            }
+        }
+        unsigned long long idA = 0ull;
+        if (want_ids) idA = (emitter_segment(P, tile_first, e) << 25) | ((unsigned long long)kind_tag(kind) << 24) | (unsigned long long)j;
+        bool sA = hA.ok, sB = hB.ok;
+        if constexpr (NT > 1) {
+            // hits on another telescope than the tile's dense one: tallied and written directly
+            const bool oA = hA.ok && hA.k != kd, oB = hB.ok && hB.k != kd;
+            if (__any_sync(0xffffffffu, oA || oB)) {
+                if (!want_ids) idA = (emitter_segment(P, tile_first, e) << 25) | ((unsigned long long)kind_tag(kind) << 24) | (unsigned long long)j;
+                Hit t = hA; t.ok = oA;
+                commit_hits<MODE_OUT>(P, sm, t, idA);
+                t = hB; t.ok = oB;
+                commit_hits<MODE_OUT>(P, sm, t, idA + 1ull);
+            }
+            sA = hA.ok && !oA; sB = hB.ok && !oB;
+        }
+        // further candidates of the two photons (several telescopes; flat photons of the generic kinds): queue
+        if (__any_sync(0xffffffffu, (cmA | cmB) != 0u)) {
+            push_candidates<TELSRC, MODE_OUT>(P, sm, tile_first, q_head, q_count, cmA, e, j, [&](int c) { return (uint32_t)c; });
+            push_candidates<TELSRC, MODE_OUT>(P, sm, tile_first, q_head, q_count, cmB, e, j + 1u, [&](int c) { return (uint32_t)c; });
+        }
+        if (sA) { part_w += hA.w; part_wt = fmaf(hA.w, hA.t, part_wt); }
+        if (sB) { part_w += hB.w; part_wt = fmaf(hB.w, hB.t, part_wt); }
+        if ((r & (kTallyTrips - 1u)) == kTallyTrips - 1u) { acc_w += (double)part_w; acc_wt += (double)part_wt; part_w = 0.0f; part_wt = 0.0f; }
+        // the block staged two trips ago leaves (its slots have been reserved meanwhile); lane 0 then makes sure the
+        // bulk copy issued in the previous trip has read its buffer, which is the one this trip stages into
+        if (r >= 2u) { if (want_ids) copy_block<true>(P, os, kd, n_2, off_2, r - 2u); else copy_block<false>(P, os, kd, n_2, off_2, r - 2u); }
+        if (lane == 0u) { bulk_commit(); bulk_wait_read<1>(); }
+        __syncwarp();
+        float *const st = os.stage[warp][r % kStageBufs];
+        const uint32_t mA = __ballot_sync(0xffffffffu, sA), mB = __ballot_sync(0xffffffffu, sB);
+        const uint32_t nA = (uint32_t)__popc(mA), n_w = nA + (uint32_t)__popc(mB);
+        acc_n += n_w;                               // warp-uniform: lane 0's copy is the one that counts
+        if (sA) {
+            const uint32_t s = (uint32_t)__popc(mA & lt);
+            float *rec = st + s * kRecWords;
+            rec[0] = hA.x; rec[1] = hA.y; rec[2] = hA.vx; rec[3] = hA.vy; rec[4] = hA.t; rec[5] = hA.lam; rec[6] = hA.w;
+            if (want_ids) os.ids[warp][r % kStageBufs][s] = idA;
+        }
+        if (sB) {
+            const uint32_t s = nA + (uint32_t)__popc(mB & lt);
+            float *rec = st + s * kRecWords;
+            rec[0] = hB.x; rec[1] = hB.y; rec[2] = hB.vx; rec[3] = hB.vy; rec[4] = hB.t; rec[5] = hB.lam; rec[6] = hB.w;
+            if (want_ids) os.ids[warp][r % kStageBufs][s] = idA + 1ull;
+        }
+        fence_proxy_async();
+        __syncwarp();
+        uint32_t old = 0u;
+        if (lane == 0u) {
+            __threadfence_block();
+            old = atomicAdd(&os.agg[r & (kRoundSlots - 1)], (n_w << 8) | 1u);
+            if ((old & 0xffu) == (uint32_t)kWarps - 1u) {
+                // last arrival of round r: reserve the round's records, publish the base
+                const uint32_t total = (old >> 8) + n_w;
+                os.agg[r & (kRoundSlots - 1)] = 0u;
+                unsigned long long b = 0ull;
+                if (total) b = atomicAdd(&P.cursors[kd], (unsigned long long)total);
+                *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)] = b;
+                __threadfence_block();
+                *(volatile uint32_t *)&os.rflag[r & (kRoundSlots - 1)] = r + 1u;
+            }
+        }
+        __syncwarp();
+        n_2 = n_1; off_2 = off_1;
+        off_1 = __shfl_sync(0xffffffffu, old >> 8, 0);
+        n_1 = n_w;
+    }
+    // the last two blocks
+    if (n_trips >= 2u) { if (want_ids) copy_block<true>(P, os, kd, n_2, off_2, n_trips - 2u); else copy_block<false>(P, os, kd, n_2, off_2, n_trips - 2u); }
+    if (n_trips >= 1u) { if (want_ids) copy_block<true>(P, os, kd, n_1, off_1, n_trips - 1u); else copy_block<false>(P, os, kd, n_1, off_1, n_trips - 1u); }
+    if (lane == 0u) { bulk_commit(); bulk_wait<0>(); }
+    __syncwarp();
+    // the warp's tally of kd into the tile's: one shared-memory atomic per warp and sum
+    acc_w += (double)part_w; acc_wt += (double)part_wt;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { acc_w += __shfl_xor_sync(0xffffffffu, acc_w, o); acc_wt += __shfl_xor_sync(0xffffffffu, acc_wt, o); }
+    if (lane == 0u && acc_n) { atomicAdd(&sm.t_hits[kd], acc_n); atomicAdd(&sm.t_sw[kd], acc_w); atomicAdd(&sm.t_swt[kd], acc_wt); }
+    n_up_out += n_up;
+}
+
 template <int TELSRC, bool COPLANAR, int NT, int MODE>
-__global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_constant__ KParams P)
+__global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONST) ? kOutCtasPerSm : 3) propagate_kernel(const __grid_constant__ KParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem &sm = *reinterpret_cast<TileSmem *>(smem_raw);
@@ -1404,10 +1720,10 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
     if (tid < kWarps) sm.wide_count[tid] = 0u;
     constexpr bool OUT = (MODE == MODE_OUT);
-    if constexpr (OUT) {
+    if constexpr (OUT && TELSRC == TEL_CONST) {
         OutSmem &os = out_smem(sm);
-        if (tid < kWarps) { os.wn[tid] = 0u; os.wk[tid] = -1; }
-        if (tid == 0) os.rounds = 1;
+        if (tid < kRoundSlots) { os.agg[tid] = 0u; os.rflag[tid] = 0u; os.rbase[tid] = 0ull; }
+        if (tid < kTelConstMax) os.probe[tid] = 0u;
     }
     if constexpr (MODE == MODE_HIST) {
         HistSmem &hs = hist_smem(sm);
@@ -1443,9 +1759,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     // generic kind (fluorescence, near-horizontal Cherenkov tracks) costs about kGenericWeight axis-kind photons.
     // Every emitter takes an even number of slots of the index space (one empty slot after an odd count), so that the
     // pairs (g, g + 1), g even, which a lane of the pair loop takes, never straddle two emitters or two warps.
-    // Only the kernels that run the pair loop pad (the brute-force tally and output kernels).
-    constexpr bool kPadded = index_space_is_padded<TELSRC, MODE>();
-    const uint32_t odd = kPadded ? (nb & 1u) : 0u;
+    const uint32_t odd = nb & 1u;
     const uint32_t nbp = nb + odd;
     sm.odd[tid] = (uint8_t)odd;
     const uint32_t n_pad_w = (uint32_t)__popc(__ballot_sync(0xffffffffu, odd != 0u));
@@ -1481,7 +1795,7 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
 #pragma unroll
         for (int w = 1; w < kWarps; ++w) {
             const unsigned long long x = wtotal / kWarps * (unsigned)w + wtotal % kWarps * (unsigned)w / kWarps;   // floor(wtotal w / 8)
-            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & (kPadded ? ~1u : ~0u);
+            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & ~1u;
         }
     }
     __syncthreads();
@@ -1491,65 +1805,71 @@ __global__ void __launch_bounds__(kTile, 3) propagate_kernel(const __grid_consta
     const unsigned long long tile_first = P.first_id + (unsigned long long)blockIdx.x * (unsigned)segs_per_tile;
     uint32_t n_up = 0;
 
-    // Every warp runs the same number of iterations (that of the longest range), so the photon-output kernels can
-    // close a round with a block-wide barrier every kRound iterations.
+    // Every warp runs the same number of iterations (that of the longest range): the dense loop of the photon-output
+    // kernels closes a round of reservations once per trip, and every warp of the tile has to arrive at it.
     uint32_t max_len = 0;
 #pragma unroll
     for (int w = 0; w < kWarps; ++w) max_len = max(max_len, sm.bound[w + 1] - sm.bound[w]);
-    const uint32_t n_iter = (max_len + 31u) / 32u;
     if (total) {
-        // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
-        WarpWalk ww;
-        {
-            const uint32_t g0 = min(lo + (uint32_t)lane, max(hi, 1u) - 1u);
-            int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
-            while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
-            ww.e = a;
-        }
-        // Loop-carried per lane: photon index g, emitter e with its end, index j within the emitter, kind, the hoisted
-        // Philox words and (brute-force kernels only; the grid kernels are short of registers and reload it from
-        // shared memory every iteration) the axis frame.
-        ww.end = sm.prefix[ww.e + 1] - sm.odd[ww.e];
-        ww.kind = sm.kind[ww.e];
-        ww.pe = philox_emitter(P, emitter_segment(P, tile_first, ww.e));
-        ww.f_reg = load_axis_frame(sm, ww.e);
-        ww.g = lo + (uint32_t)lane; ww.j = ww.g - sm.prefix[ww.e];
-        ww.n_up = 0u; ww.q_head = 0u; ww.q_count = 0u;
-        // One instance of the loop per (inline evaluation, refraction slack in the pre-tests): both are uniform over the
-        // tile, and a photon of the default path pays for neither.
-        bool rounds = false;
-#define C8_WALK(INL, FIRST, IT0, IT1, RND)                                                                                       \
-    ((P.flags & kFlagRefract) ? walk<TELSRC, COPLANAR, NT, MODE, INL, true, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND) \
-                              : walk<TELSRC, COPLANAR, NT, MODE, INL, false, FIRST>(P, sm, ww, hi, tile_first, IT0, IT1, n_iter, RND))
-#define C8_WALK_PAIRS(BASE)                                                                                                    \
-    do {                                                                                                                       \
-        if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true, MODE == MODE_HIST>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count); \
-        else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, BASE, hi, tile_first, ww.n_up, ww.q_head, ww.q_count);     \
-    } while (0)
-        if constexpr (OUT) {
-            // round 0 decides whether the tile is dense (stays in rounds mode, inline evaluation) or sparse (pair loop)
-            const uint32_t it1 = min((uint32_t)kRound, n_iter);
-            rounds = C8_WALK(true, true, 0u, it1, true);
-            if (rounds) C8_WALK(true, false, it1, n_iter, true);
-            else if constexpr (TELSRC == TEL_CONST) C8_WALK_PAIRS(min(lo + 32u * it1, hi));
-            else C8_WALK(false, false, it1, n_iter, false);
+        // One instance of a loop per setting of the refraction slack in the pre-tests: it is uniform over the launch, and
+        // a photon of the default path does not pay for it.
+        uint32_t q_head = 0u, q_count = 0u;
+        if constexpr (OUT && TELSRC != TEL_CONST) {
+            // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
+            WarpWalk ww;
+            {
+                const uint32_t g0 = min(lo + (uint32_t)lane, max(hi, 1u) - 1u);
+                int a = 0, b = kTile;                 // invariant: prefix[a] <= g0 < prefix[b]
+                while (b - a > 1) { const int m = (a + b) >> 1; if (sm.prefix[m] <= g0) a = m; else b = m; }
+                ww.e = a;
+            }
+            // Loop-carried per lane: photon index g, emitter e with its end, index j within the emitter, kind, the hoisted
+            // Philox words (the grid kernels are short of registers and reload the axis frame from shared memory).
+            ww.end = sm.prefix[ww.e + 1] - sm.odd[ww.e];
+            ww.kind = sm.kind[ww.e];
+            ww.pe = philox_emitter(P, emitter_segment(P, tile_first, ww.e));
+            ww.f_reg = load_axis_frame(sm, ww.e);
+            ww.g = lo + (uint32_t)lane; ww.j = ww.g - sm.prefix[ww.e];
+            ww.n_up = 0u; ww.q_head = 0u; ww.q_count = 0u;
+            const uint32_t n_iter = (max_len + 31u) / 32u;
+            if (P.flags & kFlagRefract) walk<TELSRC, COPLANAR, NT, MODE, true>(P, sm, ww, hi, tile_first, n_iter);
+            else walk<TELSRC, COPLANAR, NT, MODE, false>(P, sm, ww, hi, tile_first, n_iter);
+            n_up = ww.n_up; q_head = ww.q_head; q_count = ww.q_count;
         } else {
-            C8_WALK_PAIRS(lo);            // tally: candidates to the queue; ground histogram: both photons evaluated inline
+            bool dense = false;
+            int kd = 0;
+            if constexpr (OUT) {
+                // dense or sparse tile?  (tile-uniform: every thread reads the same counts after the barrier)
+                OutSmem &os = out_smem(sm);
+                if (P.flags & kFlagRefract) probe_density<COPLANAR, NT, true>(P, sm, os, lo, hi, tile_first);
+                else probe_density<COPLANAR, NT, false>(P, sm, os, lo, hi, tile_first);
+                __syncthreads();
+                uint32_t best = 0u;
+#pragma unroll
+                for (int k = 0; k < NT; ++k) { const uint32_t c = os.probe[k]; if (c > best) { best = c; kd = k; } }
+                dense = best >= (uint32_t)kProbeDense;
+            }
+            if constexpr (OUT) {
+                if (dense) {
+                    const uint32_t n_trips = (max_len + 63u) / 64u;
+                    if (P.flags & kFlagRefract) walk_dense<COPLANAR, NT, true, false>(P, sm, out_smem(sm), lo, hi, tile_first, n_trips, kd, n_up, q_head, q_count);
+                    else if (NT == 1 && COPLANAR && P.tau == nullptr && P.ids == nullptr)
+                        walk_dense<COPLANAR, NT, false, NT == 1 && COPLANAR>(P, sm, out_smem(sm), lo, hi, tile_first, n_trips, kd, n_up, q_head, q_count);
+                    else walk_dense<COPLANAR, NT, false, false>(P, sm, out_smem(sm), lo, hi, tile_first, n_trips, kd, n_up, q_head, q_count);
+                }
+            }
+            if (!dense) {
+                // tally, sparse photon output: candidates to the queue; ground histogram: both photons evaluated inline
+                if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
+                else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
+            }
         }
-#undef C8_WALK
-#undef C8_WALK_PAIRS
-        n_up = ww.n_up;
-        uint32_t q_head = ww.q_head, q_count = ww.q_count;
         if constexpr (TELSRC != TEL_CONST) {
             __syncwarp();
             const uint32_t nw = sm.wide_count[warp];
             if (nw) wide_batch<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, nw);
         }
         if (q_count) drain_queue<TELSRC, MODE>(P, sm, tile_first, q_head, q_count);
-        if constexpr (OUT) {
-            // records the last drain staged (the tile is still in rounds mode): one more flush
-            if (rounds) flush_round(P, out_smem(sm), false);
-        }
         flush_accumulator(P, sm);
     }
 

@@ -25,10 +25,12 @@ def n_threads() -> int:
 
 
 def gpu_run(cfg: dict, mode: int, want_records: bool = True, capacity_per_tel: int | None = None,
-            first_id: int = 0, host_segments: bool = False, chunks: int = 1):
+            first_id: int = 0, host_segments: bool = False, chunks: int = 1, with_ids: bool = True, region_shift: int = 0):
     """Run cfg through the CUDA path.  Returns dict(counts, tallies, counters, records, tel_count).
 
     records: structured array sorted by (id, tel) with the 7 record floats, the id and the telescope.
+    with_ids=False: no id side buffer is passed (the launch bench.py times); the records then come back in the order
+    of the regions, id = 0.  region_shift: every telescope region starts that many records later in the buffer.
     """
     import torch
 
@@ -48,11 +50,11 @@ def gpu_run(cfg: dict, mode: int, want_records: bool = True, capacity_per_tel: i
     d_rec = d_ids = None
     if mode == c8.MODE_OUTPUT:
         cap = int(capacity_per_tel if capacity_per_tel is not None else 1 << 20)
-        d_rec = torch.zeros((n_tel * cap, 7), dtype=torch.float32, device=dev)
-        d_ids = torch.zeros(n_tel * cap, dtype=torch.int64, device=dev)
-        d_off = torch.arange(n_tel, dtype=torch.int64, device=dev) * cap
+        d_rec = torch.zeros((n_tel * cap + region_shift, 7), dtype=torch.float32, device=dev)
+        d_ids = torch.zeros(n_tel * cap + region_shift, dtype=torch.int64, device=dev)
+        d_off = torch.arange(n_tel, dtype=torch.int64, device=dev) * cap + region_shift
         d_cap = torch.full((n_tel,), cap, dtype=torch.int64, device=dev)
-        kw.update(records=d_rec, tel_offset=d_off, tel_capacity=d_cap, ids=d_ids)
+        kw.update(records=d_rec, tel_offset=d_off, tel_capacity=d_cap, ids=d_ids if with_ids else None)
     if host_segments:
         h = torch.from_numpy(seg.view(np.uint8).reshape(n, 48).copy()).pin_memory()
         ctx.propagate_segments_host(h, par, n=n, first_segment_id=first_id, **kw)
@@ -75,14 +77,16 @@ def gpu_run(cfg: dict, mode: int, want_records: bool = True, capacity_per_tel: i
         for k in range(n_tel):
             m = int(tel_count[k])
             r = np.zeros(m, dtype=rec_dtype)
-            blk = h_rec[k * cap: k * cap + m]
+            blk = h_rec[region_shift + k * cap: region_shift + k * cap + m]
             for i, name in enumerate(("x", "y", "cx", "cy", "t", "lam", "w")):
                 r[name] = blk[:, i]
-            r["id"] = h_ids[k * cap: k * cap + m]
+            r["id"] = h_ids[region_shift + k * cap: region_shift + k * cap + m]
             r["tel"] = k
             parts.append(r)
         rec = np.concatenate(parts) if parts else np.zeros(0, dtype=rec_dtype)
-        out["records"] = rec[np.lexsort((rec["tel"], rec["id"]))]
+        out["records"] = rec[np.lexsort((rec["tel"], rec["id"]))] if with_ids else rec
+        if region_shift:
+            assert not h_rec[:region_shift].any(), "records written before the first region"
     ctx.close()
     return out
 

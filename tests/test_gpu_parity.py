@@ -190,6 +190,26 @@ def test_accept_all_output(c8):
     assert rep["matched"] == rep["hits_oracle"] >= 0.999 * (g["counters"]["generated"] - g["counters"]["upward"])
 
 
+@pytest.mark.parametrize("shift", [0, 1, 2, 3])
+def test_dense_output_without_ids_equals_with_ids(c8, shift):
+    """The launch bench.py times for the HBM roofline passes no id side buffer and takes the dense loop's fast path;
+    its records must be the same set, bit for bit, as those of the general path that the parity tests check by id.
+    The region starts 0..3 records into the buffer, so the 16-byte body of every block sees each alignment."""
+    import parity_util as pu
+    cfg = wl.make_config("c5g", n_segments=3000)
+    a = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=1 << 20, region_shift=shift)
+    b = pu.gpu_run(cfg, c8.MODE_OUTPUT, capacity_per_tel=1 << 20, with_ids=False, region_shift=shift)
+    assert a["counters"] == b["counters"] and len(a["records"]) == len(b["records"]) > 400_000
+    assert np.array_equal(a["tallies"]["hits"], b["tallies"]["hits"])
+    assert np.allclose(a["tallies"]["sum_w"], b["tallies"]["sum_w"], rtol=1e-6)
+    fields = ["x", "y", "cx", "cy", "t", "lam", "w"]
+    ra = np.stack([a["records"][f] for f in fields], axis=1).view(np.uint32)
+    rb = np.stack([b["records"][f] for f in fields], axis=1).view(np.uint32)
+    ra = ra[np.lexsort(ra.T[::-1])]
+    rb = rb[np.lexsort(rb.T[::-1])]
+    assert np.array_equal(ra, rb)
+
+
 def test_dense_hits_several_telescopes_misaligned_regions(c8):
     """Large overlapping spheres: most warp iterations are dense, the lanes of a warp hit different telescopes,
     a photon hits several; odd capacities make every region start off a 16-byte boundary."""
