@@ -111,7 +111,8 @@ size_t smem_bytes(int mode, bool staging = true, bool ids = true)
 {
     if (mode == c8::MODE_HIST) return sizeof(c8::TileSmem) + sizeof(c8::HistSmem);
     if (mode != c8::MODE_OUT || !staging) return sizeof(c8::TileSmem);
-    return sizeof(c8::TileSmem) + (ids ? sizeof(c8::OutSmem) : offsetof(c8::OutSmem, ids));
+    (void)ids;
+    return sizeof(c8::TileSmem) + sizeof(c8::OutSmem);
 }
 
 typedef void (*kernel_t)(const c8::KParams);

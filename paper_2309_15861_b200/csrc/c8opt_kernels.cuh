@@ -35,7 +35,8 @@ constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global m
 constexpr int kMaxLayers = 8;
 constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
 constexpr int kBlockRecs = 64;        // photon output, dense tiles: records a warp stages per trip of the dense loop (2 per lane)
-constexpr int kStageBufs = 3;         // staging buffers per warp (a block waits two trips for its slots, see walk_dense)
+constexpr int kStageBufs = 2;         // staging buffers per warp (a block waits for its slots while the next one is staged)
+constexpr int kSubMax = 2;            // trips per reservation round in the dense loop's fast path (1 in the general one)
 constexpr int kRoundSlots = 4;        // reservation rounds in flight per tile (power of two > the two a warp may lag)
 constexpr int kProbeDense = 32;       // candidates among the kTile sampled photons from which a tile takes the dense loop (12.5 %)
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
@@ -235,17 +236,17 @@ struct __align__(16) TileSmem {
 // reservation is a split arrive / wait without a block barrier (walk_dense): a warp adds its record count to agg[r & 3]
 // (bits 8.. = records so far = the warp's offset in the round, bits 0..7 = warps arrived); the last of the kWarps
 // arrivals bumps the cursor by the round's total and publishes the base in rbase[r & 3], rflag[r & 3] = r + 1; a warp
-// picks the base up two trips later and sends its block out with one bulk copy (shared -> global, TMA).
+// picks the base up after it has staged the next block and copies its block out with 16-byte vector stores.
 struct OutSmem {
     unsigned long long rbase[kRoundSlots];       // first record slot of round r in the dense telescope's region
     uint32_t agg[kRoundSlots];                   // see above
     uint32_t rflag[kRoundSlots];
     uint32_t probe[kTelConstMax];                // candidates per telescope among the sampled photons (probe_density)
-    // kStageBufs blocks per warp: block r is staged in buffer r % 3 while the bulk copies of blocks r - 1, r - 2 may
-    // still be reading theirs
-    __align__(16) float stage[kWarps][kStageBufs][kBlockRecs * kRecWords];
-    unsigned long long ids[kWarps][kStageBufs][kBlockRecs];     // last: not allocated when the caller wants no ids
+    // two blocks per warp: block r is staged in buffer r & 1 while block r - 1 waits for its slots.  The general path
+    // stages kBlockRecs records per block and keeps their ids (if the caller wants them) in the upper half of the buffer.
+    __align__(16) float stage[kWarps][kStageBufs][kSubMax * kBlockRecs * kRecWords];
 };
+static_assert(kSubMax >= 2 && sizeof(unsigned long long) * kBlockRecs <= sizeof(float) * (kSubMax - 1) * kBlockRecs * kRecWords, "id staging fits");
 
 __device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
 {
@@ -815,71 +816,70 @@ __device__ __forceinline__ void write_records_one_tel(const KParams &P, const Hi
     }
 }
 
-// Bulk asynchronous copy shared -> global (TMA, cp.async.bulk): 16-byte aligned addresses, size a multiple of 16.
-__device__ __forceinline__ void bulk_store(void *gdst, const void *ssrc, uint32_t bytes)
+// acquire load / release store / acq_rel add on shared memory, CTA scope (the reservation rounds of the dense loop)
+__device__ __forceinline__ uint32_t ld_acquire_cta(const uint32_t *p)
 {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                 :: "l"(gdst), "r"((uint32_t)__cvta_generic_to_shared(ssrc)), "r"(bytes) : "memory");
+    uint32_t v;
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
+    return v;
 }
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-// all but the N most recent bulk groups of this thread have finished READING their shared-memory source
-template <int N> __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory"); }
-template <int N> __device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" :: "n"(N) : "memory"); }
-// orders this thread's shared-memory writes before later async-proxy (bulk copy) reads of them
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-// Dense tiles: send the block of n records a warp staged in round r (words [0, 7 n) of staging buffer r % 3) to the
-// slots the round reserved for it, [base_r + off, base_r + off + n) of telescope kd's region.  Waits (lane 0 spins on
-// the flag in shared memory) until the last arrival of round r has published base_r; two trips of arithmetic lie
-// between the warp's own arrival and this call, so the wait is normally over.  Called by all 32 lanes, every round,
-// also with n == 0: the wait is what keeps a warp from running more than kRoundSlots - 1 rounds ahead of the others.
-//
-// 16-byte alignment: record slot s starts at word 7 s, so the words of a shared-memory slot and of a global slot are
-// in the same position within a 16-byte vector iff the two slot numbers agree modulo 4.  The order of the records
-// within a region is free (R22), so the block is rotated by rho = (-G) mod 4 slots, G = first global slot: staged
-// slot s goes to global slot G + rho + s, whose address is a multiple of 16 bytes for s = 0 -- the body leaves with
-// ONE bulk copy issued by lane 0 -- and the last rho (<= 3) staged records wrap around to global slots
-// G .. G + rho - 1 as scalar words, together with the <= 3 words the 16-byte body leaves over.
-template <bool IDS>
-__device__ __forceinline__ void copy_block(const KParams &P, OutSmem &os, const int kd, const uint32_t n, const uint32_t off,
-                                           const uint32_t r)
+__device__ __forceinline__ void st_release_cta(uint32_t *p, uint32_t v)
 {
-    const uint32_t lane = lane_id(), warp = threadIdx.x >> 5;
-    unsigned long long b = 0;
-    if (lane == 0u) {
-        volatile uint32_t *flag = &os.rflag[r & (kRoundSlots - 1)];
-        while (*flag != r + 1u) __nanosleep(64);
-        __threadfence_block();
-        b = *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)];
-    }
-    __syncwarp();
-    b = __shfl_sync(0xffffffffu, b, 0);
-    if (n == 0u) return;
-    const unsigned long long cap = P.tel_capacity[kd], first = b + off;
-    if (first >= cap) return;
+    asm volatile("st.release.cta.shared.u32 [%0], %1;" :: "r"((uint32_t)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t add_acq_rel_cta(uint32_t *p, uint32_t v)
+{
+    uint32_t old;
+    asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"((uint32_t)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+    return old;
+}
+
+// Dense tiles: copy the block of n records a warp staged in round r (words [0, 7 n) at st) to the slots the round
+// reserved for it, [base_r + off, base_r + off + n) of the dense telescope's region (cap records from global record
+// slot tel_off on).  Waits (every lane polls the flag in shared memory: a broadcast read, no divergence) until the
+// last arrival of round r has published base_r; a whole round of arithmetic lies between the warp's own arrival and
+// this call, so the wait is normally over.  Called by all 32 lanes, every round, also with n == 0: the wait is what
+// keeps a warp from running more than kRoundSlots - 1 rounds ahead of the others.
+//
+// 16-byte stores: record slot s starts at word 7 s, so the words of a shared-memory slot and of a global slot are in
+// the same position within a 16-byte vector iff the two slot numbers agree modulo 4.  The order of the records
+// within a region is free (R22), so the block is rotated by rho = (-G) mod 4 slots, G = first global slot: staged
+// slot s goes to global slot G + rho + s, whose address is a multiple of 16 bytes for s = 0 -- the body is copied as
+// aligned float4 vectors, 512 contiguous bytes per store instruction -- and the last rho (<= 3) staged records wrap
+// around to global slots G .. G + rho - 1 as scalar words, together with the <= 3 words the body leaves over.
+template <int SUB, bool IDS>
+__device__ __forceinline__ void copy_block(const KParams &P, OutSmem &os, const float *st, const unsigned long long cap,
+                                           const unsigned long long tel_off, const uint32_t n, const uint32_t off, const uint32_t r)
+{
+    const uint32_t lane = lane_id();
+    while (ld_acquire_cta(&os.rflag[r & (kRoundSlots - 1)]) != r + 1u) __nanosleep(100);
+    const unsigned long long first = *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)] + off;
+    if (n == 0u || first >= cap) return;
     const uint32_t m = (uint32_t)min((unsigned long long)n, cap - first);
-    const unsigned long long G = P.tel_offset[kd] + first;
-    const float *st = os.stage[warp][r % kStageBufs];
+    const unsigned long long G = tel_off + first;
     float *dst = P.records + G * (unsigned)kRecWords;
+    const unsigned long long *sid = reinterpret_cast<const unsigned long long *>(st + kBlockRecs * kRecWords);
     if ((reinterpret_cast<uintptr_t>(P.records) & 15u) == 0u) {
-        const uint32_t rho = min((0u - (uint32_t)G) & 3u, m), body = (m - rho) * kRecWords, nb16 = body & ~3u, rest = body & 3u;
-        if (lane == 0u && nb16) bulk_store(dst + rho * kRecWords, st, nb16 * 4u);
-        // lanes 0 .. 7 rho - 1: the wrapped records; the next `rest` lanes: the words the 16-byte body left over
+        const uint32_t rho = min((0u - (uint32_t)G) & 3u, m), body = (m - rho) * kRecWords, nvec = body >> 2, rest = body & 3u;
+        const float4 *src4 = reinterpret_cast<const float4 *>(st);
+        float4 *dst4 = reinterpret_cast<float4 *>(dst + rho * kRecWords);
+#pragma unroll
+        for (uint32_t v0 = 0; v0 < (uint32_t)(SUB * kBlockRecs * kRecWords) / 4u; v0 += 32u) {
+            const uint32_t v = v0 + lane;
+            if (v < nvec) __stcs(&dst4[v], src4[v]);
+        }
+        // lanes 0 .. 7 rho - 1: the wrapped records; the next `rest` lanes: the words the vectors left over
         const uint32_t nwrap = rho * kRecWords;
         if (lane < nwrap) dst[lane] = st[body + lane];
-        else if (lane < nwrap + rest) dst[nwrap + nb16 + (lane - nwrap)] = st[nb16 + (lane - nwrap)];
-        if constexpr (IDS) {
-            const unsigned long long *sid = os.ids[warp][r % kStageBufs];
+        else if (lane < nwrap + rest) dst[lane + (body - rest)] = st[lane - nwrap + (body - rest)];
+        if constexpr (IDS)
             for (uint32_t s = lane; s < m; s += 32u) P.ids[(s < m - rho) ? G + rho + s : G + s - (m - rho)] = sid[s];
-        }
     } else {
         const uint32_t nwords = m * kRecWords;
 #pragma unroll 4
         for (uint32_t i = lane; i < nwords; i += 32u) dst[i] = st[i];
-        if constexpr (IDS) {
-            const unsigned long long *sid = os.ids[warp][r % kStageBufs];
+        if constexpr (IDS)
             for (uint32_t s = lane; s < m; s += 32u) P.ids[G + s] = sid[s];
-        }
     }
 }
 
@@ -1476,25 +1476,28 @@ __device__ __noinline__ void probe_density(const KParams &P, TileSmem &sm, OutSm
 
 // The photon loop of a dense tile (photon output, brute-force kernels).  The pair loop of walk_pairs -- a lane takes
 // the adjacent slots g, g + 1 per trip, one Philox block for both (R20) -- with every candidate evaluated on the spot
-// from the values in registers, the records of the trip staged per warp (<= 64) and their slots reserved once per
-// tile and trip (OutSmem).  Per trip r:  arithmetic of trip r  ->  pick up the base of round r - 2 and send that block
-// out (copy_block: one bulk copy)  ->  stage block r  ->  arrive at round r.  The global atomic of a round, its latency
-// and the spread between the warps of the tile are thus covered by two trips of arithmetic, and there is no block
-// barrier.  Every warp of the tile runs all n_trips trips (it arrives with 0 records once its range is finished).
+// from the values in registers, the records of a round (SUB trips, <= 64 SUB records) staged per warp and their slots
+// reserved once per tile and round (OutSmem).  Per round r:  pick up the base of round r - 2 and copy that block out
+// (copy_block)  ->  arithmetic of round r, staged into the buffer that block left  ->  arrive at round r.  The global
+// atomic of a round, its latency and the spread between the warps of the tile are thus covered by a round of
+// arithmetic, and there is no block barrier.  Every warp of the tile runs all the rounds (it arrives with 0 records
+// once its range is finished).
 // kd = the tile's dense telescope; hits on other telescopes, further candidates of a photon and the generic kinds
 // take the paths of the sparse loop (queue / direct cursor bump).
 // FAST: one coplanar telescope, no refraction corrections, no transmission table, no id side buffer (the launch that
 // is measured against the HBM roofline): the exact evaluation of an axis-kind photon written out on the values the
-// loop holds, built from the same pieces as evaluate_pair (bit-identical records).
+// loop holds, built from the same pieces as evaluate_pair (bit-identical records), two trips per round.
 template <bool COPLANAR, int NT, bool REFR, bool FAST>
 __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSmem &os, const uint32_t base, const uint32_t hi,
                                            const unsigned long long tile_first, const uint32_t n_trips, const int kd,
                                            uint32_t &n_up_out, uint32_t &q_head, uint32_t &q_count)
 {
     constexpr int TELSRC = TEL_CONST;
+    constexpr uint32_t SUB = FAST ? (uint32_t)kSubMax : 1u;
     static_assert(!FAST || (NT == 1 && COPLANAR && !REFR), "fast path: one coplanar telescope, straight lines");
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5, lt = (1u << lane) - 1u;
     const bool want_ids = !FAST && P.ids != nullptr;
+    const unsigned long long cap_kd = P.tel_capacity[kd], off_kd = P.tel_offset[kd];
     uint32_t g = base + 2u * lane;
     int e;
     {
@@ -1507,192 +1510,209 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
     int kind = sm.kind[e];
     PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
     AxisFrame f = load_axis_frame(sm, e);
-    uint32_t n_1 = 0u, off_1 = 0u, n_2 = 0u, off_2 = 0u;      // the blocks staged one and two trips ago
-    // this thread's tally of hits on kd: fp32 partial sums over kTallyTrips trips (<= 2 kTallyTrips terms), then fp64
-    constexpr uint32_t kTallyTrips = 32u;
+    uint32_t n_1 = 0u, off_1 = 0u, n_2 = 0u, off_2 = 0u;      // the blocks staged one and two rounds ago
+    // this thread's tally of hits on kd: fp32 partial sums over kTallyRounds rounds (<= 4 kTallyRounds terms), then fp64
+    constexpr uint32_t kTallyRounds = 16u;
     uint32_t acc_n = 0u;
     float part_w = 0.0f, part_wt = 0.0f;
     double acc_w = 0.0, acc_wt = 0.0;
-    for (uint32_t r = 0; r < n_trips; ++r, g += 64u, j += 64u) {
-        const bool active = g < hi;
-        uint32_t cmA = 0u, cmB = 0u;
-        Hit hA, hB;
-        hA.ok = false; hB.ok = false;
-        if (active) {
-            if (g >= end) {
-                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
-                rend = end - sm.odd[e];
-                j = g - sm.prefix[e];
-                kind = sm.kind[e];
-                pe = philox_emitter(P, emitter_segment(P, tile_first, e));
-                f = load_axis_frame(sm, e);
-            }
-            const bool hasB = g + 1u < rend;                     // slot g + 1 is empty after an odd count
-            if (kind == KIND_CHER_AXIS) {
-                const Rand4 blk = philox_photon(P, pe, j >> 1, 0u);                               // a2: one block, two photons (R20; j is even)
-                // a3 / a4 as in walk_pairs, for both photons
-                const float w1A = one_two(blk.r0), w1B = one_two(blk.r2);
-                const float sdA = fmaf(w1A, f.negL, f.k0c), sdB = fmaf(w1B, f.negL, f.k0c);
-                float spA, cpA, spB, cpB;
-                __sincosf(fmaf(one_two(blk.r1), 6.2831853f, -9.42477760f), &spA, &cpA);
-                __sincosf(fmaf(one_two(blk.r3), 6.2831853f, -9.42477760f), &spB, &cpB);
-                const float vzA = fmaf(cpA, f.az, fmaf(spA, f.bz, f.cz)), vzB = fmaf(cpB, f.az, fmaf(spB, f.bz, f.cz));
-                const float rvA = rcp_approx(vzA), rvB = rcp_approx(vzB);
-                const float rhoA = sdA * rvA, rhoB = sdB * rvB;
-                const float gxA = fmaf(rhoA, fmaf(cpA, f.px, spA * f.qx), f.gx), gyA = fmaf(rhoA, fmaf(cpA, f.py, spA * f.qy), f.gy);
-                const float gxB = fmaf(rhoB, fmaf(cpB, f.px, spB * f.qx), f.gx), gyB = fmaf(rhoB, fmaf(cpB, f.py, spB * f.qy), f.gy);
-                const float *fr = &sm.frame[e * kFrameStride];
-                const float4 vc0 = *reinterpret_cast<const float4 *>(fr + F_AX);      // AX, AY, BX, BY
-                const float4 vc1 = *reinterpret_cast<const float4 *>(fr + F_CX);      // CX, CY, LEN, LAYER
-                const float4 hs = *reinterpret_cast<const float4 *>(fr + F_W0);       // W0, T0, IBC, DZ
-                const float vxA = fmaf(cpA, vc0.x, fmaf(spA, vc0.z, vc1.x)), vyA = fmaf(cpA, vc0.y, fmaf(spA, vc0.w, vc1.y));
-                const float vxB = fmaf(cpB, vc0.x, fmaf(spB, vc0.z, vc1.x)), vyB = fmaf(cpB, vc0.y, fmaf(spB, vc0.w, vc1.y));
-                if constexpr (FAST) {
-                    // evaluate_pair<TEL_CONST, true> for telescope 0, straight lines, no transmission table
-                    const float4 T = P.tel_c[0];
-                    const float telT = P.telT_c[0];
-                    const int li_frame = __float_as_int(vc1.w);
-                    {
-                        const float rv = fmaf(rvA, fmaf(-vzA, rvA, 1.0f), rvA), ez = -sdA * hs.w;
-                        float s_pl;
-                        hA.x = gxA - T.x; hA.y = gyA - T.y;
-                        const bool ok = axis_test_coplanar(hA.x, hA.y, vxA, vyA, ez, rv, T.w, &s_pl);
-                        if (!(vzA < 0.0f)) ++n_up;
-                        hA.ok = ok && (vzA < 0.0f);
-                        const float habs = P.z_ref_f + ez;
-                        float E;
-                        const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
-                        hA.t = arrival_time(P, (w1A - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
-                        hA.lam = cherenkov_lambda(P, cherenkov_u3(blk.r0, blk.r1));
-                        hA.vx = vxA; hA.vy = vyA; hA.w = hs.x;
-                    }
-                    if (hasB) {
-                        const float rv = fmaf(rvB, fmaf(-vzB, rvB, 1.0f), rvB), ez = -sdB * hs.w;
-                        float s_pl;
-                        hB.x = gxB - T.x; hB.y = gyB - T.y;
-                        const bool ok = axis_test_coplanar(hB.x, hB.y, vxB, vyB, ez, rv, T.w, &s_pl);
-                        if (!(vzB < 0.0f)) ++n_up;
-                        hB.ok = ok && (vzB < 0.0f);
-                        const float habs = P.z_ref_f + ez;
-                        float E;
-                        const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
-                        hB.t = arrival_time(P, (w1B - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
-                        hB.lam = cherenkov_lambda(P, cherenkov_u3(blk.r2, blk.r3));
-                        hB.vx = vxB; hB.vy = vyB; hB.w = hs.x;
+    const uint32_t n_rounds = (n_trips + SUB - 1u) / SUB;
+    for (uint32_t r = 0; r < n_rounds; ++r) {
+        float *const st = os.stage[warp][r & 1u];
+        unsigned long long *const sid = reinterpret_cast<unsigned long long *>(st + kBlockRecs * kRecWords);
+        // the block staged two rounds ago leaves this buffer (its slots have been reserved meanwhile)
+        if (r >= 2u) {
+            if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_2, off_2, r - 2u);
+            else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_2, off_2, r - 2u);
+        }
+        __syncwarp();
+        uint32_t cnt = 0u;                           // records staged in this round (warp-uniform)
+#pragma unroll
+        for (uint32_t t = 0; t < SUB; ++t, g += 64u, j += 64u) {
+            const bool active = g < hi;
+            uint32_t cmA = 0u, cmB = 0u;
+            Hit hA, hB;
+            hA.ok = false; hB.ok = false;
+            if (active) {
+                if (g >= end) {
+                    do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+                    rend = end - sm.odd[e];
+                    j = g - sm.prefix[e];
+                    kind = sm.kind[e];
+                    pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+                    f = load_axis_frame(sm, e);
+                }
+                const bool hasB = g + 1u < rend;                     // slot g + 1 is empty after an odd count
+                if (kind == KIND_CHER_AXIS) {
+                    const Rand4 blk = philox_photon(P, pe, j >> 1, 0u);                               // a2: one block, two photons (R20; j is even)
+                    // a3 / a4 as in walk_pairs, for both photons
+                    const float w1A = one_two(blk.r0), w1B = one_two(blk.r2);
+                    const float sdA = fmaf(w1A, f.negL, f.k0c), sdB = fmaf(w1B, f.negL, f.k0c);
+                    float spA, cpA, spB, cpB;
+                    __sincosf(fmaf(one_two(blk.r1), 6.2831853f, -9.42477760f), &spA, &cpA);
+                    __sincosf(fmaf(one_two(blk.r3), 6.2831853f, -9.42477760f), &spB, &cpB);
+                    const float vzA = fmaf(cpA, f.az, fmaf(spA, f.bz, f.cz)), vzB = fmaf(cpB, f.az, fmaf(spB, f.bz, f.cz));
+                    const float rvA = rcp_approx(vzA), rvB = rcp_approx(vzB);
+                    const float rhoA = sdA * rvA, rhoB = sdB * rvB;
+                    const float gxA = fmaf(rhoA, fmaf(cpA, f.px, spA * f.qx), f.gx), gyA = fmaf(rhoA, fmaf(cpA, f.py, spA * f.qy), f.gy);
+                    const float gxB = fmaf(rhoB, fmaf(cpB, f.px, spB * f.qx), f.gx), gyB = fmaf(rhoB, fmaf(cpB, f.py, spB * f.qy), f.gy);
+                    const float *fr = &sm.frame[e * kFrameStride];
+                    const float4 vc0 = *reinterpret_cast<const float4 *>(fr + F_AX);      // AX, AY, BX, BY
+                    const float4 vc1 = *reinterpret_cast<const float4 *>(fr + F_CX);      // CX, CY, LEN, LAYER
+                    const float4 hs = *reinterpret_cast<const float4 *>(fr + F_W0);       // W0, T0, IBC, DZ
+                    const float vxA = fmaf(cpA, vc0.x, fmaf(spA, vc0.z, vc1.x)), vyA = fmaf(cpA, vc0.y, fmaf(spA, vc0.w, vc1.y));
+                    const float vxB = fmaf(cpB, vc0.x, fmaf(spB, vc0.z, vc1.x)), vyB = fmaf(cpB, vc0.y, fmaf(spB, vc0.w, vc1.y));
+                    if constexpr (FAST) {
+                        // evaluate_pair<TEL_CONST, true> for telescope 0, straight lines, no transmission table
+                        const float4 T = P.tel_c[0];
+                        const float telT = P.telT_c[0];
+                        const int li_frame = __float_as_int(vc1.w);
+                        {
+                            const float rv = fmaf(rvA, fmaf(-vzA, rvA, 1.0f), rvA), ez = -sdA * hs.w;
+                            float s_pl;
+                            hA.x = gxA - T.x; hA.y = gyA - T.y;
+                            const bool ok = axis_test_coplanar(hA.x, hA.y, vxA, vyA, ez, rv, T.w, &s_pl);
+                            if (!(vzA < 0.0f)) ++n_up;
+                            hA.ok = ok && (vzA < 0.0f);
+                            const float habs = P.z_ref_f + ez;
+                            float E;
+                            const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
+                            hA.t = arrival_time(P, (w1A - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
+                            hA.lam = cherenkov_lambda(P, cherenkov_u3(blk.r0, blk.r1));
+                            hA.vx = vxA; hA.vy = vyA; hA.w = hs.x;
+                        }
+                        if (hasB) {
+                            const float rv = fmaf(rvB, fmaf(-vzB, rvB, 1.0f), rvB), ez = -sdB * hs.w;
+                            float s_pl;
+                            hB.x = gxB - T.x; hB.y = gyB - T.y;
+                            const bool ok = axis_test_coplanar(hB.x, hB.y, vxB, vyB, ez, rv, T.w, &s_pl);
+                            if (!(vzB < 0.0f)) ++n_up;
+                            hB.ok = ok && (vzB < 0.0f);
+                            const float habs = P.z_ref_f + ez;
+                            float E;
+                            const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
+                            hB.t = arrival_time(P, (w1B - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
+                            hB.lam = cherenkov_lambda(P, cherenkov_u3(blk.r2, blk.r3));
+                            hB.vx = vxB; hB.vy = vyB; hB.w = hs.x;
+                        }
+                    } else {
+                        // one telescope: the exact test decides; several: the conservative pre-tests pick the candidates
+                        uint2 cell;
+                        if (vzA < 0.0f) cmA = (NT == 1) ? 1u : plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxA, gyA, vxA, vyA, vzA, &cell); else ++n_up;
+                        if (hasB) {
+                            if (vzB < 0.0f) cmB = (NT == 1) ? 1u : plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cell); else ++n_up;
+                        }
+                        if (cmA != 0u) {
+                            Photon ph;
+                            ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(blk.r0, blk.r1);
+                            ph.vx = vxA; ph.vy = vyA; ph.vz = vzA; ph.gx = gxA; ph.gy = gyA; ph.rva = rvA;
+                            ph.s = (w1A - kOneMinus) * vc1.z; ph.ez = -sdA * hs.w;
+                            ph.ex = ph.ey = 0.0f;
+                            const int k = (NT == 1) ? 0 : __ffs(cmA) - 1;
+                            cmA &= cmA - 1u;
+                            hA = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
+                        }
+                        if (cmB != 0u) {
+                            Photon ph;
+                            ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(blk.r2, blk.r3);
+                            ph.vx = vxB; ph.vy = vyB; ph.vz = vzB; ph.gx = gxB; ph.gy = gyB; ph.rva = rvB;
+                            ph.s = (w1B - kOneMinus) * vc1.z; ph.ez = -sdB * hs.w;
+                            ph.ex = ph.ey = 0.0f;
+                            const int k = (NT == 1) ? 0 : __ffs(cmB) - 1;
+                            cmB &= cmB - 1u;
+                            hB = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
+                        }
                     }
                 } else {
-                    // one telescope: the exact test decides; several: the conservative pre-tests pick the candidates
-                    uint2 cell;
-                    if (vzA < 0.0f) cmA = (NT == 1) ? 1u : plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxA, gyA, vxA, vyA, vzA, &cell); else ++n_up;
+                    // generic kinds: out of line (photon in the global frame, pre-tests, exact test of the first candidate)
+                    const uint32_t tag = kind_tag(kind);
+                    const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
+                    const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u});
+                    hA = ga.h; cmA = ga.cm_left;
+                    if (ga.upward) ++n_up;
                     if (hasB) {
-                        if (vzB < 0.0f) cmB = (NT == 1) ? 1u : plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cell); else ++n_up;
-                    }
-                    if (cmA != 0u) {
-                        Photon ph;
-                        ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(blk.r0, blk.r1);
-                        ph.vx = vxA; ph.vy = vyA; ph.vz = vzA; ph.gx = gxA; ph.gy = gyA; ph.rva = rvA;
-                        ph.s = (w1A - kOneMinus) * vc1.z; ph.ez = -sdA * hs.w;
-                        ph.ex = ph.ey = 0.0f;
-                        const int k = (NT == 1) ? 0 : __ffs(cmA) - 1;
-                        cmA &= cmA - 1u;
-                        hA = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
-                    }
-                    if (cmB != 0u) {
-                        Photon ph;
-                        ph.axis = true; ph.tag = 0; ph.u3 = cherenkov_u3(blk.r2, blk.r3);
-                        ph.vx = vxB; ph.vy = vyB; ph.vz = vzB; ph.gx = gxB; ph.gy = gyB; ph.rva = rvB;
-                        ph.s = (w1B - kOneMinus) * vc1.z; ph.ez = -sdB * hs.w;
-                        ph.ex = ph.ey = 0.0f;
-                        const int k = (NT == 1) ? 0 : __ffs(cmB) - 1;
-                        cmB &= cmB - 1u;
-                        hB = evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
+                        const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u});
+                        hB = gb.h; cmB = gb.cm_left;
+                        if (gb.upward) ++n_up;
                     }
                 }
-            } else {
-                // generic kinds: out of line (photon in the global frame, pre-tests, exact test of the first candidate)
-                const uint32_t tag = kind_tag(kind);
-                const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
-                const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u});
-                hA = ga.h; cmA = ga.cm_left;
-                if (ga.upward) ++n_up;
-                if (hasB) {
-                    const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u});
-                    hB = gb.h; cmB = gb.cm_left;
-                    if (gb.upward) ++n_up;
+            }
+            unsigned long long idA = 0ull;
+            if (want_ids) idA = (emitter_segment(P, tile_first, e) << 25) | ((unsigned long long)kind_tag(kind) << 24) | (unsigned long long)j;
+            bool sA = hA.ok, sB = hB.ok;
+            if constexpr (NT > 1) {
+                // hits on another telescope than the tile's dense one: tallied and written directly
+                const bool oA = hA.ok && hA.k != kd, oB = hB.ok && hB.k != kd;
+                if (__any_sync(0xffffffffu, oA || oB)) {
+                    if (!want_ids) idA = (emitter_segment(P, tile_first, e) << 25) | ((unsigned long long)kind_tag(kind) << 24) | (unsigned long long)j;
+                    Hit h2 = hA; h2.ok = oA;
+                    commit_hits<MODE_OUT>(P, sm, h2, idA);
+                    h2 = hB; h2.ok = oB;
+                    commit_hits<MODE_OUT>(P, sm, h2, idA + 1ull);
+                }
+                sA = hA.ok && !oA; sB = hB.ok && !oB;
+            }
+            if constexpr (!FAST) {
+                // further candidates of the two photons (several telescopes; flat photons of the generic kinds): queue
+                if (__any_sync(0xffffffffu, (cmA | cmB) != 0u)) {
+                    push_candidates<TELSRC, MODE_OUT>(P, sm, tile_first, q_head, q_count, cmA, e, j, [&](int c) { return (uint32_t)c; });
+                    push_candidates<TELSRC, MODE_OUT>(P, sm, tile_first, q_head, q_count, cmB, e, j + 1u, [&](int c) { return (uint32_t)c; });
                 }
             }
-        }
-        unsigned long long idA = 0ull;
-        if (want_ids) idA = (emitter_segment(P, tile_first, e) << 25) | ((unsigned long long)kind_tag(kind) << 24) | (unsigned long long)j;
-        bool sA = hA.ok, sB = hB.ok;
-        if constexpr (NT > 1) {
-            // hits on another telescope than the tile's dense one: tallied and written directly
-            const bool oA = hA.ok && hA.k != kd, oB = hB.ok && hB.k != kd;
-            if (__any_sync(0xffffffffu, oA || oB)) {
-                if (!want_ids) idA = (emitter_segment(P, tile_first, e) << 25) | ((unsigned long long)kind_tag(kind) << 24) | (unsigned long long)j;
-                Hit t = hA; t.ok = oA;
-                commit_hits<MODE_OUT>(P, sm, t, idA);
-                t = hB; t.ok = oB;
-                commit_hits<MODE_OUT>(P, sm, t, idA + 1ull);
+            {
+                // (a miss leaves t undefined: select the product, not the factor)
+                const float wA = sA ? hA.w : 0.0f, wB = sB ? hB.w : 0.0f;
+                part_w += wA + wB;
+                part_wt += (sA ? hA.w * hA.t : 0.0f) + (sB ? hB.w * hB.t : 0.0f);
             }
-            sA = hA.ok && !oA; sB = hB.ok && !oB;
+            const uint32_t mA = __ballot_sync(0xffffffffu, sA), mB = __ballot_sync(0xffffffffu, sB);
+            const uint32_t nA = (uint32_t)__popc(mA);
+            if (sA) {
+                const uint32_t s = cnt + (uint32_t)__popc(mA & lt);
+                float *rec = st + s * kRecWords;
+                rec[0] = hA.x; rec[1] = hA.y; rec[2] = hA.vx; rec[3] = hA.vy; rec[4] = hA.t; rec[5] = hA.lam; rec[6] = hA.w;
+                if (want_ids) sid[s] = idA;
+            }
+            if (sB) {
+                const uint32_t s = cnt + nA + (uint32_t)__popc(mB & lt);
+                float *rec = st + s * kRecWords;
+                rec[0] = hB.x; rec[1] = hB.y; rec[2] = hB.vx; rec[3] = hB.vy; rec[4] = hB.t; rec[5] = hB.lam; rec[6] = hB.w;
+                if (want_ids) sid[s] = idA + 1ull;
+            }
+            cnt += nA + (uint32_t)__popc(mB);
         }
-        // further candidates of the two photons (several telescopes; flat photons of the generic kinds): queue
-        if (__any_sync(0xffffffffu, (cmA | cmB) != 0u)) {
-            push_candidates<TELSRC, MODE_OUT>(P, sm, tile_first, q_head, q_count, cmA, e, j, [&](int c) { return (uint32_t)c; });
-            push_candidates<TELSRC, MODE_OUT>(P, sm, tile_first, q_head, q_count, cmB, e, j + 1u, [&](int c) { return (uint32_t)c; });
-        }
-        if (sA) { part_w += hA.w; part_wt = fmaf(hA.w, hA.t, part_wt); }
-        if (sB) { part_w += hB.w; part_wt = fmaf(hB.w, hB.t, part_wt); }
-        if ((r & (kTallyTrips - 1u)) == kTallyTrips - 1u) { acc_w += (double)part_w; acc_wt += (double)part_wt; part_w = 0.0f; part_wt = 0.0f; }
-        // the block staged two trips ago leaves (its slots have been reserved meanwhile); lane 0 then makes sure the
-        // bulk copy issued in the previous trip has read its buffer, which is the one this trip stages into
-        if (r >= 2u) { if (want_ids) copy_block<true>(P, os, kd, n_2, off_2, r - 2u); else copy_block<false>(P, os, kd, n_2, off_2, r - 2u); }
-        if (lane == 0u) { bulk_commit(); bulk_wait_read<1>(); }
-        __syncwarp();
-        float *const st = os.stage[warp][r % kStageBufs];
-        const uint32_t mA = __ballot_sync(0xffffffffu, sA), mB = __ballot_sync(0xffffffffu, sB);
-        const uint32_t nA = (uint32_t)__popc(mA), n_w = nA + (uint32_t)__popc(mB);
-        acc_n += n_w;                               // warp-uniform: lane 0's copy is the one that counts
-        if (sA) {
-            const uint32_t s = (uint32_t)__popc(mA & lt);
-            float *rec = st + s * kRecWords;
-            rec[0] = hA.x; rec[1] = hA.y; rec[2] = hA.vx; rec[3] = hA.vy; rec[4] = hA.t; rec[5] = hA.lam; rec[6] = hA.w;
-            if (want_ids) os.ids[warp][r % kStageBufs][s] = idA;
-        }
-        if (sB) {
-            const uint32_t s = nA + (uint32_t)__popc(mB & lt);
-            float *rec = st + s * kRecWords;
-            rec[0] = hB.x; rec[1] = hB.y; rec[2] = hB.vx; rec[3] = hB.vy; rec[4] = hB.t; rec[5] = hB.lam; rec[6] = hB.w;
-            if (want_ids) os.ids[warp][r % kStageBufs][s] = idA + 1ull;
-        }
-        fence_proxy_async();
+        acc_n += cnt;                               // warp-uniform: lane 0's copy is the one that counts
+        if ((r & (kTallyRounds - 1u)) == kTallyRounds - 1u) { acc_w += (double)part_w; acc_wt += (double)part_wt; part_w = 0.0f; part_wt = 0.0f; }
         __syncwarp();
         uint32_t old = 0u;
         if (lane == 0u) {
-            __threadfence_block();
-            old = atomicAdd(&os.agg[r & (kRoundSlots - 1)], (n_w << 8) | 1u);
+            old = add_acq_rel_cta(&os.agg[r & (kRoundSlots - 1)], (cnt << 8) | 1u);
             if ((old & 0xffu) == (uint32_t)kWarps - 1u) {
                 // last arrival of round r: reserve the round's records, publish the base
-                const uint32_t total = (old >> 8) + n_w;
+                const uint32_t total = (old >> 8) + cnt;
                 os.agg[r & (kRoundSlots - 1)] = 0u;
                 unsigned long long b = 0ull;
                 if (total) b = atomicAdd(&P.cursors[kd], (unsigned long long)total);
                 *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)] = b;
-                __threadfence_block();
-                *(volatile uint32_t *)&os.rflag[r & (kRoundSlots - 1)] = r + 1u;
+                st_release_cta(&os.rflag[r & (kRoundSlots - 1)], r + 1u);
             }
         }
         __syncwarp();
         n_2 = n_1; off_2 = off_1;
         off_1 = __shfl_sync(0xffffffffu, old >> 8, 0);
-        n_1 = n_w;
+        n_1 = cnt;
     }
     // the last two blocks
-    if (n_trips >= 2u) { if (want_ids) copy_block<true>(P, os, kd, n_2, off_2, n_trips - 2u); else copy_block<false>(P, os, kd, n_2, off_2, n_trips - 2u); }
-    if (n_trips >= 1u) { if (want_ids) copy_block<true>(P, os, kd, n_1, off_1, n_trips - 1u); else copy_block<false>(P, os, kd, n_1, off_1, n_trips - 1u); }
-    if (lane == 0u) { bulk_commit(); bulk_wait<0>(); }
-    __syncwarp();
+    if (n_rounds >= 2u) {
+        const float *st = os.stage[warp][n_rounds & 1u];
+        if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_2, off_2, n_rounds - 2u);
+        else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_2, off_2, n_rounds - 2u);
+    }
+    if (n_rounds >= 1u) {
+        const float *st = os.stage[warp][(n_rounds - 1u) & 1u];
+        if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_1, off_1, n_rounds - 1u);
+        else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_1, off_1, n_rounds - 1u);
+    }
     // the warp's tally of kd into the tile's: one shared-memory atomic per warp and sum
     acc_w += (double)part_w; acc_wt += (double)part_wt;
 #pragma unroll
