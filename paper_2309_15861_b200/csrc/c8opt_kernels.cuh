@@ -35,9 +35,13 @@ constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global m
 constexpr int kMaxLayers = 8;
 constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
 constexpr int kBlockRecs = 64;        // photon output, dense tiles: records a warp stages per trip of the dense loop (2 per lane)
-constexpr int kStageBufs = 2;         // staging buffers per warp (a block waits for its slots while the next one is staged)
-constexpr int kSubMax = 2;            // trips per reservation round in the dense loop's fast path (1 in the general one)
-constexpr int kRoundSlots = 4;        // reservation rounds in flight per tile (power of two > the two a warp may lag)
+constexpr int kWarpStageWords = 2 * 2 * 64 * 7;   // floats of staging per warp: NB buffers of SUB trips x 64 records (dense loop)
+#ifndef C8_FAST_BUFS
+#define C8_FAST_BUFS 2
+#define C8_FAST_SUB 2
+#endif
+constexpr int kFastBufs = C8_FAST_BUFS, kFastSub = C8_FAST_SUB;   // the fast path's split of it: buffers, trips per reservation round
+constexpr int kRoundSlots = 8;        // reservation rounds in flight per tile (power of two > the buffers a warp may lag)
 constexpr int kProbeDense = 32;       // candidates among the kTile sampled photons from which a tile takes the dense loop (12.5 %)
 constexpr int kDenseMin = 16;         // candidates in one warp iteration from which they are evaluated on the spot
 constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-kind photons (warp load balance)
@@ -235,18 +239,20 @@ struct __align__(16) TileSmem {
 // serialise in L2 (~1 per clock), so the cursor of a telescope must not be bumped once per warp and trip.  The
 // reservation is a split arrive / wait without a block barrier (walk_dense): a warp adds its record count to agg[r & 3]
 // (bits 8.. = records so far = the warp's offset in the round, bits 0..7 = warps arrived); the last of the kWarps
-// arrivals bumps the cursor by the round's total and publishes the base in rbase[r & 3], rflag[r & 3] = r + 1; a warp
-// picks the base up after it has staged the next block and copies its block out with 16-byte vector stores.
+// arrivals bumps the cursor by the round's total, publishes the base in rbase[r & 7] and arrives at the mbarrier
+// rbar[r & 7]; a warp picks the base up after it has staged the next block (mbarrier try_wait: the hardware parks the
+// warp, no polling instructions) and copies its block out with 16-byte vector stores.
 struct OutSmem {
     unsigned long long rbase[kRoundSlots];       // first record slot of round r in the dense telescope's region
+    unsigned long long rbar[kRoundSlots];        // mbarrier (1 arrival): phase r / kRoundSlots completes when rbase[r % kRoundSlots] is round r's
     uint32_t agg[kRoundSlots];                   // see above
-    uint32_t rflag[kRoundSlots];
     uint32_t probe[kTelConstMax];                // candidates per telescope among the sampled photons (probe_density)
-    // two blocks per warp: block r is staged in buffer r & 1 while block r - 1 waits for its slots.  The general path
-    // stages kBlockRecs records per block and keeps their ids (if the caller wants them) in the upper half of the buffer.
-    __align__(16) float stage[kWarps][kStageBufs][kSubMax * kBlockRecs * kRecWords];
+    // NB buffers per warp: block r is staged in buffer r % NB while the blocks r - 1 .. r - NB + 1 wait for their slots.
+    // The general path uses two buffers of kBlockRecs records and keeps their ids (if the caller wants them) behind them.
+    __align__(16) float stage[kWarps][kWarpStageWords];
 };
-static_assert(kSubMax >= 2 && sizeof(unsigned long long) * kBlockRecs <= sizeof(float) * (kSubMax - 1) * kBlockRecs * kRecWords, "id staging fits");
+static_assert(kFastBufs * kFastSub * kBlockRecs * kRecWords <= kWarpStageWords, "fast-path staging fits");
+static_assert(2 * (kBlockRecs * kRecWords + 2 * kBlockRecs) <= kWarpStageWords, "general-path staging with ids fits");
 
 __device__ __forceinline__ OutSmem &out_smem(TileSmem &sm)
 {
@@ -277,12 +283,13 @@ __device__ __forceinline__ HistSmem &hist_smem(TileSmem &sm) { return *reinterpr
 //   F_A0..C2 (7..15): v = sth (cos' A + sin' B) + cth C.
 // Hit-only slots (all kinds): F_W0 weight, F_T0 start time, F_IBC 1/(beta c), and for the axis kind
 //   F_DZ, F_AX..F_CY (v_x, v_y coefficients), F_LEN; F_LAYER = bits of the int index of the atmosphere layer that
-//   holds the whole segment, -1 if it crosses a layer boundary; F_OMC = 1 - cos(half-angle) of a beamed emitter's cone.
+//   holds the lower end of the segment, F_HNEXT = lower bound of the next layer if the segment reaches into it (else
+//   +inf), F_LAYER = -1 if it spans more than two layers; F_OMC = 1 - cos(half-angle) of a beamed emitter's cone.
 enum {
     F_NEGL = 0, F_K0C = 1, F_AZ = 2, F_BZ = 3, F_CZ = 4, F_PX = 5, F_PY = 6, F_QX = 7, F_QY = 8, F_GX = 9, F_GY = 10,
     F_E0 = 0, F_D0 = 3, F_L = 6, F_A0 = 7, F_B0 = 10, F_C0 = 13,
     F_W0 = 16, F_T0 = 17, F_IBC = 18, F_DZ = 19, F_AX = 20, F_AY = 21, F_BX = 22, F_BY = 23, F_CX = 24, F_CY = 25,
-    F_LEN = 26, F_LAYER = 27, F_OMC = 28
+    F_LEN = 26, F_LAYER = 27, F_OMC = 28, F_HNEXT = 29
 };
 
 // ------------------------------------------------------------------------------------
@@ -457,7 +464,8 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
         const float zlo = fminf(za, zb) - 1.0f, zhi = fmaxf(za, zb) + 1.0f;
         int la = 0, lb = 0;
         for (int i = 1; i < P.n_layers; ++i) { if (zlo >= P.layerf[i].h_lo) la = i; if (zhi >= P.layerf[i].h_lo) lb = i; }
-        fr[F_LAYER] = __int_as_float(la == lb ? la : -1);
+        fr[F_LAYER] = __int_as_float(lb - la <= 1 ? la : -1);
+        fr[F_HNEXT] = (lb == la + 1) ? P.layerf[lb].h_lo : __int_as_float(0x7f800000);
     }
     *kind_out = (uint8_t)kind;
     const double e0[3] = { p0[0] - P.x_ref, p0[1] - P.y_ref, p0[2] - P.z_ref };
@@ -610,12 +618,12 @@ __device__ __forceinline__ float ex2_approx(float x)
 // an explicit fmaf, so that both callers compile to the same arithmetic and a photon's record does not depend on the
 // path that produced it.
 //
-// Index of the atmosphere layer at altitude habs: from the frame when the whole segment lies in one layer, else looked
-// up (unused layers carry h_lo = +inf, so the count is the index).
-__device__ __forceinline__ int emission_layer(const KParams &P, int li_frame, float habs)
+// Index of the atmosphere layer at altitude habs: from the frame when the segment lies in one layer or two adjacent
+// ones (the second from h_next on), else looked up (unused layers carry h_lo = +inf, so the count is the index).
+__device__ __forceinline__ int emission_layer(const KParams &P, int li_frame, float h_next, float habs)
 {
-    int li = li_frame;
-    if (li < 0) {
+    int li = li_frame + ((habs >= h_next) ? 1 : 0);
+    if (li_frame < 0) {
         li = 0;
 #pragma unroll
         for (int i = 1; i < kMaxLayers; ++i) li += (habs >= P.layerf[i].h_lo) ? 1 : 0;
@@ -671,7 +679,7 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     // layers carry h_lo = +inf, so the count is the index).
     float Te, eta_e;
     auto atmosphere_at_emission = [&]() {
-        const LayerF lf = P.layerf[emission_layer(P, __float_as_int(fr[F_LAYER]), habs)];
+        const LayerF lf = P.layerf[emission_layer(P, __float_as_int(fr[F_LAYER]), fr[F_HNEXT], habs)];
         float E;
         Te = depth_at(lf, habs, &E);
         eta_e = P.kappa_m * lf.b * (lf.k2 * 0.693147181f) * E;   // eta0 rho(h) / rho0, rho = (b / c) exp(-h / c) / 100
@@ -816,16 +824,25 @@ __device__ __forceinline__ void write_records_one_tel(const KParams &P, const Hi
     }
 }
 
-// acquire load / release store / acq_rel add on shared memory, CTA scope (the reservation rounds of the dense loop)
-__device__ __forceinline__ uint32_t ld_acquire_cta(const uint32_t *p)
+// mbarrier and acq_rel add on shared memory, CTA scope (the reservation rounds of the dense loop)
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, uint32_t count)
 {
-    uint32_t v;
-    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
-    return v;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void st_release_cta(uint32_t *p, uint32_t v)
+__device__ __forceinline__ void mbar_arrive_release(unsigned long long *bar)
 {
-    asm volatile("st.release.cta.shared.u32 [%0], %1;" :: "r"((uint32_t)__cvta_generic_to_shared(p)), "r"(v) : "memory");
+    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" :: "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
+// wait until the phase of the given parity has completed (acquire); the hardware suspends the thread between tries
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n"
+        "}\n" :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
 }
 __device__ __forceinline__ uint32_t add_acq_rel_cta(uint32_t *p, uint32_t v)
 {
@@ -852,13 +869,13 @@ __device__ __forceinline__ void copy_block(const KParams &P, OutSmem &os, const 
                                            const unsigned long long tel_off, const uint32_t n, const uint32_t off, const uint32_t r)
 {
     const uint32_t lane = lane_id();
-    while (ld_acquire_cta(&os.rflag[r & (kRoundSlots - 1)]) != r + 1u) __nanosleep(100);
+    mbar_wait(&os.rbar[r & (kRoundSlots - 1)], (r / (uint32_t)kRoundSlots) & 1u);
     const unsigned long long first = *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)] + off;
     if (n == 0u || first >= cap) return;
     const uint32_t m = (uint32_t)min((unsigned long long)n, cap - first);
     const unsigned long long G = tel_off + first;
     float *dst = P.records + G * (unsigned)kRecWords;
-    const unsigned long long *sid = reinterpret_cast<const unsigned long long *>(st + kBlockRecs * kRecWords);
+    const unsigned long long *sid = reinterpret_cast<const unsigned long long *>(st + kBlockRecs * kRecWords);   // general path
     if ((reinterpret_cast<uintptr_t>(P.records) & 15u) == 0u) {
         const uint32_t rho = min((0u - (uint32_t)G) & 3u, m), body = (m - rho) * kRecWords, nvec = body >> 2, rest = body & 3u;
         const float4 *src4 = reinterpret_cast<const float4 *>(st);
@@ -1493,7 +1510,8 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                                            uint32_t &n_up_out, uint32_t &q_head, uint32_t &q_count)
 {
     constexpr int TELSRC = TEL_CONST;
-    constexpr uint32_t SUB = FAST ? (uint32_t)kSubMax : 1u;
+    constexpr uint32_t SUB = FAST ? (uint32_t)kFastSub : 1u, NB = FAST ? (uint32_t)kFastBufs : 2u;
+    constexpr uint32_t kBufWords = (uint32_t)kWarpStageWords / NB;
     static_assert(!FAST || (NT == 1 && COPLANAR && !REFR), "fast path: one coplanar telescope, straight lines");
     const uint32_t lane = lane_id(), warp = threadIdx.x >> 5, lt = (1u << lane) - 1u;
     const bool want_ids = !FAST && P.ids != nullptr;
@@ -1510,7 +1528,9 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
     int kind = sm.kind[e];
     PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
     AxisFrame f = load_axis_frame(sm, e);
-    uint32_t n_1 = 0u, off_1 = 0u, n_2 = 0u, off_2 = 0u;      // the blocks staged one and two rounds ago
+    uint32_t n_h[NB], off_h[NB];                    // the blocks staged 1 .. NB rounds ago: records, offset in their round
+#pragma unroll
+    for (uint32_t i = 0; i < NB; ++i) { n_h[i] = 0u; off_h[i] = 0u; }
     // this thread's tally of hits on kd: fp32 partial sums over kTallyRounds rounds (<= 4 kTallyRounds terms), then fp64
     constexpr uint32_t kTallyRounds = 16u;
     uint32_t acc_n = 0u;
@@ -1518,12 +1538,12 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
     double acc_w = 0.0, acc_wt = 0.0;
     const uint32_t n_rounds = (n_trips + SUB - 1u) / SUB;
     for (uint32_t r = 0; r < n_rounds; ++r) {
-        float *const st = os.stage[warp][r & 1u];
+        float *const st = os.stage[warp] + (r % NB) * kBufWords;
         unsigned long long *const sid = reinterpret_cast<unsigned long long *>(st + kBlockRecs * kRecWords);
-        // the block staged two rounds ago leaves this buffer (its slots have been reserved meanwhile)
-        if (r >= 2u) {
-            if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_2, off_2, r - 2u);
-            else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_2, off_2, r - 2u);
+        // the block staged NB rounds ago leaves this buffer (its slots have been reserved meanwhile)
+        if (r >= NB) {
+            if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_h[NB - 1], off_h[NB - 1], r - NB);
+            else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_h[NB - 1], off_h[NB - 1], r - NB);
         }
         __syncwarp();
         uint32_t cnt = 0u;                           // records staged in this round (warp-uniform)
@@ -1567,6 +1587,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                         const float4 T = P.tel_c[0];
                         const float telT = P.telT_c[0];
                         const int li_frame = __float_as_int(vc1.w);
+                        const float h_next = fr[F_HNEXT];
                         {
                             const float rv = fmaf(rvA, fmaf(-vzA, rvA, 1.0f), rvA), ez = -sdA * hs.w;
                             float s_pl;
@@ -1576,7 +1597,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                             hA.ok = ok && (vzA < 0.0f);
                             const float habs = P.z_ref_f + ez;
                             float E;
-                            const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
+                            const float Te = depth_at(P.layerf[emission_layer(P, li_frame, h_next, habs)], habs, &E);
                             hA.t = arrival_time(P, (w1A - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
                             hA.lam = cherenkov_lambda(P, cherenkov_u3(blk.r0, blk.r1));
                             hA.vx = vxA; hA.vy = vyA; hA.w = hs.x;
@@ -1590,7 +1611,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                             hB.ok = ok && (vzB < 0.0f);
                             const float habs = P.z_ref_f + ez;
                             float E;
-                            const float Te = depth_at(P.layerf[emission_layer(P, li_frame, habs)], habs, &E);
+                            const float Te = depth_at(P.layerf[emission_layer(P, li_frame, h_next, habs)], habs, &E);
                             hB.t = arrival_time(P, (w1B - kOneMinus) * vc1.z, hs.z, hs.y, s_pl, telT, Te, rv);
                             hB.lam = cherenkov_lambda(P, cherenkov_u3(blk.r2, blk.r3));
                             hB.vx = vxB; hB.vy = vyB; hB.w = hs.x;
@@ -1694,24 +1715,24 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                 unsigned long long b = 0ull;
                 if (total) b = atomicAdd(&P.cursors[kd], (unsigned long long)total);
                 *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)] = b;
-                st_release_cta(&os.rflag[r & (kRoundSlots - 1)], r + 1u);
+                mbar_arrive_release(&os.rbar[r & (kRoundSlots - 1)]);
             }
         }
         __syncwarp();
-        n_2 = n_1; off_2 = off_1;
-        off_1 = __shfl_sync(0xffffffffu, old >> 8, 0);
-        n_1 = cnt;
+#pragma unroll
+        for (uint32_t i = NB - 1u; i > 0u; --i) { n_h[i] = n_h[i - 1u]; off_h[i] = off_h[i - 1u]; }
+        off_h[0] = __shfl_sync(0xffffffffu, old >> 8, 0);
+        n_h[0] = cnt;
     }
-    // the last two blocks
-    if (n_rounds >= 2u) {
-        const float *st = os.stage[warp][n_rounds & 1u];
-        if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_2, off_2, n_rounds - 2u);
-        else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_2, off_2, n_rounds - 2u);
-    }
-    if (n_rounds >= 1u) {
-        const float *st = os.stage[warp][(n_rounds - 1u) & 1u];
-        if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_1, off_1, n_rounds - 1u);
-        else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_1, off_1, n_rounds - 1u);
+    // the last NB blocks, oldest first
+#pragma unroll
+    for (uint32_t i = NB; i > 0u; --i) {
+        if (n_rounds >= i) {
+            const uint32_t r = n_rounds - i;
+            const float *st = os.stage[warp] + (r % NB) * kBufWords;
+            if (want_ids) copy_block<SUB, true>(P, os, st, cap_kd, off_kd, n_h[i - 1u], off_h[i - 1u], r);
+            else copy_block<SUB, false>(P, os, st, cap_kd, off_kd, n_h[i - 1u], off_h[i - 1u], r);
+        }
     }
     // the warp's tally of kd into the tile's: one shared-memory atomic per warp and sum
     acc_w += (double)part_w; acc_wt += (double)part_wt;
@@ -1742,7 +1763,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     constexpr bool OUT = (MODE == MODE_OUT);
     if constexpr (OUT && TELSRC == TEL_CONST) {
         OutSmem &os = out_smem(sm);
-        if (tid < kRoundSlots) { os.agg[tid] = 0u; os.rflag[tid] = 0u; os.rbase[tid] = 0ull; }
+        if (tid < kRoundSlots) { os.agg[tid] = 0u; os.rbase[tid] = 0ull; mbar_init(&os.rbar[tid], 1u); }
         if (tid < kTelConstMax) os.probe[tid] = 0u;
     }
     if constexpr (MODE == MODE_HIST) {
