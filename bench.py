@@ -28,19 +28,58 @@ import workloads as wl  # noqa: E402
 
 METRIC = "photons generated+propagated per second"
 UNIT = "photons/s"
-# algorithmic thread-instructions per photon: Philox 42 per block -- one block per
-# fluorescence photon, one per TWO Cherenkov photons (R20) -- + uniforms/generation/projection 40 + 6 per telescope
-# tested + loop 10
-ALG_INSTR = {"c1": 77.0, "c2": 101.0, "c5": 101.0, "c3a": 110.0, "c3b": 120.0, "c4": 110.0}
 RECORD_BYTES = 28.0
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from the round's `ncu --set full` captures under
-# profiles/, per 10^6 segments (they scale with the segment count); None = not captured for this workload.
-NCU_TRAFFIC_PER_1E6_SEGMENTS = {
-    ("c2", "tally"): 48.07e6,        # profiles/ncu_c2_tally_r01.md: the 48 MB segment table once
-    ("c4", "tally"): 99.13e6,        # profiles/ncu_c4_tally_r01.md: two passes over the segment table + 2.4 MB of spills
-    ("c5g", "output"): 5.084e9,      # profiles/ncu_c5g_output_r01.md: 5.035 GB written + 49.7 MB read
-    ("c2", "hist"): 48.11e6,         # profiles/ncu_c2_groundhist_r01.md
+SEGMENT_BYTES = 48.0
+
+# Algorithmic thread-instructions per photon (DESIGN.md section 7 has the same table, row by row): what the method must do for
+# one photon in SASS-level operations, NOT what the kernel executes (ncu's executed count is reported in profiles/).
+ALG_PARTS = {
+    "philox_block": 42.0,       # Philox4x32-10, S-halves of rounds 1-2 hoisted: 18 IMAD.WIDE + 18 LOP3 + 6
+    "uniform": 2.0,             # per uniform: SHF + LOP3 (mantissa stuffing)
+    "azimuth": 6.0,             # K0 - u1 L, phi, range scale, 2 MUFU (sin, cos)
+    "project": 12.0,            # v_z, 1/v_z (MUFU.RCP), rho, N, plane crossing, sign test
+    "pretest_per_tel": 6.0,     # 2 FADD + 2 FFMA/FMUL + FSETP + mask LOP per constant-bank telescope
+    "grid_lookup": 15.0,        # cell index, bounds test, 8-byte load, first pre-test (100-telescope array)
+    "generic_photon": 34.0,     # fluorescence / generic kinds: emission point, sincospi polynomial, polar angle, direction
+    "walk": 14.0,               # index walk, emitter-crossing test, loop
+    "queue": 4.0,               # candidate ballot / queue test
+    "exact_per_hit": 250.0,     # regenerate + exact test + time + wavelength + weight + commit, per (photon, telescope) hit
+    "preamble_per_emitter": 1200.0,   # fp64 preamble of one (segment, process)
+    "record_per_hit": 90.0,     # photon output, dense tiles: exact test, arrival time, wavelength, 7-word record staging
+    "hist_per_bunch": 92.0,     # ground histogram: v_x, v_y, arrival time, wavelength, radius, bin, 3 shared atomics
 }
+
+
+def alg_instr_per_photon(name: str, photons: float, emitters: float, hits: float, n_tel: int, ground_hist: bool = False) -> dict:
+    """Algorithmic instructions per photon of workload `name`, from ALG_PARTS and the measured counts of the run
+    (photons, emitters = (segment, process) pairs with a preamble, hits).  Returns the parts and their sum."""
+    P = ALG_PARTS
+    fluor = name in ("c3a", "c3b")
+    parts = {}
+    if fluor:
+        parts["philox"] = P["philox_block"]                     # one block per fluorescence photon
+        parts["uniforms"] = 4 * P["uniform"]
+        parts["generation"] = P["generic_photon"]
+    else:
+        parts["philox"] = P["philox_block"] / 2                 # one block per TWO Cherenkov photons (R20)
+        parts["uniforms"] = 2 * P["uniform"]
+        parts["generation"] = P["azimuth"]
+    parts["projection"] = P["project"]
+    if ground_hist:
+        parts["histogram"] = P["hist_per_bunch"]
+    elif name == "c5g":
+        parts["record"] = P["record_per_hit"] * hits / photons
+    else:
+        parts["pretests"] = P["grid_lookup"] if n_tel > 8 else P["pretest_per_tel"] * (1 if n_tel <= 1 else 4 if n_tel <= 4 else 8)
+        parts["queue"] = P["queue"]
+        parts["exact_amortised"] = P["exact_per_hit"] * hits / photons
+    parts["walk"] = P["walk"]
+    parts["preamble_amortised"] = P["preamble_per_emitter"] * emitters / photons
+    if name == "c4" and not ground_hist:
+        # both processes: the fluorescence share of the photons (~4 %) costs a full block and the generic generation
+        parts["fluorescence_share"] = 0.04 * (P["philox_block"] / 2 + 2 * P["uniform"] + P["generic_photon"] - P["azimuth"])
+    parts = {k: round(v, 2) for k, v in parts.items()}
+    return {"parts": parts, "total": round(sum(parts.values()), 2)}
 
 
 def load_peaks():
@@ -164,6 +203,8 @@ def main():
     ap.add_argument("--segments", type=int, default=None, help="override the segment count of the workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-output-leg", action="store_true",
+                    help="skip the photon-output leg (roofline_output) that the default c2 run adds")
     ap.add_argument("--ground-hist", action="store_true",
                     help="ground-plane radial profile mode (C8OPT_MODE_GROUND_HIST, PAPER.md:85-89) on the workload's "
                          "segments: 1000 bins of 1 m about the shower axis; telescopes are not consulted")
@@ -183,7 +224,7 @@ def main():
     import torch.distributed as dist
 
     import paper_2309_15861_b200 as c8
-    from paper_2309_15861_b200.sharding import shard_first_id
+    from paper_2309_15861_b200.sharding import all_reduce_results, shard_first_id
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the photon path has no CPU fallback")
@@ -194,6 +235,10 @@ def main():
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    # clocks and throttle reasons are sampled over the whole measuring part of the process (warm-up, timed region,
+    # end-to-end leg, photon-output leg), every 5 ms
+    sampler = ClockSampler(local_rank, period_s=0.005)
+    sampler.start()
 
     # ---- inputs: every rank owns a full-size segment set of its own (weak scaling, independent showers)
     cfg = wl.make_config(args.workload, n_segments=args.segments)
@@ -211,10 +256,58 @@ def main():
         par["mode"] = c8.MODE_GROUND_HIST
         par["fl_beam_telescope"] = -1
     output_mode = par["mode"] == c8.MODE_OUTPUT
+    n_procs = 2 if par["processes"] == 3 else 1
+    h_seg = torch.from_numpy(seg.view(np.uint8).reshape(n, 48).copy()).pin_memory()
+    d_seg = h_seg.to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+    peaks = load_peaks()
+
+    def time_leg(ctx, par, kw, steps, warmup, hist=False):
+        """W untimed + K timed steps of one propagate call over the whole table; device time by CUDA events on the
+        launching stream around every step, L2 flushed (untimed) between steps.  Returns (counters, ms per step array,
+        launches in the timed region, wall seconds of the timed region)."""
+        def step(ev=None):
+            flush.fill_(1)
+            ctx.reset_tallies()
+            if ev is not None:
+                ev[0].record(stream)
+            ctx.propagate_segments(d_seg, par, n=n, first_segment_id=first_id, **kw)
+            if ev is not None:
+                ev[1].record(stream)
+        for _ in range(warmup):
+            step()
+        counters = ctx.read_ground_histogram()[2] if hist else ctx.read_tallies()[1]
+        events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        l0 = ctx.launch_count
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        w0 = time.perf_counter()
+        for k in range(steps):
+            step(events[k])
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - w0
+        if world > 1:
+            dist.barrier()
+        return counters, np.array([a.elapsed_time(b) for a, b in events]), ctx.launch_count - l0, wall
+
+    def output_buffers(ctx, par, n_tel):
+        """Record regions sized by one tally-mode pass (exact record count per telescope + slack)."""
+        p0 = dict(par); p0["mode"] = c8.MODE_TALLY
+        ctx.reset_tallies()
+        ctx.propagate_segments(d_seg, p0, n=n, first_segment_id=first_id)
+        t0_, _, _ = ctx.read_tallies()
+        caps = (t0_["hits"].astype(np.int64) + 1024)
+        offs = np.concatenate([[0], np.cumsum(caps)[:-1]])
+        return dict(records=torch.empty((int(caps.sum()), 7), dtype=torch.float32, device=dev),
+                    tel_offset=torch.from_numpy(offs).to(dev), tel_capacity=torch.from_numpy(caps).to(dev))
+
     ctx = c8.Context(cfg["atmosphere"])
     ctx.add_telescopes(tel)
     if args.ground_hist:
         ctx.set_ground_histogram(0.0, 0.0, 1000.0, 1000)
+    kw = output_buffers(ctx, par, n_tel) if output_mode else {}
 
     def read_counters():
         """Synchronise, read the step's result back (D2H) and return the counters."""
@@ -222,57 +315,11 @@ def main():
             return ctx.read_ground_histogram()[2]
         return ctx.read_tallies()[1]
 
-    h_seg = torch.from_numpy(seg.view(np.uint8).reshape(n, 48).copy()).pin_memory()
-    d_seg = h_seg.to(dev)
-    kw = {}
-    cap = 0
-    if output_mode:
-        # capacity: one warm-up pass in tally mode gives the exact record count per telescope
-        p0 = dict(par); p0["mode"] = c8.MODE_TALLY
-        ctx.propagate_segments(d_seg, p0, n=n, first_segment_id=first_id)
-        t0_, _, _ = ctx.read_tallies()
-        caps = (t0_["hits"].astype(np.int64) + 1024)
-        offs = np.concatenate([[0], np.cumsum(caps)[:-1]])
-        cap = int(caps.sum())
-        kw = dict(records=torch.empty((cap, 7), dtype=torch.float32, device=dev),
-                  tel_offset=torch.from_numpy(offs).to(dev), tel_capacity=torch.from_numpy(caps).to(dev))
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-    stream = torch.cuda.current_stream()
-
-    def step(timed_events=None):
-        flush.fill_(1)                                   # L2 flush between steps (untimed)
-        ctx.reset_tallies()
-        if timed_events is not None:
-            timed_events[0].record(stream)
-        ctx.propagate_segments(d_seg, par, n=n, first_segment_id=first_id, **kw)
-        if timed_events is not None:
-            timed_events[1].record(stream)
-
-    for _ in range(args.warmup):
-        step()
-    counters = read_counters()
+    # ---- timed region: exactly K steps
+    counters, step_ms, launches, wall = time_leg(ctx, par, kw, args.steps, args.warmup, hist=args.ground_hist)
     photons_per_step = counters["generated"]
     culled_per_step = counters["culled"]
     hits_per_step = counters["hits"]
-
-    # ---- timed region: exactly K steps, device time by CUDA events on the launching stream
-    events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    launches0 = ctx.launch_count
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    wall0 = time.perf_counter()
-    for k in range(args.steps):
-        step(events[k])
-    torch.cuda.synchronize()
-    wall = time.perf_counter() - wall0
-    clocks = sampler.stop()
-    if world > 1:
-        dist.barrier()
-    launches = ctx.launch_count - launches0
-    step_ms = np.array([a.elapsed_time(b) for a, b in events])
     total_ms = float(step_ms.sum())
     if world > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
@@ -284,6 +331,14 @@ def main():
     else:
         photons_all = float(photons_per_step)
     value = photons_all * args.steps / (total_ms * 1e-3)
+
+    # ---- the job's only exchange: one sum of the per-telescope tallies and counters over the ranks, after
+    # the timed region (NCCL all-reduce of a few hundred bytes)
+    reduced = None
+    if world > 1 and not args.ground_hist:
+        tallies, cnt, _ = ctx.read_tallies()
+        tallies_all, cnt_all = all_reduce_results(tallies, cnt, device=dev)
+        reduced = {"hits_all_ranks": int(tallies_all["hits"].sum()), "generated_all_ranks": int(cnt_all["generated"])}
 
     # ---- end to end through the C-ABI with HOST buffers: H2D of the segments + kernel + D2H of the tallies
     e2e = None
@@ -311,33 +366,54 @@ def main():
                "note": "c8opt_propagate_segments_host from pinned host memory (chunked H2D overlapped with the kernels) "
                        "+ c8opt_read_tallies; wall clock"}
 
+    # ---- photon-output leg (north_star's second roofline): the same segments against one accept-all detector on the
+    # observation level, every downward photon written as a 28-byte record ("c5g" at this segment count)
+    roofline_output = None
+    if args.workload == "c2" and not (args.no_output_leg or args.cull or args.ground_hist) and rank == 0:
+        octx = c8.Context(cfg["atmosphere"])
+        g_tel = wl.make_config("c5g", n_segments=1)["telescopes"]
+        octx.add_telescopes(np.asarray(g_tel, dtype=np.float32))
+        opar = dict(par); opar["mode"] = c8.MODE_OUTPUT
+        okw = output_buffers(octx, opar, 1)
+        ko = max(3, min(args.steps, 20))
+        ocnt, oms, olaunch, _ = time_leg(octx, opar, okw, ko, 3)
+        launches += olaunch
+        o_s = float(oms.sum()) * 1e-3 / ko
+        obytes = RECORD_BYTES * ocnt["records"] + SEGMENT_BYTES * n
+        roofline_output = {
+            "bound": "hbm", "workload": f"c5g at {n} segments (the c2 segments, accept-all detector at h_obs)",
+            "achieved": obytes / o_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": obytes / o_s / 1e9 / peaks["hbm_gbs"],
+            "traffic": None, "traffic_note": "measured per round with ncu --set full: profiles/ncu_c5g_output_r02.md",
+            "peak_source": peaks["source"], "algorithmic_bytes_per_launch": obytes,
+            "bytes_per_record": RECORD_BYTES, "bytes_per_segment": SEGMENT_BYTES, "records_per_launch": ocnt["records"],
+            "kernel": "c8::propagate_kernel<TEL_CONST, coplanar, 1, output>", "kernel_ms": o_s * 1e3, "steps": ko,
+            "photons_per_s": ocnt["generated"] / o_s}
+        octx.close()
+        del okw
+
+    clocks = sampler.stop()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     # ---- roofline of the dominant (only) kernel
-    peaks = load_peaks()
     per_launch_s = total_ms * 1e-3 / args.steps
+    alg = alg_instr_per_photon(args.workload, float(photons_per_step - culled_per_step), float(n * n_procs), float(hits_per_step), n_tel,
+                               ground_hist=args.ground_hist)
     if args.workload == "c5g":
-        bytes_per_launch = RECORD_BYTES * hits_per_step + 48.0 * n
+        bytes_per_launch = RECORD_BYTES * hits_per_step + SEGMENT_BYTES * n
         roofline = {"bound": "hbm", "achieved": bytes_per_launch / per_launch_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "traffic": None, "peak_source": peaks["source"], "bytes_per_photon": RECORD_BYTES}
+                    "traffic": None, "peak_source": peaks["source"], "bytes_per_record": RECORD_BYTES, "bytes_per_segment": SEGMENT_BYTES,
+                    "algorithmic_bytes_per_launch": bytes_per_launch, "alg_instr_per_photon": alg["total"], "alg_instr_parts": alg["parts"]}
     else:
-        # ground histogram: no pre-tests (-24) but every downward bunch is carried to the plane: v_x, v_y, arrival time
-        # (exp), wavelength, radius, bin, three shared-memory atomics (+ ~90): 101 - 24 + 92; DESIGN.md §7
-        instr = 169.0 if args.ground_hist else ALG_INSTR.get(args.workload, 101.0)
         peak = 148 * 4 * 32 * peaks["sm_max_mhz"] * 1e6 / 1e12            # thread-instructions / s, issue-slot peak
         # culled bunches cost no photon-loop instructions: the roofline counts the propagated ones only
-        roofline = {"bound": "alu", "achieved": instr * (photons_per_step - culled_per_step) / per_launch_s / 1e12, "peak": peak,
+        roofline = {"bound": "alu", "achieved": alg["total"] * (photons_per_step - culled_per_step) / per_launch_s / 1e12, "peak": peak,
                     "unit": "Tinstr/s", "traffic": None, "peak_source": "148 SM x 4 schedulers x 32 lanes x sm_max_mhz "
-                    f"({peaks['source']})", "alg_instr_per_photon": instr,
-                    "hbm_achieved_gbs": (48.0 * n + RECORD_BYTES * (hits_per_step if output_mode else 0)) / per_launch_s / 1e9}
-    mode_key = "hist" if args.ground_hist else ("output" if output_mode else "tally")
-    traffic = NCU_TRAFFIC_PER_1E6_SEGMENTS.get((args.workload, mode_key))
-    if traffic is not None and not args.cull:
-        roofline["traffic"] = traffic * n / 1e6
-        roofline["traffic_source"] = "ncu --set full capture of this round (profiles/), scaled to this segment count"
+                    f"({peaks['source']})", "alg_instr_per_photon": alg["total"], "alg_instr_parts": alg["parts"],
+                    "hbm_achieved_gbs": (SEGMENT_BYTES * n + RECORD_BYTES * (hits_per_step if output_mode else 0)) / per_launch_s / 1e9}
+    roofline["traffic_note"] = "not measured in this run; the ncu --set full captures of the round are under profiles/"
     roofline["frac"] = roofline["achieved"] / roofline["peak"]
     roofline["kernel"] = "c8::propagate_kernel"
     roofline["kernel_ms"] = per_launch_s * 1e3
@@ -346,16 +422,20 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": cfg["name"], "segments_per_gpu": n, "photons_per_step_per_gpu": photons_per_step,
+        "config": {"workload": cfg["name"], "segments": n, "segments_per_gpu": n, "photons_per_step_per_gpu": photons_per_step,
                    "hits_per_step_per_gpu": hits_per_step, "telescopes": n_tel, "mode": "ground histogram (1000 x 1 m)" if args.ground_hist else "output" if output_mode else "tally",
                    "l2": "flushed between steps (256 MiB fill, untimed)", "timing": "sum of per-step CUDA-event times",
-                   "parallelism": f"segments sharded over {world} GPU(s), no data-path collective",
+                   "parallelism": f"segments sharded over {world} GPU(s), no data-path collective; one all-reduce of the tallies after the job",
                    "culling": (f"on: {culled_per_step} of the bunches per step are generated but provably miss every telescope "
                                "and skip the photon loop; value counts them (pre-cull equivalent), tallies are identical")
                               if args.cull else "off"},
         "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "wall_s_timed_region": wall, "step_ms_min_med_max": [float(step_ms.min()), float(np.median(step_ms)), float(step_ms.max())],
     }
+    if roofline_output is not None:
+        out["roofline_output"] = roofline_output
+    if reduced is not None:
+        out["all_reduce"] = reduced
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = oracle_baseline(cfg)
     print(json.dumps(out))

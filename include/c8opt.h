@@ -27,6 +27,9 @@
  *   - units: metres, nanoseconds, nanometres (wavelength), g/cm^2 (depth), MeV.
  *   - geometry: flat atmosphere, z up = altitude above sea level (R9).
  *   - one context per host thread; calls on one context must not overlap.
+ *   - a context belongs to the CUDA device that was current when it was created;
+ *     every entry point makes that device current for its own duration and
+ *     restores the caller's device before it returns.
  */
 #ifndef C8OPT_H
 #define C8OPT_H
@@ -172,11 +175,18 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n);
 
 /* Generate, propagate, intersect and tally / write the photons of n segments
  * (DEVICE array d_seg) with global ids first_segment_id + i.  Asynchronous on
- * `cuda_stream` (a cudaStream_t; NULL = default stream); accumulates into the
- * context's tallies and counters, so many batches may precede one read.
- * The random stream of photon j of segment S is Philox4x32-10 with
- * counter (j, S[31:0], S[63:32], process tag) and key = seed (R20): results do
- * not depend on how segments are batched.
+ * `cuda_stream` (a cudaStream_t; NULL = default stream) in every mode: the call
+ * only enqueues work (kernel launches and, in photon-output mode, one small
+ * device-to-device copy of tel_capacity into the context), allocates nothing
+ * and never waits for the device; it accumulates into the context's tallies
+ * and counters, so many batches may precede one read.  out->tel_offset /
+ * tel_capacity must stay valid until the enqueued work has run.
+ * Random stream (R20): Philox4x32-10, key = seed.  A fluorescence
+ * photon j of segment S draws the block with counter (j, S[31:0], S[63:32], 1);
+ * the Cherenkov photons 2k and 2k + 1 share the block with counter
+ * (k, S[31:0], S[63:32], 0) -- words (r0, r1) for the even one, (r2, r3) for the
+ * odd one.  The stream is a function of (seed, segment id, photon index) only:
+ * results do not depend on how segments are batched.
  * Errors: ARGUMENT (null, no telescopes, bad params, output mode without
  * records / offsets), CUDA. */
 int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_t n,
@@ -184,13 +194,23 @@ int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_
                              const c8opt_output *out, void *cuda_stream);
 
 /* Same path with the segments in HOST memory (pinned memory makes the copies
- * asynchronous): the segment table is cut into chunks whose host->device copy
- * overlaps the kernel of the previous chunk on two internal streams; returns
- * after all work is enqueued, ordered after prior work on `cuda_stream`, and
- * `cuda_stream` waits for it.  out->counts, if given, is still DEVICE memory. */
+ * asynchronous): the segment table is cut into chunks (a small first one, then
+ * doubling up to a quarter of the table) whose host->device copy overlaps the
+ * kernel of the previous chunk on two internal streams; returns after all work
+ * is enqueued, ordered after prior work on `cuda_stream`, and `cuda_stream`
+ * waits for it (also when an error is returned half way).  out->counts, if
+ * given, is still DEVICE memory.  Needs two device staging buffers of one
+ * chunk each: allocated by c8opt_reserve_host_staging, else by the first call
+ * that needs them (that call then synchronises the internal streams once). */
 int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, uint64_t n,
                                   uint64_t first_segment_id, const c8opt_run_params *params,
                                   const c8opt_output *out, void *cuda_stream);
+
+/* Create the internal streams and allocate the two device staging buffers of
+ * c8opt_propagate_segments_host for tables of up to max_segments segments
+ * (2 x 48 bytes x min(max(max_segments / 4, 32 Ki), 1 Mi), rounded to whole
+ * tiles), so that no later call allocates.  Errors: CUDA. */
+int c8opt_reserve_host_staging(c8opt_ctx *ctx, uint64_t max_segments);
 
 /* Synchronise with all work enqueued on the context and copy the results to
  * HOST memory: host_out[n_tel] tallies, counters[8] (may be NULL),

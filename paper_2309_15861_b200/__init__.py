@@ -35,7 +35,8 @@ RECORD_FLOATS = 7
 
 EXPORTS = ("c8opt_create_atmosphere", "c8opt_add_telescopes", "c8opt_propagate_segments",
            "c8opt_propagate_segments_host", "c8opt_read_tallies", "c8opt_reset_tallies", "c8opt_destroy",
-           "c8opt_last_error", "c8opt_launch_count", "c8opt_set_ground_histogram", "c8opt_read_ground_histogram")
+           "c8opt_last_error", "c8opt_launch_count", "c8opt_set_ground_histogram", "c8opt_read_ground_histogram",
+           "c8opt_reserve_host_staging")
 
 
 class C8optError(RuntimeError):
@@ -94,6 +95,7 @@ def lib():
         L.c8opt_launch_count.restype = C.c_uint64
         L.c8opt_set_ground_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_int32]
         L.c8opt_read_ground_histogram.argtypes = [vp, vp, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+        L.c8opt_reserve_host_staging.argtypes = [vp, C.c_uint64]
         for name in EXPORTS[:6] + EXPORTS[9:]:
             getattr(L, name).restype = C.c_int
         _lib = L
@@ -186,6 +188,10 @@ class Context:
         rp = make_run_params(params)
         self._check(lib().c8opt_propagate_segments_host(self._h, _ptr(h_seg), n, first_segment_id, C.byref(rp),
                                                         C.byref(out) if out is not None else None, _stream(stream)))
+
+    def reserve_host_staging(self, max_segments: int):
+        """Pre-allocate the device staging of propagate_segments_host (c8opt_reserve_host_staging)."""
+        self._check(lib().c8opt_reserve_host_staging(self._h, int(max_segments)))
 
     def read_tallies(self, allow_overflow: bool = False):
         """Synchronises; returns (tallies[n_tel], counters dict, records written per telescope)."""

@@ -55,10 +55,14 @@ struct c8opt_ctx {
     bool have_refract_grid = false;
     double refr_cmax = 0, r_max = 0;   // kappa T(lowest telescope) [m]; largest telescope radius
     // results
+    // one device block, laid out for n_tel telescopes as [counters 8 x u64][cursors n x u64][tallies n x 24 B]
+    // [capacity n x u64], so that a reset is one memset (all but the capacities) and a read one copy; h_results is
+    // its pinned host mirror
+    unsigned char *d_results = nullptr, *h_results = nullptr;
     c8::Tally *d_tallies = nullptr;
     unsigned long long *d_counters = nullptr;   // [8]
     unsigned long long *d_cursors = nullptr;    // [n_tel]
-    std::vector<unsigned long long> h_capacity; // capacities of the last output-mode call
+    unsigned long long *d_capacity = nullptr;   // [n_tel] capacities of the last output-mode call (device-side copy)
     bool have_capacity = false;
     unsigned long long segments_total = 0;      // host-side running count (counter 0)
     unsigned long long launches = 0;
@@ -81,6 +85,19 @@ int fail(c8opt_ctx *ctx, int code, const char *fmt, ...)
     va_end(ap);
     return code;
 }
+
+// Makes the context's device current for the duration of an entry point and restores the caller's device afterwards.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
 
 #define C8_CUDA(ctx, call)                                                                        \
     do {                                                                                          \
@@ -367,14 +384,44 @@ int launch(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, const c8opt_segment *d
     return C8OPT_OK;
 }
 
+// Photon-output mode: keep the capacities of this call for c8opt_read_tallies (records kept / dropped per telescope).
+// Device-to-device into the context's own buffer, asynchronous on the caller's stream: no host synchronisation on
+// the hot call, and the caller's tel_capacity array need not outlive it.
 int remember_capacity(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *out, cudaStream_t st)
 {
     if (rp->mode != C8OPT_MODE_OUTPUT) return C8OPT_OK;
-    ctx->h_capacity.resize(ctx->n_tel);
-    C8_CUDA(ctx, cudaMemcpyAsync(ctx->h_capacity.data(), out->tel_capacity, sizeof(unsigned long long) * ctx->n_tel,
-                                 cudaMemcpyDeviceToHost, st));
+    C8_CUDA(ctx, cudaMemcpyAsync(ctx->d_capacity, out->tel_capacity, sizeof(unsigned long long) * ctx->n_tel,
+                                 cudaMemcpyDeviceToDevice, st));
     ctx->have_capacity = true;
     return C8OPT_OK;
+}
+
+// The two internal streams, their events and the device staging buffers of c8opt_propagate_segments_host.
+int ensure_pipeline(c8opt_ctx *ctx, unsigned long long chunk_segments)
+{
+    if (!ctx->pipe_stream[0]) {
+        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->pipe_stream[i], cudaStreamNonBlocking));
+        for (int i = 0; i < 3; ++i) C8_CUDA(ctx, cudaEventCreateWithFlags(&ctx->pipe_event[i], cudaEventDisableTiming));
+    }
+    if (ctx->stage_segments < chunk_segments) {
+        for (int i = 0; i < 2; ++i) {
+            C8_CUDA(ctx, cudaStreamSynchronize(ctx->pipe_stream[i]));
+            cudaFree(ctx->d_stage[i]); ctx->d_stage[i] = nullptr;
+        }
+        ctx->stage_segments = 0;
+        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaMalloc(&ctx->d_stage[i], sizeof(c8opt_segment) * chunk_segments));
+        ctx->stage_segments = chunk_segments;
+    }
+    return C8OPT_OK;
+}
+
+// largest chunk of the host-segment pipeline: a quarter of the table, between 32 Ki and 1 Mi segments, whole tiles
+unsigned long long host_chunk_max(unsigned long long n)
+{
+    unsigned long long chunk = (n + 3) / 4;
+    if (chunk < (1ull << 15)) chunk = 1ull << 15;
+    if (chunk > (1ull << 20)) chunk = 1ull << 20;
+    return (chunk + c8::kTile - 1) / c8::kTile * c8::kTile;
 }
 
 }  // namespace
@@ -426,8 +473,11 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
         e = cudaMalloc(&ctx->d_tau, bytes);
         if (e == cudaSuccess) e = cudaMemcpy(ctx->d_tau, desc->tau, bytes, cudaMemcpyHostToDevice);
     }
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 8 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(ctx->d_counters, 0, 8 * sizeof(unsigned long long));
+    const size_t results_bytes = 64 + (size_t)C8OPT_MAX_TELESCOPES * (8 + sizeof(c8::Tally) + 8);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_results, results_bytes);
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_results, 0, results_bytes);
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_results, results_bytes);
+    ctx->d_counters = reinterpret_cast<unsigned long long *>(ctx->d_results);
     for (int ts = 0; ts < 3 && e == cudaSuccess; ++ts)
         for (int nt = 1; nt <= 8 && e == cudaSuccess; nt *= (nt == 1 ? 4 : 2))
             for (int cp = 0; cp < 4 && e == cudaSuccess; ++cp)
@@ -457,11 +507,11 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
         if (!(xyzr[4 * k + 3] > 0.0f)) return fail(ctx, C8OPT_ERR_ARGUMENT, "telescope %d: radius must be > 0", k);
         for (int i = 0; i < 3; ++i) { lo[i] = std::fmin(lo[i], xyzr[4 * k + i]); hi[i] = std::fmax(hi[i], xyzr[4 * k + i]); }
     }
-    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    DeviceGuard guard(ctx->device);
     C8_CUDA(ctx, cudaDeviceSynchronize());
     ctx->n_tel = 0;
-    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_tallies); cudaFree(ctx->d_cursors); cudaFree(ctx->d_grid);
-    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_telEta = nullptr; ctx->d_tallies = nullptr; ctx->d_cursors = nullptr; ctx->d_grid = nullptr;
+    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid);
+    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_telEta = nullptr; ctx->d_grid = nullptr;
     ctx->tel_xyzr.assign(xyzr, xyzr + 4 * (size_t)n);
     // reference point: centre of the bounding box; all device coordinates are relative to it
     ctx->x_ref = 0.5 * (lo[0] + hi[0]); ctx->y_ref = 0.5 * (lo[1] + hi[1]); ctx->z_ref = 0.5 * (lo[2] + hi[2]);
@@ -492,14 +542,16 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telA, sizeof(float4) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telT, sizeof(float) * n));
     C8_CUDA(ctx, cudaMalloc(&ctx->d_telEta, sizeof(float) * n));
-    C8_CUDA(ctx, cudaMalloc(&ctx->d_tallies, sizeof(c8::Tally) * n));
-    C8_CUDA(ctx, cudaMalloc(&ctx->d_cursors, sizeof(unsigned long long) * n));
+    ctx->d_cursors = reinterpret_cast<unsigned long long *>(ctx->d_results + 64);
+    ctx->d_tallies = reinterpret_cast<c8::Tally *>(ctx->d_results + 64 + 8 * (size_t)n);
+    ctx->d_capacity = reinterpret_cast<unsigned long long *>(ctx->d_results + 64 + 32 * (size_t)n);
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telA, A.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telT, T.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telEta, ctx->h_telEta.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
     ctx->tel_src = c8::TEL_CONST;
     if (n >= c8::kTelGridMin) {
-        // the grid lookup costs about as much as two brute-force pre-tests, so it serves from 3 telescopes up
+        // the grid lookup costs more than four brute-force pre-tests (11 instructions each), so it serves from
+        // kTelGridMin = 9 telescopes up (tried at 3: c2 1.07 -> 1.26 ms)
         std::vector<uint2> cells;
         ctx->n_tel_pending = n;
         if (build_grid(ctx, &cells)) {
@@ -523,6 +575,7 @@ int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_
 {
     if (!ctx) return C8OPT_ERR_ARGUMENT;
     if (!d_seg && n) return fail(ctx, C8OPT_ERR_ARGUMENT, "d_seg is NULL");
+    DeviceGuard guard(ctx->device);
     c8::KParams P;
     int rc = fill_params(ctx, params, out, &P);
     if (rc != C8OPT_OK) return rc;
@@ -532,11 +585,19 @@ int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_
     return launch(ctx, P, params->mode, d_seg, n, first_segment_id, out ? out->counts : nullptr, st);
 }
 
+int c8opt_reserve_host_staging(c8opt_ctx *ctx, uint64_t max_segments)
+{
+    if (!ctx) return C8OPT_ERR_ARGUMENT;
+    DeviceGuard guard(ctx->device);
+    return ensure_pipeline(ctx, host_chunk_max(max_segments));
+}
+
 int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, uint64_t n, uint64_t first_segment_id,
                                   const c8opt_run_params *params, const c8opt_output *out, void *cuda_stream)
 {
     if (!ctx) return C8OPT_ERR_ARGUMENT;
     if (!h_seg && n) return fail(ctx, C8OPT_ERR_ARGUMENT, "h_seg is NULL");
+    DeviceGuard guard(ctx->device);
     c8::KParams P;
     int rc = fill_params(ctx, params, out, &P);
     if (rc != C8OPT_OK) return rc;
@@ -544,39 +605,40 @@ int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, ui
     rc = remember_capacity(ctx, params, out, user);
     if (rc != C8OPT_OK) return rc;
     if (n == 0) return C8OPT_OK;
-    // chunking: ~1/8 of the table per chunk, between 32 Ki and 1 Mi segments, a multiple of the tile
-    unsigned long long chunk = (n + 7) / 8;
-    if (chunk < (1ull << 15)) chunk = 1ull << 15;
-    if (chunk > (1ull << 20)) chunk = 1ull << 20;
-    chunk = (chunk + c8::kTile - 1) / c8::kTile * c8::kTile;
-    if (!ctx->pipe_stream[0]) {
-        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->pipe_stream[i], cudaStreamNonBlocking));
-        for (int i = 0; i < 3; ++i) C8_CUDA(ctx, cudaEventCreateWithFlags(&ctx->pipe_event[i], cudaEventDisableTiming));
-    }
-    if (ctx->stage_segments < chunk) {
-        for (int i = 0; i < 2; ++i) {
-            C8_CUDA(ctx, cudaStreamSynchronize(ctx->pipe_stream[i]));
-            cudaFree(ctx->d_stage[i]); ctx->d_stage[i] = nullptr;
-        }
-        ctx->stage_segments = 0;
-        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaMalloc(&ctx->d_stage[i], sizeof(c8opt_segment) * chunk));
-        ctx->stage_segments = chunk;
-    }
+    // Chunk schedule: the first chunk is small (1/32 of the table, at least 32 Ki segments) so that the first kernel
+    // starts after a short copy; the chunks then double up to a quarter of the table, so that the kernels in the
+    // middle fill the GPU for several waves, and no chunk takes more than half of what is left, so that the last
+    // kernel, which nothing overlaps, is short again.  Two staging buffers, copy and kernel of a chunk on the same
+    // internal stream.
+    const unsigned long long chunk_max = host_chunk_max(n);
+    rc = ensure_pipeline(ctx, chunk_max);          // allocates on the first call unless c8opt_reserve_host_staging did
+    if (rc != C8OPT_OK) return rc;
+    unsigned long long chunk_min = (n + 31) / 32;
+    if (chunk_min < (1ull << 15)) chunk_min = 1ull << 15;
+    chunk_min = (chunk_min + c8::kTile - 1) / c8::kTile * c8::kTile;
+    if (chunk_min > chunk_max) chunk_min = chunk_max;
+    unsigned long long grow = chunk_min;
     C8_CUDA(ctx, cudaEventRecord(ctx->pipe_event[2], user));
     for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamWaitEvent(ctx->pipe_stream[i], ctx->pipe_event[2], 0));
     int c = 0;
-    for (unsigned long long off = 0; off < n; off += chunk, ++c) {
-        const unsigned long long m = (n - off < chunk) ? (n - off) : chunk;
+    cudaError_t ce = cudaSuccess;
+    for (unsigned long long off = 0, m = 0; off < n && rc == C8OPT_OK && ce == cudaSuccess; off += m, grow = std::min(2 * grow, chunk_max), ++c) {
+        const unsigned long long left = n - off, half = (left / 2 + c8::kTile - 1) / c8::kTile * c8::kTile;
+        m = std::min(left, std::max(chunk_min, std::min(grow, half)));
         cudaStream_t st = ctx->pipe_stream[c & 1];
-        C8_CUDA(ctx, cudaMemcpyAsync(ctx->d_stage[c & 1], h_seg + off, sizeof(c8opt_segment) * m, cudaMemcpyHostToDevice, st));
+        ce = cudaMemcpyAsync(ctx->d_stage[c & 1], h_seg + off, sizeof(c8opt_segment) * m, cudaMemcpyHostToDevice, st);
+        if (ce != cudaSuccess) break;
         rc = launch(ctx, P, params->mode, ctx->d_stage[c & 1], m, first_segment_id + off,
                     (out && out->counts) ? out->counts + 2 * off : nullptr, st);
-        if (rc != C8OPT_OK) return rc;
     }
+    // also after an error: the caller's stream waits for whatever was enqueued on the internal streams
     for (int i = 0; i < 2; ++i) {
-        C8_CUDA(ctx, cudaEventRecord(ctx->pipe_event[i], ctx->pipe_stream[i]));
-        C8_CUDA(ctx, cudaStreamWaitEvent(user, ctx->pipe_event[i], 0));
+        const cudaError_t e1 = cudaEventRecord(ctx->pipe_event[i], ctx->pipe_stream[i]);
+        const cudaError_t e2 = (e1 == cudaSuccess) ? cudaStreamWaitEvent(user, ctx->pipe_event[i], 0) : e1;
+        if (ce == cudaSuccess && e2 != cudaSuccess) ce = e2;
     }
+    if (rc != C8OPT_OK) return rc;
+    if (ce != cudaSuccess) return fail(ctx, C8OPT_ERR_CUDA, "host-segment pipeline: %s", cudaGetErrorString(ce));
     return C8OPT_OK;
 }
 
@@ -585,19 +647,21 @@ int c8opt_read_tallies(c8opt_ctx *ctx, c8opt_tally *host_out, int32_t n_tel, uin
     if (!ctx) return C8OPT_ERR_ARGUMENT;
     if (!host_out) return fail(ctx, C8OPT_ERR_ARGUMENT, "host_out is NULL");
     if (n_tel != ctx->n_tel || n_tel < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "n_tel = %d but the context has %d telescopes", n_tel, ctx->n_tel);
-    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    DeviceGuard guard(ctx->device);
     C8_CUDA(ctx, cudaDeviceSynchronize());
     static_assert(sizeof(c8opt_tally) == sizeof(c8::Tally), "tally layout");
-    C8_CUDA(ctx, cudaMemcpy(host_out, ctx->d_tallies, sizeof(c8::Tally) * n_tel, cudaMemcpyDeviceToHost));
-    unsigned long long cnt[8];
-    C8_CUDA(ctx, cudaMemcpy(cnt, ctx->d_counters, sizeof(cnt), cudaMemcpyDeviceToHost));
-    std::vector<unsigned long long> cur(n_tel);
-    C8_CUDA(ctx, cudaMemcpy(cur.data(), ctx->d_cursors, sizeof(unsigned long long) * n_tel, cudaMemcpyDeviceToHost));
+    // one copy of the whole result block into its pinned mirror
+    C8_CUDA(ctx, cudaMemcpy(ctx->h_results, ctx->d_results, 64 + 40 * (size_t)n_tel, cudaMemcpyDeviceToHost));
+    const unsigned long long *cnt = reinterpret_cast<const unsigned long long *>(ctx->h_results);
+    const unsigned long long *cur = cnt + 8;
+    std::memcpy(host_out, ctx->h_results + 64 + 8 * (size_t)n_tel, sizeof(c8::Tally) * n_tel);
+    std::vector<unsigned long long> capacity(n_tel, ~0ull);
+    if (ctx->have_capacity) std::memcpy(capacity.data(), ctx->h_results + 64 + 32 * (size_t)n_tel, 8 * (size_t)n_tel);
     unsigned long long hits = 0, stored = 0, dropped = 0;
     for (int k = 0; k < n_tel; ++k) {
         hits += host_out[k].hits;
         unsigned long long kept = cur[k];
-        if (ctx->have_capacity && kept > ctx->h_capacity[k]) { dropped += kept - ctx->h_capacity[k]; kept = ctx->h_capacity[k]; }
+        if (kept > capacity[k]) { dropped += kept - capacity[k]; kept = capacity[k]; }
         stored += kept;
         if (host_tel_count) host_tel_count[k] = kept;
     }
@@ -618,12 +682,9 @@ int c8opt_read_tallies(c8opt_ctx *ctx, c8opt_tally *host_out, int32_t n_tel, uin
 int c8opt_reset_tallies(c8opt_ctx *ctx, void *cuda_stream)
 {
     if (!ctx) return C8OPT_ERR_ARGUMENT;
+    DeviceGuard guard(ctx->device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    C8_CUDA(ctx, cudaMemsetAsync(ctx->d_counters, 0, 8 * sizeof(unsigned long long), st));
-    if (ctx->n_tel > 0) {
-        C8_CUDA(ctx, cudaMemsetAsync(ctx->d_tallies, 0, sizeof(c8::Tally) * ctx->n_tel, st));
-        C8_CUDA(ctx, cudaMemsetAsync(ctx->d_cursors, 0, sizeof(unsigned long long) * ctx->n_tel, st));
-    }
+    C8_CUDA(ctx, cudaMemsetAsync(ctx->d_results, 0, 64 + 32 * (size_t)ctx->n_tel, st));      // counters, cursors, tallies
     if (ctx->d_hist) C8_CUDA(ctx, cudaMemsetAsync(ctx->d_hist, 0, sizeof(c8::Tally) * (ctx->hist_bins + 1), st));
     ctx->segments_total = 0;
     return C8OPT_OK;
@@ -635,7 +696,7 @@ int c8opt_set_ground_histogram(c8opt_ctx *ctx, double core_x_m, double core_y_m,
     if (n_bins < 0 || n_bins > c8::kHistMax) return fail(ctx, C8OPT_ERR_ARGUMENT, "n_bins must be 0 .. %d", c8::kHistMax);
     if (n_bins > 0 && (!std::isfinite(core_x_m) || !std::isfinite(core_y_m) || !(r_max_m > 0.0) || !std::isfinite(r_max_m)))
         return fail(ctx, C8OPT_ERR_ARGUMENT, "need a finite core and r_max > 0");
-    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    DeviceGuard guard(ctx->device);
     C8_CUDA(ctx, cudaDeviceSynchronize());
     cudaFree(ctx->d_hist);
     ctx->d_hist = nullptr; ctx->hist_bins = 0;
@@ -651,7 +712,7 @@ int c8opt_read_ground_histogram(c8opt_ctx *ctx, c8opt_hist_bin *host_out, int32_
     if (!ctx) return C8OPT_ERR_ARGUMENT;
     if (!host_out) return fail(ctx, C8OPT_ERR_ARGUMENT, "host_out is NULL");
     if (n_bins != ctx->hist_bins || n_bins < 1) return fail(ctx, C8OPT_ERR_ARGUMENT, "n_bins = %d but the context has %d bins", n_bins, ctx->hist_bins);
-    C8_CUDA(ctx, cudaSetDevice(ctx->device));
+    DeviceGuard guard(ctx->device);
     C8_CUDA(ctx, cudaDeviceSynchronize());
     static_assert(sizeof(c8opt_hist_bin) == sizeof(c8::Tally), "histogram bin layout");
     C8_CUDA(ctx, cudaMemcpy(host_out, ctx->d_hist, sizeof(c8::Tally) * n_bins, cudaMemcpyDeviceToHost));
@@ -678,7 +739,7 @@ int c8opt_read_ground_histogram(c8opt_ctx *ctx, c8opt_hist_bin *host_out, int32_
 void c8opt_destroy(c8opt_ctx *ctx)
 {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
+    DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
     for (int i = 0; i < 2; ++i) {
         if (ctx->pipe_stream[i]) cudaStreamDestroy(ctx->pipe_stream[i]);
@@ -686,7 +747,7 @@ void c8opt_destroy(c8opt_ctx *ctx)
     }
     for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
     cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid);
-    cudaFree(ctx->d_tallies); cudaFree(ctx->d_counters); cudaFree(ctx->d_cursors); cudaFree(ctx->d_hist);
+    cudaFree(ctx->d_results); cudaFreeHost(ctx->h_results); cudaFree(ctx->d_hist);
     cudaGetLastError();
     delete ctx;
 }

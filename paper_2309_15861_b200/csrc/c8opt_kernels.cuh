@@ -146,7 +146,8 @@ __device__ __forceinline__ float rcp_refined(float x)
 
 
 // ------------------------------------------------------------------------------------
-// a2: Philox4x32-10 (Salmon et al., SC'11), counter (j, S_lo, S_hi, tag), key = seed (R20).
+// a2: Philox4x32-10 (Salmon et al., SC'11), key = seed.  Counter (R20): fluorescence photon j of segment S draws
+// the block (j, S_lo, S_hi, 1); the Cherenkov photons 2k, 2k + 1 share the block (k, S_lo, S_hi, 0).
 struct Rand4 { uint32_t r0, r1, r2, r3; };
 
 constexpr uint32_t kPhiloxM0 = 0xD2511F53u, kPhiloxM1 = 0xCD9E8D57u;
@@ -167,8 +168,8 @@ __device__ __forceinline__ Rand4 philox4x32_10(const KParams &P, uint32_t c0, ui
     return Rand4{c0, c1, c2, c3};
 }
 
-// The counter is (j, S_lo, S_hi, tag): only word 0 changes from photon to photon of one emitter, so
-// the S-dependent halves of rounds 1 and 2 are computed once per emitter (3 words) and each photon
+// The counter is (block index, S_lo, S_hi, tag): only word 0 changes from block to block of one emitter, so
+// the S-dependent halves of rounds 1 and 2 are computed once per emitter (3 words) and each block
 // does 18 instead of 20 wide multiplies.  Same function, bit for bit.
 struct PhiloxEmitter { uint32_t C, D, E; };
 
@@ -371,19 +372,19 @@ __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, 
 }
 
 // Preamble of emitter (segment i, process tag).  Writes the frame, returns n_b.
-// *bad is set when the segment is invalid (non-finite field, gamma <= 1, L < 0, |d| off unity by > 1e-3,
-// or n_b >= 2^24).
+// *bad is set when the segment is invalid: 1 = non-finite field, gamma <= 1, L < 0 or |d| off unity by > 1e-3 (the
+// same for both processes), 2 = n_b >= 2^24 for this process.
 __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1, const float4 s2, int tag,
-                             float *__restrict__ fr, uint8_t *kind_out, bool *bad, bool *culled)
+                             float *__restrict__ fr, uint8_t *kind_out, int *bad, bool *culled)
 {
-    *bad = false;
+    *bad = 0;
     *culled = false;
     const double L = (double)s1.w, gamma = (double)s2.x, zq = (double)s2.y, dE = (double)s2.z;
     const double dx = (double)s1.x, dy = (double)s1.y, dz = (double)s1.z;
     const double dn = sqrt(dadd(dadd(dmul(dx, dx), dmul(dy, dy)), dmul(dz, dz)));
     const bool finite = isfinite(s0.x) && isfinite(s0.y) && isfinite(s0.z) && isfinite(s0.w) && isfinite(dn) &&
                         isfinite(L) && isfinite(gamma) && isfinite(zq) && isfinite(dE);
-    if (!finite || !(gamma > 1.0) || !(L >= 0.0) || !(fabs(dn - 1.0) <= 1e-3)) { *bad = true; return 0; }
+    if (!finite || !(gamma > 1.0) || !(L >= 0.0) || !(fabs(dn - 1.0) <= 1e-3)) { *bad = 1; return 0; }
     const double d[3] = { ddiv(dx, dn), ddiv(dy, dn), ddiv(dz, dn) };
     const double p0[3] = { (double)s0.x, (double)s0.y, (double)s0.z };
     const double ig2 = ddiv(1.0, dmul(gamma, gamma));
@@ -445,7 +446,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     }
     if (!(mu > 0.0)) return 0;
     const double nb = ceil(ddiv(mu, P.bunch_size));              // R1: deterministic bunches
-    if (nb > 16777215.0) { *bad = true; return 0; }
+    if (nb > 16777215.0) { *bad = 2; return 0; }
     double w0 = ddiv(mu, nb);
     if (kind == KIND_CONE && P.beam_tel >= 0) w0 *= 0.5 * P.omc;  // R14 (weight form): Omega / 4 pi
     if ((P.flags & kFlagCull) && tag == 0) {
@@ -503,6 +504,16 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     }
     fr[F_L] = (float)L;
     return (uint32_t)nb;
+}
+
+// Is the segment invalid for the Cherenkov process?  (rare path of the second launch of a two-process request)
+__device__ __noinline__ int cherenkov_preamble_status(const KParams &P, const float4 s0, const float4 s1, const float4 s2, float *scratch_frame)
+{
+    int bad;
+    bool culled;
+    uint8_t kind;
+    preamble(P, s0, s1, s2, 0, scratch_frame, &kind, &bad, &culled);
+    return bad;
 }
 
 // ------------------------------------------------------------------------------------
@@ -1781,9 +1792,15 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     if (seg_local < segs_per_tile && seg_i < P.n_seg) {
         const float4 *sp = P.seg + seg_i * 3ull;
         const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
-        bool bad, culled;
+        int bad;
+        bool culled;
         nb = preamble(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled);
-        if (bad) sm.invalid[seg_local] = 1;
+        if (P.split_part == 2) {
+            // second launch of a two-process request: the first one (Cherenkov) has counted the segments that are
+            // invalid for both processes or for Cherenkov; what is left to count here is a segment whose fluorescence
+            // bunch count alone is out of range (the Cherenkov preamble is run again to find out; rare)
+            if (bad == 2 && cherenkov_preamble_status(P, s0, s1, s2, &sm.frame[tid * kFrameStride]) == 0) sm.invalid[seg_local] = 1;
+        } else if (bad) sm.invalid[seg_local] = 1;
         if (P.counts) {
             P.counts[seg_i * 2ull + (unsigned)tag] = nb;
             if (P.n_procs == 1 && P.split_part == 0) P.counts[seg_i * 2ull + (unsigned)(tag ^ 1)] = 0u;
@@ -1928,7 +1945,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         // invalid segments of this tile (each counted once)
         uint32_t nbad = (tid < kTile / (int)P.n_procs) ? sm.invalid[tid] : 0u;
         nbad = __reduce_add_sync(0xffffffffu, nbad);
-        if (lane == 0 && nbad && P.split_part != 2) atomicAdd(&P.counters[6], (unsigned long long)nbad);   // once per segment
+        if (lane == 0 && nbad) atomicAdd(&P.counters[6], (unsigned long long)nbad);   // once per segment
     }
     if constexpr (MODE == MODE_HIST) {
         // the tile's histogram into the global one (the barrier above ordered the warps' updates); bin hist_bins = overflow

@@ -169,6 +169,26 @@ def test_non_coplanar_and_generic_tracks(c8):
     assert rep["matched"] > 1000
 
 
+def test_segment_invalid_for_one_process_only(c8):
+    """Both processes (two launches): a segment whose fluorescence bunch count alone is out of range (n_b >= 2^24), one
+    whose Cherenkov count alone is, and one that is invalid for both are each counted once, as the oracle counts them."""
+    import parity_util as pu
+    cfg = wl.make_config("c4", n_segments=4000)
+    seg = cfg["segments"]
+    seg["dE"][100] = np.float32(1.0e7)              # 4 / MeV x 1e7 MeV = 4e7 bunches >= 2^24: fluorescence only
+    seg["length"][200] = np.float32(1.0e6)          # ~ 34 / m x 1e6 m along a horizontal track at 2.5 km: Cherenkov only
+    seg["z0"][200], seg["dz"][200], seg["dx"][200], seg["dy"][200] = 2500.0, 0.0, 1.0, 0.0
+    seg["gamma"][200] = np.float32(1e4)
+    seg["gamma"][300] = np.float32(0.5)             # both
+    seg["dE"][301] = np.float32(1.0e7)
+    seg["gamma"][301] = np.float32(np.nan)          # both, and the fluorescence count out of range as well
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("invalid-one-process", rep)
+    assert g["counters"]["invalid"] == 4
+
+
 def test_output_capacity_overflow(c8):
     """The kernel never writes past tel_capacity; the overflow is counted and reported as error -3."""
     import parity_util as pu
