@@ -219,6 +219,20 @@ def refraction(atm: dict, e_z, c_z, v_z):
     return dr.value, dth.value
 
 
+def intersect_refracted(atm: dict, e, v, tel):
+    """R10 / R11 with the corrections of R27.  Returns (hit, b2, s_c, s_pl, x, y, v_out[3])."""
+    e = np.ascontiguousarray(e, dtype=np.float64)
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    t = np.ascontiguousarray(tel, dtype=np.float64)
+    b2, sc, sp = C.c_double(), C.c_double(), C.c_double()
+    xy, vo = np.zeros(2), np.zeros(3)
+    f = lib().orc_intersect_refracted
+    f.argtypes = [C.POINTER(Atmosphere)] + [C.POINTER(C.c_double)] * 3 + [C.POINTER(C.c_double)] * 3 + [C.POINTER(C.c_double)] * 2
+    f.restype = C.c_int
+    hit = f(C.byref(make_atmosphere(atm)), _dp(e), _dp(v), _dp(t), C.byref(b2), C.byref(sc), C.byref(sp), _dp(xy), _dp(vo))
+    return bool(hit), b2.value, sc.value, sp.value, float(xy[0]), float(xy[1]), vo
+
+
 def optical_depth(atm: dict, h, lam) -> float:
     return lib().orc_optical_depth(C.byref(make_atmosphere(atm)), float(h), float(lam))
 

@@ -361,6 +361,8 @@ double orc_arrival_time(const orc_atmosphere *atm, double e_z, double c_z, doubl
  *   dtheta = tan(theta0) (eta(e_z) - eta(c_z)).
  * Both are negative going down (the air gets denser: the ray bends towards the vertical).  The optical path changes
  * only to second order (Fermat), so the arrival time of R8 stands. */
+#define ORC_REFRACT_VZ_MIN 0.25   /* cos(75.5 deg): where the first-order forms leave their 3e-3 bound (see below) */
+
 void orc_refraction(const orc_atmosphere *atm, double e_z, double c_z, double v_z, double *dr, double *dtheta)
 {
     double cos0 = fabs(v_z), sin0 = sqrt(fmax(0.0, 1.0 - v_z * v_z)), tan0 = sin0 / cos0;
@@ -383,9 +385,11 @@ int orc_intersect_refracted(const orc_atmosphere *atm, const double e[3], const 
     double sp = (tel[2] - e[2]) / v[2];
     double x = e[0] + sp * v[0] - tel[0], y = e[1] + sp * v[1] - tel[1];
     double sin0 = sqrt(v[0] * v[0] + v[1] * v[1]);
-    /* the planar first-order forms are for rays well away from the horizontal (the Cherenkov light of a shower):
-     * beyond a zenith angle of 60 degrees, |v_z| < 0.5, the straight line is kept (R27) */
-    if (sin0 > 0.0 && v[2] <= -0.5) {
+    /* Validity of the first-order forms (R27): the terms they drop are O(eta tan^2 theta0) of the correction.  Against
+     * a Snell ray integrated through the same n(z) they stay within 3e-3 of it up to a zenith angle of 75.5 degrees
+     * (|v_z| >= 0.25) for emission altitudes up to 30 km, and leave that bound beyond (6e-3 at 80, 2e-2 at 85 degrees;
+     * tests/test_oracle_pins.py::test_refraction_first_order_validity_bound).  Flatter rays keep the straight line. */
+    if (sin0 > 0.0 && v[2] <= -ORC_REFRACT_VZ_MIN) {
         double dr, dth;
         orc_refraction(atm, e[2], tel[2], v[2], &dr, &dth);
         double hx = v[0] / sin0, hy = v[1] / sin0;

@@ -661,6 +661,70 @@ def test_refraction_corrections_against_integrated_snell_ray(atm, theta_deg, e_z
     assert math.isclose(dth, dth_num, rel_tol=3e-3), (dth, dth_num)
 
 
+@pytest.mark.parametrize("atm", [ATM1, ATM5], ids=["one-layer", "five-layer"])
+def test_refraction_first_order_validity_bound(atm):
+    """Where R27's first-order forms hold: they drop terms of relative size O(eta tan^2 theta0).  Against the integrated
+    Snell ray they stay within 3e-3 at zenith angles 55, 60, 65 and 75 degrees for emission at 12 and 30 km, and they
+    have left that bound at 80 and 85 degrees -- which is where the oracle's cut-off |v_z| >= 0.25 (75.5 degrees) comes
+    from: it is set by this error, not by any data structure of the GPU path."""
+    for e_z in (12000.0, 30000.0):
+        for deg in (55.0, 60.0, 65.0, 75.0):
+            th = math.radians(deg)
+            dr, dth = O.refraction(atm, e_z, 2000.0, -math.cos(th))
+            dr_num, dth_num = _snell_ray(atm, e_z, 2000.0, th)
+            assert math.isclose(dr, dr_num, rel_tol=3e-3) and math.isclose(dth, dth_num, rel_tol=3e-3), (e_z, deg, dr, dr_num)
+        for deg in (80.0, 85.0):
+            th = math.radians(deg)
+            dr, _ = O.refraction(atm, e_z, 2000.0, -math.cos(th))
+            dr_num, _ = _snell_ray(atm, e_z, 2000.0, th)
+            assert abs(dr / dr_num - 1.0) > 3e-3, (e_z, deg, dr, dr_num)
+    assert math.isclose(math.degrees(math.acos(0.25)), 75.52, abs_tol=0.01)
+
+
+def _ray(zenith_deg, azimuth_deg=30.0):
+    th, ph = math.radians(zenith_deg), math.radians(azimuth_deg)
+    return np.array([math.sin(th) * math.cos(ph), math.sin(th) * math.sin(ph), -math.cos(th)])
+
+
+def test_refraction_cutoff_moves_rays_inside_and_keeps_rays_outside():
+    """A ray just steeper than the cut-off (|v_z| = 0.2501) arrives moved by dr along its horizontal flight direction and
+    turned by dtheta; a ray just flatter (|v_z| = 0.2499) arrives where the straight line does, direction unchanged."""
+    tel = np.array([0.0, 0.0, 2000.0, 1e9])
+    e = np.array([100.0, -50.0, 9000.0])
+    for vz, moved in ((0.2501, True), (0.2499, False), (0.5001, True), (0.4999, True), (0.9, True)):
+        v = _ray(math.degrees(math.acos(vz)))
+        hit0, _, _, sp0, x0, y0 = O.intersect(e, v, tel)
+        hit1, _, _, sp1, x1, y1, vo = O.intersect_refracted(ATM5, e, v, tel)
+        assert hit0 and hit1 and sp0 == sp1
+        if moved:
+            dr, dth = O.refraction(ATM5, e[2], 2000.0, v[2])
+            hx, hy = v[0] / math.hypot(v[0], v[1]), v[1] / math.hypot(v[0], v[1])
+            assert math.isclose(x1 - x0, dr * hx, rel_tol=1e-9) and math.isclose(y1 - y0, dr * hy, rel_tol=1e-9)
+            assert math.isclose(math.acos(-vo[2]) - math.acos(-v[2]), dth, rel_tol=1e-6)
+            assert abs(dr) > 0.05
+        else:
+            assert x1 == x0 and y1 == y0 and np.array_equal(vo, v)
+
+
+def test_refraction_flips_the_hit_decision_on_a_small_sphere():
+    """The sphere test runs on the corrected values: a 45-degree ray from 10 km above the plane lands 1.4 m short of its
+    straight line, so a 0.9 m sphere centred 2 m behind the straight-line point (b = 2 cos 45 = 1.41 m: a miss) is hit
+    once the correction is applied (b = 0.43 m), and a sphere centred on the straight-line point (a hit) is missed
+    (b = 0.98 m)."""
+    v = _ray(45.0, azimuth_deg=0.0)                                    # flies towards +x
+    e = np.array([0.0, 0.0, 12000.0])
+    dr, _ = O.refraction(ATM5, 12000.0, 2000.0, v[2])
+    assert -1.6 < dr < -1.2
+    x_line = 10000.0                                                   # straight-line plane crossing
+    behind = np.array([x_line - 2.0, 0.0, 2000.0, 0.9])
+    on_line = np.array([x_line, 0.0, 2000.0, 0.9])
+    assert not O.intersect(e, v, behind)[0] and O.intersect(e, v, on_line)[0]
+    hit_b, b2_b, *_ = O.intersect_refracted(ATM5, e, v, behind)
+    hit_o, b2_o, *_ = O.intersect_refracted(ATM5, e, v, on_line)
+    assert hit_b and math.isclose(math.sqrt(b2_b), abs(2.0 + dr) * math.cos(math.radians(45.0)), rel_tol=1e-3)
+    assert not hit_o and math.isclose(math.sqrt(b2_o), abs(dr) * math.cos(math.radians(45.0)), rel_tol=1e-3)
+
+
 def test_refraction_magnitude_and_vertical_ray():
     """SURVEY.md §8(f) quotes ~3 cm and ~7e-6 rad at 4 degrees from 8 km above the plane; a vertical ray is not moved."""
     dr, dth = O.refraction(ATM1, 10000.0, 2000.0, -math.cos(math.radians(4.0)))
