@@ -48,6 +48,7 @@ constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-k
 constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
 constexpr uint32_t kFlagCull = 1u;    // == C8OPT_FLAG_CULL
 constexpr uint32_t kFlagRefract = 2u; // == C8OPT_FLAG_REFRACT
+constexpr float kRefractVzMin = 0.25f;   // R27: the corrections apply to photons with |v_z| >= 0.25 (zenith <= 75.5 degrees)
 constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
 constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
@@ -359,8 +360,14 @@ __device__ __forceinline__ bool cone_reaches(float ux, float uy, float uz, float
 __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, float mz, float dx, float dy, float dz, float hl,
                                           float sin_c, float cos_c)
 {
-    // with the refraction corrections a photon may land up to 6.93 refr_cmax off its straight line (|v_z| >= 0.5)
-    const float grow = (P.flags & kFlagRefract) ? 7.0f * P.refr_cmax : 0.0f;
+    // With the refraction corrections a photon lands up to refr_cmax sin / cos^3 off its straight line (R27).  The
+    // photons of this emitter lie within theta_c of d, so |v_z| >= |d_z| cos_c - sqrt(1 - d_z^2) sin_c; the corrections
+    // stop at |v_z| = kRefractVzMin, where the reach is 62 refr_cmax.
+    float grow = 0.0f;
+    if (P.flags & kFlagRefract) {
+        const float vzm = fmaxf(fmaf(fabsf(dz), cos_c, -sqrtf(fmaxf(fmaf(-dz, dz, 1.0f), 0.0f)) * sin_c) - 1e-3f, kRefractVzMin);
+        grow = 1.02f * P.refr_cmax * sqrtf(fmaxf(fmaf(-vzm, vzm, 1.0f), 0.0f)) / (vzm * vzm * vzm) + 0.01f;
+    }
     if (!cone_reaches(-mx, -my, -mz, P.cull_Rb + grow, dx, dy, dz, hl, sin_c, cos_c)) return true;
     if (P.n_tel > kCullTelMax) return false;
     for (int k = 0; k < P.n_tel; ++k) {
@@ -696,7 +703,7 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
         eta_e = P.kappa_m * lf.b * (lf.k2 * 0.693147181f) * E;   // eta0 rho(h) / rho0, rho = (b / c) exp(-h / c) / 100
     };
     float s_pl;
-    if ((P.flags & kFlagRefract) && ph.vz <= -0.5f) {
+    if ((P.flags & kFlagRefract) && ph.vz <= -kRefractVzMin) {
         // R27: point and direction on the plane z = c_z corrected for refraction to first order, then
         // the sphere test on the corrected values.  (x, y) = straight-line plane point relative to the centre.
         float x, y, hk;
@@ -1038,13 +1045,21 @@ __device__ __forceinline__ bool plane_pretest(const float4 T, float gx, float gy
     return qq - qv * qv - add <= fmaf(qq, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f));   // slack for the fp32 cancellation
 }
 
-// Slack of the pre-tests for a photon whose arrival point the refraction corrections may move (|v_z| >= 0.5 only).
+// Slack of the pre-tests for a photon whose arrival point the refraction corrections may move (|v_z| >= kRefractVzMin).
 __device__ __forceinline__ float refraction_slack(const KParams &P, float vz)
 {
-    if (!(vz <= -0.5f)) return 0.0f;
+    if (!(vz <= -kRefractVzMin)) return 0.0f;
     const float rv = rcp_approx(vz), s2 = fmaf(-vz, vz, 1.0f);
     const float x = 1.01f * P.refr_cmax * sqrtf(fmaxf(s2, 0.0f)) * rv * rv;      // d |v_z| = cmax sin / cos^2
     return x * (P.refr_two_rmax + x);
+}
+
+// How far the refraction corrections can move the arrival point of a photon in the plane (wide test): 0 for |v_z| < kRefractVzMin
+__device__ __forceinline__ float refraction_reach(const KParams &P, float vz)
+{
+    if (!(vz <= -kRefractVzMin)) return 0.0f;
+    const float rv = rcp_approx(vz), s2 = fmaf(-vz, vz, 1.0f);
+    return 1.02f * P.refr_cmax * sqrtf(fmaxf(s2, 0.0f)) * fabsf(rv * rv * rv) + 0.01f;
 }
 
 // Candidate mask of a photon over the telescopes reachable from its plane crossing.
@@ -1102,6 +1117,9 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
             if (REFR) return grid_lookup<COPLANAR>(P, P.grid_lvl[kGridLevels], gx, gy, vx, vy, vz, cell, refraction_slack(P, vz));
             return grid_lookup<COPLANAR>(P, P.grid_lvl[0], gx, gy, vx, vy, vz, cell, 0.0f);
         }
+        // corrected photons flatter than level 0 serves: their reach (up to 62 refr_cmax) is beyond what a grid of
+        // <= 4 telescopes per cell can hold, so they take the wide test, which carries the slack
+        if (REFR && -vz >= kRefractVzMin) return kAllTelescopes;
         if (P.n_grid_levels > 1 && -vz >= P.grid_lvl[1].vzmin) return grid_lookup<COPLANAR>(P, P.grid_lvl[1], gx, gy, vx, vy, vz, cell, 0.0f);
         return kAllTelescopes;
     } else {
@@ -1132,6 +1150,9 @@ __device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned
         px = ph.axis ? ph.gx : ph.ex; py = ph.axis ? ph.gy : ph.ey; pz = ph.axis ? 0.0f : ph.ez;
         vx = ph.vx; vy = ph.vy; vz = ph.vz;
     }
+    // R27: the corrections move the ray by at most refr_cmax sin / cos^3 in the plane, so b changes by no more than that
+    const float slack = (P.flags & kFlagRefract) ? refraction_reach(P, vz) : 0.0f;
+    const float add = slack * (P.refr_two_rmax + slack);
     for (int k0 = 0; k0 < P.n_tel; k0 += 32) {
         uint32_t cm = 0u;
         const int kn = min(32, P.n_tel - k0);
@@ -1142,7 +1163,7 @@ __device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned
                 const float cx = fmaf(my, vz, -(mz * vy)), cy = fmaf(mz, vx, -(mx * vz)), cz = fmaf(mx, vy, -(my * vx));
                 const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
                 const float mm = fmaf(mx, mx, fmaf(my, my, mz * mz));
-                if (b2 <= fmaf(mm, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f))) cm |= 1u << c;
+                if (b2 <= fmaf(mm, 1e-5f, fmaf(T.w, 1.0001f, 1e-3f)) + add) cm |= 1u << c;
             }
         }
         if (__any_sync(0xffffffffu, cm != 0u))

@@ -436,6 +436,48 @@ def test_refraction_corrections(c8, name, n):
     assert len(common) > 0.9 * len(g["records"]) and 1e-3 < np.median(shift) < 1.0
 
 
+@pytest.mark.parametrize("layout", ["4 telescopes", "4 x 4 grid"])
+def test_refraction_inclined_showers(c8, layout):
+    """C8OPT_FLAG_REFRACT beyond 60 degrees: half of the tracks are tilted to zenith angles of 58 .. 78 degrees and aimed
+    at the array, so that photons on both sides of |v_z| = 0.5 (the steep candidate grid's limit) and of the cut-off
+    |v_z| = 0.25 (R27) are corrected / kept and tested with the right slack, with and without culling."""
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=40_000)
+    seg = cfg["segments"]
+    rng = np.random.Generator(np.random.PCG64(321))
+    idx = np.arange(0, len(seg), 2)
+    zen = np.radians(rng.uniform(58.0, 78.0, len(idx)))
+    az = rng.uniform(0.0, 2.0 * np.pi, len(idx))
+    d = np.stack([np.sin(zen) * np.cos(az), np.sin(zen) * np.sin(az), -np.cos(zen)], axis=1)
+    d = d.astype(np.float32).astype(np.float64)
+    d /= np.linalg.norm(d, axis=1, keepdims=True)
+    h = seg["z0"][idx].astype(np.float64) - 2000.0
+    aim = rng.normal(0.0, 30.0, (len(idx), 2))
+    seg["x0"][idx] = aim[:, 0] - h * d[:, 0] / -d[:, 2]
+    seg["y0"][idx] = aim[:, 1] - h * d[:, 1] / -d[:, 2]
+    seg["dx"][idx], seg["dy"][idx], seg["dz"][idx] = d[:, 0], d[:, 1], d[:, 2]
+    seg["length"][idx] = np.minimum(seg["length"][idx], 0.5 * h / -d[:, 2]).astype(np.float32)
+    seg["t0"][idx] = (-(h / -d[:, 2]) / 0.299792458).astype(np.float32)
+    if layout == "4 telescopes":
+        tel = cfg["telescopes"].copy(); tel[:, 3] = 25.0
+    else:
+        tel = wl.telescopes_grid(n=4, spacing=60.0, r=12.0)
+    cfg["telescopes"] = tel
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_REFRACT)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report(f"refract-inclined {layout}", rep)
+    vz = -np.sqrt(np.maximum(0.0, 1.0 - g["records"]["cx"].astype(np.float64) ** 2 - g["records"]["cy"].astype(np.float64) ** 2))
+    n_mid, n_flat = int(((vz > -0.5) & (vz <= -0.25)).sum()), int((vz > -0.25).sum())
+    print(f"[refract-inclined {layout}] records with 0.25 <= |v_z| < 0.5: {n_mid}, flatter: {n_flat}")
+    assert rep["matched"] > 5000 and n_mid > 500 and n_flat > 50
+    cfg["params"] = dict(cfg["params"], flags=c8.FLAG_REFRACT | c8.FLAG_CULL)
+    gc = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    assert np.array_equal(gc["records"]["id"], g["records"]["id"]) and np.array_equal(gc["records"]["x"], g["records"]["x"])
+    assert gc["counters"]["culled"] > 0
+
+
 def test_refraction_with_culling_non_coplanar(c8):
     """Both flags, spheres of different sizes at different altitudes: the culling test carries the refraction reach."""
     import parity_util as pu
