@@ -48,10 +48,13 @@ class Params(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("processes", C.c_uint32),
                 ("lam1", C.c_double), ("lam2", C.c_double), ("bunch_size", C.c_double),
                 ("fl_yield", C.c_double), ("fl_lam1", C.c_double), ("fl_lam2", C.c_double),
-                ("fl_beam_telescope", C.c_int), ("fl_beam_halfangle", C.c_double), ("refract", C.c_int)]
+                ("fl_beam_telescope", C.c_int), ("fl_beam_halfangle", C.c_double), ("refract", C.c_int),
+                ("cut_mode", C.c_int), ("cut_angle", C.c_double)]
 
 
 FLAG_REFRACT = 2      # the bit of params["flags"] that asks for the refraction corrections (R27)
+FLAG_CUT_CENTRE = 4   # R29: angular particle cut against the experiment centre ...
+FLAG_CUT_TELESCOPES = 8   # ... or against the nearest telescope; params["cut_angle"] in rad
 
 
 class Frame(C.Structure):
@@ -71,7 +74,7 @@ class Photon(C.Structure):
 TALLY_DTYPE = np.dtype([("hits", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
 RECORD_DTYPE = np.dtype([("x", "<f8"), ("y", "<f8"), ("cx", "<f8"), ("cy", "<f8"), ("t", "<f8"),
                          ("lam", "<f8"), ("w", "<f8"), ("id", "<u8"), ("tel", "<i4"), ("pad", "<i4")])
-COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "unused")
+COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "cut")
 
 
 def lib():
@@ -138,7 +141,9 @@ def make_atmosphere(atm: dict) -> Atmosphere:
 def make_params(p: dict) -> Params:
     return Params(int(p["seed"]), int(p["processes"]), p["lam1"], p["lam2"], p["bunch_size"],
                   p["fl_yield"], p["fl_lam1"], p["fl_lam2"], int(p["fl_beam_telescope"]), p["fl_beam_halfangle"],
-                  1 if (int(p.get("flags", 0)) & FLAG_REFRACT) else 0)
+                  1 if (int(p.get("flags", 0)) & FLAG_REFRACT) else 0,
+                  2 if (int(p.get("flags", 0)) & FLAG_CUT_TELESCOPES) else 1 if (int(p.get("flags", 0)) & FLAG_CUT_CENTRE) else 0,
+                  float(p.get("cut_angle", 0.0)))
 
 
 def _dp(a):
@@ -231,6 +236,20 @@ def intersect_refracted(atm: dict, e, v, tel):
     f.restype = C.c_int
     hit = f(C.byref(make_atmosphere(atm)), _dp(e), _dp(v), _dp(t), C.byref(b2), C.byref(sc), C.byref(sp), _dp(xy), _dp(vo))
     return bool(hit), b2.value, sc.value, sp.value, float(xy[0]), float(xy[1]), vo
+
+
+def particle_cut(p0, d, L, telescopes, mode: int, cut_angle: float) -> bool:
+    """R29: is the Cherenkov segment (start p0, unit direction d, length L) cut?  mode 1 = angle to the
+    experiment centre, 2 = smallest angle to a telescope."""
+    tel = np.ascontiguousarray(np.asarray(telescopes, dtype=np.float32).astype(np.float64))
+    centre = array_sphere(telescopes)
+    f = lib().orc_particle_cut
+    f.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double), C.c_double, C.POINTER(C.c_double), C.c_int,
+                  C.POINTER(C.c_double), C.c_int, C.c_double]
+    f.restype = C.c_int
+    p0 = np.ascontiguousarray(p0, dtype=np.float64)
+    d = np.ascontiguousarray(d, dtype=np.float64)
+    return bool(f(_dp(p0), _dp(d), float(L), _dp(tel), len(tel), _dp(np.ascontiguousarray(centre[:3])), int(mode), float(cut_angle)))
 
 
 def optical_depth(atm: dict, h, lam) -> float:

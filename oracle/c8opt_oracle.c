@@ -59,6 +59,8 @@ typedef struct {
     int fl_beam_telescope;             /* -1 = isotropic */
     double fl_beam_halfangle;          /* rad */
     int refract;                       /* R27: apply the refraction corrections of PAPER.md:77 to position and angle */
+    int cut_mode;                      /* R29: 0 none, 1 angle to the experiment centre, 2 smallest angle to a telescope */
+    double cut_angle;                  /* rad ("recommended cut of 6 degrees") */
 } orc_params;
 
 /* one fp32 segment record, 12 x 4 bytes (flags is a uint32 in the same slot) */
@@ -437,7 +439,7 @@ double orc_transmission(const orc_atmosphere *atm, double h, double lam, double 
  *   tallies  : orc_tally[n_tel], accumulated into
  *   counters : uint64[8] accumulated into:
  *              0 segments, 1 photons generated, 2 upward (v_z >= 0), 3 hits,
- *              4 records stored, 5 records dropped (capacity), 6 invalid segments, 7 unused
+ *              4 records stored, 5 records dropped (capacity), 6 invalid segments, 7 bunches of cut segments (R29)
  *   records  : NULL or orc_record[cap]; *n_rec is advanced
  * Brute force over ALL telescopes; a photon may hit several; no shadowing (R10).
  */
@@ -455,6 +457,30 @@ void orc_array_sphere(const double *tel, int n_tel, double out[4])
         rb = fmax(rb, sqrt(x * x + y * y + z * z) + tel[4 * k + 3]);
     }
     out[3] = rb;
+}
+
+/* R29, the angular particle cut of PAPER.md:57 (section 1.2.1, Fig. 2): "calculate the angle difference between the
+ * currently handled particles' flight direction and the vector to the experiment center.  For higher precision, the
+ * minimum angle to each individual telescope can be used."  A Cherenkov segment is not handled (no photon is drawn)
+ * when that angle exceeds the cut.  The vector is taken from the segment midpoint m = p0 + (L/2) d; the experiment
+ * centre is the centre of the bounding box of the telescope centres (the point of R28).  angle(d, u) > cut is decided
+ * as d.u < cos(cut) |u|, so that no inverse cosine enters.  Returns 1 when the segment is cut.  The cut is lossy: it
+ * is the paper's trade of photons for speed, unlike the exact culling of the GPU path, which the oracle never needs. */
+int orc_particle_cut(const double p0[3], const double d[3], double L, const double *tel, int n_tel, const double centre[3],
+                     int mode, double cut_angle)
+{
+    if (mode == 0) return 0;
+    double cc = cos(cut_angle);
+    int n = (mode == 2) ? n_tel : 1;
+    for (int k = 0; k < n; ++k) {
+        const double *c = (mode == 2) ? &tel[4 * k] : centre;
+        double u[3];
+        for (int i = 0; i < 3; ++i) u[i] = c[i] - (p0[i] + (0.5 * L) * d[i]);
+        double dot = (d[0] * u[0] + d[1] * u[1]) + d[2] * u[2];
+        double norm = sqrt((u[0] * u[0] + u[1] * u[1]) + u[2] * u[2]);
+        if (!(dot < cc * norm)) return 0;          /* within the cut of this target: the segment is handled */
+    }
+    return 1;
 }
 
 void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
@@ -476,6 +502,11 @@ void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
                              : (tag == 1 && par->fl_beam_telescope == -2) ? array : NULL;
             if (orc_preamble(atm, par, &seg[i], tag, bt, &f) != 0) { invalid = 1; continue; }
             if (counts) counts[2 * i + tag] = f.n_b;
+            if (tag == 0 && orc_particle_cut(f.p0, f.d, f.L, tel, n_tel, array, par->cut_mode, par->cut_angle)) {
+                counters[1] += f.n_b;          /* the bunches of a cut segment count as generated ... */
+                counters[7] += f.n_b;          /* ... and as skipped */
+                continue;
+            }
             for (uint32_t j = 0; j < f.n_b; ++j) {
                 orc_photon ph;
                 orc_make_photon(&f, par, S, j, tag, &ph);

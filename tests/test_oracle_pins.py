@@ -854,3 +854,94 @@ def test_cherenkov_pair_shares_one_philox_block_R20():
     assert abs(c[0, 1]) < 0.03 and abs(c[0, 2]) < 0.03 and abs(c[1, 2]) < 0.03
     # neighbours 2k, 2k + 1 are as independent as any other two photons
     assert abs(np.corrcoef(u[0::2, 0], u[1::2, 0])[0, 1]) < 0.03 and abs(np.corrcoef(u[0::2, 2], u[1::2, 2])[0, 1]) < 0.03
+
+
+# ------------------------------------------------------------------ angular particle cut (R29)
+def _tilted(axis, deg, azimuth_deg=40.0):
+    """Unit vector at `deg` degrees from the unit vector `axis` (independent construction: Gram-Schmidt + cos / sin)."""
+    axis = np.asarray(axis, dtype=np.float64) / np.linalg.norm(axis)
+    t = np.cross(axis, [0.3, -0.2, 0.9]); t /= np.linalg.norm(t)
+    s = np.cross(axis, t)
+    a, ph = math.radians(deg), math.radians(azimuth_deg)
+    return math.cos(a) * axis + math.sin(a) * (math.cos(ph) * t + math.sin(ph) * s)
+
+
+def test_particle_cut_hand_built_angles():
+    """A segment whose midpoint is 8 km above and 3 km beside the experiment centre: kept while its direction is within the
+    cut of the line to the centre, cut beyond; the angle is re-measured here with an inverse cosine (the oracle uses
+    none).  The vector starts at the MIDPOINT of the segment (R29)."""
+    tel = W.telescopes_square()                                       # centre (0, 0, 2000)
+    mid = np.array([3000.0, -1000.0, 10000.0])
+    to_centre = np.array([0.0, 0.0, 2000.0]) - mid
+    cut = math.radians(6.0)
+    for deg, expect_cut in ((0.0, False), (5.9, False), (5.999, False), (6.001, True), (6.1, True), (90.0, True), (170.0, True)):
+        d = _tilted(to_centre, deg)
+        L = 40.0
+        p0 = mid - 0.5 * L * d
+        ang = math.acos(np.clip(np.dot(d, to_centre) / np.linalg.norm(to_centre), -1.0, 1.0))
+        assert math.isclose(ang, math.radians(deg), abs_tol=1e-9)
+        assert O.particle_cut(p0, d, L, tel, 1, cut) is expect_cut
+    # measured from the start point instead, a long segment would be judged differently: 2 km long, aimed at the centre from its midpoint
+    d = to_centre / np.linalg.norm(to_centre)
+    assert not O.particle_cut(mid - 1000.0 * d, d, 2000.0, tel, 1, math.radians(0.01))
+    assert not O.particle_cut(mid, d, 0.0, tel, 0, 0.0)               # mode 0: never cut
+
+
+def test_particle_cut_nearest_telescope_mode():
+    """Mode 2 ("the minimum angle to each individual telescope"): a segment aimed at a telescope 400 m from
+    the array centre, 3 km up, is 7.6 degrees off the centre (cut at 6 degrees in mode 1) but 0 degrees off that telescope
+    (kept in mode 2); aimed 6.5 degrees off every telescope it is cut in both."""
+    tel = np.array([[400.0, 0.0, 2000.0, 6.0], [-400.0, 0.0, 2000.0, 6.0], [0.0, 400.0, 2000.0, 6.0], [0.0, -400.0, 2000.0, 6.0]], dtype=np.float32)
+    mid = np.array([400.0, 0.0, 5000.0])
+    d = np.array([0.0, 0.0, -1.0])
+    cut = math.radians(6.0)
+    off_centre = math.degrees(math.atan2(400.0, 3000.0))
+    assert 7.5 < off_centre < 7.7
+    assert O.particle_cut(mid - 5.0 * d, d, 10.0, tel, 1, cut) and not O.particle_cut(mid - 5.0 * d, d, 10.0, tel, 2, cut)
+    far = np.array([5000.0, 5000.0, 9000.0])
+    assert O.particle_cut(far, d, 10.0, tel, 1, cut) and O.particle_cut(far, d, 10.0, tel, 2, cut)
+    # brute force over random segments: mode 2 cuts exactly those whose smallest angle (arccos) exceeds the cut
+    rng = np.random.Generator(np.random.PCG64(11))
+    n_cut = 0
+    for _ in range(300):
+        p0 = np.array([rng.uniform(-2000, 2000), rng.uniform(-2000, 2000), rng.uniform(3000, 12000)])
+        dd = _tilted([0.0, 0.0, -1.0], rng.uniform(0.0, 25.0), rng.uniform(0.0, 360.0))
+        L = rng.uniform(0.0, 30.0)
+        m = p0 + 0.5 * L * dd
+        angs = [math.acos(np.clip(np.dot(dd, t[:3] - m) / np.linalg.norm(t[:3] - m), -1, 1)) for t in tel.astype(np.float64)]
+        if abs(min(angs) - cut) < 1e-6:
+            continue
+        assert O.particle_cut(p0, dd, L, tel, 2, cut) is (min(angs) > cut)
+        n_cut += min(angs) > cut
+    assert 50 < n_cut < 280
+
+
+def test_particle_cut_in_the_whole_path():
+    """With the cut, the run is the uncut run restricted to the kept segments: same records for them, none for the
+    others; every bunch still counts as generated, the bunches of cut segments are reported; fluorescence is never cut."""
+    cfg = W.make_config("c2", n_segments=3000)
+    cfg["telescopes"][:, 3] = 40.0
+    par = dict(cfg["params"], processes=3, fl_yield=20.0)
+    a = O.run(cfg["atmosphere"], cfg["telescopes"], cfg["segments"], par, record_capacity=1 << 20)
+    cut = math.radians(3.0)
+    b = O.run(cfg["atmosphere"], cfg["telescopes"], cfg["segments"], dict(par, flags=O.FLAG_CUT_CENTRE, cut_angle=cut), record_capacity=1 << 20)
+    assert np.array_equal(a["counts"], b["counts"])
+    ca, cb = (dict(zip(O.COUNTER_NAMES, (int(v) for v in r["counters"]))) for r in (a, b))
+    assert ca["cut"] == 0 and cb["generated"] == ca["generated"]
+    seg = cfg["segments"]
+    dn = np.stack([seg["dx"], seg["dy"], seg["dz"]], axis=1).astype(np.float64)
+    dn /= np.linalg.norm(dn, axis=1, keepdims=True)
+    mid = np.stack([seg["x0"], seg["y0"], seg["z0"]], axis=1).astype(np.float64) + 0.5 * seg["length"].astype(np.float64)[:, None] * dn
+    u = np.array([0.0, 0.0, 2000.0]) - mid
+    ang = np.arccos(np.clip(np.sum(dn * u, axis=1) / np.linalg.norm(u, axis=1), -1, 1))
+    is_cut = ang > cut
+    assert 0.2 < is_cut.mean() < 0.95
+    assert cb["cut"] == int(a["counts"][is_cut, 0].astype(np.int64).sum())
+    ra, rb = a["records"], b["records"]
+    keep = ~(is_cut[(ra["id"] >> 25).astype(np.int64)] & (((ra["id"] >> 24) & 1) == 0))
+    ra = ra[keep]
+    ka, kb = np.lexsort((ra["tel"], ra["id"])), np.lexsort((rb["tel"], rb["id"]))
+    assert len(ra) == len(rb) and 0 < len(rb) < len(a["records"])
+    for f in ("id", "tel", "x", "y", "t", "w"):
+        assert np.array_equal(ra[f][ka], rb[f][kb])
+    assert int(((rb["id"] >> 24) & 1).sum()) == int(((a["records"]["id"] >> 24) & 1).sum()) > 0      # fluorescence untouched
