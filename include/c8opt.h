@@ -78,6 +78,17 @@ extern "C" {
  * direction and the direction turns by dtheta = tan(theta0) (eta(e_z) - eta(c_z)); the sphere test and the record
  * use the corrected point and direction; the arrival time (optical path, R8) changes only to second order and stands. */
 #define C8OPT_FLAG_REFRACT 2u
+/* CUT_CENTRE / CUT_TELESCOPES: the paper's own angular particle cut (section 1.2.1, Fig. 2 :63-65; DESIGN.md
+ * R29): "calculate the angle difference between the currently handled particles' flight direction and the vector to the
+ * experiment center.  For higher precision, the minimum angle to each individual telescope can be used."  A Cherenkov
+ * segment whose direction is more than c8opt_run_params.cut_angle_rad (the paper recommends 6 degrees) off the vector
+ * from its midpoint to the experiment centre (centre of the bounding box of the telescope centres) -- or, with
+ * CUT_TELESCOPES, off the vector to every telescope centre -- is not handled: no photon is drawn.  Unlike CULL this cut
+ * is LOSSY (that is the paper's trade; its Fig. 2 is the lost light against the cut angle): tallies and records are those
+ * of the kept segments.  The bunches of a cut segment still count as generated and are reported in
+ * counters[C8OPT_CNT_CULLED].  Fluorescence is never cut.  Both flags set = CUT_TELESCOPES. */
+#define C8OPT_FLAG_CUT_CENTRE      4u
+#define C8OPT_FLAG_CUT_TELESCOPES  8u
 
 typedef struct c8opt_ctx c8opt_ctx;   /* opaque, owned by the library */
 
@@ -125,6 +136,7 @@ typedef struct {
                                       C8OPT_BEAM_ARRAY beam at the whole array (R28)        */
     uint32_t flags;                /* C8OPT_FLAG_* bits                                     */
     double   fl_beam_halfangle_rad;
+    double   cut_angle_rad;        /* C8OPT_FLAG_CUT_*: the angular particle cut, in [0, pi] */
 } c8opt_run_params;
 
 /* Optional outputs of one propagate call; every pointer is DEVICE memory owned

@@ -28,6 +28,8 @@ MODE_TALLY, MODE_OUTPUT, MODE_GROUND_HIST = 0, 1, 2
 BEAM_ARRAY = -2
 FLAG_CULL = 1
 FLAG_REFRACT = 2
+FLAG_CUT_CENTRE = 4
+FLAG_CUT_TELESCOPES = 8
 COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped", "invalid", "culled")
 TALLY_DTYPE = np.dtype([("hits", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
 HIST_DTYPE = np.dtype([("n", "<u8"), ("sum_w", "<f8"), ("sum_wt", "<f8")])
@@ -61,7 +63,8 @@ class _RunParams(C.Structure):
     _fields_ = [("seed", C.c_uint64), ("processes", C.c_uint32), ("mode", C.c_uint32),
                 ("lam1_nm", C.c_double), ("lam2_nm", C.c_double), ("bunch_size", C.c_double),
                 ("fl_yield_per_MeV", C.c_double), ("fl_lam1_nm", C.c_double), ("fl_lam2_nm", C.c_double),
-                ("fl_beam_telescope", C.c_int32), ("flags", C.c_uint32), ("fl_beam_halfangle_rad", C.c_double)]
+                ("fl_beam_telescope", C.c_int32), ("flags", C.c_uint32), ("fl_beam_halfangle_rad", C.c_double),
+                ("cut_angle_rad", C.c_double)]
 
 
 class _Output(C.Structure):
@@ -126,7 +129,8 @@ def make_run_params(p: dict) -> _RunParams:
     return _RunParams(int(p["seed"]), int(p["processes"]), int(p.get("mode", MODE_TALLY)),
                       float(p["lam1"]), float(p["lam2"]), float(p["bunch_size"]),
                       float(p["fl_yield"]), float(p["fl_lam1"]), float(p["fl_lam2"]),
-                      int(p["fl_beam_telescope"]), int(p.get("flags", 0)), float(p["fl_beam_halfangle"]))
+                      int(p["fl_beam_telescope"]), int(p.get("flags", 0)), float(p["fl_beam_halfangle"]),
+                      float(p.get("cut_angle", 0.0)))
 
 
 class Context:

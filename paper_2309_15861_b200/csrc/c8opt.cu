@@ -42,6 +42,7 @@ struct c8opt_ctx {
     int hist_bins = 0;
     double hist_core_x = 0, hist_core_y = 0, hist_r_max = 0;
     float4 *d_telA = nullptr;
+    double4 *d_telD = nullptr;         // absolute centres in double (x, y, z, R): the angular particle cut (R29)
     float *d_telT = nullptr;
     float *d_telEta = nullptr;
     std::vector<float> h_telEta;
@@ -242,7 +243,13 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     const unsigned procs = rp->processes;
     if (procs == 0 || (procs & ~3u)) return fail(ctx, C8OPT_ERR_ARGUMENT, "processes must be a combination of bits 0 and 1");
     if (rp->mode > 2u) return fail(ctx, C8OPT_ERR_ARGUMENT, "mode must be 0 (tally), 1 (photon output) or 2 (ground histogram)");
-    if (rp->flags & ~(C8OPT_FLAG_CULL | C8OPT_FLAG_REFRACT)) return fail(ctx, C8OPT_ERR_ARGUMENT, "unknown bit in flags");
+    if (rp->flags & ~(C8OPT_FLAG_CULL | C8OPT_FLAG_REFRACT | C8OPT_FLAG_CUT_CENTRE | C8OPT_FLAG_CUT_TELESCOPES))
+        return fail(ctx, C8OPT_ERR_ARGUMENT, "unknown bit in flags");
+    if (rp->flags & (C8OPT_FLAG_CUT_CENTRE | C8OPT_FLAG_CUT_TELESCOPES)) {
+        if (hist) return fail(ctx, C8OPT_ERR_ARGUMENT, "no particle cut in ground-histogram mode (every bunch counts)");
+        if (!(rp->cut_angle_rad >= 0.0 && rp->cut_angle_rad <= 3.14159265358979323846))
+            return fail(ctx, C8OPT_ERR_ARGUMENT, "cut_angle_rad must be in [0, pi]");
+    }
     if (!(rp->bunch_size > 0.0) || !std::isfinite(rp->bunch_size)) return fail(ctx, C8OPT_ERR_ARGUMENT, "bunch_size must be > 0");
     if (procs & C8OPT_PROC_CHERENKOV)
         if (!(rp->lam1_nm > 0.0) || !(rp->lam2_nm > rp->lam1_nm)) return fail(ctx, C8OPT_ERR_ARGUMENT, "need 0 < lam1 < lam2");
@@ -284,6 +291,8 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     }
     P.processes = procs; P.n_procs = (procs == 3u) ? 2u : 1u;
     P.flags = rp->flags; P.cull_Rb = ctx->cull_Rb;
+    P.telD = ctx->d_telD;
+    P.cut_cos = (rp->flags & (C8OPT_FLAG_CUT_CENTRE | C8OPT_FLAG_CUT_TELESCOPES)) ? std::cos(rp->cut_angle_rad) : -2.0;
     if (rp->flags & C8OPT_FLAG_REFRACT) {
         if (ctx->tel_src == c8::TEL_GRID && !ctx->have_refract_grid && !hist)
             return fail(ctx, C8OPT_ERR_ARGUMENT, "C8OPT_FLAG_REFRACT: no candidate grid with the refraction reach can be built for this array");
@@ -510,8 +519,8 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     DeviceGuard guard(ctx->device);
     C8_CUDA(ctx, cudaDeviceSynchronize());
     ctx->n_tel = 0;
-    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid);
-    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_telEta = nullptr; ctx->d_grid = nullptr;
+    cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid); cudaFree(ctx->d_telD);
+    ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_telEta = nullptr; ctx->d_grid = nullptr; ctx->d_telD = nullptr;
     ctx->tel_xyzr.assign(xyzr, xyzr + 4 * (size_t)n);
     // reference point: centre of the bounding box; all device coordinates are relative to it
     ctx->x_ref = 0.5 * (lo[0] + hi[0]); ctx->y_ref = 0.5 * (lo[1] + hi[1]); ctx->z_ref = 0.5 * (lo[2] + hi[2]);
@@ -545,6 +554,12 @@ int c8opt_add_telescopes(c8opt_ctx *ctx, const float *xyzr, int32_t n)
     ctx->d_cursors = reinterpret_cast<unsigned long long *>(ctx->d_results + 64);
     ctx->d_tallies = reinterpret_cast<c8::Tally *>(ctx->d_results + 64 + 8 * (size_t)n);
     ctx->d_capacity = reinterpret_cast<unsigned long long *>(ctx->d_results + 64 + 32 * (size_t)n);
+    {
+        std::vector<double4> D(n);
+        for (int k = 0; k < n; ++k) D[k] = make_double4(xyzr[4 * k], xyzr[4 * k + 1], xyzr[4 * k + 2], xyzr[4 * k + 3]);
+        C8_CUDA(ctx, cudaMalloc(&ctx->d_telD, sizeof(double4) * n));
+        C8_CUDA(ctx, cudaMemcpy(ctx->d_telD, D.data(), sizeof(double4) * n, cudaMemcpyHostToDevice));
+    }
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telA, A.data(), sizeof(float4) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telT, T.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
     C8_CUDA(ctx, cudaMemcpy(ctx->d_telEta, ctx->h_telEta.data(), sizeof(float) * n, cudaMemcpyHostToDevice));
@@ -746,6 +761,7 @@ void c8opt_destroy(c8opt_ctx *ctx)
         cudaFree(ctx->d_stage[i]);
     }
     for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
+    cudaFree(ctx->d_telD);
     cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid);
     cudaFree(ctx->d_results); cudaFreeHost(ctx->h_results); cudaFree(ctx->d_hist);
     cudaGetLastError();

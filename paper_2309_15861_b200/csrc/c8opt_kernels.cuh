@@ -48,6 +48,7 @@ constexpr int kGenericWeight = 6;     // cost of a generic-kind photon in axis-k
 constexpr int kCullTelMax = 128;      // culling tests the telescopes one by one up to this many, else only the array's bounding sphere
 constexpr uint32_t kFlagCull = 1u;    // == C8OPT_FLAG_CULL
 constexpr uint32_t kFlagRefract = 2u; // == C8OPT_FLAG_REFRACT
+constexpr uint32_t kFlagCutCentre = 4u, kFlagCutTel = 8u;   // == C8OPT_FLAG_CUT_CENTRE / _TELESCOPES
 constexpr float kRefractVzMin = 0.25f;   // R27: the corrections apply to photons with |v_z| >= 0.25 (zenith <= 75.5 degrees)
 constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
 constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
@@ -83,6 +84,8 @@ struct KParams {
     const float4 *telA;            // device: (cx - x_ref, cy - y_ref, cz - z_ref, R^2)
     const float *telT;             // device: column depth T(c_z) [g/cm^2]
     const float *telEta;           // device: refractivity eta(c_z)  (C8OPT_FLAG_REFRACT)
+    const double4 *telD;           // device: absolute centres in double (x, y, z, R), the angular particle cut (R29)
+    double cut_cos;                // cos(cut_angle_rad)
     float4 tel_c[kTelConstMax];    // the same two tables in the constant bank when n_tel <= kTelConstMax
     float telT_c[kTelConstMax];
     float telEta_c[kTelConstMax];
@@ -378,6 +381,26 @@ __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, 
     return true;
 }
 
+// The paper's angular particle cut (R29): true = the Cherenkov segment is not handled, because its
+// direction d is more than the cut angle off the vector from its midpoint to the experiment centre (or, kFlagCutTel,
+// to every telescope centre).  angle > cut is decided as d.u < cos(cut) |u|, in double, explicit round-to-nearest
+// operations in the oracle's order, so that both sides cut the same segments.
+__device__ __noinline__ bool particle_cut(const KParams &P, const double p0[3], const double d[3], double L)
+{
+    const int n = (P.flags & kFlagCutTel) ? P.n_tel : 1;
+    const double hl = dmul(0.5, L);
+    for (int k = 0; k < n; ++k) {
+        double c[3] = { P.x_ref, P.y_ref, P.z_ref };
+        if (P.flags & kFlagCutTel) { const double4 T = P.telD[k]; c[0] = T.x; c[1] = T.y; c[2] = T.z; }
+        double u[3];
+        for (int i = 0; i < 3; ++i) u[i] = dsub(c[i], dadd(p0[i], dmul(hl, d[i])));
+        const double dot = dadd(dadd(dmul(d[0], u[0]), dmul(d[1], u[1])), dmul(d[2], u[2]));
+        const double norm = sqrt(dadd(dadd(dmul(u[0], u[0]), dmul(u[1], u[1])), dmul(u[2], u[2])));
+        if (!(dot < dmul(P.cut_cos, norm))) return false;
+    }
+    return true;
+}
+
 // Preamble of emitter (segment i, process tag).  Writes the frame, returns n_b.
 // *bad is set when the segment is invalid: 1 = non-finite field, gamma <= 1, L < 0 or |d| off unity by > 1e-3 (the
 // same for both processes), 2 = n_b >= 2^24 for this process.
@@ -456,6 +479,10 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     if (nb > 16777215.0) { *bad = 2; return 0; }
     double w0 = ddiv(mu, nb);
     if (kind == KIND_CONE && P.beam_tel >= 0) w0 *= 0.5 * P.omc;  // R14 (weight form): Omega / 4 pi
+    if ((P.flags & (kFlagCutCentre | kFlagCutTel)) && tag == 0 && particle_cut(P, p0, d, L)) {
+        *culled = true;
+        return (uint32_t)nb;
+    }
     if ((P.flags & kFlagCull) && tag == 0) {
         const double hl = 0.5 * L;
         if (cull_emitter(P, (float)(p0[0] + hl * d[0] - P.x_ref), (float)(p0[1] + hl * d[1] - P.y_ref), (float)(p0[2] + hl * d[2] - P.z_ref),
@@ -1828,7 +1855,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         }
         if (culled) { n_culled = nb; nb = 0u; }           // generated, but provably no hit: not propagated
     }
-    if (P.flags & kFlagCull) {
+    if (P.flags & (kFlagCull | kFlagCutCentre | kFlagCutTel)) {
         unsigned long long c = n_culled;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);

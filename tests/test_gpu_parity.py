@@ -286,6 +286,27 @@ def test_segment_culling_changes_nothing(c8, name, n):
         assert frac > 0.2          # fluorescence (c3b) is never culled
 
 
+@pytest.mark.parametrize("name,n,flag,deg", [("c2", 50_000, "centre", 6.0), ("c2", 50_000, "telescopes", 2.0), ("c4", 60_000, "centre", 4.0),
+                                             ("c4", 60_000, "telescopes", 1.5), ("c1", None, "centre", 1.0)])
+def test_angular_particle_cut(c8, name, n, flag, deg):
+    """C8OPT_FLAG_CUT_CENTRE / _TELESCOPES (the paper's own lossy cut, R29) against the oracle with the same
+    cut: the same segments are cut on both sides (decided in double, same operation order), so counts, tallies and
+    records are compared exactly as without it; the bunches of the cut segments are reported."""
+    import parity_util as pu
+    cfg = wl.make_config(name) if n is None else wl.make_config(name, n_segments=n)
+    full = pu.gpu_run(cfg, c8.MODE_TALLY)
+    fl = c8.FLAG_CUT_CENTRE if flag == "centre" else c8.FLAG_CUT_TELESCOPES
+    cfg["params"] = dict(cfg["params"], flags=fl, cut_angle=float(np.radians(deg)))
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o, check_upward=False)
+    _report(f"cut-{name}-{flag}-{deg}", rep)
+    assert g["counters"]["culled"] == int(o["counters"][7]) > 0
+    lost = 1.0 - g["counters"]["hits"] / full["counters"]["hits"]
+    print(f"[cut {name} {flag} {deg} deg] bunches skipped {g['counters']['culled'] / g['counters']['generated']:.3f}, hits lost {lost:.4f}")
+    assert 0.0 <= lost < 1.0 and rep["matched"] > 50
+
+
 def test_segment_culling_non_coplanar_big_spheres(c8):
     """Culling with telescopes of different sizes at different altitudes, against the oracle (which never culls)."""
     import parity_util as pu
