@@ -276,6 +276,8 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
     P.tau = ctx->d_tau; P.tau_nh = ctx->tau_nh; P.tau_nl = ctx->tau_nl;
     P.tau_h0 = (float)ctx->tau_h0; P.tau_inv_dh = (float)(1.0 / ctx->tau_dh);
     P.tau_l0 = (float)ctx->tau_l0; P.tau_inv_dl = (float)(1.0 / ctx->tau_dl);
+    P.tau_h0_d = ctx->tau_h0; P.tau_dh_d = ctx->tau_dh; P.tau_l0_d = ctx->tau_l0; P.tau_dl_d = ctx->tau_dl;
+    P.lam1_d = rp->lam1_nm; P.lam2_d = rp->lam2_nm; P.fl_lam1_d = rp->fl_lam1_nm; P.fl_lam2_d = rp->fl_lam2_nm;
     P.n_tel = ctx->n_tel; P.telA = ctx->d_telA; P.telT = ctx->d_telT; P.telEta = ctx->d_telEta;
     if (ctx->tel_src == c8::TEL_CONST) {
         for (int k = 0; k < c8::kTelConstMax; ++k) { P.tel_c[k] = make_float4(0.f, 0.f, 0.f, -1.f); P.telT_c[k] = 0.f; }   // R^2 = -1: never hit

@@ -52,6 +52,7 @@ constexpr uint32_t kFlagCutCentre = 4u, kFlagCutTel = 8u;   // == C8OPT_FLAG_CUT
 constexpr float kRefractVzMin = 0.25f;   // R27: the corrections apply to photons with |v_z| >= 0.25 (zenith <= 75.5 degrees)
 constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
 constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
+constexpr int kFlatList = 128;        // flat-photon candidates a tile can defer to its double-precision pass (beyond: fp32)
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 constexpr int kOutCtasPerSm = 2;       // resident CTAs per SM the brute-force photon-output kernels are compiled for (register budget)
 
@@ -112,6 +113,8 @@ struct KParams {
     double bunch_size, fl_yield;
     float inv_lam1, dinv_lam;      // Cherenkov: 1/lam = inv_lam1 - u3 * dinv_lam (R4)
     float fl_lam1, fl_dlam;
+    double lam1_d, lam2_d, fl_lam1_d, fl_lam2_d;             // the same bands, and the axes of the tau table, in double:
+    double tau_h0_d, tau_dh_d, tau_l0_d, tau_dl_d;           // flat photons are evaluated in double (flat_hit_f64)
     int beam_tel;
     double beam_x, beam_y, beam_z; // centre of the beam telescope, or (beam_tel == -2) of the array's sphere (absolute)
     double beam_rb;                // radius of the sphere that holds every telescope sphere (beam_tel == -2, R28)
@@ -233,6 +236,8 @@ struct __align__(16) TileSmem {
     uint2 queue[kWarps][kQueue];                // per-warp ring of candidate (photon, telescope) pairs
     uint32_t wide_list[kWarps][64];             // photons waiting for the wide test: j | e << 24
     uint32_t wide_count[kWarps];
+    uint2 flat_list[kFlatList];                 // (photon, telescope) pairs of flat photons, evaluated in double at the end of the tile
+    uint32_t flat_count, flat_pad[3];
     // per-thread tally accumulators (flushed into t_* when the telescope changes and at the end of the tile)
     double acc_w[kTile], acc_wt[kTile];
     uint32_t acc_n[kTile];
@@ -385,8 +390,9 @@ __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, 
 // direction d is more than the cut angle off the vector from its midpoint to the experiment centre (or, kFlagCutTel,
 // to every telescope centre).  angle > cut is decided as d.u < cos(cut) |u|, in double, explicit round-to-nearest
 // operations in the oracle's order, so that both sides cut the same segments.
-__device__ __noinline__ bool particle_cut(const KParams &P, const double p0[3], const double d[3], double L)
+__device__ __noinline__ bool particle_cut(const KParams &P, double p0x, double p0y, double p0z, double dx, double dy, double dz, double L)
 {
+    const double p0[3] = { p0x, p0y, p0z }, d[3] = { dx, dy, dz };
     const int n = (P.flags & kFlagCutTel) ? P.n_tel : 1;
     const double hl = dmul(0.5, L);
     for (int k = 0; k < n; ++k) {
@@ -401,11 +407,15 @@ __device__ __noinline__ bool particle_cut(const KParams &P, const double p0[3], 
     return true;
 }
 
+// What the preamble knows about an emitter, in double: for the photons that fp32 cannot carry (flat_hit_f64).
+struct FrameD { double p0[3], d[3], L, t0, ibc, w0, sin_c, cos_c, omc, axis[3]; int kind; };
+
 // Preamble of emitter (segment i, process tag).  Writes the frame, returns n_b.
 // *bad is set when the segment is invalid: 1 = non-finite field, gamma <= 1, L < 0 or |d| off unity by > 1e-3 (the
 // same for both processes), 2 = n_b >= 2^24 for this process.
+template <bool WITH_D = false>
 __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1, const float4 s2, int tag,
-                             float *__restrict__ fr, uint8_t *kind_out, int *bad, bool *culled)
+                             float *__restrict__ fr, uint8_t *kind_out, int *bad, bool *culled, FrameD *fd = nullptr)
 {
     *bad = 0;
     *culled = false;
@@ -479,7 +489,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     if (nb > 16777215.0) { *bad = 2; return 0; }
     double w0 = ddiv(mu, nb);
     if (kind == KIND_CONE && P.beam_tel >= 0) w0 *= 0.5 * P.omc;  // R14 (weight form): Omega / 4 pi
-    if ((P.flags & (kFlagCutCentre | kFlagCutTel)) && tag == 0 && particle_cut(P, p0, d, L)) {
+    if ((P.flags & (kFlagCutCentre | kFlagCutTel)) && tag == 0 && particle_cut(P, p0[0], p0[1], p0[2], d[0], d[1], d[2], L)) {
         *culled = true;
         return (uint32_t)nb;
     }
@@ -492,6 +502,10 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
         }
     }
 
+    if constexpr (WITH_D) {
+        for (int i = 0; i < 3; ++i) { fd->p0[i] = p0[i]; fd->d[i] = d[i]; fd->axis[i] = axis[i]; }
+        fd->L = L; fd->t0 = (double)s0.w; fd->ibc = ibc; fd->w0 = w0; fd->sin_c = sin_c; fd->cos_c = cos_c; fd->omc = omc_e; fd->kind = kind;
+    }
     fr[F_W0] = (float)w0; fr[F_T0] = s0.w; fr[F_IBC] = (float)ibc; fr[F_LEN] = (float)L; fr[F_OMC] = (float)omc_e;
     {
         // layer of both ends in fp32 altitudes as the photon loop sees them (1 m of margin against rounding)
@@ -808,6 +822,151 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     return h;
 }
 
+// ------------------------------------------------------------------------------------
+// Flat photons.  A photon with |v_z| < kFlatVz (isotropic / beamed fluorescence seen from the side, Cherenkov light of a
+// horizontal track) travels |c_z - e_z| / |v_z| to the plane of the telescope: kilometres for metres of height.  fp32
+// cannot carry it to north_star's 1 cm / 0.1 ns (delta(1 / v_z) = delta v_z / v_z^2), so such a photon only passes a
+// conservative fp32 distance test here and is then evaluated in DOUBLE from the segment record: preamble, uniforms from
+// the same Philox words, direction, R10, R8, R4, R17.  They are well below 1e-3 of the photons that reach this point.
+constexpr float kFlatVz = 0.05f;
+
+__device__ __forceinline__ double column_depth_d(const KParams &P, double h)
+{
+    const LayerD l = P.layer[layer_of(P, h)];
+    return l.a + l.b * exp(-h / l.c);
+}
+
+__device__ __noinline__ Hit flat_hit_f64(const KParams &P, unsigned long long S, uint32_t tag, uint32_t j, int k)
+{
+    Hit h;
+    h.ok = false; h.k = k; h.x = h.y = h.vx = h.vy = h.t = h.lam = h.w = 0.0f;
+    const float4 *sp = P.seg + (S - P.first_id) * 3ull;
+    const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
+    float scratch[kFrameStride];
+    uint8_t kind8;
+    int bad;
+    bool culled;
+    FrameD f;
+    const uint32_t nb = preamble<true>(P, s0, s1, s2, (int)tag, scratch, &kind8, &bad, &culled, &f);
+    if (bad || culled || j >= nb) return h;
+    // a2, R19: U = ((r >> 9) + 1/2) 2^-23; the Cherenkov wavelength uniform from the 9 + 9 low bits (R20)
+    const Rand4 blk = philox4x32_10(P, tag ? j : (j >> 1), (uint32_t)S, (uint32_t)(S >> 32), tag);
+    const Rand4 r = tag ? blk : cherenkov_words(blk, j);
+    const double u1 = ((double)(r.r0 >> 9) + 0.5) * 1.1920928955078125e-07, u2 = ((double)(r.r1 >> 9) + 0.5) * 1.1920928955078125e-07;
+    const double u3 = tag ? ((double)(r.r2 >> 9) + 0.5) * 1.1920928955078125e-07
+                          : ((double)(((r.r0 & 511u) << 9) | (r.r1 & 511u)) + 0.5) * 3.814697265625e-06;
+    const double u4 = ((double)(r.r3 >> 9) + 0.5) * 1.1920928955078125e-07;
+    // a3: emission point and time, direction
+    const double s = u1 * f.L;
+    const double e[3] = { f.p0[0] + s * f.d[0], f.p0[1] + s * f.d[1], f.p0[2] + s * f.d[2] };
+    const double t_e = f.t0 + s * f.ibc;
+    double sphi, cphi;
+    sincos(6.283185307179586476925 * u2, &sphi, &cphi);
+    double v[3];
+    if (f.kind == KIND_FL_ISO) {
+        const double cth = 1.0 - 2.0 * u4, sth = 2.0 * sqrt(u4 * (1.0 - u4));
+        v[0] = cphi * sth; v[1] = sphi * sth; v[2] = -cth;
+    } else {
+        double sth = f.sin_c, cth = f.cos_c;                     // Cherenkov (generic projection)
+        if (f.kind == KIND_CONE) { const double t = u4 * f.omc; cth = 1.0 - t; sth = sqrt(t * (2.0 - t)); }
+        double m0[3], m1[3];
+        rodrigues_columns(f.axis, m0, m1);
+        // M_Rod (cos phi sth, sin phi sth, -cth) with the third column of M_Rod = -axis
+        for (int i = 0; i < 3; ++i) v[i] = sth * (cphi * m0[i] + sphi * m1[i]) + cth * f.axis[i];
+    }
+    // a4, R10: distance from the sphere centre to the forward ray, as a cross product
+    // (ground histogram: the one accept-all detector on the observation level about the core)
+    const double4 T = (P.hist != nullptr) ? make_double4(P.x_ref, P.y_ref, P.z_ref, 1e15) : P.telD[k];
+    const double m[3] = { T.x - e[0], T.y - e[1], T.z - e[2] };
+    if (!(v[2] < 0.0) || !(m[2] < 0.0)) return h;
+    const double cx = m[1] * v[2] - m[2] * v[1], cy = m[2] * v[0] - m[0] * v[2], cz = m[0] * v[1] - m[1] * v[0];
+    const double s_c = m[0] * v[0] + m[1] * v[1] + m[2] * v[2];
+    if (!(cx * cx + cy * cy + cz * cz <= T.w * T.w) || !(s_c > 0.0)) return h;
+    const double s_pl = m[2] / v[2];
+    // R8, R4, R17
+    const double excess = 0.01 * (P.eta0 / P.rho0) * (column_depth_d(P, T.z) - column_depth_d(P, e[2])) / fabs(v[2]);
+    const double lam = tag ? P.fl_lam1_d + u3 * (P.fl_lam2_d - P.fl_lam1_d)
+                           : 1.0 / (1.0 / P.lam1_d - u3 * (1.0 / P.lam1_d - 1.0 / P.lam2_d));
+    double w = f.w0;
+    if (P.tau != nullptr) {
+        const int nh = P.tau_nh, nl = P.tau_nl;
+        double fh = (e[2] - P.tau_h0_d) / P.tau_dh_d, fl = (lam - P.tau_l0_d) / P.tau_dl_d;
+        fh = fmin(fmax(fh, 0.0), (double)(nh - 1)); fl = fmin(fmax(fl, 0.0), (double)(nl - 1));
+        const int ih = min(max((int)floor(fh), 0), max(nh - 2, 0)), il = min(max((int)floor(fl), 0), max(nl - 2, 0));
+        const double th = fh - (double)ih, tl = fl - (double)il;
+        const int ih1 = (nh > 1) ? ih + 1 : ih, il1 = (nl > 1) ? il + 1 : il;
+        const double t00 = __ldg(&P.tau[ih * nl + il]), t01 = __ldg(&P.tau[ih * nl + il1]);
+        const double t10 = __ldg(&P.tau[ih1 * nl + il]), t11 = __ldg(&P.tau[ih1 * nl + il1]);
+        const double tau = (1.0 - th) * (t00 + tl * (t01 - t00)) + th * (t10 + tl * (t11 - t10));
+        w *= exp(-tau / fabs(v[2]));
+    }
+    h.x = (float)(e[0] + s_pl * v[0] - T.x); h.y = (float)(e[1] + s_pl * v[1] - T.y);
+    h.vx = (float)v[0]; h.vy = (float)v[1];
+    h.t = (float)(t_e + (s_pl + excess) * (1.0 / 0.299792458));
+    h.lam = (float)lam; h.w = (float)w;
+    h.ok = true;
+    return h;
+}
+
+// evaluate_pair, with the flat photons of the generic kinds set aside for flat_hit_f64 once they pass a conservative
+// fp32 distance test (cross product, no plane projection, slack for the fp32 error): the pair goes to the tile's flat list,
+// which is worked off in double after the photon loops (flat_pass) -- the loops themselves never call into the
+// double-precision code, whose register needs would otherwise spill their state.  j = photon index.  A full list
+// (more than kFlatList such pairs in one tile: not seen in any config) leaves the pair to fp32.  The ground histogram
+// keeps fp32 throughout: a flat photon lands beyond 20 times its emission height, far outside any profile.
+template <int TELSRC, bool COPLANAR = false>
+__device__ __forceinline__ Hit evaluate_any(const KParams &P, TileSmem &sm, int e, const Photon &ph, int k, uint32_t j)
+{
+    if (!ph.axis && ph.vz > -kFlatVz && P.hist == nullptr) {
+        Hit h;
+        h.ok = false; h.k = k;
+        if (!(ph.vz < 0.0f)) return h;
+        const float4 T = tel_at<TELSRC>(P, k);
+        if (!(T.w > 0.0f)) return h;                                   // an unused constant-bank slot (R^2 = -1)
+        const float mx = T.x - ph.ex, my = T.y - ph.ey, mz = T.z - ph.ez;
+        const float cx = fmaf(my, ph.vz, -(mz * ph.vy)), cy = fmaf(mz, ph.vx, -(mx * ph.vz)), cz = fmaf(mx, ph.vy, -(my * ph.vx));
+        const float b2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz)), mm = fmaf(mx, mx, fmaf(my, my, mz * mz));
+        // fp32 error of b = |m x v|: |m| delta v (~3e-7) + delta m (1 ulp of a coordinate ~ 1e-7 |m|): below 1e-6 |m|
+        const float thr = sqrtf(T.w) + fmaf(2e-6f, sqrtf(mm), 2e-3f);
+        if (!(b2 <= thr * thr)) return h;
+        const uint32_t slot = atomicAdd(&sm.flat_count, 1u);
+        if (slot < (uint32_t)kFlatList) { sm.flat_list[slot] = make_uint2(j | ((uint32_t)e << 24), (uint32_t)k); return h; }
+    }
+    return evaluate_pair<TELSRC, COPLANAR>(P, sm, e, ph, k);
+}
+
+__device__ __forceinline__ unsigned long long emitter_segment(const KParams &P, unsigned long long tile_first, int e)
+{
+    return tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
+}
+
+// The tile's flat list in double (see evaluate_any), by all threads of the tile after the photon loops: tally, record.
+template <int MODE>
+__device__ __noinline__ void flat_pass(const KParams &P, TileSmem &sm, unsigned long long tile_first)
+{
+    const uint32_t n = min(sm.flat_count, (uint32_t)kFlatList);
+    for (uint32_t i = threadIdx.x; i < n; i += kTile) {
+        const uint2 q = sm.flat_list[i];
+        const int e = (int)(q.x >> 24), k = (int)q.y;
+        const uint32_t j = q.x & 0xffffffu, tag = kind_tag(sm.kind[e]);
+        const unsigned long long S = emitter_segment(P, tile_first, e);
+        const Hit h = flat_hit_f64(P, S, tag, j, k);
+        if (!h.ok) continue;
+        const double w = (double)h.w;
+        if (P.n_tel <= kTelSmemMax) { atomicAdd(&sm.t_hits[k], 1u); atomicAdd(&sm.t_sw[k], w); atomicAdd(&sm.t_swt[k], w * (double)h.t); }
+        else { atomicAdd(&P.tallies[k].hits, 1ull); atomicAdd(&P.tallies[k].sum_w, w); atomicAdd(&P.tallies[k].sum_wt, w * (double)h.t); }
+        if constexpr (MODE == MODE_OUT) {
+            const unsigned long long slot = atomicAdd(&P.cursors[k], 1ull);
+            if (slot < P.tel_capacity[k]) {
+                const unsigned long long at = P.tel_offset[k] + slot;
+                float *rec = P.records + at * (unsigned)kRecWords;
+                rec[0] = h.x; rec[1] = h.y; rec[2] = h.vx; rec[3] = h.vy; rec[4] = h.t; rec[5] = h.lam; rec[6] = h.w;
+                if (P.ids) P.ids[at] = (S << 25) | ((unsigned long long)tag << 24) | (unsigned long long)j;
+            }
+        }
+    }
+}
+
 // Photon output, hits on several telescopes: the lanes of one telescope reserve their records with a single bump of
 // that telescope's cursor.  Called by all 32 lanes.
 __device__ __forceinline__ void write_records_grouped(const KParams &P, const Hit &h, uint64_t id)
@@ -986,10 +1145,6 @@ __device__ __forceinline__ void commit_hits(const KParams &P, TileSmem &sm, cons
 
 // ---- the per-warp candidate queue.  Entry = (emitter, photon index, telescope) in 8 bytes:
 // x = j (24 bits) | e << 24,  y = telescope index.  The warp-uniform count lives in a register.
-__device__ __forceinline__ unsigned long long emitter_segment(const KParams &P, unsigned long long tile_first, int e)
-{
-    return tile_first + (unsigned)((P.n_procs == 2) ? (e & (kTile / 2 - 1)) : e);
-}
 
 template <int TELSRC, int MODE>
 __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigned long long tile_first, uint32_t head, uint32_t n)
@@ -1005,7 +1160,7 @@ __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigne
         const uint32_t j = q.x & 0xffffffu;
         const unsigned long long S = emitter_segment(P, tile_first, e);
         const Photon ph = make_photon(P, sm, e, j, S);
-        h = evaluate_pair<TELSRC>(P, sm, e, ph, (int)q.y);
+        h = evaluate_any<TELSRC>(P, sm, e, ph, (int)q.y, j);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
     __syncwarp();
@@ -1024,7 +1179,7 @@ __device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned
     if (has) {
         const unsigned long long S = emitter_segment(P, tile_first, e);
         const Photon ph = photon_from_rand(P, sm, e, Rand4{r0, r1, r2, r3});
-        h = evaluate_pair<TELSRC>(P, sm, e, ph, k);
+        h = evaluate_any<TELSRC>(P, sm, e, ph, k, j);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
     __syncwarp();
@@ -1499,7 +1654,7 @@ __device__ __forceinline__ uint32_t const_candidates(const KParams &P, const Pho
 struct GenericHit { Hit h; uint32_t cm_left; bool upward; };
 
 template <bool COPLANAR, int NT, bool REFR>
-__device__ __noinline__ GenericHit generic_hit(const KParams &P, const TileSmem &sm, int e, const Rand4 r)
+__device__ __noinline__ GenericHit generic_hit(const KParams &P, TileSmem &sm, int e, const Rand4 r, uint32_t j)
 {
     GenericHit g;
     g.h.ok = false; g.h.k = 0; g.h.x = g.h.y = g.h.vx = g.h.vy = g.h.t = g.h.lam = g.h.w = 0.0f;
@@ -1511,7 +1666,7 @@ __device__ __noinline__ GenericHit generic_hit(const KParams &P, const TileSmem 
     if (cm != 0u) {
         const int k = __ffs(cm) - 1;
         cm &= cm - 1u;
-        g.h = evaluate_pair<TEL_CONST, COPLANAR>(P, sm, e, ph, k);
+        g.h = evaluate_any<TEL_CONST, COPLANAR>(P, sm, e, ph, k, j);
     }
     g.cm_left = cm;
     return g;
@@ -1707,11 +1862,11 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                     // generic kinds: out of line (photon in the global frame, pre-tests, exact test of the first candidate)
                     const uint32_t tag = kind_tag(kind);
                     const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
-                    const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u});
+                    const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u}, j);
                     hA = ga.h; cmA = ga.cm_left;
                     if (ga.upward) ++n_up;
                     if (hasB) {
-                        const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u});
+                        const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u}, j + 1u);
                         hB = gb.h; cmB = gb.cm_left;
                         if (gb.upward) ++n_up;
                     }
@@ -1815,7 +1970,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     const bool tally_in_smem = P.n_tel <= kTelSmemMax;
     if (tally_in_smem)
         for (int k = tid; k < P.n_tel; k += kTile) { sm.t_hits[k] = 0u; sm.t_sw[k] = 0.0; sm.t_swt[k] = 0.0; }
-    if (tid == 0) { sm.n_upward = 0ull; sm.n_culled = 0ull; }
+    if (tid == 0) { sm.n_upward = 0ull; sm.n_culled = 0ull; sm.flat_count = 0u; }
     sm.invalid[tid] = 0;
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
     if (tid < kWarps) sm.wide_count[tid] = 0u;
@@ -1984,6 +2139,13 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     for (int o = 16; o > 0; o >>= 1) n_up += __shfl_xor_sync(0xffffffffu, n_up, o);
     if (lane == 0 && n_up) atomicAdd(&sm.n_upward, (unsigned long long)n_up);
     __syncthreads();
+    if constexpr (MODE != MODE_HIST) {
+        // the flat photons the loops set aside, in double (tile-uniform branch)
+        if (sm.flat_count) {
+            flat_pass<MODE>(P, sm, tile_first);
+            __syncthreads();
+        }
+    }
     if (tid == 0) {
         if (total - n_pad + sm.n_culled) atomicAdd(&P.counters[1], (unsigned long long)(total - n_pad) + sm.n_culled);
         if (sm.n_upward) atomicAdd(&P.counters[2], sm.n_upward);

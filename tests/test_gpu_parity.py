@@ -537,15 +537,14 @@ def test_fluorescence_beamed_at_the_array(c8):
     tel[:, 3] = 12.0
     cfg["telescopes"] = tel
     cfg["params"] = dict(cfg["params"], fl_beam_telescope=c8.BEAM_ARRAY, fl_yield=4000.0)
-    # tracks a few metres above the telescopes' plane would reach them 2.9 km away along nearly horizontal rays
-    # (v_z ~ 0.003, t ~ 2e5 ns), beyond what fp32 positions and times can hold to 1 cm / 0.1 ns: keep the others
-    cfg["segments"] = cfg["segments"][cfg["segments"]["z0"] > 3000.0]
+    # (tracks a few metres above the telescopes' plane reach them 2.9 km away along nearly horizontal rays, v_z ~ 0.003:
+    # those photons are evaluated in double on the GPU, flat_hit_f64)
     iso_generated = int(np.ceil(4000.0 * cfg["segments"]["dE"].astype(np.float64)).sum())
     g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
     o = pu.oracle_run(cfg)
     rep = pu.compare(cfg, g, o)
     _report("beam-array-far", rep)
-    assert rep["matched"] > 300 and g["counters"]["upward"] == 0
+    assert rep["matched"] > 300          # (cones of tracks just above the telescopes' plane reach above the horizontal: upward > 0)
     assert g["counters"]["generated"] < 1e-3 * iso_generated          # the paper's gain: the number of photons
 
     cfg = wl.make_config("c4", n_segments=20_000)
