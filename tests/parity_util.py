@@ -170,14 +170,13 @@ def compare(cfg: dict, g: dict, o: dict, first_id: int = 0, check_records: bool 
             assert dt.max() <= TOL_T_NS, f"(d) time: {dt.max():.3e} ns"
             dl = np.abs(a["lam"] - b_["lam"]) / b_["lam"]
             assert dl.max() <= TOL_LAM_REL, f"wavelength: {dl.max():.3e}"
-            # weight = w0 exp(-tau / |v_z|): the fp32 exponential is good to ~2e-7 (1 + |argument|) relative, and the
-            # argument = ln(w0 / w) reaches tens for the flat photons of isotropic fluorescence, whose weight is ~0
-            w0_max = float(cfg["params"]["bunch_size"])
-            arg = np.log(np.maximum(w0_max / np.maximum(np.abs(b_["w"]), 1e-300), 1.0))
-            dw = np.abs(a["w"] - b_["w"]) / np.abs(b_["w"]) / (1.0 + arg)
+            # weight = w0 exp(-tau / |v_z|), plain relative error: the flat photons (|v_z| < 0.05), whose exponent reaches
+            # hundreds, are evaluated in double on the GPU; for the others the exponent stays below 20 (2e-7 x 20 in fp32)
+            dw = np.abs(a["w"] - b_["w"]) / np.maximum(np.abs(b_["w"]), 1e-300)
             assert dw.max() <= TOL_W_REL, f"weight: {dw.max():.3e}"
             rep.update(max_dxy_m=float(max(dx.max(), dy.max())), max_ang_rad=float(ang.max()), max_dt_ns=float(dt.max()),
-                       max_dlam_rel=float(dl.max()), max_dw_rel=float(dw.max()))
+                       max_dlam_rel=float(dl.max()), max_dw_rel=float(dw.max()),
+                       flat_records_two_component_direction=int((~steep).sum()))
         rep.update(matched=len(common), flips=len(flips))
     # (b) per-telescope tallies: within 1e-3 relative, or explained by the enumerated boundary flips
     B = float(cfg["params"]["bunch_size"])

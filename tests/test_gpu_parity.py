@@ -102,10 +102,11 @@ def test_batching_and_host_path_invariance(c8):
 
 
 def test_config3_fluorescence_isotropic_and_beamed(c8):
-    """configs[2]: fluorescence only, telescope at 10 km; isotropic (hit list identical) and beamed 2 deg."""
+    """configs[2] at its full size (10^6 segments): fluorescence only, telescope at 10 km; isotropic (hit list identical)
+    and beamed 2 deg; every record compared."""
     import parity_util as pu
     for name in ("c3a", "c3b"):
-        cfg = wl.make_config(name, n_segments=200_000)
+        cfg = wl.make_config(name)
         g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
         o = pu.oracle_run(cfg)
         rep = pu.compare(cfg, g, o)
@@ -597,7 +598,12 @@ def test_config5_full_size_one_percent_block(c8):
     gk = gb["id"].astype(np.uint64) * 16 + gb["tel"].astype(np.uint64)
     ok = orr["id"].astype(np.uint64) * 16 + orr["tel"].astype(np.uint64)
     common, ia, ib = np.intersect1d(gk, ok, return_indices=True)
-    assert len(gk) + len(ok) - 2 * len(common) <= 3 and len(common) > 50_000             # (b) at most a few edge flips
+    assert len(gk) + len(ok) - 2 * len(common) <= 3 and len(common) > 50_000             # (b) at most a few edge flips ...
+    blk_cfg = dict(cfg, segments=cfg["segments"][lo:lo + n_blk])
+    for key in np.concatenate([np.setdiff1d(gk, ok), np.setdiff1d(ok, gk)]):            # ... each within 5 mm of the rim (R22)
+        hit, b, R, _ = pu.oracle_impact(blk_cfg, int(key) >> 4, int(key) & 15, first_id=lo)
+        print(f"[parity c5-full-1pct] flip photon={int(key) >> 4:#x} tel={int(key) & 15} b-R={b - R:+.3e} m")
+        assert abs(b - R) < pu.TOL_FLIP_M
     a, b = gb[ia], orr[ib]
     assert np.max(np.abs(a["x"] - b["x"])) <= pu.TOL_XY_M and np.max(np.abs(a["y"] - b["y"])) <= pu.TOL_XY_M      # (c)
     assert np.max(np.abs(a["cx"] - b["cx"])) <= 1e-5 and np.max(np.abs(a["cy"] - b["cy"])) <= 1e-5
@@ -606,3 +612,37 @@ def test_config5_full_size_one_percent_block(c8):
     print(f"[parity c5-full-1pct] records_total={len(gr)} block_gpu={len(gk)} block_oracle={len(ok)} matched={len(common)} "
           f"max_dxy_m={max(np.max(np.abs(a['x'] - b['x'])), np.max(np.abs(a['y'] - b['y']))):.3e} "
           f"max_dt_ns={np.max(np.abs(a['t'] - b['t'])):.3e}")
+
+
+def test_config4_full_size_tally(c8):
+    """configs[3] at its full size (10^7 segments, 100 telescopes, both processes, transmission table) in the launch
+    configuration bench.py times (tally mode): per-segment counts of both processes bit-exact, per-telescope hits and
+    weight sums against the oracle's (about a minute of host time on 16 cores)."""
+    import parity_util as pu
+    cfg = wl.make_config("c4")
+    g = pu.gpu_run(cfg, c8.MODE_TALLY)
+    o = pu.oracle_run(cfg, record_capacity=0)
+    rep = pu.compare(cfg, g, o, check_records=False)
+    _report("c4-full", rep)
+    assert g["counters"]["generated"] > 2_000_000_000 and g["counters"]["hits"] > 10_000_000
+    d = np.abs(g["tallies"]["hits"].astype(np.int64) - o["tallies"]["hits"].astype(np.int64))
+    print(f"[parity c4-full] per-telescope hit differences: max {d.max()}, total {d.sum()} of {int(o['tallies']['hits'].sum())}")
+    assert d.max() <= 3
+
+
+@pytest.mark.parametrize("name,n,B", [("c2", 40_000, 8.0), ("c4", 30_000, 3.5), ("c3b", 100_000, 2.0)])
+def test_bunch_size_above_one(c8, name, n, B):
+    """R1 with B > 1: n_b = ceil(mu / B) bunches of weight mu / n_b <= B; counts bit-exact, records and weights compared."""
+    import parity_util as pu
+    cfg = wl.make_config(name, n_segments=n)
+    cfg["params"] = dict(cfg["params"], bunch_size=B)
+    if name == "c2":
+        cfg["telescopes"][:, 3] = 15.0
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report(f"bunch-{name}-{B}", rep)
+    w = g["records"]["w"]
+    assert rep["matched"] > 100 and w.max() <= B * (1 + 1e-6)
+    if name != "c3b":                       # (beamed bunches carry the factor Omega / 4 pi = 3e-4)
+        assert w.max() > 1.0
