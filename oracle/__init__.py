@@ -80,7 +80,8 @@ COUNTER_NAMES = ("segments", "generated", "upward", "hits", "records", "dropped"
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
+        # C8OPT_ORACLE_LIB: a build of the same source made elsewhere (the sanitizer test's ASan / UBSan build)
+        L = C.CDLL(os.environ.get("C8OPT_ORACLE_LIB") or build())
         u32p, dp = C.POINTER(C.c_uint32), C.POINTER(C.c_double)
         L.orc_philox4x32_10.argtypes = [u32p, u32p, u32p]
         L.orc_philox4x32_10.restype = None

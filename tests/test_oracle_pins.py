@@ -945,3 +945,37 @@ def test_particle_cut_in_the_whole_path():
     for f in ("id", "tel", "x", "y", "t", "w"):
         assert np.array_equal(ra[f][ka], rb[f][kb])
     assert int(((rb["id"] >> 24) & 1).sum()) == int(((a["records"]["id"] >> 24) & 1).sum()) > 0      # fluorescence untouched
+
+
+# ------------------------------------------------------------------ sanitizers
+def test_oracle_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """The oracle's C built with -fsanitize=address,undefined (errors abort) runs every branch of the whole path on a
+    small case -- both processes, transmission table, refraction, the particle cut, array beaming, records up to and
+    beyond their capacity, the ground histogram, threads -- and gives the same result as the plain build."""
+    import subprocess
+    import sys
+    src = os.path.join(os.path.dirname(O.__file__), "c8opt_oracle.c")
+    san = str(tmp_path / "liboracle_san.so")
+    subprocess.check_call(["gcc", "-std=c99", "-O1", "-g", "-ffp-contract=off", "-fPIC", "-shared", "-fsanitize=address,undefined",
+                           "-fno-sanitize-recover=all", "-o", san, src, "-lm"])
+    asan = subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
+    script = r"""
+import sys, numpy as np
+sys.path.insert(0, %r)
+import oracle as O, workloads as W
+cfg = W.make_config("c4", n_segments=400)
+par = dict(cfg["params"], flags=O.FLAG_REFRACT | O.FLAG_CUT_TELESCOPES, cut_angle=0.2)
+a = O.run(cfg["atmosphere"], cfg["telescopes"], cfg["segments"], par, record_capacity=1 << 16, threads=3)
+b = O.run(cfg["atmosphere"], cfg["telescopes"], cfg["segments"], dict(par, fl_beam_telescope=O.BEAM_ARRAY), record_capacity=8)
+h = O.ground_histogram(cfg["atmosphere"], cfg["segments"], cfg["params"], (1.0, 2.0), 800.0, 40, threads=2)
+c1 = W.make_config("c3b", n_segments=300)
+c = O.run(c1["atmosphere"], c1["telescopes"], c1["segments"], c1["params"], record_capacity=1 << 12)
+print(int(a["tallies"]["hits"].sum()), int(a["counters"][7]), int(b["counters"][5]), int(h["hist"]["n"].sum()), int(c["counters"][1]))
+""" % os.path.dirname(os.path.dirname(O.__file__))
+    outs = []
+    for env_extra in ({"LD_PRELOAD": asan, "C8OPT_ORACLE_LIB": san, "ASAN_OPTIONS": "detect_leaks=0"}, {}):
+        env = dict(os.environ, **env_extra)
+        r = subprocess.run([sys.executable, "-c", script], env=env, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        outs.append(r.stdout.strip().splitlines()[-1])
+    assert outs[0] == outs[1] and int(outs[0].split()[0]) > 100 and int(outs[0].split()[2]) > 0
