@@ -295,11 +295,13 @@ __device__ __forceinline__ HistSmem &hist_smem(TileSmem &sm) { return *reinterpr
 //   F_DZ, F_AX..F_CY (v_x, v_y coefficients), F_LEN; F_LAYER = bits of the int index of the atmosphere layer that
 //   holds the lower end of the segment, F_HNEXT = lower bound of the next layer if the segment reaches into it (else
 //   +inf), F_LAYER = -1 if it spans more than two layers; F_OMC = 1 - cos(half-angle) of a beamed emitter's cone.
+// Fluorescence kinds: the polar window outside of which no photon of the emitter can reach the array (polar_cull):
+//   F_VZLO, F_VZHI bound v_z of an isotropic photon, F_TMAX bounds 1 - cos(theta') of a beamed one.
 enum {
     F_NEGL = 0, F_K0C = 1, F_AZ = 2, F_BZ = 3, F_CZ = 4, F_PX = 5, F_PY = 6, F_QX = 7, F_QY = 8, F_GX = 9, F_GY = 10,
     F_E0 = 0, F_D0 = 3, F_L = 6, F_A0 = 7, F_B0 = 10, F_C0 = 13,
     F_W0 = 16, F_T0 = 17, F_IBC = 18, F_DZ = 19, F_AX = 20, F_AY = 21, F_BX = 22, F_BY = 23, F_CX = 24, F_CY = 25,
-    F_LEN = 26, F_LAYER = 27, F_OMC = 28, F_HNEXT = 29
+    F_LEN = 26, F_LAYER = 27, F_OMC = 28, F_HNEXT = 29, F_VZLO = 30, F_VZHI = 31, F_TMAX = 32
 };
 
 // ------------------------------------------------------------------------------------
@@ -518,6 +520,38 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     }
     *kind_out = (uint8_t)kind;
     const double e0[3] = { p0[0] - P.x_ref, p0[1] - P.y_ref, p0[2] - P.z_ref };
+    if (kind == KIND_FL_ISO || kind == KIND_CONE) {
+        // Exact cull per photon ("it is vital that the above method must be very fast"): a photon can hit a
+        // telescope only if it passes within R_b of the array centre c, i.e. only if its direction is within
+        // A = asin(R_b / D) + asin((L/2) / D) of the line from the segment midpoint to c (D = |c - m| - L/2).  For an
+        // isotropic photon that bounds v_z = -cos(theta), which the polar uniform alone gives, to a window; for a
+        // beamed one it bounds the polar angle about the cone axis.  Photons outside are dropped before their
+        // direction is built (polar_cull); the ground histogram takes every photon.
+        // (fp32 is ample: the window carries 2e-5 rad of slack against 1e-6 of rounding)
+        float vz_lo = -1.0f, vz_hi = 1.0f, t_max = __int_as_float(0x7f800000);
+        if (P.hist == nullptr) {
+            const float hl = (float)(0.5 * L);
+            const float ux = -(float)(e0[0] + 0.5 * L * d[0]), uy = -(float)(e0[1] + 0.5 * L * d[1]), uz = -(float)(e0[2] + 0.5 * L * d[2]);
+            const float Dm = sqrtf(fmaf(ux, ux, fmaf(uy, uy, uz * uz))), D = Dm - hl;
+            const float Rb = P.cull_Rb * 1.00001f + ((P.flags & kFlagRefract) ? 62.5f * P.refr_cmax : 0.0f) + 0.02f;
+            if (D > Rb * 1.0001f) {
+                const float A = asinf(Rb / D) + asinf(fminf(1.0f, hl / D)) + 2e-5f;
+                if (kind == KIND_FL_ISO) {
+                    const float thu = acosf(fminf(1.0f, fmaxf(-1.0f, uz / Dm)));
+                    vz_lo = cosf(fminf(3.14159265f, thu + A)) - 1e-5f;
+                    vz_hi = cosf(fmaxf(0.0f, thu - A)) + 1e-5f;
+                } else {
+                    const float ca = ((float)axis[0] * ux + (float)axis[1] * uy + (float)axis[2] * uz) / Dm;
+                    const float th_max = acosf(fminf(1.0f, fmaxf(-1.0f, ca))) + A + 6e-4f;      // (acos near 1 loses digits: 1e-7 in its argument is 4.5e-4 rad)
+                    const float alpha_b = acosf(fmaxf(-1.0f, 1.0f - (float)omc_e));
+                    // only when the whole cone points below the horizon: a dropped photon is then known to go down
+                    if (acosf(fminf(1.0f, fmaxf(-1.0f, -(float)axis[2]))) + alpha_b < 1.5697f && th_max < 3.1415f)
+                    { const float sh = sinf(0.5f * th_max); t_max = 2.0f * sh * sh * 1.0001f + 1e-12f; }   // 1 - cos, without cancellation
+                }
+            }
+        }
+        fr[F_VZLO] = vz_lo; fr[F_VZHI] = vz_hi; fr[F_TMAX] = t_max;
+    }
     if (kind == KIND_FL_ISO) {
         for (int i = 0; i < 3; ++i) { fr[F_E0 + i] = (float)e0[i]; fr[F_D0 + i] = (float)d[i]; }
         fr[F_L] = (float)L;
@@ -1375,6 +1409,21 @@ __device__ __forceinline__ void wide_push(const KParams &P, TileSmem &sm, unsign
     if (lane == 0u) sm.wide_count[warp] = n;
 }
 
+// The polar window of a fluorescence emitter (see the preamble): true = the photon with polar word r3 cannot reach the
+// array, or goes up (*up; counted by the caller) -- decided from one uniform, before the direction is built.
+__device__ __forceinline__ bool polar_cull(const TileSmem &sm, int e, int kind, uint32_t r3, bool *up)
+{
+    const float *fr = &sm.frame[e * kFrameStride];
+    *up = false;
+    if (kind == KIND_FL_ISO) {
+        const float vz = fmaf(2.0f, uniform01(r3), -1.0f);             // - cos(theta), exact (R16)
+        *up = !(vz < 0.0f);
+        return *up || vz < fr[F_VZLO] || vz > fr[F_VZHI];
+    }
+    if (kind == KIND_CONE) return uniform01(r3) * fr[F_OMC] > fr[F_TMAX];
+    return false;
+}
+
 // a2-a4 of the hot loop for the generic kinds.  Returns the candidate mask (see plane_candidates); *upward is
 // set when the photon does not go down.  Photons flatter than |v_z| = 0.05 are tested against all telescopes.
 template <int TELSRC, bool COPLANAR, int NT, bool REFR>
@@ -1467,7 +1516,8 @@ __device__ __forceinline__ void walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 // the same hoisted Philox as the axis kind (the process tag is counter word 3)
                 r = kind_tag(kind) ? philox_photon(P, pe, j, 1u) : cherenkov_words(philox_photon(P, pe, j >> 1, 0u), j);
                 bool up;
-                cm = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, r.r0, r.r1, r.r2, r.r3, &cell, &up);
+                if (!polar_cull(sm, e, kind, r.r3, &up))
+                    cm = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, r.r0, r.r1, r.r2, r.r3, &cell, &up);
                 if (up) ++n_up;
             }
         }
@@ -1589,11 +1639,13 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                 bool up;
                 const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
                 rA = tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u};
-                cmA = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rA.r0, rA.r1, rA.r2, rA.r3, &cellA, &up);
+                if (!polar_cull(sm, e, kind, rA.r3, &up))
+                    cmA = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rA.r0, rA.r1, rA.r2, rA.r3, &cellA, &up);
                 if (up) ++n_up;
                 if (hasB) {
                     rB = tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u};
-                    cmB = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rB.r0, rB.r1, rB.r2, rB.r3, &cellB, &up);
+                    if (!polar_cull(sm, e, kind, rB.r3, &up))
+                        cmB = generic_candidates<TELSRC, COPLANAR, NT, REFR>(P, sm, e, rB.r0, rB.r1, rB.r2, rB.r3, &cellB, &up);
                     if (up) ++n_up;
                 }
             }
@@ -1862,13 +1914,19 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                     // generic kinds: out of line (photon in the global frame, pre-tests, exact test of the first candidate)
                     const uint32_t tag = kind_tag(kind);
                     const Rand4 blk0 = philox_photon(P, pe, tag ? j : (j >> 1), tag);
-                    const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u}, j);
-                    hA = ga.h; cmA = ga.cm_left;
-                    if (ga.upward) ++n_up;
+                    bool up;
+                    if (!polar_cull(sm, e, kind, blk0.r3, &up)) {
+                        const GenericHit ga = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? blk0 : Rand4{blk0.r0, blk0.r1, 0u, 0u}, j);
+                        hA = ga.h; cmA = ga.cm_left; up = ga.upward;
+                    }
+                    if (up) ++n_up;
                     if (hasB) {
-                        const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u}, j + 1u);
-                        hB = gb.h; cmB = gb.cm_left;
-                        if (gb.upward) ++n_up;
+                        const Rand4 rB = tag ? philox_photon(P, pe, j + 1u, 1u) : Rand4{blk0.r2, blk0.r3, 0u, 0u};
+                        if (!polar_cull(sm, e, kind, rB.r3, &up)) {
+                            const GenericHit gb = generic_hit<COPLANAR, NT, REFR>(P, sm, e, rB, j + 1u);
+                            hB = gb.h; cmB = gb.cm_left; up = gb.upward;
+                        }
+                        if (up) ++n_up;
                     }
                 }
             }
