@@ -52,7 +52,7 @@ constexpr uint32_t kFlagCutCentre = 4u, kFlagCutTel = 8u;   // == C8OPT_FLAG_CUT
 constexpr float kRefractVzMin = 0.25f;   // R27: the corrections apply to photons with |v_z| >= 0.25 (zenith <= 75.5 degrees)
 constexpr int MODE_TALLY = 0, MODE_OUT = 1, MODE_HIST = 2;   // == C8OPT_MODE_*
 constexpr int kHistMax = 1024;        // radial bins of the ground-plane profile
-constexpr int kFlatList = 128;        // flat-photon candidates a tile can defer to its double-precision pass (beyond: fp32)
+constexpr int kFlatList = 96;         // flat-photon candidates a tile can defer to its double-precision pass (beyond: fp32)
 constexpr int kQueue = 64;            // candidate-queue entries per warp (power of two, >= 2 * 32)
 constexpr int kOutCtasPerSm = 2;       // resident CTAs per SM the brute-force photon-output kernels are compiled for (register budget)
 
@@ -225,6 +225,7 @@ struct __align__(16) TileSmem {
     uint32_t prefix[kTile + 8];                 // exclusive scan of n_b; prefix[kTile] = total
     float frame[kTile * kFrameStride];          // fp32 frames, see frame slots below
     uint8_t kind[kTile];
+    uint8_t tmask[kTile];                       // constant-bank telescopes the emitter can reach (reach_mask)
     uint8_t invalid[kTile];
     uint32_t warp_sum[kWarps], warp_pad[kWarps];
     uint8_t odd[kTile + 8];                     // 1 = the emitter's count is odd: its last slot of the index space is empty
@@ -388,6 +389,28 @@ __device__ __noinline__ bool cull_emitter(const KParams &P, float mx, float my, 
     return true;
 }
 
+// Which of the <= kTelConstMax constant-bank telescopes can a photon of this Cherenkov emitter reach at all?  The culling
+// test, telescope by telescope (bit k = telescope k); 0xff when the question does not apply (ground histogram).  The
+// pair loop skips the pre-tests of the telescopes that no lane of the warp can reach (walk_pairs).
+__device__ __noinline__ uint32_t reach_mask(const KParams &P, float mx, float my, float mz, float dx, float dy, float dz, float hl,
+                                            float sin_c, float cos_c)
+{
+    if (P.hist != nullptr || P.n_tel > kTelConstMax) return 0xffu;
+    float grow = 0.0f;
+    if (P.flags & kFlagRefract) {
+        const float vzm = fmaxf(fmaf(fabsf(dz), cos_c, -sqrtf(fmaxf(fmaf(-dz, dz, 1.0f), 0.0f)) * sin_c) - 1e-3f, kRefractVzMin);
+        grow = 1.02f * P.refr_cmax * sqrtf(fmaxf(fmaf(-vzm, vzm, 1.0f), 0.0f)) / (vzm * vzm * vzm) + 0.01f;
+    }
+    if (!cone_reaches(-mx, -my, -mz, P.cull_Rb + grow, dx, dy, dz, hl, sin_c, cos_c)) return 0u;
+    uint32_t m = 0u;
+    for (int k = 0; k < P.n_tel; ++k) {
+        const float4 T = P.tel_c[k];
+        const float R = T.w * rsqrtf(fmaxf(T.w, 1e-30f)) + grow;
+        if (cone_reaches(T.x - mx, T.y - my, T.z - mz, R, dx, dy, dz, hl, sin_c, cos_c)) m |= 1u << k;
+    }
+    return m;
+}
+
 // The paper's angular particle cut (R29): true = the Cherenkov segment is not handled, because its
 // direction d is more than the cut angle off the vector from its midpoint to the experiment centre (or, kFlagCutTel,
 // to every telescope centre).  angle > cut is decided as d.u < cos(cut) |u|, in double, explicit round-to-nearest
@@ -415,10 +438,12 @@ struct FrameD { double p0[3], d[3], L, t0, ibc, w0, sin_c, cos_c, omc, axis[3]; 
 // Preamble of emitter (segment i, process tag).  Writes the frame, returns n_b.
 // *bad is set when the segment is invalid: 1 = non-finite field, gamma <= 1, L < 0 or |d| off unity by > 1e-3 (the
 // same for both processes), 2 = n_b >= 2^24 for this process.
-template <bool WITH_D = false>
+template <bool WITH_D = false, bool WITH_MASK = false>
 __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1, const float4 s2, int tag,
-                             float *__restrict__ fr, uint8_t *kind_out, int *bad, bool *culled, FrameD *fd = nullptr)
+                             float *__restrict__ fr, uint8_t *kind_out, int *bad, bool *culled, FrameD *fd = nullptr,
+                             uint8_t *tmask_out = nullptr)
 {
+    if constexpr (WITH_MASK) *tmask_out = 0xffu;
     *bad = 0;
     *culled = false;
     const double L = (double)s1.w, gamma = (double)s2.x, zq = (double)s2.y, dE = (double)s2.z;
@@ -495,7 +520,17 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
         *culled = true;
         return (uint32_t)nb;
     }
-    if ((P.flags & kFlagCull) && tag == 0) {
+    if (WITH_MASK && tag == 0 && P.n_tel <= kTelConstMax) {
+        // small arrays: the telescopes this emitter can reach at all; none = culled (C8OPT_FLAG_CULL)
+        const double hl = 0.5 * L;
+        const uint32_t tm = reach_mask(P, (float)(p0[0] + hl * d[0] - P.x_ref), (float)(p0[1] + hl * d[1] - P.y_ref), (float)(p0[2] + hl * d[2] - P.z_ref),
+                                       (float)d[0], (float)d[1], (float)d[2], (float)hl, (float)sin_c, (float)cos_c);
+        *tmask_out = (uint8_t)tm;
+        if ((P.flags & kFlagCull) && tm == 0u) {
+            *culled = true;
+            return (uint32_t)nb;
+        }
+    } else if ((P.flags & kFlagCull) && tag == 0) {
         const double hl = 0.5 * L;
         if (cull_emitter(P, (float)(p0[0] + hl * d[0] - P.x_ref), (float)(p0[1] + hl * d[1] - P.y_ref), (float)(p0[2] + hl * d[2] - P.z_ref),
                          (float)d[0], (float)d[1], (float)d[2], (float)hl, (float)sin_c, (float)cos_c)) {
@@ -1571,6 +1606,20 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
     AxisFrame f_reg = load_axis_frame(sm, e);
     for (uint32_t b0 = base; b0 < hi; b0 += 64u, g += 64u, j += 64u) {
         const bool active = g < hi;
+        // brute-force kernels: the telescopes that any lane's emitter can reach at all (reach_mask); the pre-tests of the
+        // others are skipped for the whole warp (most emitters of a shower reach none; a trip spans one or two emitters)
+        uint32_t umask = 0xffu;
+        if constexpr (TELSRC == TEL_CONST) {
+            if (active && g >= end) {
+                do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
+                rend = end - sm.odd[e];
+                j = g - sm.prefix[e];
+                kind = sm.kind[e];
+                pe = philox_emitter(P, emitter_segment(P, tile_first, e));
+                f_reg = load_axis_frame(sm, e);
+            }
+            umask = __reduce_or_sync(0xffffffffu, active ? (uint32_t)sm.tmask[e] : 0u);
+        }
         uint32_t cmA = 0u, cmB = 0u;
         uint2 cellA = make_uint2(0xffffffffu, 0xffffffffu), cellB = cellA;
         Rand4 rA = {0u, 0u, 0u, 0u}, rB = rA;
@@ -1578,7 +1627,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
         hA.ok = false; hA.k = 0; hA.x = hA.y = hA.vx = hA.vy = hA.t = hA.lam = hA.w = 0.0f;
         hB = hA;
         if (active) {
-            if (g >= end) {
+            if (TELSRC != TEL_CONST && g >= end) {
                 do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
                 rend = end - sm.odd[e];
                 j = g - sm.prefix[e];
@@ -1607,9 +1656,24 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                     vxA = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); vyA = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
                     vxB = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); vyB = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
                 }
-                if (vzA < 0.0f) cmA = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxA, gyA, vxA, vyA, vzA, &cellA); else ++n_up;
-                if (hasB) {
-                    if (vzB < 0.0f) cmB = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cellB); else ++n_up;
+                if constexpr (TELSRC == TEL_CONST) {
+                    // the pre-tests of both photons, telescope by telescope, for the telescopes in reach of the warp
+                    const bool dnA = vzA < 0.0f, dnB = hasB && vzB < 0.0f;
+                    n_up += (dnA ? 0u : 1u) + ((hasB && !dnB) ? 1u : 0u);
+                    const float vz2sA = vzA * vzA * 0.9999f, vz2sB = vzB * vzB * 0.9999f;
+                    const float addA = REFR ? refraction_slack(P, vzA) : 0.0f, addB = REFR ? refraction_slack(P, vzB) : 0.0f;
+#pragma unroll
+                    for (int k = 0; k < NT; ++k) {
+                        if ((umask >> k) & 1u) {
+                            if (dnA && plane_pretest<COPLANAR>(P.tel_c[k], gxA, gyA, vxA, vyA, vzA, vz2sA, addA)) cmA |= 1u << k;
+                            if (dnB && plane_pretest<COPLANAR>(P.tel_c[k], gxB, gyB, vxB, vyB, vzB, vz2sB, addB)) cmB |= 1u << k;
+                        }
+                    }
+                } else {
+                    if (vzA < 0.0f) cmA = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxA, gyA, vxA, vyA, vzA, &cellA); else ++n_up;
+                    if (hasB) {
+                        if (vzB < 0.0f) cmB = plane_candidates<TELSRC, COPLANAR, NT, REFR>(P, gxB, gyB, vxB, vyB, vzB, &cellB); else ++n_up;
+                    }
                 }
                 if constexpr (INLINE) {
                     const float *fr = &sm.frame[e * kFrameStride];
@@ -2055,7 +2119,8 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
         int bad;
         bool culled;
-        nb = preamble(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled);
+        nb = preamble<false, TELSRC == TEL_CONST>(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled, nullptr,
+                                                  &sm.tmask[tid]);
         if (P.split_part == 2) {
             // second launch of a two-process request: the first one (Cherenkov) has counted the segments that are
             // invalid for both processes or for Cherenkov; what is left to count here is a segment whose fluorescence
