@@ -1114,7 +1114,10 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, uint32_t pari
         ".reg .pred p;\n"
         "WAIT_%=:\n"
         "mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%0], %1;\n"
-        "@!p bra WAIT_%=;\n"
+        "@p bra DONE_%=;\n"
+        "nanosleep.u32 200;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
         "}\n" :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
 }
 __device__ __forceinline__ uint32_t add_acq_rel_cta(uint32_t *p, uint32_t v)
@@ -1867,6 +1870,17 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
     float part_w = 0.0f, part_wt = 0.0f;
     double acc_w = 0.0, acc_wt = 0.0;
     const uint32_t n_rounds = (n_trips + SUB - 1u) / SUB;
+    // The warp that arrives last at a round bumps the cursor, but does not wait for the answer (2-3 us under the write
+    // load): it publishes the base only after the arithmetic of its next trip (lane 0: pend_b is the pending result).
+    unsigned long long pend_b = 0ull;
+    uint32_t pend_r = 0xffffffffu;
+    auto publish_pending = [&]() {
+        if (lane == 0u && pend_r != 0xffffffffu) {
+            *(volatile unsigned long long *)&os.rbase[pend_r & (kRoundSlots - 1)] = pend_b;
+            mbar_arrive_release(&os.rbar[pend_r & (kRoundSlots - 1)]);
+            pend_r = 0xffffffffu;
+        }
+    };
     for (uint32_t r = 0; r < n_rounds; ++r) {
         float *const st = os.stage[warp] + (r % NB) * kBufWords;
         unsigned long long *const sid = reinterpret_cast<unsigned long long *>(st + kBlockRecs * kRecWords);
@@ -2022,6 +2036,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                 part_w += wA + wB;
                 part_wt += (sA ? hA.w * hA.t : 0.0f) + (sB ? hB.w * hB.t : 0.0f);
             }
+            if (t == 0u) publish_pending();
             const uint32_t mA = __ballot_sync(0xffffffffu, sA), mB = __ballot_sync(0xffffffffu, sB);
             const uint32_t nA = (uint32_t)__popc(mA);
             if (sA) {
@@ -2048,10 +2063,9 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                 // last arrival of round r: reserve the round's records, publish the base
                 const uint32_t total = (old >> 8) + cnt;
                 os.agg[r & (kRoundSlots - 1)] = 0u;
-                unsigned long long b = 0ull;
-                if (total) b = atomicAdd(&P.cursors[kd], (unsigned long long)total);
-                *(volatile unsigned long long *)&os.rbase[r & (kRoundSlots - 1)] = b;
-                mbar_arrive_release(&os.rbar[r & (kRoundSlots - 1)]);
+                pend_b = 0ull;
+                if (total) pend_b = atomicAdd(&P.cursors[kd], (unsigned long long)total);
+                pend_r = r;
             }
         }
         __syncwarp();
@@ -2060,6 +2074,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
         off_h[0] = __shfl_sync(0xffffffffu, old >> 8, 0);
         n_h[0] = cnt;
     }
+    publish_pending();
     // the last NB blocks, oldest first
 #pragma unroll
     for (uint32_t i = NB; i > 0u; --i) {
