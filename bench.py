@@ -203,6 +203,8 @@ def main():
     ap.add_argument("--segments", type=int, default=None, help="override the segment count of the workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--output-segments", type=int, default=None,
+                    help="segment count of the photon-output leg (default: configs[4]'s 10^7)")
     ap.add_argument("--no-output-leg", action="store_true",
                     help="skip the photon-output leg (roofline_output) that the default c2 run adds")
     ap.add_argument("--ground-hist", action="store_true",
@@ -370,18 +372,24 @@ def main():
     # observation level, every downward photon written as a 28-byte record ("c5g" at this segment count)
     roofline_output = None
     if args.workload == "c2" and not (args.no_output_leg or args.cull or args.ground_hist) and rank == 0:
-        octx = c8.Context(cfg["atmosphere"])
-        g_tel = wl.make_config("c5g", n_segments=1)["telescopes"]
-        octx.add_telescopes(np.asarray(g_tel, dtype=np.float32))
-        opar = dict(par); opar["mode"] = c8.MODE_OUTPUT
+        # "c5g": configs[4]'s segment set (the c2 generator at 10^7 segments) with one accept-all detector
+        del kw
+        ocfg = wl.make_config("c5g", n_segments=args.output_segments)
+        oseg = ocfg["segments"]
+        on = len(oseg)
+        d_seg = torch.from_numpy(oseg.view(np.uint8).reshape(on, 48).copy()).to(dev)
+        n_saved, n = n, on                              # time_leg / output_buffers read n and d_seg
+        octx = c8.Context(ocfg["atmosphere"])
+        octx.add_telescopes(np.asarray(ocfg["telescopes"], dtype=np.float32))
+        opar = dict(ocfg["params"]); opar["mode"] = c8.MODE_OUTPUT
         okw = output_buffers(octx, opar, 1)
-        ko = max(3, min(args.steps, 20))
+        ko = max(3, min(args.steps, 10))
         ocnt, oms, olaunch, _ = time_leg(octx, opar, okw, ko, 3)
         launches += olaunch
         o_s = float(oms.sum()) * 1e-3 / ko
-        obytes = RECORD_BYTES * ocnt["records"] + SEGMENT_BYTES * n
+        obytes = RECORD_BYTES * ocnt["records"] + SEGMENT_BYTES * on
         roofline_output = {
-            "bound": "hbm", "workload": f"c5g at {n} segments (the c2 segments, accept-all detector at h_obs)",
+            "bound": "hbm", "workload": f"c5g: {on} segments of configs[4] (seed 2), one accept-all detector at h_obs, photon-output mode",
             "achieved": obytes / o_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": obytes / o_s / 1e9 / peaks["hbm_gbs"],
             "traffic": None, "traffic_note": "measured per round with ncu --set full: profiles/ncu_c5g_output_r02.md",
             "peak_source": peaks["source"], "algorithmic_bytes_per_launch": obytes,
@@ -389,7 +397,8 @@ def main():
             "kernel": "c8::propagate_kernel<TEL_CONST, coplanar, 1, output>", "kernel_ms": o_s * 1e3, "steps": ko,
             "photons_per_s": ocnt["generated"] / o_s}
         octx.close()
-        del okw
+        del okw, d_seg
+        n = n_saved
 
     clocks = sampler.stop()
     if rank != 0:
