@@ -349,7 +349,9 @@ int launch_one(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, unsigned long long
 {
     // Full tiles for large inputs; small inputs are cut into about one wave of tiles (3 CTAs on each of the SMs), at
     // least 8 segments each, so that 10^4 segments do not run on a quarter of the GPU.
-    const unsigned long long per_tile_max = c8::kTile / P.n_procs;
+    // At most kTile - 1 segments per tile: the tile's photon index space is 32 bits wide and an emitter holds up to
+    // 2^24 - 1 bunches (R23), padded to 2^24 slots, so 255 emitters stay below 2^32 - 2^24 whatever their counts.
+    const unsigned long long per_tile_max = (c8::kTile - 1) / P.n_procs;
     const unsigned long long one_wave = 3ull * (unsigned long long)ctx->n_sm;
     unsigned long long per_tile = (n + one_wave - 1) / one_wave;
     per_tile = std::min(per_tile_max, std::max(8ull, per_tile));

@@ -646,3 +646,25 @@ def test_bunch_size_above_one(c8, name, n, B):
     assert rep["matched"] > 100 and w.max() <= B * (1 + 1e-6)
     if name != "c3b":                       # (beamed bunches carry the factor Omega / 4 pi = 3e-4)
         assert w.max() > 1.0
+
+
+def test_full_tile_of_emitters_near_the_bunch_limit(c8):
+    """the tile's photon index space is 32 bits wide.  300 segments of ~1.6e7 bunches each (the limit is 2^24 - 1)
+    fill one tile of 255 segments with 4.1e9 photon slots (255 x 2^24 < 2^32) and start a second one; counts bit-exact,
+    tallies against the oracle (about half a minute of host time)."""
+    import parity_util as pu
+    cfg = wl.make_config("c1", n_segments=300)
+    seg = cfg["segments"]
+    seg["x0"], seg["y0"], seg["z0"] = 0.0, 0.0, 9000.0
+    seg["dx"], seg["dy"], seg["dz"] = 0.0, 0.0, -1.0
+    seg["length"], seg["gamma"] = np.float32(50.0), np.float32(1e5)
+    seg["z0"] += np.arange(300, dtype=np.float32)                     # (distinct emitters)
+    seg["t0"] = -(seg["z0"] - 2000.0) / 0.299792458
+    cfg["params"] = dict(cfg["params"], bunch_size=4.7e-5)
+    cfg["telescopes"] = np.array([[70.0, 60.0, 2000.0, 8.0]], dtype=np.float32)
+    g = pu.gpu_run(cfg, c8.MODE_TALLY)
+    assert g["counts"][:, 0].min() > 12_000_000 and g["counts"][:, 0].max() < (1 << 24)
+    assert g["counters"]["generated"] > 4_000_000_000
+    o = pu.oracle_run(cfg, record_capacity=0)
+    rep = pu.compare(cfg, g, o, check_records=False)
+    _report("255-big-emitters", rep)
