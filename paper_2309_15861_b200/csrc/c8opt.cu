@@ -135,8 +135,13 @@ size_t smem_bytes(int mode, bool staging = true, bool ids = true)
 
 typedef void (*kernel_t)(const c8::KParams);
 
-template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar, bool out)
+// out: 0 tally, 1 photon output with the dense loop, 2 photon output without it (brute-force kernels only)
+template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar, int out)
 {
+    if constexpr (TELSRC == c8::TEL_CONST) {
+        if (out == 2)
+            return coplanar ? c8::propagate_kernel<TELSRC, true, NT, c8::MODE_OUT, false> : c8::propagate_kernel<TELSRC, false, NT, c8::MODE_OUT, false>;
+    }
     if (out) return coplanar ? c8::propagate_kernel<TELSRC, true, NT, c8::MODE_OUT> : c8::propagate_kernel<TELSRC, false, NT, c8::MODE_OUT>;
     return coplanar ? c8::propagate_kernel<TELSRC, true, NT, c8::MODE_TALLY> : c8::propagate_kernel<TELSRC, false, NT, c8::MODE_TALLY>;
 }
@@ -144,7 +149,7 @@ template <int TELSRC, int NT> kernel_t pick_kernel2(bool coplanar, bool out)
 // nt = number of constant-bank telescope slots the hot loop tests (n_tel rounded up to 1, 4 or 8)
 int padded_count(int n_tel) { return n_tel <= 1 ? 1 : (n_tel <= 4 ? 4 : 8); }
 
-kernel_t pick_kernel(int tel_src, bool coplanar, int nt, bool out)
+kernel_t pick_kernel(int tel_src, bool coplanar, int nt, int out)
 {
     if (tel_src == c8::TEL_CONST) {
         if (nt == 1) return pick_kernel2<c8::TEL_CONST, 1>(coplanar, out);
@@ -154,6 +159,11 @@ kernel_t pick_kernel(int tel_src, bool coplanar, int nt, bool out)
     if (tel_src == c8::TEL_GRID) return pick_kernel2<c8::TEL_GRID, 0>(coplanar, out);
     return pick_kernel2<c8::TEL_GLOBAL, 0>(coplanar, out);
 }
+
+// A tile of a shower's light is "dense" on a telescope (a good part of its photons hit it) only when the telescope is
+// of the size of the light pool.  Below this radius the photon-output launch takes the kernel instance without the dense
+// loop (3 CTAs/SM instead of 2); both instances are correct for any input.
+constexpr double kDenseRadiusMin_m = 30.0;
 
 // Ground-plane candidate grid: a photon with |v_z| >= vzmin that hits telescope k crosses the
 // plane z_ref within rho_k = R / vzmin + |c_z - z_ref| sqrt(1 / vzmin^2 - 1) of (c_x, c_y).  Every cell lists the
@@ -363,8 +373,9 @@ int launch_one(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, unsigned long long
         c8::propagate_kernel<c8::TEL_CONST, true, 1, c8::MODE_HIST><<<(unsigned)tiles, c8::kTile, smem_bytes(c8::MODE_HIST), st>>>(P);
     } else {
         const bool out = P.records != nullptr;
-        kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out);
-        k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, ctx->tel_src == c8::TEL_CONST, P.ids != nullptr), st>>>(P);
+        const bool dense_loop = out && ctx->tel_src == c8::TEL_CONST && ctx->r_max >= kDenseRadiusMin_m;
+        kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out ? (dense_loop || ctx->tel_src != c8::TEL_CONST ? 1 : 2) : 0);
+        k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, dense_loop, P.ids != nullptr), st>>>(P);
     }
     C8_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
@@ -494,8 +505,12 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
     for (int ts = 0; ts < 3 && e == cudaSuccess; ++ts)
         for (int nt = 1; nt <= 8 && e == cudaSuccess; nt *= (nt == 1 ? 4 : 2))
             for (int cp = 0; cp < 4 && e == cudaSuccess; ++cp)
-                e = cudaFuncSetAttribute(pick_kernel(ts, (cp & 1) != 0, nt, (cp & 2) != 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                e = cudaFuncSetAttribute(pick_kernel(ts, (cp & 1) != 0, nt, (cp & 2) ? 1 : 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)smem_bytes((cp & 2) ? c8::MODE_OUT : c8::MODE_TALLY));
+    for (int nt = 1; nt <= 8 && e == cudaSuccess; nt *= (nt == 1 ? 4 : 2))
+        for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
+            e = cudaFuncSetAttribute(pick_kernel(c8::TEL_CONST, cp != 0, nt, 2), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)smem_bytes(c8::MODE_OUT, false));
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(c8::propagate_kernel<c8::TEL_CONST, true, 1, c8::MODE_HIST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)smem_bytes(c8::MODE_HIST));

@@ -2093,8 +2093,11 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
     n_up_out += n_up;
 }
 
-template <int TELSRC, bool COPLANAR, int NT, int MODE>
-__global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONST) ? kOutCtasPerSm : 3) propagate_kernel(const __grid_constant__ KParams P)
+// DENSE (brute-force photon-output kernels only): with the dense loop and its record staging, compiled for 2 CTAs/SM;
+// without, every tile takes the sparse paths (correct for any input, 3 CTAs/SM): the host launches that instance when
+// no telescope is large enough to catch a good part of a shower's light (c8opt.cu, pick_kernel).
+template <int TELSRC, bool COPLANAR, int NT, int MODE, bool DENSE = true>
+__global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONST && DENSE) ? kOutCtasPerSm : 3) propagate_kernel(const __grid_constant__ KParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem &sm = *reinterpret_cast<TileSmem *>(smem_raw);
@@ -2112,7 +2115,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
     if (tid < kWarps) sm.wide_count[tid] = 0u;
     constexpr bool OUT = (MODE == MODE_OUT);
-    if constexpr (OUT && TELSRC == TEL_CONST) {
+    if constexpr (OUT && TELSRC == TEL_CONST && DENSE) {
         OutSmem &os = out_smem(sm);
         if (tid < kRoundSlots) { os.agg[tid] = 0u; os.rbase[tid] = 0ull; mbar_init(&os.rbar[tid], 1u); }
         if (tid < kTelConstMax) os.probe[tid] = 0u;
@@ -2237,7 +2240,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         } else {
             bool dense = false;
             int kd = 0;
-            if constexpr (OUT) {
+            if constexpr (OUT && DENSE) {
                 // dense or sparse tile?  (tile-uniform: every thread reads the same counts after the barrier)
                 OutSmem &os = out_smem(sm);
                 if (P.flags & kFlagRefract) probe_density<COPLANAR, NT, true>(P, sm, os, lo, hi, tile_first);
@@ -2248,7 +2251,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
                 for (int k = 0; k < NT; ++k) { const uint32_t c = os.probe[k]; if (c > best) { best = c; kd = k; } }
                 dense = best >= (uint32_t)kProbeDense;
             }
-            if constexpr (OUT) {
+            if constexpr (OUT && DENSE) {
                 if (dense) {
                     const uint32_t n_trips = (max_len + 63u) / 64u;
                     if (P.flags & kFlagRefract) walk_dense<COPLANAR, NT, true, false>(P, sm, out_smem(sm), lo, hi, tile_first, n_trips, kd, n_up, q_head, q_count);
