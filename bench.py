@@ -371,7 +371,7 @@ def main():
     # ---- photon-output leg (north_star's second roofline): the same segments against one accept-all detector on the
     # observation level, every downward photon written as a 28-byte record ("c5g" at this segment count)
     roofline_output = None
-    if args.workload == "c2" and not (args.no_output_leg or args.cull or args.ground_hist) and rank == 0:
+    if args.workload == "c2" and not (args.no_output_leg or args.cull or args.ground_hist) and world == 1:
         # "c5g": configs[4]'s segment set (the c2 generator at 10^7 segments) with one accept-all detector
         del kw
         ocfg = wl.make_config("c5g", n_segments=args.output_segments)
