@@ -2036,7 +2036,6 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                 part_w += wA + wB;
                 part_wt += (sA ? hA.w * hA.t : 0.0f) + (sB ? hB.w * hB.t : 0.0f);
             }
-            if (t == 0u) publish_pending();
             const uint32_t mA = __ballot_sync(0xffffffffu, sA), mB = __ballot_sync(0xffffffffu, sB);
             const uint32_t nA = (uint32_t)__popc(mA);
             if (sA) {
@@ -2052,6 +2051,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
                 if (want_ids) sid[s] = idA + 1ull;
             }
             cnt += nA + (uint32_t)__popc(mB);
+            if (t == 0u) publish_pending();
         }
         acc_n += cnt;                               // warp-uniform: lane 0's copy is the one that counts
         if ((r & (kTallyRounds - 1u)) == kTallyRounds - 1u) { acc_w += (double)part_w; acc_wt += (double)part_wt; part_w = 0.0f; part_wt = 0.0f; }
