@@ -16,7 +16,11 @@
 // telescope) pairs can be hits (~0.4 % of the photons) and pushes their 8-byte ids into a
 // per-warp queue; whenever 32 are queued the warp processes them with all lanes busy:
 // regenerate the photon from its counter-based random stream, exact sphere test, arrival
-// time, wavelength, weight, tally / record.
+// time, wavelength, weight, tally / record.  Photon output with a detector that catches a
+// good part of the light takes the dense loop instead (walk_dense: every candidate is
+// evaluated on the spot, records staged per warp, slots reserved once per tile and round
+// without a block barrier, 16-byte vector stores).  Flat photons (|v_z| < 0.05) are set
+// aside and evaluated in double at the end of the tile (flat_pass).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -1583,7 +1587,7 @@ __device__ __forceinline__ void walk(const KParams &P, TileSmem &sm, WarpWalk &w
     ww.pe = pe; ww.f_reg = f_reg;
 }
 
-// The pair loop (tally kernels, and the sparse tiles of the photon-output kernels after round 0): a lane takes the two
+// The pair loop (tally kernels, ground histogram, and the sparse tiles of the photon-output kernels): a lane takes the two
 // adjacent slots g, g + 1 (g even) of the index space per trip, a warp 64.  Both photons belong to the same emitter
 // (the index space is padded to even counts), so one emitter state serves both; their Philox chains and geometry are
 // independent and interleave, which halves the dependent-issue stalls per photon, and the round keys / telescope
