@@ -153,7 +153,11 @@ def compare(cfg: dict, g: dict, o: dict, first_id: int = 0, check_records: bool 
         a, b_ = gr[gi], orr[oi]
         if len(a):
             dx, dy = np.abs(a["x"] - b_["x"]), np.abs(a["y"] - b_["y"])
-            assert dx.max() <= TOL_XY_M and dy.max() <= TOL_XY_M, f"(c) position: {dx.max():.3e} {dy.max():.3e} m"
+            # 1 cm, plus half an fp32 ulp of the stored number: the record holds x, y as fp32, and the plane crossing of a
+            # nearly horizontal photon that clips a sphere can lie > 131 km from the centre, where an ulp exceeds 1.5 cm
+            tol_x, tol_y = TOL_XY_M + 2.0 ** -24 * np.abs(b_["x"]), TOL_XY_M + 2.0 ** -24 * np.abs(b_["y"])
+            assert (dx <= tol_x).all() and (dy <= tol_y).all(), f"(c) position: {dx.max():.3e} {dy.max():.3e} m"
+            rep.update(records_beyond_100km=int(((np.abs(b_["x"]) > 1e5) | (np.abs(b_["y"]) > 1e5)).sum()))
             # direction: the record stores (cos_x, cos_y) only.  The two stored components are compared
             # directly; the full angle (v_z rebuilt from the unit norm) is compared where the rebuild is
             # well conditioned, |v_z| >= 0.05 (a near-horizontal photon's v_z is not recoverable from fp32

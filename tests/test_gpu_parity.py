@@ -668,3 +668,18 @@ def test_full_tile_of_emitters_near_the_bunch_limit(c8):
     o = pu.oracle_run(cfg, record_capacity=0)
     rep = pu.compare(cfg, g, o, check_records=False)
     _report("255-big-emitters", rep)
+
+
+def test_many_flat_photons_in_one_tile(c8):
+    """Isotropic fluorescence at 250 photons per segment beside a 150 m sphere 300 m away: every tile sets tens of flat
+    (|v_z| < 0.05) photons aside for its double-precision pass, some of them so flat that they cross the telescope's plane
+    hundreds of kilometres away (the fp32 record then carries half an ulp of rounding on top of the 1 cm)."""
+    import parity_util as pu
+    cfg = wl.make_config("c3a", n_segments=3000)
+    cfg["telescopes"] = np.array([[300.0, 0.0, 2000.0, 150.0]], dtype=np.float32)
+    cfg["params"] = dict(cfg["params"], fl_yield=250.0)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("flat-many", rep)
+    assert rep["flat_records_two_component_direction"] > 150 and rep["matched"] > 10_000
