@@ -49,7 +49,7 @@ class Params(C.Structure):
                 ("lam1", C.c_double), ("lam2", C.c_double), ("bunch_size", C.c_double),
                 ("fl_yield", C.c_double), ("fl_lam1", C.c_double), ("fl_lam2", C.c_double),
                 ("fl_beam_telescope", C.c_int), ("fl_beam_halfangle", C.c_double), ("refract", C.c_int),
-                ("cut_mode", C.c_int), ("cut_angle", C.c_double)]
+                ("cut_mode", C.c_int), ("cut_angle", C.c_double), ("cauchy_b", C.c_double)]
 
 
 FLAG_REFRACT = 2      # the bit of params["flags"] that asks for the refraction corrections (R27)
@@ -63,7 +63,8 @@ class Frame(C.Structure):
                 ("L", C.c_double), ("t0", C.c_double), ("inv_beta_c", C.c_double),
                 ("sin_c", C.c_double), ("cos_c", C.c_double),
                 ("A", C.c_double * 3), ("M", (C.c_double * 3) * 3),
-                ("one_minus_cos_ab", C.c_double), ("kind", C.c_int)]
+                ("one_minus_cos_ab", C.c_double), ("kind", C.c_int),
+                ("disp_eta", C.c_double), ("disp_beta2", C.c_double), ("disp_mean", C.c_double)]
 
 
 class Photon(C.Structure):
@@ -144,7 +145,7 @@ def make_params(p: dict) -> Params:
                   p["fl_yield"], p["fl_lam1"], p["fl_lam2"], int(p["fl_beam_telescope"]), p["fl_beam_halfangle"],
                   1 if (int(p.get("flags", 0)) & FLAG_REFRACT) else 0,
                   2 if (int(p.get("flags", 0)) & FLAG_CUT_TELESCOPES) else 1 if (int(p.get("flags", 0)) & FLAG_CUT_CENTRE) else 0,
-                  float(p.get("cut_angle", 0.0)))
+                  float(p.get("cut_angle", 0.0)), float(p.get("cauchy_b", 0.0)))
 
 
 def _dp(a):
@@ -251,6 +252,14 @@ def particle_cut(p0, d, L, telescopes, mode: int, cut_angle: float) -> bool:
     p0 = np.ascontiguousarray(p0, dtype=np.float64)
     d = np.ascontiguousarray(d, dtype=np.float64)
     return bool(f(_dp(p0), _dp(d), float(L), _dp(tel), len(tel), _dp(np.ascontiguousarray(centre[:3])), int(mode), float(cut_angle)))
+
+
+def dispersion_integral(eta: float, beta2: float, b: float, x1: float, x2: float) -> float:
+    """R30: int_{x2}^{x1} max(0, sin^2 theta_c(x)) dx by the oracle's 16-interval Simpson rule (x = 1 / lambda)."""
+    f = lib().orc_dispersion_integral
+    f.argtypes = [C.c_double] * 5
+    f.restype = C.c_double
+    return f(eta, beta2, b, x1, x2)
 
 
 def optical_depth(atm: dict, h, lam) -> float:

@@ -61,6 +61,7 @@ typedef struct {
     int refract;                       /* R27: apply the refraction corrections of PAPER.md:77 to position and angle */
     int cut_mode;                      /* R29: 0 none, 1 angle to the experiment centre, 2 smallest angle to a telescope */
     double cut_angle;                  /* rad ("recommended cut of 6 degrees") */
+    double cauchy_b;                   /* R30: dispersion n(lambda, h) - 1 = eta(h) (1 + b / lambda^2), b in nm^2; 0 = none */
 } orc_params;
 
 /* one fp32 segment record, 12 x 4 bytes (flags is a uint32 in the same slot) */
@@ -78,6 +79,7 @@ typedef struct {
     double M[3][3];     /* M_Rod                                       */
     double one_minus_cos_ab; /* beamed fluorescence: 1 - cos(alpha_b)                */
     int kind;           /* 0 Cherenkov, 1 fluorescence isotropic, 2 fluorescence beamed */
+    double disp_eta, disp_beta2, disp_mean;  /* R30 (cauchy_b > 0): eta(h_mid), beta^2, band average of sin^2 theta_c */
 } orc_frame;
 
 typedef struct {
@@ -188,6 +190,27 @@ static void orc_rodrigues(const double dir[3], double A[3], double M[3][3])
  *   beamed (R14, R15): weight *= Omega / 4 pi, Omega = 2 pi (1 - cos alpha_b),
  *   line of sight from the segment midpoint to the telescope centre.
  */
+/* R30: sin^2 theta_c at x = 1 / lambda [1/nm] for refractivity eta (long-wavelength value), beta^2, Cauchy coefficient b;
+ * <= 0 below the threshold. */
+double orc_dispersion_sin2(double eta, double beta2, double b, double x)
+{
+    double n = 1.0 + eta * (1.0 + (b * x) * x);
+    double bn2 = (beta2 * n) * n;
+    return 1.0 - 1.0 / bn2;
+}
+
+/* int_{x2}^{x1} max(0, sin^2 theta_c(x)) dx, composite Simpson, 16 intervals */
+double orc_dispersion_integral(double eta, double beta2, double b, double x1, double x2)
+{
+    double h = (x1 - x2) / 16.0, odd = 0.0, even = 0.0, ends = 0.0;
+    for (int k = 0; k <= 16; ++k) {
+        double f = orc_dispersion_sin2(eta, beta2, b, x2 + (double)k * h);
+        if (!(f > 0.0)) f = 0.0;
+        if (k == 0 || k == 16) ends += f; else if (k & 1) odd += f; else even += f;
+    }
+    return (h / 3.0) * ((ends + 4.0 * odd) + 2.0 * even);
+}
+
 int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_segment *s, int tag,
                  const double *beam_tel_xyz, orc_frame *f)
 {
@@ -213,6 +236,20 @@ int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_seg
         f->kind = 0;
         double h_mid = f->p0[2] + 0.5 * L * f->d[2];      /* R3 */
         double eta = orc_refractivity(atm, h_mid);
+        if (par->cauchy_b > 0.0) {
+            /* R30: the Frank-Tamm integrand with n(lambda): in x = 1 / lambda,
+             *   N = 2 pi alpha z^2 L int_{x2}^{x1} sin^2 theta_c(x) Theta(...) dx,  sin^2 theta_c(x) = 1 - 1 / (beta^2 n(x)^2),
+             *   n(x) - 1 = eta (1 + b x^2)  (two-term Cauchy form; the paper gives no dispersion law),
+             * by composite Simpson with 16 intervals; Theta cuts the integrand at 0 where beta n(x) < 1. */
+            if (!(L > 0.0)) return 0;
+            double S = orc_dispersion_integral(eta, 1.0 - ig2, par->cauchy_b, 1.0 / par->lam1, 1.0 / par->lam2);
+            if (!(S > 0.0)) return 0;
+            mu = 2.0 * ORC_PI * ORC_ALPHA * 1.0e9 * zq * zq * L * S;
+            f->disp_eta = eta; f->disp_beta2 = 1.0 - ig2;
+            f->disp_mean = S / (1.0 / par->lam1 - 1.0 / par->lam2);
+            orc_rodrigues(f->d, f->A, f->M);
+            goto bunches;
+        }
         double q = 2.0 * eta + eta * eta - (1.0 + eta) * (1.0 + eta) * ig2;
         if (!(q > 0.0) || !(L > 0.0)) return 0;          /* threshold Theta(beta - 1/n) */
         double bn2 = (1.0 - ig2) * (1.0 + eta) * (1.0 + eta); /* beta^2 n^2 */
@@ -222,6 +259,7 @@ int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_seg
         double c_ft = 2.0 * ORC_PI * ORC_ALPHA * (1.0 / par->lam1 - 1.0 / par->lam2) * 1.0e9; /* per metre */
         mu = c_ft * zq * zq * L * sin2;
         orc_rodrigues(f->d, f->A, f->M);
+        f->disp_eta = eta; f->disp_beta2 = 1.0 - ig2; f->disp_mean = sin2;
     } else {
         mu = par->fl_yield * (double)s->dE;               /* constant yield x total energy loss */
         if (par->fl_beam_telescope == -2) {
@@ -260,6 +298,7 @@ int orc_preamble(const orc_atmosphere *atm, const orc_params *par, const orc_seg
             f->kind = 1;
         }
     }
+bunches:
     if (!(mu > 0.0)) return 0;
     double nb = ceil(mu / par->bunch_size);
     if (nb > 16777215.0) return -1;                      /* photon index must fit 24 bits of the record id */
@@ -305,8 +344,20 @@ void orc_make_photon(const orc_frame *f, const orc_params *par, uint64_t S, uint
     double phi = 2.0 * ORC_PI * u2;                        /* R5: c_rng */
     double p[3];
     if (f->kind == 0) {
-        p[0] = cos(phi) * f->sin_c; p[1] = sin(phi) * f->sin_c; p[2] = -f->cos_c;
-        ph->lam = 1.0 / (1.0 / par->lam1 - u3 * (1.0 / par->lam1 - 1.0 / par->lam2)); /* R4: pdf ~ lambda^-2 */
+        double sin_c = f->sin_c, cos_c = f->cos_c;
+        double x = 1.0 / par->lam1 - u3 * (1.0 / par->lam1 - 1.0 / par->lam2);
+        if (par->cauchy_b > 0.0) {
+            /* R30: the photon of wavelength 1 / x leaves at ITS Cherenkov angle, cos theta_c = 1 / (beta n(x)); x is still
+             * drawn uniformly (R4), so the bunch carries sin^2 theta_c(x) / <sin^2 theta_c> as a weight factor (0 below
+             * the threshold at this wavelength: the bunch is dropped by the caller) */
+            double n = 1.0 + f->disp_eta * (1.0 + (par->cauchy_b * x) * x);
+            double s2 = orc_dispersion_sin2(f->disp_eta, f->disp_beta2, par->cauchy_b, x);
+            if (!(s2 > 0.0)) { ph->w = 0.0; s2 = 0.0; }
+            else ph->w = f->w0 * (s2 / f->disp_mean);
+            sin_c = sqrt(s2); cos_c = 1.0 / (sqrt(f->disp_beta2) * n);
+        }
+        p[0] = cos(phi) * sin_c; p[1] = sin(phi) * sin_c; p[2] = -cos_c;
+        ph->lam = 1.0 / x;                                                /* R4: pdf ~ lambda^-2 */
     } else if (f->kind == 1) {
         double cth = 1.0 - 2.0 * u4, sth = 2.0 * sqrt(u4 * (1.0 - u4));            /* R16 isotropic */
         ph->v[0] = cos(phi) * sth; ph->v[1] = sin(phi) * sth; ph->v[2] = -cth;
@@ -511,6 +562,7 @@ void orc_run(const orc_atmosphere *atm, const double *tel, int n_tel,
                 orc_photon ph;
                 orc_make_photon(&f, par, S, j, tag, &ph);
                 counters[1] += 1;
+                if (par->cauchy_b > 0.0 && tag == 0 && !(ph.w > 0.0)) continue;   /* R30: below the threshold at its wavelength */
                 if (!(ph.v[2] < 0.0)) { counters[2] += 1; continue; }
                 for (int k = 0; k < n_tel; ++k) {
                     double b2, s_c, s_pl, xy[2], va[3] = { ph.v[0], ph.v[1], ph.v[2] };

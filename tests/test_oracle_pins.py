@@ -979,3 +979,72 @@ print(int(a["tallies"]["hits"].sum()), int(a["counters"][7]), int(b["counters"][
         assert r.returncode == 0, r.stderr[-2000:]
         outs.append(r.stdout.strip().splitlines()[-1])
     assert outs[0] == outs[1] and int(outs[0].split()[0]) > 100 and int(outs[0].split()[2]) > 0
+
+
+# ------------------------------------------------------------------ wavelength-dependent refractive index (R30)
+def _sin2_disp(eta, beta2, b, x):
+    n = 1.0 + eta * (1.0 + b * x * x)
+    return 1.0 - 1.0 / (beta2 * n * n)
+
+
+def test_dispersion_integral_against_fine_quadrature_and_the_closed_form():
+    """The Frank-Tamm lambda integral with n(lambda) - 1 = eta (1 + b / lambda^2): the oracle's 16-interval Simpson rule
+    against a 2e5-point trapezoid of the same integrand (1e-9 relative: the integrand is a smooth, nearly quadratic
+    function of x = 1 / lambda), and with b -> 0 against the closed form sin^2 theta_c (1/lam1 - 1/lam2) of R2."""
+    x1, x2 = 1.0 / 300.0, 1.0 / 600.0
+    for eta, gamma, b in ((2.83e-4, 1e4, 5670.0), (1.0e-4, 200.0, 5670.0), (2.2e-4, 80.0, 20000.0)):
+        beta2 = 1.0 - 1.0 / gamma ** 2
+        xs = np.linspace(x2, x1, 200001)
+        ref = np.trapezoid(np.maximum(0.0, _sin2_disp(eta, beta2, b, xs)), xs)
+        got = O.dispersion_integral(eta, beta2, b, x1, x2)
+        assert ref > 0 and math.isclose(got, ref, rel_tol=1e-9), (got, ref)
+    eta, beta2 = 2.83e-4, 1.0 - 1e-8
+    closed = (1.0 - 1.0 / (beta2 * (1 + eta) ** 2)) * (x1 - x2)
+    assert math.isclose(O.dispersion_integral(eta, beta2, 0.0, x1, x2), closed, rel_tol=1e-11)        # (1 - 1 / (beta n)^2 cancels 3 digits)
+    # dispersion raises the yield: n is larger at every wavelength of the band
+    assert O.dispersion_integral(eta, beta2, 5670.0, x1, x2) > closed * 1.03
+
+
+def test_dispersion_threshold_inside_the_band():
+    """A particle that is above the Cherenkov threshold only for the blue end of the band (n grows towards short
+    wavelengths): the integrand is cut at 0 (the Theta of PAPER.md:45), the integral is that of the radiating part --
+    to the accuracy of a 16-interval rule across a kink, a few 1e-3 -- and far below the no-threshold value."""
+    eta, b = 2.0e-4, 5670.0
+    x1, x2 = 1.0 / 300.0, 1.0 / 600.0
+    n_mid = 1.0 + eta * (1.0 + b * (0.5 * (x1 + x2)) ** 2)
+    beta2 = 1.0 / n_mid ** 2                                   # threshold exactly at the middle of the band in x
+    xs = np.linspace(x2, x1, 400001)
+    f = _sin2_disp(eta, beta2, b, xs)
+    assert f[0] < 0 < f[-1]
+    ref = np.trapezoid(np.maximum(0.0, f), xs)
+    got = O.dispersion_integral(eta, beta2, b, x1, x2)
+    assert math.isclose(got, ref, rel_tol=2e-2) and got < 0.3 * abs(np.trapezoid(np.abs(f), xs)) + ref
+
+
+def test_dispersion_photons_leave_at_the_angle_of_their_wavelength():
+    """R30 per photon: v . d = 1 / (beta n(lambda)) with n(lambda) - 1 = eta (1 + b / lambda^2), weight = w0 sin^2(lambda) /
+    <sin^2>, so that the weights of all bunches sum to mu; blue photons open wider than red ones; with b = 0 the
+    photons are those of R2 - R4 bit for bit."""
+    seg = one_segment(z0=8000.0, d=(0.1, 0.2, -1.0), length=30.0, gamma=300.0)
+    par0 = W.default_params(bunch_size=0.05, seed=5)
+    par = dict(par0, cauchy_b=5670.0)
+    st, f = O.preamble(ATM5, par, seg[0], 0)
+    st0, f0 = O.preamble(ATM5, par0, seg[0], 0)
+    assert st == 0 and f.n_b > f0.n_b > 2000
+    eta = O.refractivity(ATM5, 8000.0 + 0.5 * 30.0 * f.d[2])
+    beta2 = 1.0 - 1.0 / 300.0 ** 2
+    assert math.isclose(f.mu, 2 * math.pi * 7.2973525693e-3 * 1e9 * 30.0 * O.dispersion_integral(eta, beta2, 5670.0, 1 / 300.0, 1 / 600.0), rel_tol=1e-12)
+    sw, cs = 0.0, []
+    for j in range(f.n_b):
+        ph = O.make_photon(f, par, 0, j, 0)
+        n = 1.0 + eta * (1.0 + 5670.0 / ph.lam ** 2)
+        cos_c = 1.0 / (math.sqrt(beta2) * n)
+        assert math.isclose(float(np.dot(ph.v, f.d)), cos_c, rel_tol=0, abs_tol=1e-12)
+        assert math.isclose(ph.w, f.w0 * (1.0 - cos_c ** 2) / f.disp_mean, rel_tol=1e-9)
+        sw += ph.w; cs.append((ph.lam, cos_c))
+    assert math.isclose(sw, f.mu, rel_tol=0.02)                      # Monte-Carlo mean of sin^2 over the band
+    cs.sort()
+    assert cs[0][1] < cs[-1][1]                                      # shortest wavelength: smallest cos, widest cone
+    for j in (0, 1, 17):
+        a, b_ = O.make_photon(f0, par0, 0, j, 0), O.make_photon(f0, dict(par0, cauchy_b=0.0), 0, j, 0)
+        assert tuple(a.v) == tuple(b_.v) and a.w == b_.w and a.lam == b_.lam
