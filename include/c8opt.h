@@ -257,6 +257,35 @@ const char *c8opt_last_error(const c8opt_ctx *ctx);
  * gpu_launches). */
 uint64_t c8opt_launch_count(const c8opt_ctx *ctx);
 
+/* ---- the entry point that allocates nothing --------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the tally-mode pass (the same kernels as c8opt_propagate_segments with C8OPT_MODE_TALLY) with
+ * no context and no allocation.  What the context path keeps in cudaMalloc'ed memory -- the counters and tallies the
+ * kernel accumulates into, and the telescope tables -- lives in ONE file-scope `static __device__` array of
+ * C8OPT_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until exit); its stated
+ * limit is C8OPT_STATIC_MAX_TELESCOPES telescopes.  The call makes no cudaMalloc / cudaFree / cudaMallocHost and no
+ * allocating library call; it enqueues a set-up kernel (tables written, accumulators zeroed: the array keeps the last
+ * call's contents), the propagate kernel(s) and a kernel that writes the results, all on `cuda_stream`, and returns
+ * without synchronising.  The first call on a device also looks up the array's address and raises the kernels'
+ * shared-memory limit (once per device, the CURRENT device is used).
+ *   atmosphere   HOST, as for c8opt_create_atmosphere, except that atmosphere->tau is ignored:
+ *   d_tau        DEVICE, the transmission table tau[tau_nh][tau_nl] (shape / axes from `atmosphere`), or NULL for none;
+ *                the caller's memory, read by the kernels
+ *   xyzr, n_tel  HOST, as for c8opt_add_telescopes; 1 <= n_tel <= C8OPT_STATIC_MAX_TELESCOPES
+ *   d_seg, n, first_segment_id, params   as for c8opt_propagate_segments; params->mode must be C8OPT_MODE_TALLY
+ *   d_tallies_out    DEVICE, [n_tel] c8opt_tally, written (not accumulated into)
+ *   d_counters_out   DEVICE, [8] uint64 in the order of C8OPT_CNT_* (RECORDS = DROPPED = 0), or NULL
+ * Every call shares the one array per device: calls that overlap on the GPU (different streams, or two processes'
+ * worth of threads on one device) RACE; order them on one stream or with events.  Results equal the context path's
+ * up to the order of the floating-point atomics.  Errors: ARGUMENT (also: too many telescopes, a mode other than
+ * tally; message from c8opt_last_error(NULL)), CUDA. */
+#define C8OPT_STATIC_MAX_TELESCOPES 8
+#define C8OPT_STATIC_SCRATCH_BYTES 1024
+int c8opt_tally_static(const c8opt_atmosphere_desc *atmosphere, const float *d_tau, const float *xyzr, int32_t n_tel,
+                       const c8opt_segment *d_seg, uint64_t n, uint64_t first_segment_id,
+                       const c8opt_run_params *params, c8opt_tally *d_tallies_out, uint64_t *d_counters_out,
+                       void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,7 +38,8 @@ RECORD_FLOATS = 7
 EXPORTS = ("c8opt_create_atmosphere", "c8opt_add_telescopes", "c8opt_propagate_segments",
            "c8opt_propagate_segments_host", "c8opt_read_tallies", "c8opt_reset_tallies", "c8opt_destroy",
            "c8opt_last_error", "c8opt_launch_count", "c8opt_set_ground_histogram", "c8opt_read_ground_histogram",
-           "c8opt_reserve_host_staging")
+           "c8opt_reserve_host_staging", "c8opt_tally_static")
+STATIC_MAX_TELESCOPES = 8
 
 
 class C8optError(RuntimeError):
@@ -99,6 +100,8 @@ def lib():
         L.c8opt_set_ground_histogram.argtypes = [vp, C.c_double, C.c_double, C.c_double, C.c_int32]
         L.c8opt_read_ground_histogram.argtypes = [vp, vp, C.c_int32, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
         L.c8opt_reserve_host_staging.argtypes = [vp, C.c_uint64]
+        L.c8opt_tally_static.argtypes = [C.POINTER(_AtmosphereDesc), vp, C.POINTER(C.c_float), C.c_int32, vp, C.c_uint64,
+                                         C.c_uint64, C.POINTER(_RunParams), vp, vp, vp]
         for name in EXPORTS[:6] + EXPORTS[9:]:
             getattr(L, name).restype = C.c_int
         _lib = L
@@ -133,23 +136,46 @@ def make_run_params(p: dict) -> _RunParams:
                       float(p.get("cut_angle", 0.0)))
 
 
+def _atmosphere_desc(atmosphere: dict):
+    """(c8opt_atmosphere_desc, the float32 table it points at or None)."""
+    d = _AtmosphereDesc()
+    layers = atmosphere["layers"]
+    d.n_layers = len(layers)
+    for i, (h_lo, a, b, c) in enumerate(layers[:MAX_LAYERS]):
+        d.layers[i] = _Layer(h_lo, a, b, c)
+    d.eta0, d.rho0_gcm3, d.h_obs_m = atmosphere["eta0"], atmosphere["rho0"], atmosphere["h_obs"]
+    tau = atmosphere.get("tau")
+    if tau is not None:
+        tau = np.ascontiguousarray(tau, dtype=np.float32)
+        d.tau_nh, d.tau_nl = tau.shape
+        d.tau_h0_m, d.tau_dh_m = atmosphere["tau_h0"], atmosphere["tau_dh"]
+        d.tau_l0_nm, d.tau_dl_nm = atmosphere["tau_l0"], atmosphere["tau_dl"]
+        d.tau = tau.ctypes.data_as(C.POINTER(C.c_float))
+    return d, tau
+
+
+def tally_static(atmosphere: dict, xyzr, d_seg, params: dict, d_tallies_out, d_counters_out=None, d_tau=None,
+                 n: int | None = None, first_segment_id: int = 0, stream=None):
+    """c8opt_tally_static: the tally pass with no context and no allocation (asynchronous on `stream`).
+    d_seg, d_tallies_out ([n_tel] x 24 bytes), d_counters_out ([8] uint64) and d_tau (the transmission table, float32
+    [tau_nh, tau_nl], or None) are the caller's CUDA tensors; atmosphere["tau"] only gives the table's shape."""
+    d, _tau = _atmosphere_desc(atmosphere)
+    d.tau = None
+    t = np.ascontiguousarray(xyzr, dtype=np.float32).reshape(-1, 4)
+    if n is None:
+        n = d_seg.numel() * d_seg.element_size() // 48
+    rp = make_run_params(params)
+    rc = lib().c8opt_tally_static(C.byref(d), _ptr(d_tau), t.ctypes.data_as(C.POINTER(C.c_float)), len(t), _ptr(d_seg), n,
+                                  first_segment_id, C.byref(rp), _ptr(d_tallies_out), _ptr(d_counters_out), _stream(stream))
+    if rc != 0:
+        raise C8optError(rc, lib().c8opt_last_error(None).decode())
+
+
 class Context:
     """Owns one c8opt_ctx."""
 
     def __init__(self, atmosphere: dict):
-        d = _AtmosphereDesc()
-        layers = atmosphere["layers"]
-        d.n_layers = len(layers)
-        for i, (h_lo, a, b, c) in enumerate(layers[:MAX_LAYERS]):
-            d.layers[i] = _Layer(h_lo, a, b, c)
-        d.eta0, d.rho0_gcm3, d.h_obs_m = atmosphere["eta0"], atmosphere["rho0"], atmosphere["h_obs"]
-        tau = atmosphere.get("tau")
-        if tau is not None:
-            tau = np.ascontiguousarray(tau, dtype=np.float32)
-            d.tau_nh, d.tau_nl = tau.shape
-            d.tau_h0_m, d.tau_dh_m = atmosphere["tau_h0"], atmosphere["tau_dh"]
-            d.tau_l0_nm, d.tau_dl_nm = atmosphere["tau_l0"], atmosphere["tau_dl"]
-            d.tau = tau.ctypes.data_as(C.POINTER(C.c_float))
+        d, _tau = _atmosphere_desc(atmosphere)
         self._h = C.c_void_p()
         self.n_tel = 0
         self.hist_bins = 0

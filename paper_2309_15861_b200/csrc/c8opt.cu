@@ -9,6 +9,7 @@
 #include <cstddef>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -792,3 +793,195 @@ const char *c8opt_last_error(const c8opt_ctx *ctx) { return ctx ? ctx->error : g
 uint64_t c8opt_launch_count(const c8opt_ctx *ctx) { return ctx ? ctx->launches : 0; }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------------
+// c8opt_tally_static: the tally pass with no context and no allocation (include/c8opt.h).  Everything the context
+// path keeps in cudaMalloc'ed memory sits in this one array; host code must not pass its NAME to a kernel (that is a
+// host-side stand-in): static_device() asks for the device address once per device, kernels in this file name it
+// directly.
+// Layout: [0, 384) the result block of 8 telescopes as in c8opt_ctx (counters 8 x u64, cursors, tallies, capacities);
+// [512, 640) telA float4[8]; [640, 672) telT; [672, 704) telEta; [704, 960) telD double4[8].
+static __device__ __align__(256) unsigned char g_c8opt_static_scratch[C8OPT_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kStaticTel = C8OPT_STATIC_MAX_TELESCOPES;
+static_assert(kStaticTel == c8::kTelConstMax, "the static entry point serves the brute-force kernels (telescopes in the constant bank)");
+constexpr size_t kStOffCursors = 64, kStOffTallies = 64 + 8 * kStaticTel, kStOffTelA = 512, kStOffTelT = 640,
+                 kStOffTelEta = 672, kStOffTelD = 704;
+static_assert(kStOffTallies + (sizeof(c8::Tally) + 8) * kStaticTel <= kStOffTelA, "result block overlaps the tables");
+static_assert(kStOffTelD + sizeof(double4) * kStaticTel <= C8OPT_STATIC_SCRATCH_BYTES, "static scratch too small");
+
+struct StaticTables { float4 telA[kStaticTel]; double4 telD[kStaticTel]; float telT[kStaticTel], telEta[kStaticTel]; };
+
+// Writes the telescope tables and zeroes the accumulators (the array keeps the last call's contents).
+__global__ void static_setup_kernel(const StaticTables t)
+{
+    unsigned char *s = g_c8opt_static_scratch;
+    const int i = threadIdx.x;
+    if (i < (int)(kStOffTelA / 8)) reinterpret_cast<unsigned long long *>(s)[i] = 0ull;
+    if (i < kStaticTel) {
+        reinterpret_cast<float4 *>(s + kStOffTelA)[i] = t.telA[i];
+        reinterpret_cast<float *>(s + kStOffTelT)[i] = t.telT[i];
+        reinterpret_cast<float *>(s + kStOffTelEta)[i] = t.telEta[i];
+        reinterpret_cast<double4 *>(s + kStOffTelD)[i] = t.telD[i];
+    }
+}
+
+// Results to the caller's buffers: the tallies, and the counters in the order of C8OPT_CNT_*.
+__global__ void static_finish_kernel(c8::Tally *tallies_out, unsigned long long *counters_out, int n_tel, unsigned long long n_seg)
+{
+    const unsigned char *s = g_c8opt_static_scratch;
+    const c8::Tally *t = reinterpret_cast<const c8::Tally *>(s + kStOffTallies);
+    const int i = threadIdx.x;
+    if (i < n_tel) tallies_out[i] = t[i];
+    if (i == 0 && counters_out) {
+        const unsigned long long *cnt = reinterpret_cast<const unsigned long long *>(s);
+        unsigned long long hits = 0;
+        for (int k = 0; k < n_tel; ++k) hits += t[k].hits;
+        counters_out[C8OPT_CNT_SEGMENTS] = n_seg; counters_out[C8OPT_CNT_GENERATED] = cnt[1];
+        counters_out[C8OPT_CNT_UPWARD] = cnt[2]; counters_out[C8OPT_CNT_HITS] = hits;
+        counters_out[C8OPT_CNT_RECORDS] = 0; counters_out[C8OPT_CNT_DROPPED] = 0;
+        counters_out[C8OPT_CNT_INVALID] = cnt[6]; counters_out[C8OPT_CNT_CULLED] = cnt[7];
+    }
+}
+
+// Once per device, with that device current: the array's device address, the SM count, the shared-memory limit of the
+// six brute-force tally kernels.  No allocation.
+struct StaticDevice { bool ready = false; unsigned char *scratch = nullptr; int n_sm = 148; };
+constexpr int kStaticDevices = 64;
+StaticDevice g_static_device[kStaticDevices];
+std::mutex g_static_mutex;
+
+int static_device(int dev, StaticDevice *out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice &d = g_static_device[dev];
+    if (!d.ready) {
+        int major = 0, n_sm = 0;
+        C8_CUDA(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+        if (major != 10) return fail(nullptr, C8OPT_ERR_CUDA, "device is sm_%dx, this library is built for sm_100a only", major);
+        C8_CUDA(nullptr, cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+        unsigned char *ptr = nullptr;
+        C8_CUDA(nullptr, cudaGetSymbolAddress((void **)&ptr, g_c8opt_static_scratch));
+        if (!ptr) return fail(nullptr, C8OPT_ERR_CUDA, "cudaGetSymbolAddress gave no address for the static scratch");
+        for (int nt = 1; nt <= 8; nt *= (nt == 1 ? 4 : 2))
+            for (int cp = 0; cp < 2; ++cp)
+                C8_CUDA(nullptr, cudaFuncSetAttribute(pick_kernel(c8::TEL_CONST, cp != 0, nt, 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                      (int)smem_bytes(c8::MODE_TALLY)));
+        d.scratch = ptr; d.n_sm = n_sm > 0 ? n_sm : 148; d.ready = true;
+    }
+    *out = d;
+    return C8OPT_OK;
+}
+
+}  // namespace
+
+extern "C" int c8opt_tally_static(const c8opt_atmosphere_desc *desc, const float *d_tau, const float *xyzr, int32_t n_tel,
+                                  const c8opt_segment *d_seg, uint64_t n, uint64_t first_segment_id,
+                                  const c8opt_run_params *params, c8opt_tally *d_tallies_out, uint64_t *d_counters_out,
+                                  void *cuda_stream)
+{
+    if (!desc || !xyzr || !params || !d_tallies_out) return fail(nullptr, C8OPT_ERR_ARGUMENT, "c8opt_tally_static: atmosphere, xyzr, params or d_tallies_out is NULL");
+    if (!d_seg && n) return fail(nullptr, C8OPT_ERR_ARGUMENT, "c8opt_tally_static: d_seg is NULL");
+    if (n_tel < 1) return fail(nullptr, C8OPT_ERR_ARGUMENT, "c8opt_tally_static: telescope count %d must be >= 1", n_tel);
+    if (n_tel > kStaticTel)
+        return fail(nullptr, C8OPT_ERR_ARGUMENT, "c8opt_tally_static: %d telescopes, but the static scratch (%d bytes) holds the tables and "
+                    "accumulators of at most %d: use a context (c8opt_create_atmosphere)", n_tel, C8OPT_STATIC_SCRATCH_BYTES, kStaticTel);
+    if (params->mode != C8OPT_MODE_TALLY) return fail(nullptr, C8OPT_ERR_ARGUMENT, "c8opt_tally_static: mode must be C8OPT_MODE_TALLY");
+    if (desc->n_layers < 1 || desc->n_layers > C8OPT_MAX_LAYERS) return fail(nullptr, C8OPT_ERR_ARGUMENT, "n_layers out of range");
+    for (int i = 0; i < desc->n_layers; ++i) {
+        const c8opt_layer &l = desc->layers[i];
+        if (!std::isfinite(l.h_lo_m) || !std::isfinite(l.a_gcm2) || !std::isfinite(l.b_gcm2) || !(l.c_m > 0.0) || !std::isfinite(l.c_m))
+            return fail(nullptr, C8OPT_ERR_ARGUMENT, "layer %d: non-finite coefficient or c <= 0", i);
+        if (i > 0 && !(l.h_lo_m > desc->layers[i - 1].h_lo_m)) return fail(nullptr, C8OPT_ERR_ARGUMENT, "layer bounds must ascend");
+    }
+    if (!(desc->rho0_gcm3 > 0.0) || !std::isfinite(desc->eta0) || !(desc->eta0 >= 0.0) || !std::isfinite(desc->h_obs_m))
+        return fail(nullptr, C8OPT_ERR_ARGUMENT, "need rho0 > 0, eta0 >= 0, finite h_obs");
+    if (d_tau && (desc->tau_nh < 1 || desc->tau_nl < 1 || desc->tau_nh > 4096 || desc->tau_nl > 4096 || !(desc->tau_dh_m > 0.0) || !(desc->tau_dl_nm > 0.0)))
+        return fail(nullptr, C8OPT_ERR_ARGUMENT, "bad transmission table shape / spacing");
+    for (int k = 0; k < n_tel; ++k) {
+        for (int i = 0; i < 4; ++i)
+            if (!std::isfinite(xyzr[4 * k + i])) return fail(nullptr, C8OPT_ERR_ARGUMENT, "telescope %d: non-finite value", k);
+        if (!(xyzr[4 * k + 3] > 0.0f)) return fail(nullptr, C8OPT_ERR_ARGUMENT, "telescope %d: radius must be > 0", k);
+    }
+    int ndev = 0, dev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, C8OPT_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    C8_CUDA(nullptr, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticDevices) return fail(nullptr, C8OPT_ERR_CUDA, "device ordinal %d out of range", dev);
+    StaticDevice sd;
+    int rc = static_device(dev, &sd);
+    if (rc != C8OPT_OK) return rc;
+
+    // Host-side description of the run (what c8opt_create_atmosphere and c8opt_add_telescopes keep in a context), with
+    // the device pointers aimed at the static array.  Per thread; its small host vectors are sized on the first call.
+    thread_local c8opt_ctx host;
+    c8opt_ctx *ctx = &host;
+    ctx->device = dev; ctx->n_sm = sd.n_sm;
+    ctx->n_layers = desc->n_layers;
+    for (int i = 0; i < desc->n_layers; ++i)
+        ctx->layer[i] = HostLayer{desc->layers[i].h_lo_m, desc->layers[i].a_gcm2, desc->layers[i].b_gcm2, desc->layers[i].c_m};
+    ctx->eta0 = desc->eta0; ctx->rho0 = desc->rho0_gcm3; ctx->h_obs = desc->h_obs_m;
+    ctx->d_tau = const_cast<float *>(d_tau);
+    ctx->tau_nh = d_tau ? desc->tau_nh : 0; ctx->tau_nl = d_tau ? desc->tau_nl : 0;
+    ctx->tau_h0 = d_tau ? desc->tau_h0_m : 0.0; ctx->tau_dh = d_tau ? desc->tau_dh_m : 1.0;
+    ctx->tau_l0 = d_tau ? desc->tau_l0_nm : 0.0; ctx->tau_dl = d_tau ? desc->tau_dl_nm : 1.0;
+    // telescopes: the host part of c8opt_add_telescopes
+    double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (int k = 0; k < n_tel; ++k)
+        for (int i = 0; i < 3; ++i) { lo[i] = std::fmin(lo[i], xyzr[4 * k + i]); hi[i] = std::fmax(hi[i], xyzr[4 * k + i]); }
+    ctx->tel_xyzr.assign(xyzr, xyzr + 4 * (size_t)n_tel);
+    ctx->x_ref = 0.5 * (lo[0] + hi[0]); ctx->y_ref = 0.5 * (lo[1] + hi[1]); ctx->z_ref = 0.5 * (lo[2] + hi[2]);
+    ctx->coplanar = (lo[2] == hi[2]);
+    ctx->h_telA.resize(n_tel); ctx->h_telT.resize(n_tel); ctx->h_telEta.resize(n_tel);
+    StaticTables tab;
+    std::memset(&tab, 0, sizeof(tab));
+    double z_low = INFINITY, rb = 0.0;
+    ctx->r_max = 0.0;
+    for (int k = 0; k < n_tel; ++k) {
+        const double x = xyzr[4 * k], y = xyzr[4 * k + 1], z = xyzr[4 * k + 2], r = xyzr[4 * k + 3];
+        ctx->h_telA[k] = make_float4((float)(x - ctx->x_ref), (float)(y - ctx->y_ref), (float)(z - ctx->z_ref), (float)(r * r));
+        ctx->h_telT[k] = (float)host_depth(ctx, z);
+        ctx->h_telEta[k] = (float)host_refractivity(ctx, z);
+        z_low = std::fmin(z_low, z); ctx->r_max = std::fmax(ctx->r_max, r);
+        const double dx = x - ctx->x_ref, dy = y - ctx->y_ref, dz = z - ctx->z_ref;
+        rb = std::fmax(rb, std::sqrt(dx * dx + dy * dy + dz * dz) + r);
+        tab.telA[k] = ctx->h_telA[k]; tab.telT[k] = ctx->h_telT[k]; tab.telEta[k] = ctx->h_telEta[k];
+        tab.telD[k] = make_double4(x, y, z, r);
+    }
+    ctx->refr_cmax = 0.01 * ctx->eta0 / ctx->rho0 * host_depth(ctx, z_low);
+    ctx->cull_Rb = (float)(rb * (1.0 + 1e-6));
+    ctx->array_rb = rb;
+    ctx->tel_src = c8::TEL_CONST; ctx->n_tel = n_tel; ctx->n_grid_levels = 0; ctx->d_grid = nullptr; ctx->have_refract_grid = false;
+    ctx->d_results = sd.scratch;
+    ctx->d_counters = reinterpret_cast<unsigned long long *>(sd.scratch);
+    ctx->d_cursors = reinterpret_cast<unsigned long long *>(sd.scratch + kStOffCursors);
+    ctx->d_tallies = reinterpret_cast<c8::Tally *>(sd.scratch + kStOffTallies);
+    ctx->d_telA = reinterpret_cast<float4 *>(sd.scratch + kStOffTelA);
+    ctx->d_telT = reinterpret_cast<float *>(sd.scratch + kStOffTelT);
+    ctx->d_telEta = reinterpret_cast<float *>(sd.scratch + kStOffTelEta);
+    ctx->d_telD = reinterpret_cast<double4 *>(sd.scratch + kStOffTelD);
+
+    c8::KParams P;
+    rc = fill_params(ctx, params, nullptr, &P);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (rc == C8OPT_OK) {
+        static_setup_kernel<<<1, 64, 0, st>>>(tab);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) rc = fail(ctx, C8OPT_ERR_CUDA, "static_setup_kernel: %s", cudaGetErrorString(e));
+    }
+    if (rc == C8OPT_OK) rc = launch(ctx, P, params->mode, d_seg, n, first_segment_id, nullptr, st);
+    if (rc == C8OPT_OK) {
+        static_finish_kernel<<<1, 32, 0, st>>>(reinterpret_cast<c8::Tally *>(d_tallies_out),
+                                              reinterpret_cast<unsigned long long *>(d_counters_out), n_tel, n);
+        const cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) rc = fail(ctx, C8OPT_ERR_CUDA, "static_finish_kernel: %s", cudaGetErrorString(e));
+    }
+    // the thread's host object must not own (and its destructor does not touch) the static array or the caller's table
+    ctx->d_results = nullptr; ctx->d_tau = nullptr; ctx->d_telA = nullptr; ctx->d_telT = nullptr; ctx->d_telEta = nullptr; ctx->d_telD = nullptr;
+    if (rc != C8OPT_OK) { std::memcpy(g_create_error, ctx->error, sizeof(g_create_error)); g_create_error[255] = 0; }
+    return rc;
+}
