@@ -137,6 +137,13 @@ typedef struct {
     uint32_t flags;                /* C8OPT_FLAG_* bits                                     */
     double   fl_beam_halfangle_rad;
     double   cut_angle_rad;        /* C8OPT_FLAG_CUT_*: the angular particle cut, in [0, pi] */
+    double   cauchy_b_nm2;         /* b >= 0 [nm^2] of n(lambda, h) - 1 = eta(h) (1 + b / lambda^2); 0: n does not depend on
+                                      lambda.  > 0 (the Frank-Tamm integrand with n(lambda); R30): the
+                                      yield is the integral over the band (16-interval Simpson in 1 / lambda, cut at the
+                                      threshold), every photon leaves at the Cherenkov angle of its own wavelength and carries
+                                      sin^2(lambda) / <sin^2> as a weight factor.  Runs on brute-force kernel instances of
+                                      its own (every photon against every telescope); not with C8OPT_FLAG_CULL, not in
+                                      C8OPT_MODE_GROUND_HIST.  Air in the band 300-600 nm: b ~ 5.7e3 nm^2 */
 } c8opt_run_params;
 
 /* Optional outputs of one propagate call; every pointer is DEVICE memory owned

@@ -65,7 +65,7 @@ class _RunParams(C.Structure):
                 ("lam1_nm", C.c_double), ("lam2_nm", C.c_double), ("bunch_size", C.c_double),
                 ("fl_yield_per_MeV", C.c_double), ("fl_lam1_nm", C.c_double), ("fl_lam2_nm", C.c_double),
                 ("fl_beam_telescope", C.c_int32), ("flags", C.c_uint32), ("fl_beam_halfangle_rad", C.c_double),
-                ("cut_angle_rad", C.c_double)]
+                ("cut_angle_rad", C.c_double), ("cauchy_b_nm2", C.c_double)]
 
 
 class _Output(C.Structure):
@@ -133,7 +133,7 @@ def make_run_params(p: dict) -> _RunParams:
                       float(p["lam1"]), float(p["lam2"]), float(p["bunch_size"]),
                       float(p["fl_yield"]), float(p["fl_lam1"]), float(p["fl_lam2"]),
                       int(p["fl_beam_telescope"]), int(p.get("flags", 0)), float(p["fl_beam_halfangle"]),
-                      float(p.get("cut_angle", 0.0)))
+                      float(p.get("cut_angle", 0.0)), float(p.get("cauchy_b", 0.0)))
 
 
 def _atmosphere_desc(atmosphere: dict):

@@ -161,6 +161,13 @@ kernel_t pick_kernel(int tel_src, bool coplanar, int nt, int out)
     return pick_kernel2<c8::TEL_GLOBAL, 0>(coplanar, out);
 }
 
+// R30 (cauchy_b_nm2 > 0): the Cherenkov launch runs on the instances with the wavelength-dependent refractive index,
+// brute force over the telescopes in global memory whatever the array (out: 0 tally, else photon output).
+kernel_t pick_disp_kernel(int out)
+{
+    return out ? c8::propagate_kernel<c8::TEL_GLOBAL_DISP, false, 0, c8::MODE_OUT> : c8::propagate_kernel<c8::TEL_GLOBAL_DISP, false, 0, c8::MODE_TALLY>;
+}
+
 // A tile of a shower's light is "dense" on a telescope (a good part of its photons hit it) only when the telescope is
 // of the size of the light pool.  Below this radius the photon-output launch takes the kernel instance without the dense
 // loop (3 CTAs/SM instead of 2); both instances are correct for any input.
@@ -262,6 +269,12 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
             return fail(ctx, C8OPT_ERR_ARGUMENT, "cut_angle_rad must be in [0, pi]");
     }
     if (!(rp->bunch_size > 0.0) || !std::isfinite(rp->bunch_size)) return fail(ctx, C8OPT_ERR_ARGUMENT, "bunch_size must be > 0");
+    if (!(rp->cauchy_b_nm2 >= 0.0) || !std::isfinite(rp->cauchy_b_nm2)) return fail(ctx, C8OPT_ERR_ARGUMENT, "cauchy_b_nm2 must be >= 0");
+    if (rp->cauchy_b_nm2 > 0.0 && (procs & C8OPT_PROC_CHERENKOV)) {
+        if (hist) return fail(ctx, C8OPT_ERR_ARGUMENT, "cauchy_b_nm2 > 0 is not served in ground-histogram mode");
+        if (rp->flags & C8OPT_FLAG_CULL)
+            return fail(ctx, C8OPT_ERR_ARGUMENT, "cauchy_b_nm2 > 0: no segment culling (the cull assumes one Cherenkov angle per segment)");
+    }
     if (procs & C8OPT_PROC_CHERENKOV)
         if (!(rp->lam1_nm > 0.0) || !(rp->lam2_nm > rp->lam1_nm)) return fail(ctx, C8OPT_ERR_ARGUMENT, "need 0 < lam1 < lam2");
     if (procs & C8OPT_PROC_FLUORESCENCE) {
@@ -317,6 +330,10 @@ int fill_params(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_output *
         P.c_ft = two_pi_alpha * (1.0 / rp->lam1_nm - 1.0 / rp->lam2_nm) * 1.0e9;
         P.inv_lam1 = (float)(1.0 / rp->lam1_nm);
         P.dinv_lam = (float)(1.0 / rp->lam1_nm - 1.0 / rp->lam2_nm);
+        // R30: n(lambda, h) - 1 = eta(h) (1 + b / lambda^2); the yield integral runs over x = 1 / lambda in the preamble
+        P.cauchy_b = rp->cauchy_b_nm2; P.cauchy_b_f = (float)rp->cauchy_b_nm2;
+        P.x1_d = 1.0 / rp->lam1_nm; P.x2_d = 1.0 / rp->lam2_nm;
+        P.c_ft0 = two_pi_alpha * 1.0e9;
     }
     P.bunch_size = rp->bunch_size; P.fl_yield = rp->fl_yield_per_MeV;
     P.fl_lam1 = (float)rp->fl_lam1_nm; P.fl_dlam = (float)(rp->fl_lam2_nm - rp->fl_lam1_nm);
@@ -375,8 +392,13 @@ int launch_one(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, unsigned long long
     } else {
         const bool out = P.records != nullptr;
         const bool dense_loop = out && ctx->tel_src == c8::TEL_CONST && ctx->r_max >= kDenseRadiusMin_m;
-        kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out ? (dense_loop || ctx->tel_src != c8::TEL_CONST ? 1 : 2) : 0);
-        k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, dense_loop, P.ids != nullptr), st>>>(P);
+        const bool disp = P.cauchy_b > 0.0 && (P.processes & C8OPT_PROC_CHERENKOV);
+        if (disp) {
+            pick_disp_kernel(out)<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, false), st>>>(P);
+        } else {
+            kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out ? (dense_loop || ctx->tel_src != c8::TEL_CONST ? 1 : 2) : 0);
+            k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, dense_loop, P.ids != nullptr), st>>>(P);
+        }
     }
     C8_CUDA(ctx, cudaGetLastError());
     ctx->launches += 1;
@@ -512,6 +534,8 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
         for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
             e = cudaFuncSetAttribute(pick_kernel(c8::TEL_CONST, cp != 0, nt, 2), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)smem_bytes(c8::MODE_OUT, false));
+    for (int o = 0; o < 2 && e == cudaSuccess; ++o)
+        e = cudaFuncSetAttribute(pick_disp_kernel(o), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(o ? c8::MODE_OUT : c8::MODE_TALLY, false));
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(c8::propagate_kernel<c8::TEL_CONST, true, 1, c8::MODE_HIST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)smem_bytes(c8::MODE_HIST));
@@ -869,6 +893,7 @@ int static_device(int dev, StaticDevice *out)
             for (int cp = 0; cp < 2; ++cp)
                 C8_CUDA(nullptr, cudaFuncSetAttribute(pick_kernel(c8::TEL_CONST, cp != 0, nt, 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                       (int)smem_bytes(c8::MODE_TALLY)));
+        C8_CUDA(nullptr, cudaFuncSetAttribute(pick_disp_kernel(0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(c8::MODE_TALLY)));
         d.scratch = ptr; d.n_sm = n_sm > 0 ? n_sm : 148; d.ready = true;
     }
     *out = d;

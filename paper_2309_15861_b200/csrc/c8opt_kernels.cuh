@@ -36,6 +36,9 @@ constexpr int kTelGridMin = 9;        // from this many telescopes on, the groun
 constexpr int TEL_CONST = 0;          // brute force over <= kTelConstMax telescopes read from the constant bank
 constexpr int TEL_GRID = 1;           // candidate lookup in the ground-plane grid
 constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global memory (grid not buildable)
+constexpr int TEL_GLOBAL_DISP = 3;    // TEL_GLOBAL with the wavelength-dependent refractive index (R30): the instances
+                                      // a request with cauchy_b > 0 runs on, whatever the array (every code path that
+                                      // compares TELSRC with TEL_CONST / TEL_GRID treats it as TEL_GLOBAL)
 constexpr int kMaxLayers = 8;
 constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
 constexpr int kBlockRecs = 64;        // photon output, dense tiles: records a warp stages per trip of the dense loop (2 per lane)
@@ -137,6 +140,9 @@ struct KParams {
     int hist_bins;
     float hist_inv_dr, hist_wscale;        // bins per metre; 2^16 / B (fixed-point unit of the tile's weight sums)
     double hist_winv;                      // B / 2^16
+    // R30 (at the end: the offsets of everything above stay as they were)
+    double cauchy_b, x1_d, x2_d, c_ft0;    // n - 1 = eta (1 + b / lambda^2), b [nm^2]; 1 / lam1, 1 / lam2 [1/nm]; 2 pi alpha 1e9
+    float cauchy_b_f;
 };
 
 __device__ __forceinline__ uint32_t lane_id() { return threadIdx.x & 31u; }
@@ -306,7 +312,10 @@ enum {
     F_NEGL = 0, F_K0C = 1, F_AZ = 2, F_BZ = 3, F_CZ = 4, F_PX = 5, F_PY = 6, F_QX = 7, F_QY = 8, F_GX = 9, F_GY = 10,
     F_E0 = 0, F_D0 = 3, F_L = 6, F_A0 = 7, F_B0 = 10, F_C0 = 13,
     F_W0 = 16, F_T0 = 17, F_IBC = 18, F_DZ = 19, F_AX = 20, F_AY = 21, F_BX = 22, F_BY = 23, F_CX = 24, F_CY = 25,
-    F_LEN = 26, F_LAYER = 27, F_OMC = 28, F_HNEXT = 29, F_VZLO = 30, F_VZHI = 31, F_TMAX = 32
+    F_LEN = 26, F_LAYER = 27, F_OMC = 28, F_HNEXT = 29, F_VZLO = 30, F_VZHI = 31, F_TMAX = 32,
+    // R30 (Cherenkov emitters of the TEL_GLOBAL_DISP instances, generic kind; slots of the axis kind): eta(h_mid) and
+    // 1 / gamma^2, each as fp32 head + tail, and 1 / <sin^2 theta_c>
+    F_DETA = 19, F_DIG2 = 20, F_DINVM = 21, F_DETA_LO = 22, F_DIG2_LO = 23
 };
 
 // ------------------------------------------------------------------------------------
@@ -438,14 +447,16 @@ __device__ __noinline__ bool particle_cut(const KParams &P, double p0x, double p
 
 // What the preamble knows about an emitter, in double: for the photons that fp32 cannot carry (flat_hit_f64).
 struct FrameD { double p0[3], d[3], L, t0, ibc, w0, sin_c, cos_c, omc, axis[3]; int kind; };
+struct FrameDisp { double d_eta, d_beta2, d_mean; };     // R30: refractivity at the midpoint, beta^2, band average of sin^2
 
 // Preamble of emitter (segment i, process tag).  Writes the frame, returns n_b.
 // *bad is set when the segment is invalid: 1 = non-finite field, gamma <= 1, L < 0 or |d| off unity by > 1e-3 (the
 // same for both processes), 2 = n_b >= 2^24 for this process.
-template <bool WITH_D = false, bool WITH_MASK = false>
+// DISP: the Cherenkov yield and angle with n(lambda) (R30).
+template <bool WITH_D = false, bool WITH_MASK = false, bool DISP = false>
 __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1, const float4 s2, int tag,
                              float *__restrict__ fr, uint8_t *kind_out, int *bad, bool *culled, FrameD *fd = nullptr,
-                             uint8_t *tmask_out = nullptr)
+                             uint8_t *tmask_out = nullptr, FrameDisp *fdisp = nullptr)
 {
     if constexpr (WITH_MASK) *tmask_out = 0xffu;
     *bad = 0;
@@ -463,23 +474,47 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     const double ibc = 1.0 / (beta * 0.299792458);        // R7: the particle moves at beta c  [ns/m]
 
     double mu, sin_c = 0.0, cos_c = 1.0, omc_e = P.omc;      // omc_e = 1 - cos(alpha) of this emitter's cone
+    double d_eta = 0.0, d_beta2 = 1.0, d_mean = 1.0;         // R30: refractivity at the midpoint, beta^2, band average of sin^2
+    constexpr bool disp = DISP;
     int kind;
     double axis[3];
     if (tag == 0) {
         // Frank-Tamm with the atmosphere homogeneous over the step (R3: midpoint altitude).
         const double h_mid = dadd(p0[2], dmul(dmul(0.5, L), d[2]));
         const double eta = refractivity(P, h_mid);
-        const double n1 = dadd(1.0, eta);
-        // q = beta^2 n^2 - 1 without cancellation; q <= 0 is the threshold Theta(beta - 1/n).
-        const double q = dsub(dadd(dmul(2.0, eta), dmul(eta, eta)), dmul(dmul(n1, n1), ig2));
-        if (!(q > 0.0) || !(L > 0.0)) return 0;
-        const double bn2 = dmul(dmul(dsub(1.0, ig2), n1), n1);
-        const double sin2 = ddiv(q, bn2);
-        cos_c = 1.0 / sqrt(bn2);
-        sin_c = sqrt(sin2);
-        mu = dmul(dmul(dmul(dmul(P.c_ft, zq), zq), L), sin2);
         axis[0] = d[0]; axis[1] = d[1]; axis[2] = d[2];
-        kind = (d[2] <= -0.1) ? KIND_CHER_AXIS : KIND_CHER_GEN;
+        if (disp) {
+            // R30 (PAPER.md:45 with n(lambda)): N = 2 pi alpha z^2 L int sin^2 theta_c(x) Theta dx over x = 1 / lambda,
+            // n(x) - 1 = eta (1 + b x^2), composite Simpson with 16 intervals; the oracle's operation order (feeds n_b).
+            // Every photon then leaves at the angle of its own wavelength (photon_from_rand): generic projection.
+            if (!(L > 0.0)) return 0;
+            d_eta = eta; d_beta2 = dsub(1.0, ig2);
+            const double h = ddiv(dsub(P.x1_d, P.x2_d), 16.0);
+            double ends = 0.0, odd = 0.0, even = 0.0;
+            for (int k = 0; k <= 16; ++k) {
+                const double x = dadd(P.x2_d, dmul((double)k, h));
+                const double n = dadd(1.0, dmul(eta, dadd(1.0, dmul(dmul(P.cauchy_b, x), x))));
+                double f = dsub(1.0, ddiv(1.0, dmul(dmul(d_beta2, n), n)));
+                if (!(f > 0.0)) f = 0.0;
+                if (k == 0 || k == 16) ends = dadd(ends, f); else if (k & 1) odd = dadd(odd, f); else even = dadd(even, f);
+            }
+            const double S = dmul(ddiv(h, 3.0), dadd(dadd(ends, dmul(4.0, odd)), dmul(2.0, even)));
+            if (!(S > 0.0)) return 0;
+            mu = dmul(dmul(dmul(dmul(P.c_ft0, zq), zq), L), S);
+            d_mean = ddiv(S, dsub(P.x1_d, P.x2_d));
+            kind = KIND_CHER_GEN;
+        } else {
+            const double n1 = dadd(1.0, eta);
+            // q = beta^2 n^2 - 1 without cancellation; q <= 0 is the threshold Theta(beta - 1/n).
+            const double q = dsub(dadd(dmul(2.0, eta), dmul(eta, eta)), dmul(dmul(n1, n1), ig2));
+            if (!(q > 0.0) || !(L > 0.0)) return 0;
+            const double bn2 = dmul(dmul(dsub(1.0, ig2), n1), n1);
+            const double sin2 = ddiv(q, bn2);
+            cos_c = 1.0 / sqrt(bn2);
+            sin_c = sqrt(sin2);
+            mu = dmul(dmul(dmul(dmul(P.c_ft, zq), zq), L), sin2);
+            kind = (d[2] <= -0.1) ? KIND_CHER_AXIS : KIND_CHER_GEN;
+        }
     } else {
         // constant yield x total energy loss over the track (R13).
         mu = dmul(P.fl_yield, dE);
@@ -546,6 +581,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
     if constexpr (WITH_D) {
         for (int i = 0; i < 3; ++i) { fd->p0[i] = p0[i]; fd->d[i] = d[i]; fd->axis[i] = axis[i]; }
         fd->L = L; fd->t0 = (double)s0.w; fd->ibc = ibc; fd->w0 = w0; fd->sin_c = sin_c; fd->cos_c = cos_c; fd->omc = omc_e; fd->kind = kind;
+        if constexpr (DISP) { fdisp->d_eta = d_eta; fdisp->d_beta2 = d_beta2; fdisp->d_mean = d_mean; }
     }
     fr[F_W0] = (float)w0; fr[F_T0] = s0.w; fr[F_IBC] = (float)ibc; fr[F_LEN] = (float)L; fr[F_OMC] = (float)omc_e;
     {
@@ -618,12 +654,21 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
         return (uint32_t)nb;
     }
     // KIND_CONE / KIND_CHER_GEN: v = sth (cos' A + sin' B) + cth C
-    const double sa = (kind == KIND_CHER_GEN) ? sin_c : 1.0, sc = (kind == KIND_CHER_GEN) ? cos_c : 1.0;
+    // (R30: sin / cos of the Cherenkov angle are the photon's own, so the columns stay unscaled as for the cone)
+    const bool scaled = (kind == KIND_CHER_GEN) && !disp;
+    const double sa = scaled ? sin_c : 1.0, sc = scaled ? cos_c : 1.0;
     for (int i = 0; i < 3; ++i) {
         fr[F_E0 + i] = (float)e0[i]; fr[F_D0 + i] = (float)d[i];
         fr[F_A0 + i] = (float)(-sa * m0[i]); fr[F_B0 + i] = (float)(-sa * m1[i]); fr[F_C0 + i] = (float)(sc * axis[i]);
     }
     fr[F_L] = (float)L;
+    if constexpr (DISP) {
+        if (kind == KIND_CHER_GEN) {
+            fr[F_DETA] = (float)d_eta; fr[F_DETA_LO] = (float)(d_eta - (double)(float)d_eta);
+            fr[F_DIG2] = (float)ig2; fr[F_DIG2_LO] = (float)(ig2 - (double)(float)ig2);
+            fr[F_DINVM] = (float)(1.0 / d_mean);
+        }
+    }
     return (uint32_t)nb;
 }
 
@@ -634,6 +679,15 @@ __device__ __noinline__ int cherenkov_preamble_status(const KParams &P, const fl
     bool culled;
     uint8_t kind;
     preamble(P, s0, s1, s2, 0, scratch_frame, &kind, &bad, &culled);
+    return bad;
+}
+// the same with n(lambda) (R30: another yield, so another bunch count)
+__device__ __noinline__ int cherenkov_preamble_status_disp(const KParams &P, const float4 s0, const float4 s1, const float4 s2, float *scratch_frame)
+{
+    int bad;
+    bool culled;
+    uint8_t kind;
+    preamble<false, false, true>(P, s0, s1, s2, 0, scratch_frame, &kind, &bad, &culled);
     return bad;
 }
 
@@ -674,6 +728,9 @@ __device__ __forceinline__ void sincospi_unit(float x, float *s, float *c)
 struct Photon { float ex, ey, ez, gx, gy, vx, vy, vz, s, u3, rva; int tag; bool axis; };   // u3 = the wavelength uniform; rva = MUFU.RCP(v_z), axis kind
 
 // a3 for a photon of emitter e, any kind, from its four random words.
+// DISP (R30): a Cherenkov photon of the generic kind leaves at the angle of its own wavelength; ph.rva then carries its
+// weight factor sin^2 theta_c(lambda) / <sin^2 theta_c>, 0 = below the threshold at this wavelength (no photon).
+template <bool DISP = false>
 __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileSmem &sm, int e, const Rand4 r)
 {
     const float *fr = &sm.frame[e * kFrameStride];
@@ -717,6 +774,26 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
             const float t = uniform01(r.r3) * fr[F_OMC];
             cth = 1.0f - t; sth = sqrtf(t * (2.0f - t));     // beamed: sin(theta') sets the aim at 10 km, keep the IEEE root
         }
+        if constexpr (DISP) {
+            if (kind == KIND_CHER_GEN) {
+                // n(x) - 1 = eta' = eta (1 + b x^2), x = 1 / lambda; sin^2 = q / (beta n)^2 with
+                // q = 2 eta' + eta'^2 - (1 + eta')^2 / gamma^2.  Near the threshold q is a small difference of 2 eta' and
+                // 1 / gamma^2, each ~1e-4: in double (head + tail of eta and 1 / gamma^2 from the frame), so that the weight
+                // factor keeps the 1e-5 of the parity criterion.
+                const float x = fmaf(-ph.u3, P.dinv_lam, P.inv_lam1);
+                const double eta = (double)fr[F_DETA] + (double)fr[F_DETA_LO], ig2 = (double)fr[F_DIG2] + (double)fr[F_DIG2_LO];
+                const double etap = eta * (1.0 + (double)(P.cauchy_b_f * x) * (double)x), n1 = 1.0 + etap;
+                const double q = 2.0 * etap + etap * etap - n1 * n1 * ig2, bn2 = (1.0 - ig2) * n1 * n1;
+                const float s2 = (float)(q / bn2);
+                sth = sqrtf(fmaxf(s2, 0.0f)); cth = rsqrtf((float)bn2);
+                ph.vx = fmaf(sth, fmaf(cp, fr[F_A0 + 0], sp * fr[F_B0 + 0]), cth * fr[F_C0 + 0]);
+                ph.vy = fmaf(sth, fmaf(cp, fr[F_A0 + 1], sp * fr[F_B0 + 1]), cth * fr[F_C0 + 1]);
+                ph.vz = fmaf(sth, fmaf(cp, fr[F_A0 + 2], sp * fr[F_B0 + 2]), cth * fr[F_C0 + 2]);
+                ph.gx = ph.gy = 0.0f;
+                ph.rva = (q > 0.0) ? s2 * fr[F_DINVM] : 0.0f;
+                return ph;
+            }
+        }
         ph.vx = fmaf(sth, fmaf(cp, fr[F_A0 + 0], sp * fr[F_B0 + 0]), cth * fr[F_C0 + 0]);
         ph.vy = fmaf(sth, fmaf(cp, fr[F_A0 + 1], sp * fr[F_B0 + 1]), cth * fr[F_C0 + 1]);
         ph.vz = fmaf(sth, fmaf(cp, fr[F_A0 + 2], sp * fr[F_B0 + 2]), cth * fr[F_C0 + 2]);
@@ -728,11 +805,12 @@ __device__ __forceinline__ Photon photon_from_rand(const KParams &P, const TileS
 __device__ __forceinline__ uint32_t kind_tag(int kind) { return (kind == KIND_CHER_AXIS || kind == KIND_CHER_GEN) ? 0u : 1u; }
 
 // a2 + a3 for photon j of emitter e, any kind (used by the queue drain, the wide test and the generic kinds' hot path).
+template <bool DISP = false>
 __device__ __forceinline__ Photon make_photon(const KParams &P, const TileSmem &sm, int e, uint32_t j, unsigned long long S)
 {
     const uint32_t tag = kind_tag(sm.kind[e]);
     const Rand4 blk = philox4x32_10(P, tag ? j : (j >> 1), (uint32_t)S, (uint32_t)(S >> 32), tag);
-    return photon_from_rand(P, sm, e, tag ? blk : cherenkov_words(blk, j));
+    return photon_from_rand<DISP>(P, sm, e, tag ? blk : cherenkov_words(blk, j));
 }
 
 // One accepted (photon, telescope) pair, ready for the tally / record.
@@ -879,6 +957,7 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     h.lam = (ph.tag == 0) ? cherenkov_lambda(P, u3) : fmaf(u3, P.fl_dlam, P.fl_lam1);
     // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
     h.w = fr[F_W0];
+    if constexpr (TELSRC == TEL_GLOBAL_DISP) { if (ph.tag == 0) h.w *= ph.rva; }      // R30: sin^2(lambda) / <sin^2>
     if (P.tau != nullptr) {
         const int nh = P.tau_nh, nl = P.tau_nl;
         float fh = (habs - P.tau_h0) * P.tau_inv_dh, fl = (h.lam - P.tau_l0) * P.tau_inv_dl;
@@ -909,6 +988,7 @@ __device__ __forceinline__ double column_depth_d(const KParams &P, double h)
     return l.a + l.b * exp(-h / l.c);
 }
 
+template <bool DISP>
 __device__ __noinline__ Hit flat_hit_f64(const KParams &P, unsigned long long S, uint32_t tag, uint32_t j, int k)
 {
     Hit h;
@@ -920,7 +1000,8 @@ __device__ __noinline__ Hit flat_hit_f64(const KParams &P, unsigned long long S,
     int bad;
     bool culled;
     FrameD f;
-    const uint32_t nb = preamble<true>(P, s0, s1, s2, (int)tag, scratch, &kind8, &bad, &culled, &f);
+    [[maybe_unused]] FrameDisp fx;
+    const uint32_t nb = preamble<true, false, DISP>(P, s0, s1, s2, (int)tag, scratch, &kind8, &bad, &culled, &f, nullptr, &fx);
     if (bad || culled || j >= nb) return h;
     // a2, R19: U = ((r >> 9) + 1/2) 2^-23; the Cherenkov wavelength uniform from the 9 + 9 low bits (R20)
     const Rand4 blk = philox4x32_10(P, tag ? j : (j >> 1), (uint32_t)S, (uint32_t)(S >> 32), tag);
@@ -936,12 +1017,22 @@ __device__ __noinline__ Hit flat_hit_f64(const KParams &P, unsigned long long S,
     double sphi, cphi;
     sincos(6.283185307179586476925 * u2, &sphi, &cphi);
     double v[3];
+    [[maybe_unused]] double wfac = 1.0;
     if (f.kind == KIND_FL_ISO) {
         const double cth = 1.0 - 2.0 * u4, sth = 2.0 * sqrt(u4 * (1.0 - u4));
         v[0] = cphi * sth; v[1] = sphi * sth; v[2] = -cth;
     } else {
         double sth = f.sin_c, cth = f.cos_c;                     // Cherenkov (generic projection)
         if (f.kind == KIND_CONE) { const double t = u4 * f.omc; cth = 1.0 - t; sth = sqrt(t * (2.0 - t)); }
+        if constexpr (DISP) {
+            if (f.kind == KIND_CHER_GEN) {                       // R30: the angle and weight factor of this wavelength
+                const double x = P.x1_d - u3 * (P.x1_d - P.x2_d), n = 1.0 + fx.d_eta * (1.0 + P.cauchy_b * x * x);
+                const double s2 = 1.0 - 1.0 / (fx.d_beta2 * n * n);
+                if (!(s2 > 0.0)) return h;
+                sth = sqrt(s2); cth = 1.0 / (sqrt(fx.d_beta2) * n);
+                wfac = s2 / fx.d_mean;
+            }
+        }
         double m0[3], m1[3];
         rodrigues_columns(f.axis, m0, m1);
         // M_Rod (cos phi sth, sin phi sth, -cth) with the third column of M_Rod = -axis
@@ -961,6 +1052,7 @@ __device__ __noinline__ Hit flat_hit_f64(const KParams &P, unsigned long long S,
     const double lam = tag ? P.fl_lam1_d + u3 * (P.fl_lam2_d - P.fl_lam1_d)
                            : 1.0 / (1.0 / P.lam1_d - u3 * (1.0 / P.lam1_d - 1.0 / P.lam2_d));
     double w = f.w0;
+    if constexpr (DISP) w *= wfac;
     if (P.tau != nullptr) {
         const int nh = P.tau_nh, nl = P.tau_nl;
         double fh = (e[2] - P.tau_h0_d) / P.tau_dh_d, fl = (lam - P.tau_l0_d) / P.tau_dl_d;
@@ -1014,7 +1106,7 @@ __device__ __forceinline__ unsigned long long emitter_segment(const KParams &P, 
 }
 
 // The tile's flat list in double (see evaluate_any), by all threads of the tile after the photon loops: tally, record.
-template <int MODE>
+template <int MODE, bool DISP>
 __device__ __noinline__ void flat_pass(const KParams &P, TileSmem &sm, unsigned long long tile_first)
 {
     const uint32_t n = min(sm.flat_count, (uint32_t)kFlatList);
@@ -1023,7 +1115,7 @@ __device__ __noinline__ void flat_pass(const KParams &P, TileSmem &sm, unsigned 
         const int e = (int)(q.x >> 24), k = (int)q.y;
         const uint32_t j = q.x & 0xffffffu, tag = kind_tag(sm.kind[e]);
         const unsigned long long S = emitter_segment(P, tile_first, e);
-        const Hit h = flat_hit_f64(P, S, tag, j, k);
+        const Hit h = flat_hit_f64<DISP>(P, S, tag, j, k);
         if (!h.ok) continue;
         const double w = (double)h.w;
         if (P.n_tel <= kTelSmemMax) { atomicAdd(&sm.t_hits[k], 1u); atomicAdd(&sm.t_sw[k], w); atomicAdd(&sm.t_swt[k], w * (double)h.t); }
@@ -1235,7 +1327,7 @@ __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigne
         const int e = (int)(q.x >> 24);
         const uint32_t j = q.x & 0xffffffu;
         const unsigned long long S = emitter_segment(P, tile_first, e);
-        const Photon ph = make_photon(P, sm, e, j, S);
+        const Photon ph = make_photon<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, j, S);
         h = evaluate_any<TELSRC>(P, sm, e, ph, (int)q.y, j);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
@@ -1254,7 +1346,7 @@ __device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned
     uint64_t id = 0;
     if (has) {
         const unsigned long long S = emitter_segment(P, tile_first, e);
-        const Photon ph = photon_from_rand(P, sm, e, Rand4{r0, r1, r2, r3});
+        const Photon ph = photon_from_rand<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, Rand4{r0, r1, r2, r3});
         h = evaluate_any<TELSRC>(P, sm, e, ph, k, j);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
@@ -1402,7 +1494,7 @@ __device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned
     if (lane < n) {
         const uint32_t q = sm.wide_list[warp][lane];
         e = (int)(q >> 24); j = q & 0xffffffu;
-        const Photon ph = make_photon(P, sm, e, j, emitter_segment(P, tile_first, e));
+        const Photon ph = make_photon<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, j, emitter_segment(P, tile_first, e));
         live = ph.vz < 0.0f;
         // a point of the ray relative to (x_ref, y_ref, z_ref): the plane crossing (axis kind) or the emission point
         px = ph.axis ? ph.gx : ph.ex; py = ph.axis ? ph.gy : ph.ey; pz = ph.axis ? 0.0f : ph.ez;
@@ -1472,7 +1564,10 @@ template <int TELSRC, bool COPLANAR, int NT, bool REFR>
 __device__ __noinline__ uint32_t generic_candidates(const KParams &P, const TileSmem &sm, int e, uint32_t r0, uint32_t r1, uint32_t r2,
                                                     uint32_t r3, uint2 *cell, bool *upward)
 {
-    const Photon ph = photon_from_rand(P, sm, e, Rand4{r0, r1, r2, r3});
+    const Photon ph = photon_from_rand<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, Rand4{r0, r1, r2, r3});
+    if constexpr (TELSRC == TEL_GLOBAL_DISP) {
+        if (ph.tag == 0 && ph.rva == 0.0f) { *upward = false; return 0u; }      // R30: below the threshold at its wavelength
+    }
     *upward = !(ph.vz < 0.0f);
     if (*upward) return 0u;
     if (ph.vz > -0.05f) return kAllTelescopes;
@@ -2141,13 +2236,14 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
         int bad;
         bool culled;
-        nb = preamble<false, TELSRC == TEL_CONST>(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled, nullptr,
+        nb = preamble<false, TELSRC == TEL_CONST, TELSRC == TEL_GLOBAL_DISP>(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled, nullptr,
                                                   &sm.tmask[tid]);
         if (P.split_part == 2) {
             // second launch of a two-process request: the first one (Cherenkov) has counted the segments that are
             // invalid for both processes or for Cherenkov; what is left to count here is a segment whose fluorescence
             // bunch count alone is out of range (the Cherenkov preamble is run again to find out; rare)
-            if (bad == 2 && cherenkov_preamble_status(P, s0, s1, s2, &sm.frame[tid * kFrameStride]) == 0) sm.invalid[seg_local] = 1;
+            if (bad == 2 && (P.cauchy_b > 0.0 ? cherenkov_preamble_status_disp(P, s0, s1, s2, &sm.frame[tid * kFrameStride])
+                                              : cherenkov_preamble_status(P, s0, s1, s2, &sm.frame[tid * kFrameStride])) == 0) sm.invalid[seg_local] = 1;
         } else if (bad) sm.invalid[seg_local] = 1;
         if (P.counts) {
             P.counts[seg_i * 2ull + (unsigned)tag] = nb;
@@ -2287,7 +2383,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     if constexpr (MODE != MODE_HIST) {
         // the flat photons the loops set aside, in double (tile-uniform branch)
         if (sm.flat_count) {
-            flat_pass<MODE>(P, sm, tile_first);
+            flat_pass<MODE, TELSRC == TEL_GLOBAL_DISP>(P, sm, tile_first);
             __syncthreads();
         }
     }

@@ -41,7 +41,7 @@ def test_struct_layouts_match_header(c8):
     assert c8.TALLY_DTYPE.itemsize == 24                        # c8opt_tally
     assert C.sizeof(c8._Layer) == 32
     assert C.sizeof(c8._AtmosphereDesc) == 8 + 8 * 32 + 24 + 8 + 32 + 8
-    assert C.sizeof(c8._RunParams) == 8 + 8 + 6 * 8 + 8 + 8 + 8
+    assert C.sizeof(c8._RunParams) == 8 + 8 + 6 * 8 + 8 + 8 + 8 + 8
     assert C.sizeof(c8._Output) == 5 * 8
 
 

@@ -683,3 +683,37 @@ def test_many_flat_photons_in_one_tile(c8):
     rep = pu.compare(cfg, g, o)
     _report("flat-many", rep)
     assert rep["flat_records_two_component_direction"] > 150 and rep["matched"] > 10_000
+
+
+@pytest.mark.parametrize("name,n,b", [("c2", 40_000, 5670.0), ("c1", None, 5670.0), ("c4", 60_000, 5670.0), ("c2", 30_000, 60_000.0)])
+def test_wavelength_dependent_refractive_index(c8, name, n, b):
+    """R30 (PAPER.md:45 with n(lambda)): n - 1 = eta(h) (1 + b / lambda^2).  The yield is the Simpson integral over the
+    band (bunch counts bit-exact), every photon leaves at the Cherenkov angle of its own wavelength with the weight
+    factor sin^2 / <sin^2>; records against the oracle on one telescope, on configs[1]'s array, with both processes
+    on configs[3]'s array, and with a dispersion ten times that of air (thresholds inside the band for many emitters)."""
+    import parity_util as pu
+    cfg = wl.make_config(name, n_segments=n)
+    base = pu.gpu_run(cfg, c8.MODE_TALLY)
+    cfg["params"] = dict(cfg["params"], cauchy_b=b)
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report(f"dispersion-{name}-b{b:g}", rep)
+    assert rep["matched"] > 100
+    # more light than with the long-wavelength n (n grows towards the blue), and tally mode sees the same photons
+    assert g["counters"]["generated"] > base["counters"]["generated"]
+    t = pu.gpu_run(cfg, c8.MODE_TALLY)
+    assert np.array_equal(t["tallies"]["hits"], g["tallies"]["hits"])
+    assert np.allclose(t["tallies"]["sum_w"], g["tallies"]["sum_w"], rtol=1e-12)
+    assert t["counters"]["generated"] == g["counters"]["generated"] and t["counters"]["upward"] == g["counters"]["upward"]
+
+
+def test_wavelength_dependent_refractive_index_argument_errors(c8):
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=1000)
+    for over, msg in ((dict(cauchy_b=-1.0), "cauchy_b_nm2"), (dict(cauchy_b=5670.0, flags=c8.FLAG_CULL), "culling")):
+        cfg["params"] = dict(cfg["params"], **over)
+        with pytest.raises(c8.C8optError) as ei:
+            pu.gpu_run(cfg, c8.MODE_TALLY)
+        assert ei.value.code == -1 and msg in str(ei.value)
+        cfg["params"].pop("flags", None)
