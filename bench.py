@@ -212,6 +212,9 @@ def main():
                          "segments: 1000 bins of 1 m about the shower axis; telescopes are not consulted")
     ap.add_argument("--cull", action="store_true",
                     help="segment culling on (C8OPT_FLAG_CULL): same tallies, `value` then counts culled bunches too")
+    ap.add_argument("--cauchy-b", type=float, default=0.0,
+                    help="wavelength-dependent refractive index n - 1 = eta (1 + b / lambda^2), b in nm^2 (DESIGN.md R30; "
+                         "air: 5670); not the headline configuration, the roofline fraction then does not apply")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -254,6 +257,9 @@ def main():
     par = dict(cfg["params"])
     if args.cull:
         par["flags"] = c8.FLAG_CULL
+    if args.cauchy_b > 0.0:
+        par["cauchy_b"] = args.cauchy_b
+        cfg["params"] = dict(cfg["params"], cauchy_b=args.cauchy_b)       # the oracle leg times the same physics
     if args.ground_hist:
         par["mode"] = c8.MODE_GROUND_HIST
         par["fl_beam_telescope"] = -1
@@ -371,7 +377,7 @@ def main():
     # ---- photon-output leg (north_star's second roofline): the same segments against one accept-all detector on the
     # observation level, every downward photon written as a 28-byte record ("c5g" at this segment count)
     roofline_output = None
-    if args.workload == "c2" and not (args.no_output_leg or args.cull or args.ground_hist) and world == 1:
+    if args.workload == "c2" and not (args.no_output_leg or args.cull or args.ground_hist or args.cauchy_b > 0.0) and world == 1:
         # "c5g": configs[4]'s segment set (the c2 generator at 10^7 segments) with one accept-all detector
         del kw
         ocfg = wl.make_config("c5g", n_segments=args.output_segments)
@@ -437,7 +443,8 @@ def main():
                    "parallelism": f"segments sharded over {world} GPU(s), no data-path collective; one all-reduce of the tallies after the job",
                    "culling": (f"on: {culled_per_step} of the bunches per step are generated but provably miss every telescope "
                                "and skip the photon loop; value counts them (pre-cull equivalent), tallies are identical")
-                              if args.cull else "off"},
+                              if args.cull else "off",
+                   "cauchy_b_nm2": args.cauchy_b},
         "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "wall_s_timed_region": wall, "step_ms_min_med_max": [float(step_ms.min()), float(np.median(step_ms)), float(step_ms.max())],
     }

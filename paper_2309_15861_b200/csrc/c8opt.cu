@@ -161,11 +161,19 @@ kernel_t pick_kernel(int tel_src, bool coplanar, int nt, int out)
     return pick_kernel2<c8::TEL_GLOBAL, 0>(coplanar, out);
 }
 
-// R30 (cauchy_b_nm2 > 0): the Cherenkov launch runs on the instances with the wavelength-dependent refractive index,
-// brute force over the telescopes in global memory whatever the array (out: 0 tally, else photon output).
-kernel_t pick_disp_kernel(int out)
+// R30 (cauchy_b_nm2 > 0): the Cherenkov launch runs on the instances with the wavelength-dependent refractive index:
+// one per telescope source and mode (out: 0 tally, else photon output), the general ones -- telescopes at any height,
+// eight constant-bank slots (the unused ones never hit), no dense loop.
+kernel_t pick_disp_kernel(int tel_src, int out)
 {
-    return out ? c8::propagate_kernel<c8::TEL_GLOBAL_DISP, false, 0, c8::MODE_OUT> : c8::propagate_kernel<c8::TEL_GLOBAL_DISP, false, 0, c8::MODE_TALLY>;
+    if (tel_src == c8::TEL_CONST)
+        return out ? c8::propagate_kernel<c8::TEL_CONST | c8::TEL_DISP, false, 8, c8::MODE_OUT, false>
+                   : c8::propagate_kernel<c8::TEL_CONST | c8::TEL_DISP, false, 8, c8::MODE_TALLY>;
+    if (tel_src == c8::TEL_GRID)
+        return out ? c8::propagate_kernel<c8::TEL_GRID | c8::TEL_DISP, false, 0, c8::MODE_OUT>
+                   : c8::propagate_kernel<c8::TEL_GRID | c8::TEL_DISP, false, 0, c8::MODE_TALLY>;
+    return out ? c8::propagate_kernel<c8::TEL_GLOBAL | c8::TEL_DISP, false, 0, c8::MODE_OUT>
+               : c8::propagate_kernel<c8::TEL_GLOBAL | c8::TEL_DISP, false, 0, c8::MODE_TALLY>;
 }
 
 // A tile of a shower's light is "dense" on a telescope (a good part of its photons hit it) only when the telescope is
@@ -394,7 +402,7 @@ int launch_one(c8opt_ctx *ctx, c8::KParams &P, unsigned mode, unsigned long long
         const bool dense_loop = out && ctx->tel_src == c8::TEL_CONST && ctx->r_max >= kDenseRadiusMin_m;
         const bool disp = P.cauchy_b > 0.0 && (P.processes & C8OPT_PROC_CHERENKOV);
         if (disp) {
-            pick_disp_kernel(out)<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, false), st>>>(P);
+            pick_disp_kernel(ctx->tel_src, out)<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, false), st>>>(P);
         } else {
             kernel_t k = pick_kernel(ctx->tel_src, ctx->coplanar, padded_count(ctx->n_tel), out ? (dense_loop || ctx->tel_src != c8::TEL_CONST ? 1 : 2) : 0);
             k<<<(unsigned)tiles, c8::kTile, smem_bytes(out ? c8::MODE_OUT : c8::MODE_TALLY, dense_loop, P.ids != nullptr), st>>>(P);
@@ -534,8 +542,9 @@ int c8opt_create_atmosphere(const c8opt_atmosphere_desc *desc, c8opt_ctx **out)
         for (int cp = 0; cp < 2 && e == cudaSuccess; ++cp)
             e = cudaFuncSetAttribute(pick_kernel(c8::TEL_CONST, cp != 0, nt, 2), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)smem_bytes(c8::MODE_OUT, false));
-    for (int o = 0; o < 2 && e == cudaSuccess; ++o)
-        e = cudaFuncSetAttribute(pick_disp_kernel(o), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(o ? c8::MODE_OUT : c8::MODE_TALLY, false));
+    for (int ts = 0; ts < 3 && e == cudaSuccess; ++ts)
+        for (int o = 0; o < 2 && e == cudaSuccess; ++o)
+            e = cudaFuncSetAttribute(pick_disp_kernel(ts, o), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(o ? c8::MODE_OUT : c8::MODE_TALLY, false));
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(c8::propagate_kernel<c8::TEL_CONST, true, 1, c8::MODE_HIST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)smem_bytes(c8::MODE_HIST));
@@ -893,7 +902,7 @@ int static_device(int dev, StaticDevice *out)
             for (int cp = 0; cp < 2; ++cp)
                 C8_CUDA(nullptr, cudaFuncSetAttribute(pick_kernel(c8::TEL_CONST, cp != 0, nt, 0), cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                       (int)smem_bytes(c8::MODE_TALLY)));
-        C8_CUDA(nullptr, cudaFuncSetAttribute(pick_disp_kernel(0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(c8::MODE_TALLY)));
+        C8_CUDA(nullptr, cudaFuncSetAttribute(pick_disp_kernel(c8::TEL_CONST, 0), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(c8::MODE_TALLY)));
         d.scratch = ptr; d.n_sm = n_sm > 0 ? n_sm : 148; d.ready = true;
     }
     *out = d;

@@ -36,9 +36,10 @@ constexpr int kTelGridMin = 9;        // from this many telescopes on, the groun
 constexpr int TEL_CONST = 0;          // brute force over <= kTelConstMax telescopes read from the constant bank
 constexpr int TEL_GRID = 1;           // candidate lookup in the ground-plane grid
 constexpr int TEL_GLOBAL = 2;         // brute force over telescopes in global memory (grid not buildable)
-constexpr int TEL_GLOBAL_DISP = 3;    // TEL_GLOBAL with the wavelength-dependent refractive index (R30): the instances
-                                      // a request with cauchy_b > 0 runs on, whatever the array (every code path that
-                                      // compares TELSRC with TEL_CONST / TEL_GRID treats it as TEL_GLOBAL)
+constexpr int TEL_DISP = 4;           // + TEL_DISP: the same with the wavelength-dependent refractive index (R30): the
+                                      // instances the Cherenkov launch of a request with cauchy_b > 0 runs on
+__host__ __device__ constexpr int tel_base(int telsrc) { return telsrc & 3; }
+__host__ __device__ constexpr bool tel_disp(int telsrc) { return (telsrc & TEL_DISP) != 0; }
 constexpr int kMaxLayers = 8;
 constexpr int kRecWords = 7;          // floats per photon record {x, y, cos_x, cos_y, t, lambda, w}
 constexpr int kBlockRecs = 64;        // photon output, dense tiles: records a warp stages per trip of the dense loop (2 per lane)
@@ -559,7 +560,7 @@ __device__ uint32_t preamble(const KParams &P, const float4 s0, const float4 s1,
         *culled = true;
         return (uint32_t)nb;
     }
-    if (WITH_MASK && tag == 0 && P.n_tel <= kTelConstMax) {
+    if (WITH_MASK && !DISP && tag == 0 && P.n_tel <= kTelConstMax) {        // (R30: no single cone, the mask stays full)
         // small arrays: the telescopes this emitter can reach at all; none = culled (C8OPT_FLAG_CULL)
         const double hl = 0.5 * L;
         const uint32_t tm = reach_mask(P, (float)(p0[0] + hl * d[0] - P.x_ref), (float)(p0[1] + hl * d[1] - P.y_ref), (float)(p0[2] + hl * d[2] - P.z_ref),
@@ -694,17 +695,17 @@ __device__ __noinline__ int cherenkov_preamble_status_disp(const KParams &P, con
 // ------------------------------------------------------------------------------------
 template <int TELSRC> __device__ __forceinline__ float4 tel_at(const KParams &P, int k)
 {
-    if (TELSRC == TEL_CONST) return P.tel_c[k];
+    if (tel_base(TELSRC) == TEL_CONST) return P.tel_c[k];
     return __ldg(&P.telA[k]);
 }
 template <int TELSRC> __device__ __forceinline__ float telT_at(const KParams &P, int k)
 {
-    if (TELSRC == TEL_CONST) return P.telT_c[k];
+    if (tel_base(TELSRC) == TEL_CONST) return P.telT_c[k];
     return __ldg(&P.telT[k]);
 }
 template <int TELSRC> __device__ __forceinline__ float telEta_at(const KParams &P, int k)
 {
-    if (TELSRC == TEL_CONST) return P.telEta_c[k];
+    if (tel_base(TELSRC) == TEL_CONST) return P.telEta_c[k];
     return __ldg(&P.telEta[k]);
 }
 
@@ -957,7 +958,7 @@ __device__ __forceinline__ Hit evaluate_pair(const KParams &P, const TileSmem &s
     h.lam = (ph.tag == 0) ? cherenkov_lambda(P, u3) : fmaf(u3, P.fl_dlam, P.fl_lam1);
     // R17: transmission weight exp(-tau(h, lambda) / |v_z|)
     h.w = fr[F_W0];
-    if constexpr (TELSRC == TEL_GLOBAL_DISP) { if (ph.tag == 0) h.w *= ph.rva; }      // R30: sin^2(lambda) / <sin^2>
+    if constexpr (tel_disp(TELSRC)) { if (ph.tag == 0) h.w *= ph.rva; }      // R30: sin^2(lambda) / <sin^2>
     if (P.tau != nullptr) {
         const int nh = P.tau_nh, nl = P.tau_nl;
         float fh = (habs - P.tau_h0) * P.tau_inv_dh, fl = (h.lam - P.tau_l0) * P.tau_inv_dl;
@@ -1327,7 +1328,7 @@ __device__ __noinline__ void drain_queue(const KParams &P, TileSmem &sm, unsigne
         const int e = (int)(q.x >> 24);
         const uint32_t j = q.x & 0xffffffu;
         const unsigned long long S = emitter_segment(P, tile_first, e);
-        const Photon ph = make_photon<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, j, S);
+        const Photon ph = make_photon<tel_disp(TELSRC)>(P, sm, e, j, S);
         h = evaluate_any<TELSRC>(P, sm, e, ph, (int)q.y, j);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
@@ -1346,7 +1347,7 @@ __device__ __noinline__ void dense_eval(const KParams &P, TileSmem &sm, unsigned
     uint64_t id = 0;
     if (has) {
         const unsigned long long S = emitter_segment(P, tile_first, e);
-        const Photon ph = photon_from_rand<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, Rand4{r0, r1, r2, r3});
+        const Photon ph = photon_from_rand<tel_disp(TELSRC)>(P, sm, e, Rand4{r0, r1, r2, r3});
         h = evaluate_any<TELSRC>(P, sm, e, ph, k, j);
         id = (S << 25) | ((unsigned long long)ph.tag << 24) | (unsigned long long)j;
     }
@@ -1420,7 +1421,7 @@ constexpr uint32_t kAllTelescopes = 0x80000000u;
 // telescope index of candidate bit c
 template <int TELSRC> __device__ __forceinline__ uint32_t slot_telescope(const uint2 cell, int c)
 {
-    if (TELSRC == TEL_GRID) return ((c < 2 ? cell.x : cell.y) >> (16 * (c & 1))) & 0xffffu;
+    if (tel_base(TELSRC) == TEL_GRID) return ((c < 2 ? cell.x : cell.y) >> (16 * (c & 1))) & 0xffffu;
     return (uint32_t)c;
 }
 
@@ -1450,7 +1451,7 @@ __device__ __forceinline__ uint32_t grid_lookup(const KParams &P, const GridLeve
 template <int TELSRC, bool COPLANAR, int NT, bool REFR>
 __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx, float gy, float vx, float vy, float vz, uint2 *cell)
 {
-    if constexpr (TELSRC == TEL_CONST) {
+    if constexpr (tel_base(TELSRC) == TEL_CONST) {
         const float vz2s = vz * vz * 0.9999f, add = REFR ? refraction_slack(P, vz) : 0.0f;
         uint32_t cm = 0u;
         // NT = n_tel rounded up to 1, 4 or 8; the unused slots hold R^2 = -1 (never a candidate).  Unrolled so that the
@@ -1459,7 +1460,7 @@ __device__ __forceinline__ uint32_t plane_candidates(const KParams &P, float gx,
         for (int k = 0; k < NT; ++k)
             if (plane_pretest<COPLANAR>(P.tel_c[k], gx, gy, vx, vy, vz, vz2s, add)) cm |= 1u << k;
         return cm;
-    } else if constexpr (TELSRC == TEL_GRID) {
+    } else if constexpr (tel_base(TELSRC) == TEL_GRID) {
         // steep photons use level 0; flatter ones the coarser level 1 when it exists, else the wide test.  One code
         // path per level, so that the level's parameters are constant-bank operands.
         if (-vz >= P.grid_lvl[0].vzmin) {
@@ -1494,7 +1495,7 @@ __device__ __noinline__ void wide_batch(const KParams &P, TileSmem &sm, unsigned
     if (lane < n) {
         const uint32_t q = sm.wide_list[warp][lane];
         e = (int)(q >> 24); j = q & 0xffffffu;
-        const Photon ph = make_photon<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, j, emitter_segment(P, tile_first, e));
+        const Photon ph = make_photon<tel_disp(TELSRC)>(P, sm, e, j, emitter_segment(P, tile_first, e));
         live = ph.vz < 0.0f;
         // a point of the ray relative to (x_ref, y_ref, z_ref): the plane crossing (axis kind) or the emission point
         px = ph.axis ? ph.gx : ph.ex; py = ph.axis ? ph.gy : ph.ey; pz = ph.axis ? 0.0f : ph.ez;
@@ -1564,8 +1565,8 @@ template <int TELSRC, bool COPLANAR, int NT, bool REFR>
 __device__ __noinline__ uint32_t generic_candidates(const KParams &P, const TileSmem &sm, int e, uint32_t r0, uint32_t r1, uint32_t r2,
                                                     uint32_t r3, uint2 *cell, bool *upward)
 {
-    const Photon ph = photon_from_rand<TELSRC == TEL_GLOBAL_DISP>(P, sm, e, Rand4{r0, r1, r2, r3});
-    if constexpr (TELSRC == TEL_GLOBAL_DISP) {
+    const Photon ph = photon_from_rand<tel_disp(TELSRC)>(P, sm, e, Rand4{r0, r1, r2, r3});
+    if constexpr (tel_disp(TELSRC)) {
         if (ph.tag == 0 && ph.rva == 0.0f) { *upward = false; return 0u; }      // R30: below the threshold at its wavelength
     }
     *upward = !(ph.vz < 0.0f);
@@ -1602,7 +1603,7 @@ template <int TELSRC, bool COPLANAR, int NT, int MODE, bool REFR>
 __device__ __forceinline__ void walk(const KParams &P, TileSmem &sm, WarpWalk &ww, const uint32_t hi, const unsigned long long tile_first,
                                      const uint32_t n_iter)
 {
-    constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
+    constexpr bool kFrameInRegs = (tel_base(TELSRC) == TEL_CONST);
     int e = ww.e, kind = ww.kind;
     uint32_t end = ww.end, g = ww.g, j = ww.j, n_up = ww.n_up, q_head = ww.q_head, q_count = ww.q_count;
     PhiloxEmitter pe = ww.pe;
@@ -1658,7 +1659,7 @@ __device__ __forceinline__ void walk(const KParams &P, TileSmem &sm, WarpWalk &w
                 if (up) ++n_up;
             }
         }
-        if constexpr (TELSRC == TEL_CONST) {
+        if constexpr (tel_base(TELSRC) == TEL_CONST) {
             if (cm == kAllTelescopes) cm = (1u << NT) - 1u;          // flat photon: all slots go to the exact test
         } else {
             const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
@@ -1691,7 +1692,7 @@ template <int TELSRC, bool COPLANAR, int NT, int MODE, bool REFR, bool INLINE>
 __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const uint32_t base, const uint32_t hi,
                                            const unsigned long long tile_first, uint32_t &n_up_out, uint32_t &q_head, uint32_t &q_count)
 {
-    constexpr bool kFrameInRegs = (TELSRC == TEL_CONST);
+    constexpr bool kFrameInRegs = (tel_base(TELSRC) == TEL_CONST);
     const int lane = threadIdx.x & 31;
     if (base >= hi) return;
     uint32_t g = base + 2u * (uint32_t)lane;
@@ -1711,7 +1712,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
         // brute-force kernels: the telescopes that any lane's emitter can reach at all (reach_mask); the pre-tests of the
         // others are skipped for the whole warp (most emitters of a shower reach none; a trip spans one or two emitters)
         uint32_t umask = 0xffu;
-        if constexpr (TELSRC == TEL_CONST) {
+        if constexpr (tel_base(TELSRC) == TEL_CONST) {
             if (active && g >= end) {
                 do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
                 rend = end - sm.odd[e];
@@ -1729,7 +1730,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
         hA.ok = false; hA.k = 0; hA.x = hA.y = hA.vx = hA.vy = hA.t = hA.lam = hA.w = 0.0f;
         hB = hA;
         if (active) {
-            if (TELSRC != TEL_CONST && g >= end) {
+            if (tel_base(TELSRC) != TEL_CONST && g >= end) {
                 do { ++e; end = sm.prefix[e + 1]; } while (g >= end);
                 rend = end - sm.odd[e];
                 j = g - sm.prefix[e];
@@ -1758,7 +1759,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                     vxA = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); vyA = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
                     vxB = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); vyB = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
                 }
-                if constexpr (TELSRC == TEL_CONST) {
+                if constexpr (tel_base(TELSRC) == TEL_CONST) {
                     // the pre-tests of both photons, telescope by telescope, for the telescopes in reach of the warp
                     const bool dnA = vzA < 0.0f, dnB = hasB && vzB < 0.0f;
                     n_up += (dnA ? 0u : 1u) + ((hasB && !dnB) ? 1u : 0u);
@@ -1828,7 +1829,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
             const uint2 cell = s ? cellB : cellA;
             const Rand4 r = s ? rB : rA;
             const uint32_t jj = j + (uint32_t)s;
-            if constexpr (TELSRC == TEL_CONST) {
+            if constexpr (tel_base(TELSRC) == TEL_CONST) {
                 if (cm == kAllTelescopes) cm = (1u << NT) - 1u;
             } else {
                 const uint32_t wide = __ballot_sync(0xffffffffu, cm == kAllTelescopes);
@@ -2196,7 +2197,7 @@ __device__ __forceinline__ void walk_dense(const KParams &P, TileSmem &sm, OutSm
 // without, every tile takes the sparse paths (correct for any input, 3 CTAs/SM): the host launches that instance when
 // no telescope is large enough to catch a good part of a shower's light (c8opt.cu, pick_kernel).
 template <int TELSRC, bool COPLANAR, int NT, int MODE, bool DENSE = true>
-__global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONST && DENSE) ? kOutCtasPerSm : 3) propagate_kernel(const __grid_constant__ KParams P)
+__global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && tel_base(TELSRC) == TEL_CONST && DENSE) ? kOutCtasPerSm : 3) propagate_kernel(const __grid_constant__ KParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     TileSmem &sm = *reinterpret_cast<TileSmem *>(smem_raw);
@@ -2214,7 +2215,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     sm.acc_n[tid] = 0u; sm.acc_k[tid] = -1; sm.acc_w[tid] = 0.0; sm.acc_wt[tid] = 0.0;
     if (tid < kWarps) sm.wide_count[tid] = 0u;
     constexpr bool OUT = (MODE == MODE_OUT);
-    if constexpr (OUT && TELSRC == TEL_CONST && DENSE) {
+    if constexpr (OUT && tel_base(TELSRC) == TEL_CONST && DENSE) {
         OutSmem &os = out_smem(sm);
         if (tid < kRoundSlots) { os.agg[tid] = 0u; os.rbase[tid] = 0ull; mbar_init(&os.rbar[tid], 1u); }
         if (tid < kTelConstMax) os.probe[tid] = 0u;
@@ -2236,7 +2237,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         const float4 s0 = __ldg(sp), s1 = __ldg(sp + 1), s2 = __ldg(sp + 2);
         int bad;
         bool culled;
-        nb = preamble<false, TELSRC == TEL_CONST, TELSRC == TEL_GLOBAL_DISP>(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled, nullptr,
+        nb = preamble<false, tel_base(TELSRC) == TEL_CONST, tel_disp(TELSRC)>(P, s0, s1, s2, tag, &sm.frame[tid * kFrameStride], &sm.kind[tid], &bad, &culled, nullptr,
                                                   &sm.tmask[tid]);
         if (P.split_part == 2) {
             // second launch of a two-process request: the first one (Cherenkov) has counted the segments that are
@@ -2316,7 +2317,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
         // One instance of a loop per setting of the refraction slack in the pre-tests: it is uniform over the launch, and
         // a photon of the default path does not pay for it.
         uint32_t q_head = 0u, q_count = 0u;
-        if constexpr (OUT && TELSRC != TEL_CONST) {
+        if constexpr (OUT && tel_base(TELSRC) != TEL_CONST) {
             // emitter of this lane's first photon: the e with prefix[e] <= g < prefix[e+1] (skips empty emitters)
             WarpWalk ww;
             {
@@ -2366,7 +2367,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
                 else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
             }
         }
-        if constexpr (TELSRC != TEL_CONST) {
+        if constexpr (tel_base(TELSRC) != TEL_CONST) {
             __syncwarp();
             const uint32_t nw = sm.wide_count[warp];
             if (nw) wide_batch<TELSRC, MODE>(P, sm, tile_first, q_head, q_count, nw);
@@ -2383,7 +2384,7 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && TELSRC == TEL_CONS
     if constexpr (MODE != MODE_HIST) {
         // the flat photons the loops set aside, in double (tile-uniform branch)
         if (sm.flat_count) {
-            flat_pass<MODE, TELSRC == TEL_GLOBAL_DISP>(P, sm, tile_first);
+            flat_pass<MODE, tel_disp(TELSRC)>(P, sm, tile_first);
             __syncthreads();
         }
     }
