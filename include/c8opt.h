@@ -141,9 +141,9 @@ typedef struct {
                                       lambda.  > 0 (the Frank-Tamm integrand with n(lambda); R30): the
                                       yield is the integral over the band (16-interval Simpson in 1 / lambda, cut at the
                                       threshold), every photon leaves at the Cherenkov angle of its own wavelength and carries
-                                      sin^2(lambda) / <sin^2> as a weight factor.  Runs on brute-force kernel instances of
-                                      its own (every photon against every telescope); not with C8OPT_FLAG_CULL, not in
-                                      C8OPT_MODE_GROUND_HIST.  Air in the band 300-600 nm: b ~ 5.7e3 nm^2 */
+                                      sin^2(lambda) / <sin^2> as a weight factor.  Runs on kernel instances of its own (the
+                                      general photon loop: about 3.6 x the time of the plain run on configs[1]); not with
+                                      C8OPT_FLAG_CULL, not in C8OPT_MODE_GROUND_HIST.  Air in the band 300-600 nm: b ~ 5.7e3 nm^2 */
 } c8opt_run_params;
 
 /* Optional outputs of one propagate call; every pointer is DEVICE memory owned

@@ -1705,6 +1705,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
     }
     uint32_t end = sm.prefix[e + 1], rend = end - sm.odd[e], j = g - sm.prefix[e], n_up = 0u;
     int kind = sm.kind[e];
+    uint32_t reach = sm.tmask[e];                 // brute-force kernels: the telescopes this lane's emitter can reach
     PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
     AxisFrame f_reg = load_axis_frame(sm, e);
     for (uint32_t b0 = base; b0 < hi; b0 += 64u, g += 64u, j += 64u) {
@@ -1718,10 +1719,11 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                 rend = end - sm.odd[e];
                 j = g - sm.prefix[e];
                 kind = sm.kind[e];
+                reach = sm.tmask[e];
                 pe = philox_emitter(P, emitter_segment(P, tile_first, e));
                 f_reg = load_axis_frame(sm, e);
             }
-            umask = __reduce_or_sync(0xffffffffu, active ? (uint32_t)sm.tmask[e] : 0u);
+            umask = __reduce_or_sync(0xffffffffu, active ? reach : 0u);
         }
         uint32_t cmA = 0u, cmB = 0u;
         uint2 cellA = make_uint2(0xffffffffu, 0xffffffffu), cellB = cellA;
@@ -1823,6 +1825,8 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
             commit_hits<MODE>(P, sm, hB, id0 + 1ull);
         }
         // candidates of slot A, then of slot B: wide test / on-the-spot evaluation / queue, as in walk()
+        // (most trips of a shower's light hold none: one vote skips the lot)
+        if (!__any_sync(0xffffffffu, (cmA | cmB) != 0u)) continue;
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
             uint32_t cm = s ? cmB : cmA;
