@@ -42,6 +42,7 @@ ALG_PARTS = {
     "grid_lookup": 15.0,        # cell index, bounds test, 8-byte load, first pre-test (100-telescope array)
     "generic_photon": 34.0,     # fluorescence / generic kinds: emission point, sincospi polynomial, polar angle, direction
     "walk": 14.0,               # index walk, emitter-crossing test, loop
+    "reach_vote": 3.0,          # brute-force kernels: OR of the lanes' reach masks over the warp, test, branch
     "queue": 4.0,               # candidate ballot / queue test
     "exact_per_hit": 250.0,     # regenerate + exact test + time + wavelength + weight + commit, per (photon, telescope) hit
     "preamble_per_emitter": 1200.0,   # fp64 preamble of one (segment, process)
@@ -50,9 +51,13 @@ ALG_PARTS = {
 }
 
 
-def alg_instr_per_photon(name: str, photons: float, emitters: float, hits: float, n_tel: int, ground_hist: bool = False) -> dict:
+def alg_instr_per_photon(name: str, photons: float, emitters: float, hits: float, n_tel: int, ground_hist: bool = False,
+                         reach_frac: float = 1.0) -> dict:
     """Algorithmic instructions per photon of workload `name`, from ALG_PARTS and the measured counts of the run
-    (photons, emitters = (segment, process) pairs with a preamble, hits).  Returns the parts and their sum."""
+    (photons, emitters = (segment, process) pairs with a preamble, hits).  Returns the parts and their sum.
+    reach_frac (brute-force kernels, <= 8 telescopes): the share of the photons whose emitter can reach a telescope at
+    all (reach mask of the preamble, measured by bench.py with one culling pass); the plane crossing, the pre-tests and
+    the candidate dispatch are the method's work for those photons only -- the others are generated and counted."""
     P = ALG_PARTS
     fluor = name in ("c3a", "c3b")
     parts = {}
@@ -64,14 +69,18 @@ def alg_instr_per_photon(name: str, photons: float, emitters: float, hits: float
         parts["philox"] = P["philox_block"] / 2                 # one block per TWO Cherenkov photons (R20)
         parts["uniforms"] = 2 * P["uniform"]
         parts["generation"] = P["azimuth"]
-    parts["projection"] = P["project"]
+    brute = n_tel <= 8 and not ground_hist and name != "c5g"
+    rf = reach_frac if brute else 1.0
+    parts["projection"] = P["project"] * rf + (2.0 * (1.0 - rf) if brute else 0.0)      # v_z and its sign test stay (upward count)
     if ground_hist:
         parts["histogram"] = P["hist_per_bunch"]
     elif name == "c5g":
         parts["record"] = P["record_per_hit"] * hits / photons
     else:
-        parts["pretests"] = P["grid_lookup"] if n_tel > 8 else P["pretest_per_tel"] * (1 if n_tel <= 1 else 4 if n_tel <= 4 else 8)
-        parts["queue"] = P["queue"]
+        parts["pretests"] = P["grid_lookup"] if n_tel > 8 else P["pretest_per_tel"] * (1 if n_tel <= 1 else 4 if n_tel <= 4 else 8) * rf
+        parts["queue"] = P["queue"] * rf
+        if brute:
+            parts["reach_vote"] = P["reach_vote"] / 2           # once per trip of two photons per lane
         parts["exact_amortised"] = P["exact_per_hit"] * hits / photons
     parts["walk"] = P["walk"]
     parts["preamble_amortised"] = P["preamble_per_emitter"] * emitters / photons
@@ -340,6 +349,17 @@ def main():
         photons_all = float(photons_per_step)
     value = photons_all * args.steps / (total_ms * 1e-3)
 
+    # brute-force kernels: the share of the Cherenkov photons whose emitter can reach a telescope at all, from one
+    # untimed pass with the exact culling on (it culls exactly the emitters whose reach mask is empty)
+    reach_frac = 1.0
+    if (n_tel <= 8 and (par["processes"] & 1) and not (args.ground_hist or args.cull or args.cauchy_b > 0.0)
+            and args.workload not in ("c5g", "c3a", "c3b") and rank == 0):
+        pc = dict(par, mode=c8.MODE_TALLY, flags=c8.FLAG_CULL)
+        ctx.reset_tallies()
+        ctx.propagate_segments(d_seg, pc, n=n, first_segment_id=first_id)
+        cc = ctx.read_tallies()[1]
+        reach_frac = 1.0 - cc["culled"] / max(cc["generated"], 1)
+
     # ---- the job's only exchange: one sum of the per-telescope tallies and counters over the ranks, after
     # the timed region (NCCL all-reduce of a few hundred bytes)
     reduced = None
@@ -415,7 +435,7 @@ def main():
     # ---- roofline of the dominant (only) kernel
     per_launch_s = total_ms * 1e-3 / args.steps
     alg = alg_instr_per_photon(args.workload, float(photons_per_step - culled_per_step), float(n * n_procs), float(hits_per_step), n_tel,
-                               ground_hist=args.ground_hist)
+                               ground_hist=args.ground_hist, reach_frac=reach_frac)
     if args.workload == "c5g":
         bytes_per_launch = RECORD_BYTES * hits_per_step + SEGMENT_BYTES * n
         roofline = {"bound": "hbm", "achieved": bytes_per_launch / per_launch_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
@@ -426,7 +446,7 @@ def main():
         # culled bunches cost no photon-loop instructions: the roofline counts the propagated ones only
         roofline = {"bound": "alu", "achieved": alg["total"] * (photons_per_step - culled_per_step) / per_launch_s / 1e12, "peak": peak,
                     "unit": "Tinstr/s", "traffic": None, "peak_source": "148 SM x 4 schedulers x 32 lanes x sm_max_mhz "
-                    f"({peaks['source']})", "alg_instr_per_photon": alg["total"], "alg_instr_parts": alg["parts"],
+                    f"({peaks['source']})", "alg_instr_per_photon": alg["total"], "alg_instr_parts": alg["parts"], "reach_frac": reach_frac,
                     "hbm_achieved_gbs": (SEGMENT_BYTES * n + RECORD_BYTES * (hits_per_step if output_mode else 0)) / per_launch_s / 1e9}
     roofline["traffic_note"] = "not measured in this run; the ncu --set full captures of the round are under profiles/"
     roofline["frac"] = roofline["achieved"] / roofline["peak"]

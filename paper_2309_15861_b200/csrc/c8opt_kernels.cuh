@@ -1752,26 +1752,32 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                 __sincosf(fmaf(one_two(rA.r1), 6.2831853f, -9.42477760f), &spA, &cpA);
                 __sincosf(fmaf(one_two(rB.r1), 6.2831853f, -9.42477760f), &spB, &cpB);
                 const float vzA = fmaf(cpA, f.az, fmaf(spA, f.bz, f.cz)), vzB = fmaf(cpB, f.az, fmaf(spB, f.bz, f.cz));
-                const float rhoA = sdA * rcp_approx(vzA), rhoB = sdB * rcp_approx(vzB);
-                const float gxA = fmaf(rhoA, fmaf(cpA, f.px, spA * f.qx), f.gx), gyA = fmaf(rhoA, fmaf(cpA, f.py, spA * f.qy), f.gy);
-                const float gxB = fmaf(rhoB, fmaf(cpB, f.px, spB * f.qx), f.gx), gyB = fmaf(rhoB, fmaf(cpB, f.py, spB * f.qy), f.gy);
-                float vxA = 0.0f, vyA = 0.0f, vxB = 0.0f, vyB = 0.0f;
-                if (!COPLANAR) {
-                    const float *fr = &sm.frame[e * kFrameStride];
-                    vxA = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); vyA = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
-                    vxB = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); vyB = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
+                // the crossing of the reference plane and (non-coplanar arrays) the horizontal direction: only where a
+                // telescope is in reach of the warp (brute-force kernels: umask; a shower's light mostly reaches none)
+                float gxA = 0.0f, gyA = 0.0f, gxB = 0.0f, gyB = 0.0f, vxA = 0.0f, vyA = 0.0f, vxB = 0.0f, vyB = 0.0f;
+                if (tel_base(TELSRC) != TEL_CONST || umask != 0u) {
+                    const float rhoA = sdA * rcp_approx(vzA), rhoB = sdB * rcp_approx(vzB);
+                    gxA = fmaf(rhoA, fmaf(cpA, f.px, spA * f.qx), f.gx); gyA = fmaf(rhoA, fmaf(cpA, f.py, spA * f.qy), f.gy);
+                    gxB = fmaf(rhoB, fmaf(cpB, f.px, spB * f.qx), f.gx); gyB = fmaf(rhoB, fmaf(cpB, f.py, spB * f.qy), f.gy);
+                    if (!COPLANAR) {
+                        const float *fr = &sm.frame[e * kFrameStride];
+                        vxA = fmaf(cpA, fr[F_AX], fmaf(spA, fr[F_BX], fr[F_CX])); vyA = fmaf(cpA, fr[F_AY], fmaf(spA, fr[F_BY], fr[F_CY]));
+                        vxB = fmaf(cpB, fr[F_AX], fmaf(spB, fr[F_BX], fr[F_CX])); vyB = fmaf(cpB, fr[F_AY], fmaf(spB, fr[F_BY], fr[F_CY]));
+                    }
                 }
                 if constexpr (tel_base(TELSRC) == TEL_CONST) {
                     // the pre-tests of both photons, telescope by telescope, for the telescopes in reach of the warp
                     const bool dnA = vzA < 0.0f, dnB = hasB && vzB < 0.0f;
                     n_up += (dnA ? 0u : 1u) + ((hasB && !dnB) ? 1u : 0u);
-                    const float vz2sA = vzA * vzA * 0.9999f, vz2sB = vzB * vzB * 0.9999f;
-                    const float addA = REFR ? refraction_slack(P, vzA) : 0.0f, addB = REFR ? refraction_slack(P, vzB) : 0.0f;
+                    if (umask != 0u) {
+                        const float vz2sA = vzA * vzA * 0.9999f, vz2sB = vzB * vzB * 0.9999f;
+                        const float addA = REFR ? refraction_slack(P, vzA) : 0.0f, addB = REFR ? refraction_slack(P, vzB) : 0.0f;
 #pragma unroll
-                    for (int k = 0; k < NT; ++k) {
-                        if ((umask >> k) & 1u) {
-                            if (dnA && plane_pretest<COPLANAR>(P.tel_c[k], gxA, gyA, vxA, vyA, vzA, vz2sA, addA)) cmA |= 1u << k;
-                            if (dnB && plane_pretest<COPLANAR>(P.tel_c[k], gxB, gyB, vxB, vyB, vzB, vz2sB, addB)) cmB |= 1u << k;
+                        for (int k = 0; k < NT; ++k) {
+                            if ((umask >> k) & 1u) {
+                                if (dnA && plane_pretest<COPLANAR>(P.tel_c[k], gxA, gyA, vxA, vyA, vzA, vz2sA, addA)) cmA |= 1u << k;
+                                if (dnB && plane_pretest<COPLANAR>(P.tel_c[k], gxB, gyB, vxB, vyB, vzB, vz2sB, addB)) cmB |= 1u << k;
+                            }
                         }
                     }
                 } else {
