@@ -1705,7 +1705,9 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
     }
     uint32_t end = sm.prefix[e + 1], rend = end - sm.odd[e], j = g - sm.prefix[e], n_up = 0u;
     int kind = sm.kind[e];
-    uint32_t reach = sm.tmask[e];                 // brute-force kernels: the telescopes this lane's emitter can reach
+    // brute-force kernels: the telescopes this lane's emitter can reach; bit 8 = not the axis kind (its candidates do
+    // not come from the pre-tests below)
+    uint32_t reach = (uint32_t)sm.tmask[e] | ((kind != KIND_CHER_AXIS) ? 0x100u : 0u);
     PhiloxEmitter pe = philox_emitter(P, emitter_segment(P, tile_first, e));
     AxisFrame f_reg = load_axis_frame(sm, e);
     for (uint32_t b0 = base; b0 < hi; b0 += 64u, g += 64u, j += 64u) {
@@ -1719,7 +1721,7 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
                 rend = end - sm.odd[e];
                 j = g - sm.prefix[e];
                 kind = sm.kind[e];
-                reach = sm.tmask[e];
+                reach = (uint32_t)sm.tmask[e] | ((kind != KIND_CHER_AXIS) ? 0x100u : 0u);
                 pe = philox_emitter(P, emitter_segment(P, tile_first, e));
                 f_reg = load_axis_frame(sm, e);
             }
@@ -1832,6 +1834,9 @@ __device__ __forceinline__ void walk_pairs(const KParams &P, TileSmem &sm, const
         }
         // candidates of slot A, then of slot B: wide test / on-the-spot evaluation / queue, as in walk()
         // (most trips of a shower's light hold none: one vote skips the lot)
+        // (photon output: nothing in reach of the warp = no candidate, without the vote; the tally kernels, whose dispatch
+        // below is one test, measured slower with this branch: c2 0.678 -> 0.685 ms, c5 7.21 -> 7.01 ms)
+        if constexpr (tel_base(TELSRC) == TEL_CONST && MODE != MODE_TALLY) { if (umask == 0u) continue; }
         if (!__any_sync(0xffffffffu, (cmA | cmB) != 0u)) continue;
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
@@ -2276,7 +2281,9 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && tel_base(TELSRC) =
     const uint32_t nbp = nb + odd;
     sm.odd[tid] = (uint8_t)odd;
     const uint32_t n_pad_w = (uint32_t)__popc(__ballot_sync(0xffffffffu, odd != 0u));
-    const uint32_t weight = (nb != 0u && sm.kind[tid] != KIND_CHER_AXIS) ? (uint32_t)kGenericWeight : 1u;
+    // (brute-force kernels: an axis-kind emitter that reaches a telescope pays the plane crossing and the pre-tests)
+    uint32_t weight = (nb != 0u && sm.kind[tid] != KIND_CHER_AXIS) ? 2u * (uint32_t)kGenericWeight : 2u;
+    if constexpr (tel_base(TELSRC) == TEL_CONST) { if (weight == 2u && sm.tmask[tid] != 0u) weight = 4u; }      // measured: 3: c2 0.683 ms, 4: 0.679, 5: 0.679 (unweighted 0.700)
     const unsigned long long wnb = (unsigned long long)nbp * weight;
     uint32_t inc = nbp;
     unsigned long long winc = wnb;
