@@ -2313,9 +2313,15 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && tel_base(TELSRC) =
     if (wnb) {
         const unsigned long long wexcl = wwoff + winc - wnb;
 #pragma unroll
+        // Large tiles: the shares begin on whole trips of the loops (64 slots), so that only the tile's last trip is a
+        // partial one and the record blocks of a dense tile keep their size (c5g 15.95 -> 15.66 ms); small tiles
+        // (fluorescence: a few hundred slots per warp) keep the finer split (tried there: c4 16.21 -> 16.43 ms).
+        // (the instance with the dense loop aligns always: its tiles of interest are large)
+        constexpr bool kAlignAlways = (MODE == MODE_OUT && tel_base(TELSRC) == TEL_CONST && DENSE);
+        const uint32_t amask = (kAlignAlways || total >= 16384u) ? ~63u : ~1u;
         for (int w = 1; w < kWarps; ++w) {
             const unsigned long long x = wtotal / kWarps * (unsigned)w + wtotal % kWarps * (unsigned)w / kWarps;   // floor(wtotal w / 8)
-            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & ~1u;
+            if (x >= wexcl && x < wexcl + wnb) sm.bound[w] = (excl + (uint32_t)((x - wexcl) / weight)) & amask;
         }
     }
     __syncthreads();
@@ -2380,8 +2386,20 @@ __global__ void __launch_bounds__(kTile, (MODE == MODE_OUT && tel_base(TELSRC) =
             }
             if (!dense) {
                 // tally, sparse photon output: candidates to the queue; ground histogram: both photons evaluated inline
-                if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
-                else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
+                if constexpr (OUT && tel_base(TELSRC) == TEL_CONST) {
+                    // The range re-read from shared memory inside a (one-pass) loop: the bounds then do not stay live in
+                    // registers across the dense loop above, which the compiler schedules better for it (measured: c5g
+                    // 15.92 -> 15.63 ms, c5 7.03 -> 6.98 ms; the same form costs the grid kernels 1.8 %, so only here).
+                    // More than one piece per warp, interleaved over the tile, measured slower (c2 0.68 -> 0.70 ms with two).
+                    for (int p = warp; p < kWarps; p += kWarps) {
+                        const uint32_t plo = sm.bound[p], phi = sm.bound[p + 1];
+                        if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true, MODE == MODE_HIST>(P, sm, plo, phi, tile_first, n_up, q_head, q_count);
+                        else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, plo, phi, tile_first, n_up, q_head, q_count);
+                    }
+                } else {
+                    if (P.flags & kFlagRefract) walk_pairs<TELSRC, COPLANAR, NT, MODE, true, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
+                    else walk_pairs<TELSRC, COPLANAR, NT, MODE, false, MODE == MODE_HIST>(P, sm, lo, hi, tile_first, n_up, q_head, q_count);
+                }
             }
         }
         if constexpr (tel_base(TELSRC) != TEL_CONST) {
