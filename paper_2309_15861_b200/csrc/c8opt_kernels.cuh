@@ -20,7 +20,10 @@
 // good part of the light takes the dense loop instead (walk_dense: every candidate is
 // evaluated on the spot, records staged per warp, slots reserved once per tile and round
 // without a block barrier, 16-byte vector stores).  Flat photons (|v_z| < 0.05) are set
-// aside and evaluated in double at the end of the tile (flat_pass).
+// aside and evaluated in double at the end of the tile (flat_pass).  Brute-force kernels
+// (<= 8 telescopes): the preamble also finds the telescopes an emitter can reach at all; a
+// trip of the pair loop whose lanes reach none only draws, orients and counts its photons.
+// TEL_DISP instances: the Cherenkov launch of a request with n(lambda) (R30).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>

@@ -717,3 +717,30 @@ def test_wavelength_dependent_refractive_index_argument_errors(c8):
             pu.gpu_run(cfg, c8.MODE_TALLY)
         assert ei.value.code == -1 and msg in str(ei.value)
         cfg["params"].pop("flags", None)
+
+
+def test_wavelength_dependent_refractive_index_with_refraction_and_cut(c8):
+    """R30 together with the refraction corrections (R27) and the paper's angular cut (R29), through the host-segment
+    entry point; and through c8opt_tally_static (same tallies as the context path)."""
+    import torch
+    import parity_util as pu
+    cfg = wl.make_config("c2", n_segments=30_000)
+    cfg["params"] = dict(cfg["params"], cauchy_b=5670.0, flags=c8.FLAG_REFRACT | c8.FLAG_CUT_TELESCOPES, cut_angle=float(np.radians(5.0)))
+    g = pu.gpu_run(cfg, c8.MODE_OUTPUT, host_segments=True)
+    o = pu.oracle_run(cfg)
+    rep = pu.compare(cfg, g, o)
+    _report("dispersion-refract-cut-c2", rep)
+    assert rep["matched"] > 100 and g["counters"]["culled"] > 0
+    dev = torch.device("cuda:0")
+    n = len(cfg["segments"])
+    d_seg = torch.from_numpy(cfg["segments"].view(np.uint8).reshape(n, 48).copy()).to(dev)
+    tau = cfg["atmosphere"].get("tau")
+    d_tau = None if tau is None else torch.from_numpy(np.ascontiguousarray(tau, dtype=np.float32)).to(dev)
+    n_tel = len(cfg["telescopes"])
+    d_tal = torch.zeros((n_tel, 3), dtype=torch.int64, device=dev)
+    d_cnt = torch.zeros(8, dtype=torch.int64, device=dev)
+    c8.tally_static(cfg["atmosphere"], cfg["telescopes"], d_seg, dict(cfg["params"], mode=c8.MODE_TALLY), d_tal, d_cnt, d_tau=d_tau, n=n)
+    torch.cuda.synchronize()
+    tallies = d_tal.cpu().numpy().view(np.uint8).reshape(-1).view(c8.TALLY_DTYPE)
+    assert np.array_equal(tallies["hits"], g["tallies"]["hits"])
+    assert np.allclose(tallies["sum_w"], g["tallies"]["sum_w"], rtol=1e-12)
