@@ -218,16 +218,16 @@ int c8opt_propagate_segments(c8opt_ctx *ctx, const c8opt_segment *d_seg, uint64_
  * kernel of the previous chunk on two internal streams; returns after all work
  * is enqueued, ordered after prior work on `cuda_stream`, and `cuda_stream`
  * waits for it (also when an error is returned half way).  out->counts, if
- * given, is still DEVICE memory.  Needs two device staging buffers of one
+ * given, is still DEVICE memory.  Needs three device staging buffers of one
  * chunk each: allocated by c8opt_reserve_host_staging, else by the first call
  * that needs them (that call then synchronises the internal streams once). */
 int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, uint64_t n,
                                   uint64_t first_segment_id, const c8opt_run_params *params,
                                   const c8opt_output *out, void *cuda_stream);
 
-/* Create the internal streams and allocate the two device staging buffers of
+/* Create the internal streams and allocate the three device staging buffers of
  * c8opt_propagate_segments_host for tables of up to max_segments segments
- * (2 x 48 bytes x min(max(max_segments / 4, 32 Ki), 1 Mi), rounded to whole
+ * (3 x 48 bytes x min(max(max_segments / 4, 32 Ki), 1 Mi), rounded to whole
  * tiles), so that no later call allocates.  Errors: CUDA. */
 int c8opt_reserve_host_staging(c8opt_ctx *ctx, uint64_t max_segments);
 

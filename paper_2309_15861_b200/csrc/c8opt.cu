@@ -69,9 +69,10 @@ struct c8opt_ctx {
     unsigned long long segments_total = 0;      // host-side running count (counter 0)
     unsigned long long launches = 0;
     // host-segment pipeline
-    cudaStream_t pipe_stream[2] = {nullptr, nullptr};
-    cudaEvent_t pipe_event[3] = {nullptr, nullptr, nullptr};
-    c8opt_segment *d_stage[2] = {nullptr, nullptr};
+    static constexpr int kPipe = 3;             // staging buffers / internal streams of the host-segment pipeline
+    cudaStream_t pipe_stream[kPipe] = {};
+    cudaEvent_t pipe_event[kPipe + 1] = {};
+    c8opt_segment *d_stage[kPipe] = {};
     unsigned long long stage_segments = 0;
     char error[256] = "";
 };
@@ -451,20 +452,20 @@ int remember_capacity(c8opt_ctx *ctx, const c8opt_run_params *rp, const c8opt_ou
     return C8OPT_OK;
 }
 
-// The two internal streams, their events and the device staging buffers of c8opt_propagate_segments_host.
+// The internal streams, their events and the device staging buffers of c8opt_propagate_segments_host.
 int ensure_pipeline(c8opt_ctx *ctx, unsigned long long chunk_segments)
 {
     if (!ctx->pipe_stream[0]) {
-        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->pipe_stream[i], cudaStreamNonBlocking));
-        for (int i = 0; i < 3; ++i) C8_CUDA(ctx, cudaEventCreateWithFlags(&ctx->pipe_event[i], cudaEventDisableTiming));
+        for (int i = 0; i < c8opt_ctx::kPipe; ++i) C8_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->pipe_stream[i], cudaStreamNonBlocking));
+        for (int i = 0; i <= c8opt_ctx::kPipe; ++i) C8_CUDA(ctx, cudaEventCreateWithFlags(&ctx->pipe_event[i], cudaEventDisableTiming));
     }
     if (ctx->stage_segments < chunk_segments) {
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < c8opt_ctx::kPipe; ++i) {
             C8_CUDA(ctx, cudaStreamSynchronize(ctx->pipe_stream[i]));
             cudaFree(ctx->d_stage[i]); ctx->d_stage[i] = nullptr;
         }
         ctx->stage_segments = 0;
-        for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaMalloc(&ctx->d_stage[i], sizeof(c8opt_segment) * chunk_segments));
+        for (int i = 0; i < c8opt_ctx::kPipe; ++i) C8_CUDA(ctx, cudaMalloc(&ctx->d_stage[i], sizeof(c8opt_segment) * chunk_segments));
         ctx->stage_segments = chunk_segments;
     }
     return C8OPT_OK;
@@ -675,9 +676,11 @@ int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, ui
     if (n == 0) return C8OPT_OK;
     // Chunk schedule: the first chunk is small (1/32 of the table, at least 32 Ki segments) so that the first kernel
     // starts after a short copy; the chunks then double up to a quarter of the table, so that the kernels in the
-    // middle fill the GPU for several waves, and no chunk takes more than half of what is left, so that the last
-    // kernel, which nothing overlaps, is short again.  Two staging buffers, copy and kernel of a chunk on the same
-    // internal stream.
+    // middle fill the GPU for several waves, and no chunk takes more than a quarter of what is left, so that the last
+    // kernels, which no copy overlaps, are short again (a half: 1.085 ms end to end on c2, a third: 1.063, a quarter:
+    // 1.050; the copy alone takes 0.88 ms, in these chunks 0.92).  Three staging buffers, copy and kernel of a chunk on
+    // the same internal stream: the copy of chunk c + 3 waits for the kernel of chunk c (with two buffers the copy
+    // engine stood still in the tapering part, where the kernel of a chunk outlasts the copy of the next: 1.158 ms).
     const unsigned long long chunk_max = host_chunk_max(n);
     rc = ensure_pipeline(ctx, chunk_max);          // allocates on the first call unless c8opt_reserve_host_staging did
     if (rc != C8OPT_OK) return rc;
@@ -686,21 +689,22 @@ int c8opt_propagate_segments_host(c8opt_ctx *ctx, const c8opt_segment *h_seg, ui
     chunk_min = (chunk_min + c8::kTile - 1) / c8::kTile * c8::kTile;
     if (chunk_min > chunk_max) chunk_min = chunk_max;
     unsigned long long grow = chunk_min;
-    C8_CUDA(ctx, cudaEventRecord(ctx->pipe_event[2], user));
-    for (int i = 0; i < 2; ++i) C8_CUDA(ctx, cudaStreamWaitEvent(ctx->pipe_stream[i], ctx->pipe_event[2], 0));
+    constexpr int kPipe = c8opt_ctx::kPipe;
+    C8_CUDA(ctx, cudaEventRecord(ctx->pipe_event[kPipe], user));
+    for (int i = 0; i < kPipe; ++i) C8_CUDA(ctx, cudaStreamWaitEvent(ctx->pipe_stream[i], ctx->pipe_event[kPipe], 0));
     int c = 0;
     cudaError_t ce = cudaSuccess;
     for (unsigned long long off = 0, m = 0; off < n && rc == C8OPT_OK && ce == cudaSuccess; off += m, grow = std::min(2 * grow, chunk_max), ++c) {
-        const unsigned long long left = n - off, half = (left / 2 + c8::kTile - 1) / c8::kTile * c8::kTile;
+        const unsigned long long left = n - off, half = (left / 4 + c8::kTile - 1) / c8::kTile * c8::kTile;   // (a quarter)
         m = std::min(left, std::max(chunk_min, std::min(grow, half)));
-        cudaStream_t st = ctx->pipe_stream[c & 1];
-        ce = cudaMemcpyAsync(ctx->d_stage[c & 1], h_seg + off, sizeof(c8opt_segment) * m, cudaMemcpyHostToDevice, st);
+        cudaStream_t st = ctx->pipe_stream[c % kPipe];
+        ce = cudaMemcpyAsync(ctx->d_stage[c % kPipe], h_seg + off, sizeof(c8opt_segment) * m, cudaMemcpyHostToDevice, st);
         if (ce != cudaSuccess) break;
-        rc = launch(ctx, P, params->mode, ctx->d_stage[c & 1], m, first_segment_id + off,
+        rc = launch(ctx, P, params->mode, ctx->d_stage[c % kPipe], m, first_segment_id + off,
                     (out && out->counts) ? out->counts + 2 * off : nullptr, st);
     }
     // also after an error: the caller's stream waits for whatever was enqueued on the internal streams
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < kPipe; ++i) {
         const cudaError_t e1 = cudaEventRecord(ctx->pipe_event[i], ctx->pipe_stream[i]);
         const cudaError_t e2 = (e1 == cudaSuccess) ? cudaStreamWaitEvent(user, ctx->pipe_event[i], 0) : e1;
         if (ce == cudaSuccess && e2 != cudaSuccess) ce = e2;
@@ -809,11 +813,11 @@ void c8opt_destroy(c8opt_ctx *ctx)
     if (!ctx) return;
     DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < c8opt_ctx::kPipe; ++i) {
         if (ctx->pipe_stream[i]) cudaStreamDestroy(ctx->pipe_stream[i]);
         cudaFree(ctx->d_stage[i]);
     }
-    for (int i = 0; i < 3; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
+    for (int i = 0; i <= c8opt_ctx::kPipe; ++i) if (ctx->pipe_event[i]) cudaEventDestroy(ctx->pipe_event[i]);
     cudaFree(ctx->d_telD);
     cudaFree(ctx->d_tau); cudaFree(ctx->d_telA); cudaFree(ctx->d_telT); cudaFree(ctx->d_telEta); cudaFree(ctx->d_grid);
     cudaFree(ctx->d_results); cudaFreeHost(ctx->h_results); cudaFree(ctx->d_hist);
